@@ -1,0 +1,428 @@
+"""Pins for the CPU oracle (`oracle/`): every oracle function is checked against something
+other than itself -- hand-computed worked examples (tests/golden/*.json, each with its
+citation), closed forms, invariants, numpy/scipy library routines, brute force.
+
+CPU only (`-m "not gpu"`).  Nothing here touches the CUDA path.
+"""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy.special import expit, softmax
+
+import oracle
+from workloads.configs import RouterCfg, SIGMOID, SOFTMAX
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _bf16_bits(x: np.ndarray) -> np.ndarray:
+    """fp32 -> bf16 bit patterns (round to nearest even), numpy only."""
+    u = np.ascontiguousarray(x, np.float32).view(np.uint32).astype(np.uint64)
+    r = ((u >> 16) & 1) + 0x7FFF
+    return ((u + r) >> 16).astype(np.uint16)
+
+
+def _bf16_val(b: np.ndarray) -> np.ndarray:
+    return (b.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+
+
+# =========================================================================== a1 GEMM
+def test_logits_match_library_fp64_matmul():
+    rng = np.random.default_rng(1)
+    T, H, E, S = 37, 96, 24, 3
+    h = _bf16_bits(rng.standard_normal((T, H)))
+    w = _bf16_bits(0.02 * rng.standard_normal((E, H)))
+    off = np.array([0, 10, 10, 37], np.int32)          # one empty source
+    bias = rng.standard_normal((S, E)).astype(np.float32)
+    l64, l32 = oracle.router_logits(h, w, bias, off)
+    ref = _bf16_val(h) @ _bf16_val(w).T                  # library routine
+    src = np.repeat(np.arange(S), np.diff(off))
+    ref = ref + bias[src].astype(np.float64)
+    np.testing.assert_allclose(l64, ref, rtol=1e-13, atol=1e-13)
+    np.testing.assert_array_equal(l32, ref.astype(np.float32))
+
+
+def test_logits_special_cases():
+    rng = np.random.default_rng(2)
+    T, H = 5, 64
+    hid = rng.standard_normal((T, H))
+    h = _bf16_bits(hid)
+    off = np.array([0, T], np.int32)
+    # one-hot W rows return a column of hidden exactly
+    w = np.zeros((3, H), np.float32); w[0, 7] = 1; w[1, 0] = 1; w[2, 63] = 1
+    l64, _ = oracle.router_logits(h, _bf16_bits(w), None, off)
+    np.testing.assert_array_equal(l64, _bf16_val(h)[:, [7, 0, 63]])
+    # all ones give H; transposed-operand mistakes would fail the next (non-square) check
+    l64, _ = oracle.router_logits(_bf16_bits(np.ones((T, H))), _bf16_bits(np.ones((2, H))), None, off)
+    assert np.all(l64 == H)
+    # H = 1
+    l64, _ = oracle.router_logits(_bf16_bits(np.array([[2.0], [3.0]])), _bf16_bits(np.array([[0.5], [4.0], [-1.0]])), None,
+                                  np.array([0, 2], np.int32))
+    np.testing.assert_array_equal(l64, [[1.0, 8.0, -2.0], [1.5, 12.0, -3.0]])
+
+
+# =========================================================================== a2 gating
+def _gold(name):
+    with open(os.path.join(GOLD, name)) as f:
+        return json.load(f)
+
+
+def _rcfg(c, **kw):
+    d = dict(L=1, H=1, E=c["E"], k=c["k"], S=1, score_fn=SIGMOID if c["score_fn"] == "sigmoid" else SOFTMAX,
+             renorm=c.get("renorm", 0), n_groups=c.get("n_groups", 1), topk_groups=c.get("topk_groups", 1),
+             group_score_topn=c.get("group_score_topn", 1), routed_scale=c.get("routed_scale", 1.0))
+    d.update(kw)
+    return RouterCfg(**d)
+
+
+@pytest.mark.parametrize("tier", [0, 1])
+def test_gating_worked_examples(tier):
+    g = _gold("gating_worked_examples.json")
+    assert "PAPER.md:47" in g["citation"]
+    for c in g["cases"]:
+        x = np.array(c["logits"] if "logits" in c else np.log(c["logits_ln"]), np.float32)[None, :]
+        sb = np.array(c["select_bias"], np.float32) if "select_bias" in c else None
+        if "ids_grouped" in c:
+            ids, _ = oracle.gate(x, _rcfg(c), sb, tier)
+            assert ids[0].tolist() == c["ids_grouped"], c["name"]
+            ids, _ = oracle.gate(x, _rcfg(c, n_groups=1, topk_groups=1, group_score_topn=1), sb, tier)
+            assert ids[0].tolist() == c["ids_ungrouped"], c["name"]
+        else:
+            ids, w = oracle.gate(x, _rcfg(c), sb, tier)
+            assert ids[0].tolist() == c["ids"], c["name"]
+            np.testing.assert_allclose(w[0], c["weights"], rtol=2e-7, err_msg=c["name"])
+
+
+def test_sig32_is_a_sigmoid():
+    """the fp32 decision routine vs the mathematical function (scipy expit in fp64)."""
+    x = np.concatenate([np.linspace(-100, 100, 400001), np.random.default_rng(0).standard_normal(200000) * 3,
+                        [0.0, -0.0, 87.0, -87.0, 88.8, -88.8, 1e30, -1e30, np.inf, -np.inf]]).astype(np.float32)
+    s = oracle.sig32(x).astype(np.float64)
+    ref = expit(x.astype(np.float64))
+    # absolute error ~1.5 ulp of 1.0 everywhere (what a key = s + bias comparison sees) ...
+    assert np.max(np.abs(s - ref)) < 1.2e-7
+    # ... and relative error of a few ulp while t = -x*log2(e) is itself exact to ~1e-6 (|x| <= 16);
+    # for very negative x the rounding of t (|t| up to 125) bounds it at ~4e-6, and below
+    # x = -125 ln 2 the result saturates at ~2^-125 (fp32 denormal range of the true value).
+    mid = np.abs(x) <= 16
+    assert np.max(np.abs(s[mid] / ref[mid] - 1.0)) < 1.2e-6
+    far = (x > -86.0) & np.isfinite(x)
+    assert np.max(np.abs(s[far] / ref[far] - 1.0)) < 5e-6
+    assert np.all(s[x < -86.6] < 3e-38) and np.all(s >= 0) and np.all(s <= 1)
+    assert oracle.sig32(np.float32(0.0))[0] == np.float32(0.5)
+    xs = np.sort(x[np.isfinite(x)])
+    assert np.all(np.diff(oracle.sig32(xs)) >= -6e-8)     # monotone up to one ulp of 1.0
+
+
+def test_topk_matches_library_stable_sort():
+    rng = np.random.default_rng(3)
+    T, E, k = 500, 64, 6
+    x = np.round(rng.standard_normal((T, E)) * 4).astype(np.float32) / 4     # many exact ties
+    x[0, :] = -np.inf; x[1, 5] = np.nan; x[2, :3] = [0.0, -0.0, 0.0]
+    cfg = RouterCfg(L=1, H=1, E=E, k=k, S=1)
+    ids, w = oracle.gate(x, cfg, None, 1)
+    key = np.where(np.isnan(x), -np.inf, x).astype(np.float64)
+    ref = np.argsort(-key, axis=1, kind="stable")[:, :k]                     # library: (key desc, index asc)
+    np.testing.assert_array_equal(ids, ref)
+    # softmax weights vs scipy
+    fin = np.isfinite(x).all(1)
+    p = softmax(x[fin].astype(np.float64), axis=1)
+    np.testing.assert_allclose(w[fin], np.take_along_axis(p, ids[fin].astype(np.int64), 1), rtol=1e-12)
+
+
+def test_gating_invariants():
+    rng = np.random.default_rng(4)
+    T, E, k = 300, 32, 4
+    x = (rng.standard_normal((T, E)) * 2).astype(np.float32)
+    soft = RouterCfg(L=1, H=1, E=E, k=k, S=1)
+    sig = RouterCfg(L=1, H=1, E=E, k=k, S=1, score_fn=SIGMOID, renorm=1, routed_scale=2.5)
+    ids_s, _ = oracle.gate(x, soft, None, 1)
+    for tier in (0, 1):
+        ids_g, w_g = oracle.gate(x, sig, None, tier)
+        # sigmoid, zero bias, no groups selects the same SET as softmax mode (monotone score)
+        assert np.array_equal(np.sort(ids_s, 1), np.sort(ids_g, 1)) or tier == 1
+        np.testing.assert_allclose(w_g.sum(1), 2.5, rtol=1e-12)            # renormalised weights sum to routed_scale
+    ids0, _ = oracle.gate(x, sig, None, 0)
+    assert np.array_equal(np.sort(ids_s, 1), np.sort(ids0, 1))
+    # n_groups = 1 is the ungrouped rule; keeping all groups is too
+    grp_all = RouterCfg(L=1, H=1, E=E, k=k, S=1, n_groups=4, topk_groups=4, group_score_topn=2)
+    np.testing.assert_array_equal(oracle.gate(x, grp_all, None, 1)[0], ids_s)
+    # group-limited: every token's experts lie in <= topk_groups groups, and inside the kept set it is plain top-k
+    grp = RouterCfg(L=1, H=1, E=E, k=k, S=1, score_fn=SIGMOID, n_groups=8, topk_groups=2, group_score_topn=2)
+    sb = (0.05 * rng.standard_normal(E)).astype(np.float32)
+    ids, _ = oracle.gate(x, grp, sb, 1)
+    assert np.all([len(set((r // 4).tolist())) <= 2 for r in ids])
+    assert np.all([len(set(r.tolist())) == k for r in ids])
+
+
+def test_gating_tiers_differ_only_on_near_ties():
+    rng = np.random.default_rng(5)
+    T, E, k = 20000, 64, 6
+    x = (rng.standard_normal((T, E)) * 1.7).astype(np.float32)
+    sb = (0.05 * rng.standard_normal(E)).astype(np.float32)
+    cfg = RouterCfg(L=1, H=1, E=E, k=k, S=1, score_fn=SIGMOID, n_groups=8, topk_groups=4, group_score_topn=2)
+    i0, _ = oracle.gate(x, cfg, sb, 0)
+    i1, _ = oracle.gate(x, cfg, sb, 1)
+    bad = np.nonzero((i0 != i1).any(1))[0]
+    assert bad.size < 0.002 * T
+    for t in bad:                                        # every disagreement is a near-tie of the fp64 keys
+        key = expit(x[t].astype(np.float64)) + sb
+        d = set(i0[t]) ^ set(i1[t])
+        if d:
+            assert np.ptp(key[list(d)]) < 2e-6
+        else:                                            # same set, different order: adjacent near-tie
+            assert np.min(np.abs(np.diff(np.sort(key[i0[t]])))) < 2e-6
+
+
+# =========================================================================== a3 counts
+def test_counts_against_library_and_invariants():
+    rng = np.random.default_rng(6)
+    T, k, S, E = 1000, 4, 5, 32
+    ids = np.stack([rng.permutation(E)[:k] for _ in range(T)]).astype(np.int32)
+    off = np.array([0, 100, 100, 420, 999, 1000], np.int32)
+    Cm = oracle.counts(ids, off, S, E)
+    src = np.repeat(np.arange(S), np.diff(off))
+    ref = np.zeros((S, E), np.int64)
+    np.add.at(ref, (np.repeat(src, k), ids.ravel()), 1)                      # library scatter-add
+    np.testing.assert_array_equal(Cm, ref)
+    np.testing.assert_array_equal(Cm.sum(1), np.diff(off) * k)               # row sums = n_s * k
+    assert Cm.sum() == T * k and Cm.min() >= 0
+    # permuting tokens inside a source leaves C unchanged
+    perm = np.concatenate([lo + rng.permutation(hi - lo) for lo, hi in zip(off[:-1], off[1:])])
+    np.testing.assert_array_equal(oracle.counts(ids[perm], off, S, E), Cm)
+
+
+# =========================================================================== a4 update
+def test_update_closed_forms():
+    rng = np.random.default_rng(7)
+    n = 50
+    Cs = [rng.integers(0, 1000, n) for _ in range(12)]
+    A = np.zeros(n); [oracle.update_ema(A, c, 0.0) for c in Cs]
+    np.testing.assert_array_equal(A, Cs[-1])                                  # d=0 -> last step
+    A = np.zeros(n); [oracle.update_ema(A, c, 1.0) for c in Cs]
+    np.testing.assert_array_equal(A, np.sum(Cs, 0))                           # d=1 -> cumulative
+    A = np.zeros(n); d = 0.9
+    for _ in range(32):
+        oracle.update_ema(A, Cs[0], d)
+    np.testing.assert_allclose(A, Cs[0] * (1 - d ** 32) / (1 - d), rtol=1e-13)  # geometric closed form
+    # window: published exactly at multiples of window_len, equal to the window's sum, then reset
+    win = np.zeros(n, np.int64); pub = np.full(n, -1, np.int64)
+    for step, c in enumerate(Cs):
+        p = oracle.update_window(win, c, pub, step, 4)
+        assert p == ((step + 1) % 4 == 0)
+        if p:
+            np.testing.assert_array_equal(pub, np.sum(Cs[step - 3: step + 1], 0))
+            assert not win.any()
+    assert not win.any()
+
+
+# =========================================================================== a5 derived
+def test_derived_invariants_and_hand_example():
+    g = _gold("objective_worked_examples.json")["cases"][1]          # one replica
+    A = np.array(g["A"], np.float64)
+    d = oracle.derived(A, np.array(g["prev"], np.int16), np.array([0, 1], np.int32), g["G"], g["slots_per_rank"])
+    np.testing.assert_array_equal(d["B"], g["B"])
+    np.testing.assert_array_equal(d["Lrank"][0], g["candidates"][0]["L"])
+    np.testing.assert_array_equal(d["pressure_raw"], [10, 8])
+    np.testing.assert_allclose(d["pressure_rel"], [10 / 9, 8 / 9], rtol=1e-15)
+    rng = np.random.default_rng(8)
+    L, S, E, G, sp = 3, 4, 12, 4, 4                                  # 16 slots, 4 replicas
+    A = rng.integers(0, 500, (L, S, E)).astype(np.float64)
+    place = np.stack([np.array([0, 1, 2, 3, 4, 5, 6, 0, 7, 8, 9, 1, 10, 11, 2, 3], np.int16)] * L)
+    d = oracle.derived(A, place, np.array([0, 1, 2, 3], np.int32), G, sp)
+    assert d["ok"]
+    np.testing.assert_allclose(d["B"].sum(1), A.sum((1, 2)))
+    np.testing.assert_allclose(d["Lrank"].sum(1), d["B"].sum(1), rtol=1e-14)   # also with replicas
+    np.testing.assert_allclose(d["pressure_raw"].sum(), d["B"].sum(), rtol=1e-14)
+    assert abs(d["pressure_rel"].mean() - 1.0) < 1e-14
+    bad = place.copy(); bad[0, 1] = 0                                 # expert 0 twice on rank 0
+    assert not oracle.derived(A, bad, np.array([0, 1, 2, 3], np.int32), G, sp)["ok"]
+
+
+# =========================================================================== a6 objective
+def test_objective_worked_examples():
+    g = _gold("objective_worked_examples.json")
+    assert "PAPER.md:240" in g["citation"] and "PAPER.md:244" in g["citation"] and "PAPER.md:248" in g["citation"]
+    for case in g["cases"]:
+        A, B, D = np.array(case["A"], float), np.array(case["B"], float), np.array(case["D"], float)
+        prev = np.array(case["prev"], np.int16)
+        kw = dict(G=case["G"], sp=case["slots_per_rank"])
+        for c in case["candidates"]:
+            cand = np.array(c["slots"], np.int16)
+            o111 = oracle.objective(cand, prev, A, B, D, None, case["M_scalar"], weights=(1, 1, 1), **kw)
+            if c.get("invalid"):
+                assert np.isnan(o111).all()
+                continue
+            ocal, pl = oracle.objective(cand, prev, A, B, D, None, case["M_scalar"], per_layer=True, **kw)
+            np.testing.assert_allclose(o111, [c["J_111"], c["C_load"], c["C_comm"], c["C_mig"], c["maxload"]], rtol=1e-14)
+            np.testing.assert_allclose(ocal[0], c["J_cal"], rtol=1e-14)
+            np.testing.assert_allclose(pl[0], [c["C_load"], c["C_comm"], c["C_mig"], c["maxload"]], rtol=1e-14)
+        cands = np.array([c["slots"] for c in case["candidates"]], np.int16)
+        ob = oracle.objective_batch(cands, prev, A, B, D, None, case["M_scalar"], **kw)
+        for i, c in enumerate(case["candidates"]):
+            if c.get("invalid"):
+                assert np.isnan(ob[i]).all()
+            else:
+                np.testing.assert_allclose(ob[i, 0], c["J_cal"], rtol=1e-14)
+
+
+def _random_instance(rng, L=2, S=3, E=12, G=4, sp=4, replicas=True):
+    NS = G * sp
+    A = rng.integers(0, 400, (L, S, E)).astype(np.float64)
+    B = A.sum(1) * rng.integers(50, 150, (L, E))          # B and A live on different scales
+    D = 1.0 + rng.random((S, G)); D[np.arange(S), np.arange(S) % G] = 0.0
+    M = 1.0 + 0.5 * rng.random((L, E, G))
+
+    def rand_place():
+        while True:
+            rows = []
+            for _ in range(L):
+                extra = rng.permutation(E)[: NS - E] if replicas else np.array([], int)
+                rows.append(rng.permutation(np.concatenate([np.arange(E), extra])))
+            p = np.array(rows, np.int16)
+            x = p.reshape(L, G, sp)
+            if all(len(set(x[l, g])) == sp for l in range(L) for g in range(G)):
+                return p
+    return A, B, D, M, rand_place
+
+
+def test_objective_closed_forms_and_invariants():
+    rng = np.random.default_rng(9)
+    L, S, E, G, sp = 2, 3, 12, 4, 4
+    A, B, D, M, rand_place = _random_instance(rng, L, S, E, G, sp)
+    prev, cand = rand_place(), rand_place()
+    kw = dict(G=G, sp=sp)
+    w = (1.0, 0.0025, 1.0)
+    o = oracle.objective(cand, prev, A, B, D, M, **kw)
+    # C_mig(x0) = 0 (BASELINE.json invariant)
+    assert oracle.objective(prev, prev, A, B, D, M, **kw)[3] == 0.0
+    # D == 1 -> C_comm = sum A, whatever the placement (also with replicas)
+    o1 = oracle.objective(cand, prev, A, B, np.ones((S, G)), M, **kw)
+    np.testing.assert_allclose(o1[2], A.sum(), rtol=1e-13)
+    # D in {0,1}: remote + local = sum A
+    Dbin = (rng.random((S, G)) < 0.5).astype(float)
+    rem = oracle.objective(cand, prev, A, B, Dbin, M, **kw)[2]
+    loc = oracle.objective(cand, prev, A, B, 1.0 - Dbin, M, **kw)[2]
+    np.testing.assert_allclose(rem + loc, A.sum(), rtol=1e-13)
+    # uniform B, no replicas, equal slots -> C_load = 0 and maxload = L * sp * b
+    A2, B2, D2, M2, rp2 = _random_instance(rng, L, S, 16, 4, 4, replicas=False)
+    o2 = oracle.objective(rp2(), rp2(), A2, np.full((L, 16), 7.0), D2, M2, G=4, sp=4)
+    assert o2[1] == 0.0 and o2[4] == L * 4 * 7.0
+    # per-rank loads sum to the total routed tokens: maxload >= mean load, C_load >= 0
+    assert o[1] >= 0 and o[4] >= B.sum() / G - 1e-9
+    # scaling (alpha, beta, gamma) by c scales J by c; J is the weighted sum of the returned terms
+    np.testing.assert_allclose(oracle.objective(cand, prev, A, B, D, M, weights=(3.0, 0.0075, 3.0), **kw)[0], 3 * o[0], rtol=1e-13)
+    np.testing.assert_allclose(o[0], w[0] * o[2] + w[1] * o[1] + w[2] * o[3], rtol=1e-13)
+    # relabelling experts consistently leaves everything unchanged
+    perm = rng.permutation(E)                    # new label of expert e is perm[e]
+    inv = np.argsort(perm)
+    o3 = oracle.objective(perm[cand].astype(np.int16), perm[prev].astype(np.int16), A[:, :, inv], B[:, inv], D, M[:, inv, :], **kw)
+    np.testing.assert_allclose(o3, o, rtol=1e-12)
+    # relabelling ranks consistently (rank blocks of slots, D and M columns)
+    gp = rng.permutation(G)                      # new position of rank g is gp[g]
+    def mv(p):
+        q = np.empty_like(p).reshape(L, G, sp); q[:, gp, :] = p.reshape(L, G, sp); return q.reshape(L, G * sp)
+    D4 = np.empty_like(D); D4[:, gp] = D
+    M4 = np.empty_like(M); M4[:, :, gp] = M
+    np.testing.assert_allclose(oracle.objective(mv(cand), mv(prev), A, B, D4, M4, **kw), o, rtol=1e-12)
+    # scalar M: C_mig = M * (number of (expert,rank) cells that changed)
+    xs = lambda p: {(l, int(e), j // sp) for l in range(L) for j, e in enumerate(p[l])}
+    assert oracle.objective(cand, prev, A, B, D, None, 1.5, **kw)[3] == 1.5 * len(xs(cand) ^ xs(prev))
+
+
+# =========================================================================== a7 moves
+def test_move_deltas_closed_forms():
+    rng = np.random.default_rng(10)
+    L, S, E, G, sp = 2, 3, 16, 4, 4
+    A, B, D, M, rand_place = _random_instance(rng, L, S, E, G, sp, replicas=False)
+    cur, prev = rand_place(), rand_place()
+    kw = dict(G=G, sp=sp)
+    moves = oracle.all_pair_moves(L, G * sp)
+    assert moves.shape == (L * 120, 3) and moves[0].tolist() == [0, 0, 1] and moves[119].tolist() == [0, 14, 15]
+    d = oracle.move_deltas(cur, prev, moves, A, B, D, M, **kw)
+    Lr = oracle.derived(A, cur, np.arange(G, dtype=np.int32) % S, G, sp)
+    base = oracle.objective(cur, prev, A, B, D, M, **kw)
+    for i in rng.choice(len(moves), 60, replace=False):
+        l, a, b = moves[i]
+        g1, g2, e1, e2 = a // sp, b // sp, cur[l, a], cur[l, b]
+        if g1 == g2:
+            assert np.all(d[i] == 0.0)                               # same-rank swap -> 0
+            continue
+        # load: with delta = b2 - b1 moved onto g1, dC_load = 2 delta (L_g1 - L_g2) + 2 delta^2 (the mean cancels)
+        Lg = np.array([B[l, cur[l, g * sp:(g + 1) * sp]].sum() for g in range(G)])
+        dl = B[l, e2] - B[l, e1]
+        np.testing.assert_allclose(d[i, 1], 2 * dl * (Lg[g1] - Lg[g2]) + 2 * dl * dl, rtol=1e-9, atol=1e-6)
+        c = lambda e, g: (A[l, :, e] * D[:, g]).sum()
+        np.testing.assert_allclose(d[i, 2], c(e1, g2) + c(e2, g1) - c(e1, g1) - c(e2, g2), rtol=1e-9, atol=1e-9)
+        # delta equals the difference of two full evaluations of the WHOLE objective
+        nxt = cur.copy(); nxt[l, a], nxt[l, b] = cur[l, b], cur[l, a]
+        np.testing.assert_allclose(d[i], oracle.objective(nxt, prev, A, B, D, M, **kw) - base, rtol=1e-9, atol=1e-5)
+        # applying the swap twice returns to the start
+        back = oracle.move_deltas(nxt, prev, moves[i:i + 1], A, B, D, M, **kw)[0]
+        np.testing.assert_allclose(back + d[i], 0.0, atol=1e-6)
+    assert Lr["ok"]
+
+
+def test_move_worked_example_and_invalid_move():
+    case = _gold("objective_worked_examples.json")["cases"][0]
+    A, B, D = np.array(case["A"], float), np.array(case["B"], float), np.array(case["D"], float)
+    prev = np.array(case["prev"], np.int16)
+    sw = case["swap_example"]
+    d = oracle.move_deltas(prev, prev, np.array([sw["move"]], np.int32), A, B, D, None, 1.0, G=2, sp=2, weights=(1, 1, 1))[0]
+    np.testing.assert_allclose(d[1:], [sw["dC_load"], sw["dC_comm"], sw["dC_mig"], sw["dmaxload"]], rtol=1e-14)
+    # a move that would put a second copy of an expert on a rank is invalid -> NaN
+    rep = _gold("objective_worked_examples.json")["cases"][1]
+    A, B, D = np.array(rep["A"], float), np.array(rep["B"], float), np.array(rep["D"], float)
+    cur = np.array(rep["prev"], np.int16)                  # [0,1 | 0,2]: swapping slots 1 and 3 gives [0,2 | 0,1]: valid
+    ok = oracle.move_deltas(cur, cur, np.array([[0, 1, 3]], np.int32), A, B, D, G=2, sp=2)[0]
+    assert np.isfinite(ok).all()
+    bad = oracle.move_deltas(cur, cur, np.array([[0, 1, 2]], np.int32), A, B, D, G=2, sp=2)[0]   # -> [0,0 | 1,2]
+    assert np.isnan(bad).all()
+    same = oracle.move_deltas(cur, cur, np.array([[0, 0, 2]], np.int32), A, B, D, G=2, sp=2)[0]  # two replicas of expert 0
+    assert np.all(same == 0.0)
+
+
+# =========================================================================== brute force
+def test_bruteforce_worked_example_and_count():
+    case = _gold("objective_worked_examples.json")["cases"][0]
+    A, B, D = np.array(case["A"][0], float), np.array(case["B"][0], float), np.array(case["D"], float)
+    n, bj, bp = oracle.bruteforce(np.array(case["prev"][0], np.int16), A, B, D, None, 1.0, G=2, sp=2)
+    assert n == case["bruteforce"]["count"]
+    np.testing.assert_allclose(bj, case["bruteforce"]["best_J_cal"], rtol=1e-14)
+    assert bp.tolist() == case["bruteforce"]["best_slots"]
+
+
+def test_bruteforce_global_minimum_properties():
+    rng = np.random.default_rng(11)
+    S, E, G, sp = 2, 12, 3, 4
+    A, B, D, M, rand_place = _random_instance(rng, 1, S, E, G, sp, replicas=False)
+    prev = rand_place()
+    n, bj, bp = oracle.bruteforce(prev[0], A[0], B[0], D, M[0], G=G, sp=sp)
+    assert n == math.factorial(E) // math.factorial(sp) ** G == 34650          # closed form for the count
+    kw = dict(G=G, sp=sp)
+    np.testing.assert_allclose(oracle.objective(bp[None], prev, A, B, D, M, **kw)[0], bj, rtol=1e-14)
+    # no sampled placement beats it, and no single swap improves it
+    for _ in range(200):
+        assert oracle.objective(rand_place(), prev, A, B, D, M, **kw)[0] >= bj - 1e-9
+    d = oracle.move_deltas(bp[None], prev, oracle.all_pair_moves(1, E), A, B, D, M, **kw)
+    assert d[:, 0].min() >= -1e-7
+    # every non-optimal start has an improving chain: the optimum of a relabelled problem has the same J
+    perm = rng.permutation(E); inv = np.argsort(perm)
+    n2, bj2, _ = oracle.bruteforce(perm[prev[0]].astype(np.int16), A[0][:, inv], B[0][inv], D, M[0][inv], G=G, sp=sp)
+    np.testing.assert_allclose(bj2, bj, rtol=1e-12)
+
+
+@pytest.mark.slow
+def test_bruteforce_tiny_config_full_enumeration():
+    """tiny config: all 16!/(4!)^4 = 63,063,000 placements of 16 experts on 4 ranks x 4 slots."""
+    rng = np.random.default_rng(12)
+    S, E, G, sp = 2, 16, 4, 4
+    A, B, D, M, rand_place = _random_instance(rng, 1, S, E, G, sp, replicas=False)
+    prev = rand_place()
+    n, bj, bp = oracle.bruteforce(prev[0], A[0], B[0], D, None, 1.0, G=G, sp=sp)
+    assert n == 63063000
+    d = oracle.move_deltas(bp[None], prev, oracle.all_pair_moves(1, E), A, B, D, None, 1.0, G=G, sp=sp)
+    assert d[:, 0].min() >= -1e-7
