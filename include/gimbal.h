@@ -1,0 +1,248 @@
+/*
+ * gimbal.h -- C ABI of libgimbal: the data-parallel hot path behind Gimbal's coordinated
+ * MoE scheduling (arxiv/paper_2606_15177), hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * Citations are PAPER.md:<line> (+ section / equation) and DESIGN.md "R<n>" for the
+ * readings taken where the paper is silent.
+ *
+ * Conventions (all entry points):
+ *   - plain C, no C++ / torch types.  `gimbal_stream_t` is a cudaStream_t passed as void*.
+ *   - every array argument is a DEVICE pointer owned by the caller unless the name ends in
+ *     `_host` (the *_host entry points take HOST pointers, pinned for full speed, and do
+ *     their own host<->device copies on the stream).  The library never frees or keeps a
+ *     caller pointer past the call; scratch memory is a caller-owned device workspace whose
+ *     size comes from the matching gimbal_*_workspace_bytes().
+ *   - calls are asynchronous on `stream`, allocate nothing, never synchronise the host (the
+ *     *_host variants synchronise the stream once, before returning), and can be captured
+ *     in a CUDA graph.
+ *   - return value: GIMBAL_OK or a negative error.  Host-detectable problems (NULL, shape,
+ *     alignment, unsupported size) are reported here and nothing is launched.  Data errors
+ *     only visible on the device (expert id out of range, invalid candidate) never trap:
+ *     the affected outputs are NaN and bit 0 of the optional `status` word is set.
+ *   - there is no CPU fallback: without a CUDA device of compute capability 10.x every
+ *     compute entry point returns GIMBAL_ERR_UNSUPPORTED.
+ */
+#ifndef GIMBAL_H
+#define GIMBAL_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define GIMBAL_API __attribute__((visibility("default")))
+#else
+#define GIMBAL_API
+#endif
+
+#define GIMBAL_OK 0
+#define GIMBAL_ERR_INVALID_ARG (-1)
+#define GIMBAL_ERR_UNSUPPORTED (-2)
+#define GIMBAL_ERR_CUDA (-3)
+#define GIMBAL_ERR_WORKSPACE (-4)
+
+#define GIMBAL_SCORE_SOFTMAX 0
+#define GIMBAL_SCORE_SIGMOID 1
+
+#define GIMBAL_LOGITS_NONE 0 /* logits never leave the chip */
+#define GIMBAL_LOGITS_OUT 1  /* logits computed and written to `logits` */
+#define GIMBAL_LOGITS_IN 2   /* router GEMM skipped; gating reads `logits` */
+
+#define GIMBAL_MODE_WINDOW 0
+#define GIMBAL_MODE_EMA 1
+
+#define GIMBAL_COUNTS_I32 0
+#define GIMBAL_COUNTS_F32 1
+
+#define GIMBAL_MAX_TOPK 8
+#define GIMBAL_MAX_SOURCES 64
+
+typedef void *gimbal_stream_t; /* cudaStream_t */
+
+/* Router / gating shape.  The paper only says "lightweight router to select top-k experts
+ * for each token"; score function, group limit and tie-break are set by the
+ * model-shaped configs (R1, R3, R4).  Total order everywhere: (key descending,
+ * index ascending), -0 == +0, NaN logits count as -inf.
+ *   softmax : key_e = logit_e;  p = softmax over all E;  w_j = p_{id_j}
+ *   sigmoid : s_e = sig32(logit_e);  key_e = fl32(s_e + select_bias_e);  w_j = s_{id_j}
+ *   n_groups > 1 : E/n_groups contiguous experts per group; group score = fp32 sum (best
+ *             first) of its group_score_topn largest keys; only the topk_groups best
+ *             groups are eligible.
+ *   renorm  : w_j /= sum of the k selected scores.   All weights are then * routed_scale.
+ * Supported: E in {16,32,64,128,256}; 1 <= k <= 8; H % 64 == 0; S <= 64;
+ *            n_groups | E with E/n_groups == 32 when n_groups > 1.                        */
+typedef struct gimbal_router_cfg {
+    int32_t L, H, E, k, S;
+    int32_t score_fn, renorm, n_groups, topk_groups, group_score_topn;
+    float routed_scale;
+} gimbal_router_cfg;
+
+/* Online routing profile (section 5.1).  All pointers are device memory.
+ *   A_step [L,S,E] i32  out   this step's counts C (a3): tokens from DP source s routed to
+ *                             expert e in layer l
+ *   WINDOW mode: A_win += C; when (step+1) % window_len == 0 the window
+ *     is published (A_pub = A_win, B_pub = B) and A_win is zeroed.
+ *   A_win  [L,S,E] i32  inout   A_pub [L,S,E] i32 out   B_pub [L,E] i32 out
+ *   EMA mode (BASELINE.json; R2): A_ema = fl32(ema_decay * A_ema + C), un-normalised.
+ *   A_ema  [L,S,E] f32  inout
+ *   B      [L,E]  i32 (WINDOW) / f32 (EMA)  out   B[l,e] = sum_s A[l,s,e] of the live profile
+ *                             (A_win after this step's accumulation and before any reset,
+ *                             or A_ema)
+ *   pressure_raw [S] f32 out  MoE pressure of DP engine s: tokens processed by experts on its
+ *                             EP ranks, sum_l sum_{g: dp_of_rank[g]=s} L[l,g]
+ *   pressure_rel [S] f32 out  the same normalised to mean 1 (R14)
+ *   step_counter [1] i64 inout  device-side step index; incremented by every call
+ *   status [1] i32 inout|NULL  bit 0 set on device-side data errors                        */
+typedef struct gimbal_stats_state {
+    int32_t mode, window_len;
+    float ema_decay;
+    int32_t reserved;
+    int32_t *A_step;
+    int32_t *A_win;
+    int32_t *A_pub;
+    int32_t *B_pub;
+    float *A_ema;
+    void *B;
+    float *pressure_raw;
+    float *pressure_rel;
+    int64_t *step_counter;
+    int32_t *status;
+} gimbal_stats_state;
+
+/* Placement problem (section 5.2).  A placement is stored slot -> expert:
+ * int16 [L,NS], NS = G*slots_per_rank, slot j of a layer lives on rank j / slots_per_rank.
+ * x[l,e,g] in {0,1} = rank g hosts expert e.  With redundant slots (NS > E,
+ * DESIGN.md R12) an expert may be hosted by r >= 1 ranks and its tokens split evenly over
+ * them.  A valid placement hosts every expert at least once and never twice on one rank.
+ * counts_dtype says whether A and B hold int32 or float.                                  */
+typedef struct gimbal_placement_cfg {
+    int32_t L, E, G, slots_per_rank, S;
+    float alpha, beta, gamma; /* J = alpha*C_comm + beta*C_load + gamma*C_mig; paper's
+                                 calibrated (1.0, 0.0025, 1.0); R6 */
+    int32_t counts_dtype;
+} gimbal_placement_cfg;
+
+/* Library / device probe.  gimbal_version() never touches CUDA. */
+GIMBAL_API int gimbal_version(void);
+/* Writes the last CUDA / validation error string (NUL-terminated, truncated to n). */
+GIMBAL_API void gimbal_last_error(char *buf, size_t n);
+
+/* ---------------------------------------------------------------------------------------
+ * gimbal_route_stats -- steps a1..a5 for layers [layer0, layer0+n_layers) of one step:
+ *   a1 logits[i,t,e] = sum_h hidden[i,t,h] * w_router[layer0+i,e,h]   (bf16 in, fp32 accumulate)
+ *                      + src_logit_bias[layer0+i, src(t), e]           (optional; workload skew)
+ *   a2 top-k gating (see gimbal_router_cfg)  ->  topk_ids, topk_w (both optional outputs)
+ *   a3 A_step[l,s,e] = #{(t,j): src(t)=s, ids[l,t,j]=e}
+ *   a4 window / EMA update, a5 B and MoE pressure (see gimbal_stats_state); a4-a5 cover all
+ *      L layers of the state and run only when layer0 + n_layers == L (last slice of a step).
+ * Arguments
+ *   hidden        [n_layers,T,H] bf16, row-major, 16-byte aligned         (NULL if LOGITS_IN)
+ *   w_router      [L,E,H] bf16 (row e = expert e's weights, K-major)      (NULL if LOGITS_IN)
+ *   select_bias   [L,E] f32 | NULL     added to the sigmoid score for selection only
+ *   src_logit_bias[L,S,E] f32 | NULL
+ *   src_offsets   [S+1] i32            tokens are concatenated by source DP engine
+ *                                      (PAPER.md:31); src_offsets[S] == T; empty sources ok
+ *   logits        [n_layers,T,E] f32   written (OUT), read (IN) or ignored (NONE); holds the
+ *                                      post-bias values fl32(acc + src_logit_bias)
+ *   topk_ids      [n_layers,T,k] i32 | NULL   best first
+ *   topk_w        [n_layers,T,k] f32 | NULL
+ *   cur_placement [L,NS] i16 | NULL,  dp_of_rank [G] i32 | NULL : needed for the pressure
+ *                                      outputs only (both NULL: pressure is left untouched)
+ *   G, slots_per_rank                  shape of cur_placement
+ * Errors: INVALID_ARG (NULL / shape / alignment), UNSUPPORTED (shape outside the compiled
+ * range, no sm_100 device), WORKSPACE (workspace_bytes too small), CUDA.                  */
+GIMBAL_API size_t gimbal_route_stats_workspace_bytes(const gimbal_router_cfg *cfg, int n_layers, int T);
+
+GIMBAL_API int gimbal_route_stats(const gimbal_router_cfg *cfg, int layer0, int n_layers, int T,
+                       const void *hidden, const void *w_router,
+                       const float *select_bias, const float *src_logit_bias,
+                       const int32_t *src_offsets, int logits_mode, float *logits,
+                       int32_t *topk_ids, float *topk_w,
+                       const int16_t *cur_placement, const int32_t *dp_of_rank, int G, int slots_per_rank,
+                       gimbal_stats_state *state, void *workspace, size_t workspace_bytes,
+                       gimbal_stream_t stream);
+
+/* Same step with the per-step inputs in HOST memory: hidden_host [n_layers,T,H] bf16 and
+ * src_offsets_host [S+1] are copied to the device staging buffers the caller provides
+ * (hidden_stage: at least 2 layers of [T,H] bf16; copies overlap the kernels layer by layer),
+ * and after the step A_step, B and both pressure vectors are copied back to
+ * result_host (layout: A_step i32 [L,S,E] | B [L,E] | pressure_raw [S] | pressure_rel [S]),
+ * gimbal_route_stats_result_bytes() bytes.  logits_mode is NONE.  Weights, biases, the
+ * placement and the state stay device-resident (they persist across steps).  Synchronises
+ * `stream` before returning.                                                              */
+GIMBAL_API size_t gimbal_route_stats_result_bytes(const gimbal_router_cfg *cfg);
+GIMBAL_API int gimbal_route_stats_host(const gimbal_router_cfg *cfg, int T,
+                            const void *hidden_host, const int32_t *src_offsets_host,
+                            void *hidden_stage, size_t hidden_stage_bytes, int32_t *src_offsets_stage,
+                            const void *w_router, const float *select_bias, const float *src_logit_bias,
+                            const int16_t *cur_placement, const int32_t *dp_of_rank, int G, int slots_per_rank,
+                            gimbal_stats_state *state, void *result_host,
+                            void *workspace, size_t workspace_bytes, gimbal_stream_t stream);
+
+/* ---------------------------------------------------------------------------------------
+ * gimbal_eval_placements -- step a6: score P candidate placements against the profile.
+ *   L[p,l,g] = sum_e B[l,e] x[l,e,g] / r[l,e]
+ *   C_load   = sum_l sum_g (L[l,g] - mean_g L[l,g])^2
+ *   C_comm   = sum_l sum_s sum_e sum_g A[l,s,e] D[s,g] x[l,e,g] / r[l,e]
+ *   C_mig    = sum_l sum_e sum_g M[l,e,g] |x[l,e,g] - x0[l,e,g]|
+ *   J        = alpha*C_comm + beta*C_load + gamma*C_mig
+ *   maxload  = sum_l max_g L[l,g]                                           (R7)
+ * Arguments
+ *   candidates [P,L,NS] i16   slot -> expert
+ *   A [L,S,E], B [L,E]        i32 or f32 (cfg->counts_dtype); B is an input of its own
+ *                             because the paper collects it on another window (R9)
+ *   D [S,G] f32 (>= 0)        source -> rank communication cost
+ *   M [L,E,G] f32 | NULL      migration cost; NULL: M_scalar everywhere
+ *   prev [L,NS] i16           x0, the placement before rebalancing (must be valid)
+ *   out [P,5] f32             {J, C_load, C_comm, C_mig, maxload}; an invalid candidate
+ *                             (id out of range, expert missing, expert twice on a rank)
+ *                             gets five NaNs
+ *   argmin [1] i32 | NULL     lowest index among the candidates of minimal J (NaNs skipped;
+ *                             -1 if none is valid)
+ * Supported: E <= 256, G <= 64, slots_per_rank <= 16, S <= 64.                            */
+GIMBAL_API size_t gimbal_eval_placements_workspace_bytes(const gimbal_placement_cfg *cfg, int P);
+
+GIMBAL_API int gimbal_eval_placements(const gimbal_placement_cfg *cfg, int P, const int16_t *candidates,
+                           const void *A, const void *B, const float *D, const float *M, float M_scalar,
+                           const int16_t *prev, float *out, int32_t *argmin,
+                           void *workspace, size_t workspace_bytes, gimbal_stream_t stream);
+
+/* Candidates and results in HOST memory (cand_stage: device buffer of P*L*NS int16;
+ * out_stage: device [P,5] f32).  Synchronises `stream` before returning.                  */
+GIMBAL_API int gimbal_eval_placements_host(const gimbal_placement_cfg *cfg, int P, const int16_t *candidates_host,
+                                int16_t *cand_stage, float *out_stage,
+                                const void *A, const void *B, const float *D, const float *M, float M_scalar,
+                                const int16_t *prev, float *out_host, int32_t *argmin_host,
+                                void *workspace, size_t workspace_bytes, gimbal_stream_t stream);
+
+/* ---------------------------------------------------------------------------------------
+ * gimbal_eval_moves -- step a7: objective deltas of single moves from placement `cur`.
+ * A move (l, slot_a, slot_b) exchanges the contents of two slots of layer l (a move into a
+ * redundant slot is a swap with that slot).  delta equals J(moved) - J(cur) term by term:
+ *   delta [n,5] f32 = {dJ, dC_load, dC_comm, dC_mig, dmaxload}
+ * Same-rank moves and exchanges of two replicas of one expert give zeros; a move that would
+ * put a second copy of an expert on a rank gives NaNs.
+ *   moves [n,3] i32 | NULL   NULL = the whole neighbourhood in canonical order: for l in
+ *                            [0,L), for a < b (a outer, b inner); then n_moves must equal
+ *                            L*NS*(NS-1)/2
+ *   best_per_layer [L] i32 | NULL  index (into the n moves) of the lowest dJ of each layer,
+ *                            lowest index on ties, -1 if the layer has no valid move
+ * Other arguments as in gimbal_eval_placements; `cur` and `prev` must be valid.            */
+GIMBAL_API size_t gimbal_eval_moves_workspace_bytes(const gimbal_placement_cfg *cfg);
+
+GIMBAL_API int gimbal_eval_moves(const gimbal_placement_cfg *cfg, const int16_t *cur, const int16_t *prev,
+                      int64_t n_moves, const int32_t *moves,
+                      const void *A, const void *B, const float *D, const float *M, float M_scalar,
+                      float *delta, int32_t *best_per_layer,
+                      void *workspace, size_t workspace_bytes, gimbal_stream_t stream);
+
+/* Counters for bench.py: kernels launched by this library since load. */
+GIMBAL_API int64_t gimbal_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GIMBAL_H */

@@ -1,0 +1,263 @@
+"""ctypes binding of include/gimbal.h -- argument marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+LOGITS_NONE, LOGITS_OUT, LOGITS_IN = 0, 1, 2
+MODE_WINDOW, MODE_EMA = 0, 1
+SCORE_SOFTMAX, SCORE_SIGMOID = 0, 1
+COUNTS_I32, COUNTS_F32 = 0, 1
+
+EXPORTED_SYMBOLS = [
+    "gimbal_version", "gimbal_last_error", "gimbal_launch_count",
+    "gimbal_route_stats_workspace_bytes", "gimbal_route_stats", "gimbal_route_stats_result_bytes",
+    "gimbal_route_stats_host",
+    "gimbal_eval_placements_workspace_bytes", "gimbal_eval_placements", "gimbal_eval_placements_host",
+    "gimbal_eval_moves_workspace_bytes", "gimbal_eval_moves",
+]
+
+
+class GimbalError(RuntimeError):
+    pass
+
+
+class _RouterCfg(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("L", "H", "E", "k", "S", "score_fn", "renorm", "n_groups", "topk_groups",
+                                          "group_score_topn")] + [("routed_scale", C.c_float)]
+
+
+class _StatsState(C.Structure):
+    _fields_ = [("mode", C.c_int32), ("window_len", C.c_int32), ("ema_decay", C.c_float), ("reserved", C.c_int32),
+                ("A_step", C.c_void_p), ("A_win", C.c_void_p), ("A_pub", C.c_void_p), ("B_pub", C.c_void_p),
+                ("A_ema", C.c_void_p), ("B", C.c_void_p), ("pressure_raw", C.c_void_p), ("pressure_rel", C.c_void_p),
+                ("step_counter", C.c_void_p), ("status", C.c_void_p)]
+
+
+class _PlacementCfg(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("L", "E", "G", "slots_per_rank", "S")] + \
+               [(n, C.c_float) for n in ("alpha", "beta", "gamma")] + [("counts_dtype", C.c_int32)]
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libgimbal.so")
+
+
+_lib = None
+
+
+def lib():
+    """Load libgimbal.so (built in-tree by build.py / __graft_entry__.build()).  No fallback."""
+    global _lib
+    if _lib is None:
+        path = lib_path()
+        if not os.path.exists(path):
+            raise GimbalError(f"{path} is missing: run `python -m paper_2606_15177_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(path)
+        L.gimbal_version.restype = C.c_int
+        L.gimbal_launch_count.restype = C.c_int64
+        for n in ("gimbal_route_stats_workspace_bytes", "gimbal_route_stats_result_bytes",
+                  "gimbal_eval_placements_workspace_bytes", "gimbal_eval_moves_workspace_bytes"):
+            getattr(L, n).restype = C.c_size_t
+        for n in ("gimbal_route_stats", "gimbal_route_stats_host", "gimbal_eval_placements",
+                  "gimbal_eval_placements_host", "gimbal_eval_moves"):
+            getattr(L, n).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def last_error() -> str:
+    buf = C.create_string_buffer(512)
+    lib().gimbal_last_error(buf, C.c_size_t(512))
+    return buf.value.decode()
+
+
+def launch_count() -> int:
+    return int(lib().gimbal_launch_count())
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise GimbalError(f"{what} failed ({rc}): {last_error()}")
+
+
+def _ptr(t):
+    if t is None:
+        return C.c_void_p(None)
+    if isinstance(t, torch.Tensor):
+        assert t.is_contiguous(), "tensors passed to libgimbal must be contiguous"
+        return C.c_void_p(t.data_ptr())
+    return C.c_void_p(int(t))
+
+
+def _stream(stream=None):
+    if stream is None:
+        if not torch.cuda.is_available():      # the library itself reports "no CUDA device"
+            return C.c_void_p(None)
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+@dataclass
+class RouterCfg:
+    L: int
+    H: int
+    E: int
+    k: int
+    S: int
+    score_fn: int = SCORE_SOFTMAX
+    renorm: int = 0
+    n_groups: int = 1
+    topk_groups: int = 1
+    group_score_topn: int = 1
+    routed_scale: float = 1.0
+
+    @classmethod
+    def from_workload(cls, r):
+        return cls(r.L, r.H, r.E, r.k, r.S, r.score_fn, r.renorm, r.n_groups, r.topk_groups, r.group_score_topn,
+                   r.routed_scale)
+
+    def c(self):
+        return _RouterCfg(self.L, self.H, self.E, self.k, self.S, self.score_fn, self.renorm, self.n_groups,
+                          self.topk_groups, self.group_score_topn, self.routed_scale)
+
+
+@dataclass
+class PlacementCfg:
+    L: int
+    E: int
+    G: int
+    slots_per_rank: int
+    S: int
+    alpha: float = 1.0
+    beta: float = 0.0025
+    gamma: float = 1.0
+    counts_dtype: int = COUNTS_I32
+
+    @property
+    def NS(self):
+        return self.G * self.slots_per_rank
+
+    def c(self):
+        return _PlacementCfg(self.L, self.E, self.G, self.slots_per_rank, self.S, self.alpha, self.beta, self.gamma,
+                             self.counts_dtype)
+
+
+class StatsState:
+    """Device-resident routing profile (gimbal_stats_state).  Allocation only."""
+
+    def __init__(self, cfg: RouterCfg, mode: int, window_len: int = 1, ema_decay: float = 0.0, device="cuda"):
+        L, S, E = cfg.L, cfg.S, cfg.E
+        self.cfg, self.mode, self.window_len, self.ema_decay = cfg, mode, window_len, ema_decay
+        i32 = dict(dtype=torch.int32, device=device)
+        f32 = dict(dtype=torch.float32, device=device)
+        self.A_step = torch.zeros(L, S, E, **i32)
+        self.A_win = torch.zeros(L, S, E, **i32)
+        self.A_pub = torch.zeros(L, S, E, **i32)
+        self.B_pub = torch.zeros(L, E, **i32)
+        self.A_ema = torch.zeros(L, S, E, **f32)
+        self.B = torch.zeros(L, E, **(i32 if mode == MODE_WINDOW else f32))
+        self.pressure_raw = torch.zeros(S, **f32)
+        self.pressure_rel = torch.zeros(S, **f32)
+        self.step_counter = torch.zeros(1, dtype=torch.int64, device=device)
+        self.status = torch.zeros(1, **i32)
+
+    @property
+    def A_live(self):
+        return self.A_win if self.mode == MODE_WINDOW else self.A_ema
+
+    def c(self):
+        return _StatsState(self.mode, self.window_len, self.ema_decay, 0, self.A_step.data_ptr(), self.A_win.data_ptr(),
+                           self.A_pub.data_ptr(), self.B_pub.data_ptr(), self.A_ema.data_ptr(), self.B.data_ptr(),
+                           self.pressure_raw.data_ptr(), self.pressure_rel.data_ptr(), self.step_counter.data_ptr(),
+                           self.status.data_ptr())
+
+
+def route_stats_workspace_bytes(cfg: RouterCfg, n_layers: int, T: int) -> int:
+    c = cfg.c()
+    return int(lib().gimbal_route_stats_workspace_bytes(C.byref(c), C.c_int(n_layers), C.c_int(T)))
+
+
+def route_stats(cfg: RouterCfg, state: StatsState, *, T: int, hidden=None, w_router=None, select_bias=None,
+                src_logit_bias=None, src_offsets=None, layer0: int = 0, n_layers: int | None = None,
+                logits_mode: int = LOGITS_NONE, logits=None, topk_ids=None, topk_w=None, cur_placement=None,
+                dp_of_rank=None, G: int = 0, slots_per_rank: int = 0, workspace=None, stream=None):
+    """gimbal_route_stats (a1..a5).  All tensors are CUDA tensors owned by the caller."""
+    n_layers = cfg.L - layer0 if n_layers is None else n_layers
+    c, s = cfg.c(), state.c()
+    rc = lib().gimbal_route_stats(C.byref(c), C.c_int(layer0), C.c_int(n_layers), C.c_int(T), _ptr(hidden), _ptr(w_router),
+                                  _ptr(select_bias), _ptr(src_logit_bias), _ptr(src_offsets), C.c_int(logits_mode),
+                                  _ptr(logits), _ptr(topk_ids), _ptr(topk_w), _ptr(cur_placement), _ptr(dp_of_rank),
+                                  C.c_int(G), C.c_int(slots_per_rank), C.byref(s), _ptr(workspace),
+                                  C.c_size_t(0 if workspace is None else workspace.numel() * workspace.element_size()),
+                                  _stream(stream))
+    _check(rc, "gimbal_route_stats")
+
+
+def route_stats_host(cfg: RouterCfg, state: StatsState, *, T: int, hidden_host, src_offsets_host, hidden_stage,
+                     src_offsets_stage, w_router, select_bias=None, src_logit_bias=None, cur_placement=None,
+                     dp_of_rank=None, G: int = 0, slots_per_rank: int = 0, result_host=None, workspace=None, stream=None):
+    """gimbal_route_stats_host: hidden / src_offsets in (pinned) host memory, results back to host."""
+    c, s = cfg.c(), state.c()
+    rc = lib().gimbal_route_stats_host(C.byref(c), C.c_int(T), _ptr(hidden_host), _ptr(src_offsets_host), _ptr(hidden_stage),
+                                       C.c_size_t(hidden_stage.numel() * hidden_stage.element_size()), _ptr(src_offsets_stage),
+                                       _ptr(w_router), _ptr(select_bias), _ptr(src_logit_bias), _ptr(cur_placement),
+                                       _ptr(dp_of_rank), C.c_int(G), C.c_int(slots_per_rank), C.byref(s), _ptr(result_host),
+                                       _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()),
+                                       _stream(stream))
+    _check(rc, "gimbal_route_stats_host")
+
+
+def route_stats_result_bytes(cfg: RouterCfg) -> int:
+    c = cfg.c()
+    return int(lib().gimbal_route_stats_result_bytes(C.byref(c)))
+
+
+def eval_placements_workspace_bytes(cfg: PlacementCfg, P: int) -> int:
+    c = cfg.c()
+    return int(lib().gimbal_eval_placements_workspace_bytes(C.byref(c), C.c_int(P)))
+
+
+def eval_moves_workspace_bytes(cfg: PlacementCfg) -> int:
+    c = cfg.c()
+    return int(lib().gimbal_eval_moves_workspace_bytes(C.byref(c)))
+
+
+def eval_placements(cfg: PlacementCfg, candidates, A, B, D, prev, out, *, M=None, M_scalar: float = 1.0, argmin=None,
+                    workspace=None, stream=None):
+    """gimbal_eval_placements (a6): out [P,5] = {J, C_load, C_comm, C_mig, maxload}."""
+    c = cfg.c()
+    P = candidates.shape[0]
+    rc = lib().gimbal_eval_placements(C.byref(c), C.c_int(P), _ptr(candidates), _ptr(A), _ptr(B), _ptr(D), _ptr(M),
+                                      C.c_float(M_scalar), _ptr(prev), _ptr(out), _ptr(argmin), _ptr(workspace),
+                                      C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream))
+    _check(rc, "gimbal_eval_placements")
+
+
+def eval_placements_host(cfg: PlacementCfg, candidates_host, cand_stage, out_stage, A, B, D, prev, out_host, *, M=None,
+                         M_scalar: float = 1.0, argmin_host=None, workspace=None, stream=None):
+    c = cfg.c()
+    P = candidates_host.shape[0]
+    rc = lib().gimbal_eval_placements_host(C.byref(c), C.c_int(P), _ptr(candidates_host), _ptr(cand_stage), _ptr(out_stage),
+                                           _ptr(A), _ptr(B), _ptr(D), _ptr(M), C.c_float(M_scalar), _ptr(prev),
+                                           _ptr(out_host), _ptr(argmin_host), _ptr(workspace),
+                                           C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream))
+    _check(rc, "gimbal_eval_placements_host")
+
+
+def eval_moves(cfg: PlacementCfg, cur, prev, A, B, D, delta, *, moves=None, n_moves: int | None = None, M=None,
+               M_scalar: float = 1.0, best_per_layer=None, workspace=None, stream=None):
+    """gimbal_eval_moves (a7): delta [n,5] = {dJ, dC_load, dC_comm, dC_mig, dmaxload}."""
+    c = cfg.c()
+    if n_moves is None:
+        n_moves = moves.shape[0] if moves is not None else cfg.L * cfg.NS * (cfg.NS - 1) // 2
+    rc = lib().gimbal_eval_moves(C.byref(c), _ptr(cur), _ptr(prev), C.c_int64(n_moves), _ptr(moves), _ptr(A), _ptr(B),
+                                 _ptr(D), _ptr(M), C.c_float(M_scalar), _ptr(delta), _ptr(best_per_layer), _ptr(workspace),
+                                 C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream))
+    _check(rc, "gimbal_eval_moves")

@@ -1,0 +1,471 @@
+// C-ABI entry points of libgimbal (include/gimbal.h): argument validation, workspace
+// carving, TMA descriptor encoding and kernel launches.  Every step of the hot path runs in
+// the kernels of this directory; there is no CPU fallback.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+
+#include "host_common.h"
+#include "placement.cuh"
+#include "stats_update.cuh"
+
+using namespace gimbal;
+
+namespace gimbal {
+int64_t launches();
+void copy_last_error(char* buf, size_t n);
+}
+
+namespace {
+
+// ---- workspace carving ---------------------------------------------------------------------
+struct Carver {
+    unsigned char* base;
+    size_t off = 0;
+    explicit Carver(void* p) : base(static_cast<unsigned char*>(p)) {}
+    template <class T>
+    T* take(size_t n) {
+        off = (off + 255) & ~size_t(255);
+        T* r = base ? reinterpret_cast<T*>(base + off) : nullptr;
+        off += n * sizeof(T);
+        return r;
+    }
+};
+
+int launch_gemm(const RouteArgs& a) {
+    switch (a.cfg->E) {
+        case 16: return launch_gemm_e16(a);
+        case 32: return launch_gemm_e32(a);
+        case 64: return launch_gemm_e64(a);
+        case 128: return launch_gemm_e128(a);
+        case 256: return launch_gemm_e256(a);
+    }
+    return fail(GIMBAL_ERR_UNSUPPORTED, "E=%d not in {16,32,64,128,256}", a.cfg->E);
+}
+
+int launch_gate(const RouteArgs& a) {
+    switch (a.cfg->E) {
+        case 16: return launch_gate_e16(a);
+        case 32: return launch_gate_e32(a);
+        case 64: return launch_gate_e64(a);
+        case 128: return launch_gate_e128(a);
+        case 256: return launch_gate_e256(a);
+    }
+    return fail(GIMBAL_ERR_UNSUPPORTED, "E=%d not in {16,32,64,128,256}", a.cfg->E);
+}
+
+int validate_router_cfg(const gimbal_router_cfg* c) {
+    if (!c) return fail(GIMBAL_ERR_INVALID_ARG, "cfg is NULL");
+    if (c->L < 1 || c->H < 1 || c->S < 1 || c->k < 1) return fail(GIMBAL_ERR_INVALID_ARG, "L, H, S, k must be >= 1");
+    if (c->E != 16 && c->E != 32 && c->E != 64 && c->E != 128 && c->E != 256)
+        return fail(GIMBAL_ERR_UNSUPPORTED, "E=%d not in {16,32,64,128,256}", c->E);
+    if (c->k > GIMBAL_MAX_TOPK || c->k > c->E) return fail(GIMBAL_ERR_UNSUPPORTED, "k=%d (max %d, <= E)", c->k, GIMBAL_MAX_TOPK);
+    if (c->S > GIMBAL_MAX_SOURCES) return fail(GIMBAL_ERR_UNSUPPORTED, "S=%d (max %d)", c->S, GIMBAL_MAX_SOURCES);
+    if (c->H % 64 != 0) return fail(GIMBAL_ERR_UNSUPPORTED, "H=%d must be a multiple of 64", c->H);
+    if (c->score_fn != GIMBAL_SCORE_SOFTMAX && c->score_fn != GIMBAL_SCORE_SIGMOID)
+        return fail(GIMBAL_ERR_INVALID_ARG, "score_fn=%d", c->score_fn);
+    if (c->n_groups < 1) return fail(GIMBAL_ERR_INVALID_ARG, "n_groups=%d", c->n_groups);
+    if (c->n_groups > 1) {
+        if (c->E % c->n_groups != 0 || c->E / c->n_groups != 32)
+            return fail(GIMBAL_ERR_UNSUPPORTED, "group-limited routing needs E/n_groups == 32 (E=%d, n_groups=%d)", c->E, c->n_groups);
+        if (c->topk_groups < 1 || c->topk_groups > c->n_groups) return fail(GIMBAL_ERR_INVALID_ARG, "topk_groups=%d", c->topk_groups);
+        if (c->group_score_topn != 1 && c->group_score_topn != 2)
+            return fail(GIMBAL_ERR_UNSUPPORTED, "group_score_topn=%d not in {1,2}", c->group_score_topn);
+        if (c->topk_groups * 32 < c->k) return fail(GIMBAL_ERR_INVALID_ARG, "topk_groups*32 < k");
+    }
+    return GIMBAL_OK;
+}
+
+struct RouteWs {
+    double* partial;           // [L,S]
+    unsigned int* done;        // [1] (+pad)
+};
+
+size_t route_ws_carve(const gimbal_router_cfg* c, void* ws, RouteWs* out) {
+    Carver cv(ws);
+    RouteWs w;
+    w.partial = cv.take<double>((size_t)c->L * c->S);
+    w.done = cv.take<unsigned int>(64);
+    if (out) *out = w;
+    return cv.off + 256;
+}
+
+// force 1-CTA or 2-CTA pairs from the environment (debug / A-B measurement); default 2
+int pick_cta_group(int T) {
+    const char* e = getenv("GIMBAL_CTA_GROUP");     // read per call: tests flip it
+    const int forced = e ? atoi(e) : 0;
+    if (forced == 1 || forced == 2) return forced;
+    return T > 128 ? 2 : 1;
+}
+
+int pick_fuse() {
+    const char* e = getenv("GIMBAL_FUSE_GATE");
+    return e ? atoi(e) : 1;
+}
+
+// ------------------------------------------------------------------------------------------
+static int validate_place_cfg(const gimbal_placement_cfg* c) {
+    if (!c) return fail(GIMBAL_ERR_INVALID_ARG, "cfg is NULL");
+    if (c->L < 1 || c->E < 1 || c->G < 1 || c->slots_per_rank < 1 || c->S < 1) return fail(GIMBAL_ERR_INVALID_ARG, "L, E, G, slots_per_rank, S must be >= 1");
+    if (c->E > kMaxE) return fail(GIMBAL_ERR_UNSUPPORTED, "E=%d (max %d)", c->E, kMaxE);
+    if (c->G > kMaxG || (c->G & (c->G - 1))) return fail(GIMBAL_ERR_UNSUPPORTED, "G=%d must be a power of two <= %d", c->G, kMaxG);
+    if (c->slots_per_rank > 16) return fail(GIMBAL_ERR_UNSUPPORTED, "slots_per_rank=%d (max 16)", c->slots_per_rank);
+    if (c->S > GIMBAL_MAX_SOURCES) return fail(GIMBAL_ERR_UNSUPPORTED, "S=%d (max %d)", c->S, GIMBAL_MAX_SOURCES);
+    if ((long)c->G * c->slots_per_rank < c->E) return fail(GIMBAL_ERR_INVALID_ARG, "G*slots_per_rank < E");
+    if (c->counts_dtype != GIMBAL_COUNTS_I32 && c->counts_dtype != GIMBAL_COUNTS_F32) return fail(GIMBAL_ERR_INVALID_ARG, "counts_dtype=%d", c->counts_dtype);
+    if (c->E % 2 != 0) return fail(GIMBAL_ERR_UNSUPPORTED, "E must be even");
+    return GIMBAL_OK;
+}
+
+struct PlaceWs {
+    PlaceTables t;
+    float4* partial;                // [P,L]
+    unsigned long long* best;       // [max(L,1)]
+    MovePrep mp;
+};
+
+static size_t place_ws_carve(const gimbal_placement_cfg* c, int P, void* ws, PlaceWs* out) {
+    Carver cv(ws);
+    PlaceWs w{};
+    const int GP = place_gp(c->G);
+    const size_t LE = (size_t)c->L * c->E;
+    w.t.wc = cv.take<float2>(LE * GP);
+    w.t.m = cv.take<float>(LE * GP);
+    w.t.w_e = cv.take<float>(LE);
+    w.t.hsum = cv.take<uint32_t>(c->L);
+    w.t.base_mig = cv.take<float>(c->L);
+    w.t.sumB = cv.take<double>(c->L);
+    w.t.r = cv.take<int32_t>(LE);
+    w.t.pmask = cv.take<uint64_t>(LE);
+    w.t.bad = cv.take<int32_t>(64);
+    w.partial = cv.take<float4>((size_t)P * c->L);
+    w.best = cv.take<unsigned long long>(c->L + 1);
+    w.mp.Lg = cv.take<float>((size_t)c->L * c->G);
+    w.mp.top = cv.take<float>((size_t)c->L * 4);
+    w.mp.top_g = cv.take<int32_t>((size_t)c->L * 4);
+    w.mp.cmask = cv.take<uint64_t>(LE);
+    w.mp.bad = cv.take<int32_t>(64);
+    if (out) *out = w;
+    return cv.off + 256;
+}
+
+static int launch_tables(const gimbal_placement_cfg* c, const void* A, const void* B, const float* D, const float* M, float M_scalar,
+                         const int16_t* prev, const PlaceWs& w, cudaStream_t stream) {
+    CUDA_TRY(cudaMemsetAsync(w.t.bad, 0, sizeof(int32_t), stream));
+    TableParams tp{};
+    tp.L = c->L; tp.E = c->E; tp.G = c->G; tp.sp = c->slots_per_rank; tp.S = c->S; tp.counts_f32 = c->counts_dtype == GIMBAL_COUNTS_F32;
+    tp.A = A; tp.B = B; tp.D = D; tp.M = M; tp.M_scalar = M_scalar; tp.prev = prev; tp.t = w.t;
+    place_tables_kernel<<<c->L, 256, 0, stream>>>(tp);
+    LAUNCH_CHECK("place_tables_kernel");
+    return GIMBAL_OK;
+}
+
+template <int SP>
+static int launch_score(const ScoreParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
+    auto kern = place_score_kernel<SP>;
+    CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<grid, kScoreThreads, smem, stream>>>(sp);
+    LAUNCH_CHECK("place_score_kernel");
+    return GIMBAL_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gimbal_version(void) { return 100; }
+
+void gimbal_last_error(char* buf, size_t n) {
+    if (!buf || n == 0) return;
+    gimbal::copy_last_error(buf, n);
+}
+
+int64_t gimbal_launch_count(void) { return gimbal::launches(); }
+
+size_t gimbal_route_stats_workspace_bytes(const gimbal_router_cfg* cfg, int n_layers, int T) {
+    (void)n_layers; (void)T;
+    if (!cfg) return 0;
+    return route_ws_carve(cfg, nullptr, nullptr);
+}
+
+size_t gimbal_route_stats_result_bytes(const gimbal_router_cfg* cfg) {
+    if (!cfg) return 0;
+    return sizeof(int32_t) * (size_t)cfg->L * cfg->S * cfg->E + 4 * (size_t)cfg->L * cfg->E + 2 * sizeof(float) * (size_t)cfg->S;
+}
+
+int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, int T, const void* hidden, const void* w_router,
+                       const float* select_bias, const float* src_logit_bias, const int32_t* src_offsets, int logits_mode,
+                       float* logits, int32_t* topk_ids, float* topk_w, const int16_t* cur_placement, const int32_t* dp_of_rank,
+                       int G, int slots_per_rank, gimbal_stats_state* st, void* workspace, size_t workspace_bytes,
+                       gimbal_stream_t stream_) {
+    int rc = validate_router_cfg(cfg);
+    if (rc) return rc;
+    if (layer0 < 0 || n_layers < 1 || layer0 + n_layers > cfg->L) return fail(GIMBAL_ERR_INVALID_ARG, "layer range [%d,%d) outside [0,%d)", layer0, layer0 + n_layers, cfg->L);
+    if (T < 0) return fail(GIMBAL_ERR_INVALID_ARG, "T=%d", T);
+    if (!src_offsets) return fail(GIMBAL_ERR_INVALID_ARG, "src_offsets is NULL");
+    if (!st || !st->A_step || !st->step_counter || !st->B) return fail(GIMBAL_ERR_INVALID_ARG, "state / A_step / B / step_counter is NULL");
+    if (st->mode == GIMBAL_MODE_WINDOW) {
+        if (!st->A_win || !st->A_pub || !st->B_pub || st->window_len < 1) return fail(GIMBAL_ERR_INVALID_ARG, "WINDOW mode needs A_win, A_pub, B_pub, window_len >= 1");
+    } else if (st->mode == GIMBAL_MODE_EMA) {
+        if (!st->A_ema) return fail(GIMBAL_ERR_INVALID_ARG, "EMA mode needs A_ema");
+    } else return fail(GIMBAL_ERR_INVALID_ARG, "state mode=%d", st->mode);
+    if (logits_mode != GIMBAL_LOGITS_NONE && logits_mode != GIMBAL_LOGITS_OUT && logits_mode != GIMBAL_LOGITS_IN)
+        return fail(GIMBAL_ERR_INVALID_ARG, "logits_mode=%d", logits_mode);
+    if (logits_mode != GIMBAL_LOGITS_NONE && !logits) return fail(GIMBAL_ERR_INVALID_ARG, "logits is NULL");
+    if (logits_mode != GIMBAL_LOGITS_IN) {
+        if (!hidden || !w_router) return fail(GIMBAL_ERR_INVALID_ARG, "hidden / w_router is NULL");
+        if ((reinterpret_cast<uintptr_t>(hidden) & 15) || (reinterpret_cast<uintptr_t>(w_router) & 15))
+            return fail(GIMBAL_ERR_INVALID_ARG, "hidden / w_router must be 16-byte aligned");
+    }
+    if ((cur_placement != nullptr) != (dp_of_rank != nullptr)) return fail(GIMBAL_ERR_INVALID_ARG, "cur_placement and dp_of_rank go together");
+    if (cur_placement) {
+        if (G < 1 || G > kMaxG || slots_per_rank < 1 || (long)G * slots_per_rank < cfg->E || !st->pressure_raw || !st->pressure_rel)
+            return fail(GIMBAL_ERR_INVALID_ARG, "pressure needs 1 <= G <= 64, G*slots >= E, pressure_raw/rel");
+    }
+    RouteWs ws;
+    const size_t need = route_ws_carve(cfg, workspace, &ws);
+    if (!workspace || workspace_bytes < need) return fail(GIMBAL_ERR_WORKSPACE, "workspace %zu < %zu bytes", workspace_bytes, need);
+    rc = require_device();
+    if (rc) return rc;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+
+    // a3 accumulates into A_step: zero the slice of this call
+    CUDA_TRY(cudaMemsetAsync(st->A_step + (size_t)layer0 * cfg->S * cfg->E, 0, sizeof(int32_t) * (size_t)n_layers * cfg->S * cfg->E, stream));
+    if (layer0 == 0) CUDA_TRY(cudaMemsetAsync(ws.done, 0, sizeof(unsigned int), stream));
+
+    if (T > 0) {
+        RouteArgs a{};
+        a.cfg = cfg; a.layer0 = layer0; a.n_layers = n_layers; a.T = T; a.hidden = hidden; a.w_router = w_router;
+        a.select_bias = select_bias; a.src_logit_bias = src_logit_bias; a.src_offsets = src_offsets;
+        a.topk_ids = topk_ids; a.topk_w = topk_w; a.A_step = st->A_step; a.stream = stream;
+        a.cta_group = pick_cta_group(T);
+        if (logits_mode == GIMBAL_LOGITS_IN) {
+            a.logits = logits;
+            rc = launch_gate(a);
+            if (rc) return rc;
+        } else {
+            // fused epilogue needs the block histogram next to the ring; fall back to two kernels otherwise
+            const bool can_fuse = pick_fuse() && (size_t)cfg->S * cfg->E * 4 <= 32 * 1024;
+            if (can_fuse) {
+                a.logits = logits_mode == GIMBAL_LOGITS_OUT ? logits : nullptr;
+                a.fuse_gate = 1;
+                rc = launch_gemm(a);
+                if (rc) return rc;
+            } else {
+                if (logits_mode != GIMBAL_LOGITS_OUT) return fail(GIMBAL_ERR_UNSUPPORTED, "unfused path needs logits_mode OUT (a logits buffer)");
+                a.logits = logits; a.fuse_gate = 0;
+                rc = launch_gemm(a);
+                if (rc) return rc;
+                rc = launch_gate(a);
+                if (rc) return rc;
+            }
+        }
+    }
+
+    if (layer0 + n_layers == cfg->L) {
+        UpdateParams u{};
+        u.L = cfg->L; u.S = cfg->S; u.E = cfg->E; u.G = G; u.sp = slots_per_rank;
+        u.mode = st->mode; u.window_len = st->window_len; u.ema_decay = st->ema_decay;
+        u.A_step = st->A_step; u.A_win = st->A_win; u.A_pub = st->A_pub; u.B_pub = st->B_pub; u.A_ema = st->A_ema; u.B = st->B;
+        u.pressure_raw = st->pressure_raw; u.pressure_rel = st->pressure_rel; u.step_counter = st->step_counter; u.status = st->status;
+        u.cur_placement = cur_placement; u.dp_of_rank = dp_of_rank; u.partial = ws.partial; u.done_counter = ws.done;
+        stats_update_kernel<<<cfg->L, kUpdateThreads, 0, stream>>>(u);
+        LAUNCH_CHECK("stats_update_kernel");
+    }
+    return GIMBAL_OK;
+}
+
+int gimbal_route_stats_host(const gimbal_router_cfg* cfg, int T, const void* hidden_host, const int32_t* src_offsets_host,
+                            void* hidden_stage, size_t hidden_stage_bytes, int32_t* src_offsets_stage, const void* w_router,
+                            const float* select_bias, const float* src_logit_bias, const int16_t* cur_placement,
+                            const int32_t* dp_of_rank, int G, int slots_per_rank, gimbal_stats_state* st, void* result_host,
+                            void* workspace, size_t workspace_bytes, gimbal_stream_t stream_) {
+    int rc = validate_router_cfg(cfg);
+    if (rc) return rc;
+    if (!hidden_host || !src_offsets_host || !hidden_stage || !src_offsets_stage || !result_host || !st)
+        return fail(GIMBAL_ERR_INVALID_ARG, "NULL host / staging pointer");
+    const size_t layer_bytes = (size_t)T * cfg->H * 2;
+    if (T < 1) return fail(GIMBAL_ERR_INVALID_ARG, "T=%d", T);
+    const size_t slots = hidden_stage_bytes / layer_bytes;
+    if (slots < 2) return fail(GIMBAL_ERR_WORKSPACE, "hidden_stage must hold at least 2 layers (%zu bytes)", 2 * layer_bytes);
+    rc = require_device();
+    if (rc) return rc;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    // a second stream carries the copies so that layer i+1 streams in while layer i computes
+    static cudaStream_t copy_stream = nullptr;
+    static cudaEvent_t ev_copied[64], ev_done[64];
+    if (!copy_stream) {
+        CUDA_TRY(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 64; ++i) {
+            CUDA_TRY(cudaEventCreateWithFlags(&ev_copied[i], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&ev_done[i], cudaEventDisableTiming));
+        }
+    }
+    const size_t nslot = slots > 64 ? 64 : slots;
+    CUDA_TRY(cudaMemcpyAsync(src_offsets_stage, src_offsets_host, sizeof(int32_t) * (cfg->S + 1), cudaMemcpyHostToDevice, stream));
+    cudaEvent_t ev_start = ev_done[0];
+    CUDA_TRY(cudaEventRecord(ev_start, stream));
+    CUDA_TRY(cudaStreamWaitEvent(copy_stream, ev_start, 0));
+    for (int l = 0; l < cfg->L; ++l) {
+        const size_t slot = (size_t)l % nslot;
+        unsigned char* dst = static_cast<unsigned char*>(hidden_stage) + slot * layer_bytes;
+        if ((size_t)l >= nslot) CUDA_TRY(cudaStreamWaitEvent(copy_stream, ev_done[slot], 0));   // slot's previous layer consumed
+        CUDA_TRY(cudaMemcpyAsync(dst, static_cast<const unsigned char*>(hidden_host) + (size_t)l * layer_bytes, layer_bytes,
+                                 cudaMemcpyHostToDevice, copy_stream));
+        CUDA_TRY(cudaEventRecord(ev_copied[slot], copy_stream));
+        CUDA_TRY(cudaStreamWaitEvent(stream, ev_copied[slot], 0));
+        rc = gimbal_route_stats(cfg, l, 1, T, dst, w_router, select_bias, src_logit_bias, src_offsets_stage, GIMBAL_LOGITS_NONE,
+                                nullptr, nullptr, nullptr, cur_placement, dp_of_rank, G, slots_per_rank, st, workspace,
+                                workspace_bytes, stream_);
+        if (rc) return rc;
+        CUDA_TRY(cudaEventRecord(ev_done[slot], stream));
+    }
+    unsigned char* out = static_cast<unsigned char*>(result_host);
+    const size_t nA = sizeof(int32_t) * (size_t)cfg->L * cfg->S * cfg->E, nB = 4 * (size_t)cfg->L * cfg->E, nP = sizeof(float) * cfg->S;
+    CUDA_TRY(cudaMemcpyAsync(out, st->A_step, nA, cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaMemcpyAsync(out + nA, st->B, nB, cudaMemcpyDeviceToHost, stream));
+    if (st->pressure_raw && st->pressure_rel) {
+        CUDA_TRY(cudaMemcpyAsync(out + nA + nB, st->pressure_raw, nP, cudaMemcpyDeviceToHost, stream));
+        CUDA_TRY(cudaMemcpyAsync(out + nA + nB + nP, st->pressure_rel, nP, cudaMemcpyDeviceToHost, stream));
+    }
+    CUDA_TRY(cudaStreamSynchronize(stream));
+    return GIMBAL_OK;
+}
+
+size_t gimbal_eval_placements_workspace_bytes(const gimbal_placement_cfg* cfg, int P) {
+    if (!cfg || P < 0) return 0;
+    return place_ws_carve(cfg, P, nullptr, nullptr);
+}
+
+size_t gimbal_eval_moves_workspace_bytes(const gimbal_placement_cfg* cfg) {
+    if (!cfg) return 0;
+    return place_ws_carve(cfg, 0, nullptr, nullptr);
+}
+
+int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const int16_t* candidates, const void* A, const void* B,
+                           const float* D, const float* M, float M_scalar, const int16_t* prev, float* out, int32_t* argmin,
+                           void* workspace, size_t workspace_bytes, gimbal_stream_t stream_) {
+    int rc = validate_place_cfg(cfg);
+    if (rc) return rc;
+    if (P < 0) return fail(GIMBAL_ERR_INVALID_ARG, "P=%d", P);
+    if (!A || !B || !D || !prev || (P > 0 && (!candidates || !out))) return fail(GIMBAL_ERR_INVALID_ARG, "NULL argument");
+    if (reinterpret_cast<uintptr_t>(candidates) & 15) return fail(GIMBAL_ERR_INVALID_ARG, "candidates must be 16-byte aligned");
+    PlaceWs w;
+    const size_t need = place_ws_carve(cfg, P, workspace, &w);
+    if (!workspace || workspace_bytes < need) return fail(GIMBAL_ERR_WORKSPACE, "workspace %zu < %zu bytes", workspace_bytes, need);
+    const int GP = place_gp(cfg->G);
+    const size_t smem = (size_t)cfg->E * GP * (M ? 12 : 8);
+    if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "E=%d G=%d with an M table needs %zu B of shared memory", cfg->E, cfg->G, smem);
+    rc = require_device();
+    if (rc) return rc;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    if (argmin) {
+        fill_u64_kernel<<<1, 32, 0, stream>>>(w.best, ~0ull, 1);
+        LAUNCH_CHECK("fill_u64_kernel");
+    }
+    if (P > 0) {
+        rc = launch_tables(cfg, A, B, D, M, M_scalar, prev, w, stream);
+        if (rc) return rc;
+        ScoreParams sp{};
+        sp.P = P; sp.L = cfg->L; sp.E = cfg->E; sp.G = cfg->G; sp.sp = cfg->slots_per_rank; sp.M_scalar = M_scalar; sp.has_M = M != nullptr;
+        sp.cand = candidates; sp.t = w.t; sp.partial = w.partial;
+        const int sms = device_info().sms;
+        int nchunk = (2 * sms + cfg->L - 1) / cfg->L;
+        const int units_per_pass = (kScoreThreads / 32) * (cfg->G < 32 ? 32 / cfg->G : 1);
+        int max_chunks = (P + units_per_pass - 1) / units_per_pass;
+        if (nchunk > max_chunks) nchunk = max_chunks;
+        if (nchunk < 1) nchunk = 1;
+        sp.chunk = (P + nchunk - 1) / nchunk;
+        dim3 grid((P + sp.chunk - 1) / sp.chunk, cfg->L);
+        switch (cfg->slots_per_rank) {
+            case 4: rc = launch_score<4>(sp, grid, smem, stream); break;
+            case 8: rc = launch_score<8>(sp, grid, smem, stream); break;
+            case 9: rc = launch_score<9>(sp, grid, smem, stream); break;
+            default: rc = launch_score<0>(sp, grid, smem, stream); break;
+        }
+        if (rc) return rc;
+        FinalizeParams fp{};
+        fp.P = P; fp.L = cfg->L; fp.G = cfg->G; fp.alpha = cfg->alpha; fp.beta = cfg->beta; fp.gamma = cfg->gamma;
+        fp.partial = w.partial; fp.bad_prev = w.t.bad; fp.out = out; fp.best = argmin ? w.best : nullptr;
+        place_finalize_kernel<<<(P + 255) / 256, 256, 0, stream>>>(fp);
+        LAUNCH_CHECK("place_finalize_kernel");
+    }
+    if (argmin) {
+        best_to_index_kernel<<<1, 32, 0, stream>>>(w.best, argmin, 1);
+        LAUNCH_CHECK("best_to_index_kernel");
+    }
+    return GIMBAL_OK;
+}
+
+int gimbal_eval_placements_host(const gimbal_placement_cfg* cfg, int P, const int16_t* candidates_host, int16_t* cand_stage,
+                                float* out_stage, const void* A, const void* B, const float* D, const float* M, float M_scalar,
+                                const int16_t* prev, float* out_host, int32_t* argmin_host, void* workspace, size_t workspace_bytes,
+                                gimbal_stream_t stream_) {
+    int rc = validate_place_cfg(cfg);
+    if (rc) return rc;
+    if (!candidates_host || !cand_stage || !out_stage || !out_host) return fail(GIMBAL_ERR_INVALID_ARG, "NULL host / staging pointer");
+    rc = require_device();
+    if (rc) return rc;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const size_t nb = sizeof(int16_t) * (size_t)P * cfg->L * cfg->G * cfg->slots_per_rank;
+    CUDA_TRY(cudaMemcpyAsync(cand_stage, candidates_host, nb, cudaMemcpyHostToDevice, stream));
+    PlaceWs w;
+    place_ws_carve(cfg, P, workspace, &w);
+    int32_t* argmin_dev = argmin_host ? reinterpret_cast<int32_t*>(w.mp.bad + 32) : nullptr;
+    rc = gimbal_eval_placements(cfg, P, cand_stage, A, B, D, M, M_scalar, prev, out_stage, argmin_dev, workspace, workspace_bytes, stream_);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(out_host, out_stage, sizeof(float) * 5 * (size_t)P, cudaMemcpyDeviceToHost, stream));
+    if (argmin_host) CUDA_TRY(cudaMemcpyAsync(argmin_host, argmin_dev, sizeof(int32_t), cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaStreamSynchronize(stream));
+    return GIMBAL_OK;
+}
+
+int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const int16_t* prev, int64_t n_moves, const int32_t* moves,
+                      const void* A, const void* B, const float* D, const float* M, float M_scalar, float* delta,
+                      int32_t* best_per_layer, void* workspace, size_t workspace_bytes, gimbal_stream_t stream_) {
+    int rc = validate_place_cfg(cfg);
+    if (rc) return rc;
+    if (n_moves < 0) return fail(GIMBAL_ERR_INVALID_ARG, "n_moves < 0");
+    if (!cur || !prev || !A || !B || !D || (n_moves > 0 && !delta)) return fail(GIMBAL_ERR_INVALID_ARG, "NULL argument");
+    const long long NS = (long long)cfg->G * cfg->slots_per_rank;
+    if (!moves && n_moves != (long long)cfg->L * NS * (NS - 1) / 2)
+        return fail(GIMBAL_ERR_INVALID_ARG, "implicit neighbourhood has %lld moves, got %lld", (long long)cfg->L * NS * (NS - 1) / 2, (long long)n_moves);
+    if (n_moves > 0xffffffffll) return fail(GIMBAL_ERR_UNSUPPORTED, "n_moves > 2^32-1");
+    PlaceWs w;
+    const size_t need = place_ws_carve(cfg, 0, workspace, &w);
+    if (!workspace || workspace_bytes < need) return fail(GIMBAL_ERR_WORKSPACE, "workspace %zu < %zu bytes", workspace_bytes, need);
+    rc = require_device();
+    if (rc) return rc;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    rc = launch_tables(cfg, A, B, D, M, M_scalar, prev, w, stream);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemsetAsync(w.mp.bad, 0, sizeof(int32_t), stream));
+    MovePrepParams pp{};
+    pp.L = cfg->L; pp.E = cfg->E; pp.G = cfg->G; pp.sp = cfg->slots_per_rank; pp.cur = cur; pp.t = w.t; pp.mp = w.mp;
+    move_prep_kernel<<<cfg->L, 256, 0, stream>>>(pp);
+    LAUNCH_CHECK("move_prep_kernel");
+    if (best_per_layer) {
+        fill_u64_kernel<<<(cfg->L + 255) / 256, 256, 0, stream>>>(w.best, ~0ull, cfg->L);
+        LAUNCH_CHECK("fill_u64_kernel");
+    }
+    if (n_moves > 0) {
+        MoveParams mp{};
+        mp.L = cfg->L; mp.E = cfg->E; mp.G = cfg->G; mp.sp = cfg->slots_per_rank; mp.n_moves = n_moves; mp.moves = moves; mp.cur = cur;
+        mp.alpha = cfg->alpha; mp.beta = cfg->beta; mp.gamma = cfg->gamma; mp.M_scalar = M_scalar; mp.has_M = M != nullptr;
+        mp.t = w.t; mp.mp = w.mp; mp.delta = delta; mp.best = best_per_layer ? w.best : nullptr;
+        const long long blocks = (n_moves + 255) / 256;
+        move_delta_kernel<<<(unsigned)blocks, 256, 0, stream>>>(mp);
+        LAUNCH_CHECK("move_delta_kernel");
+    }
+    if (best_per_layer) {
+        best_to_index_kernel<<<(cfg->L + 255) / 256, 256, 0, stream>>>(w.best, best_per_layer, cfg->L);
+        LAUNCH_CHECK("best_to_index_kernel");
+    }
+    return GIMBAL_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,97 @@
+// Definitions of host_common.h.
+#include "host_common.h"
+
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <mutex>
+
+namespace gimbal {
+
+static std::mutex g_err_mu;
+static char g_err[512] = "";
+static std::atomic<int64_t> g_launches{0};
+
+int fail(int code, const char* fmt, ...) {
+    std::lock_guard<std::mutex> lk(g_err_mu);
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+int64_t launches() { return g_launches.load(); }
+void copy_last_error(char* buf, size_t n) {
+    std::lock_guard<std::mutex> lk(g_err_mu);
+    snprintf(buf, n, "%s", g_err);
+}
+
+const DeviceInfo& device_info() {
+    static DeviceInfo info = [] {
+        DeviceInfo d;
+        int n = 0;
+        if (cudaGetDeviceCount(&n) != cudaSuccess || n == 0) {
+            snprintf(d.why, sizeof d.why, "no CUDA device");
+            cudaGetLastError();
+            return d;
+        }
+        int dev = 0, major = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+        cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev);
+        if (major != 10) {
+            snprintf(d.why, sizeof d.why, "device compute capability %d.x, need 10.x (sm_100a)", major);
+            return d;
+        }
+        d.ok = true;
+        return d;
+    }();
+    return info;
+}
+
+int require_device() {
+    const DeviceInfo& d = device_info();
+    if (!d.ok) return fail(GIMBAL_ERR_UNSUPPORTED, "%s", d.why);
+    return GIMBAL_OK;
+}
+
+// ---- TMA descriptors -----------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess) f = nullptr;
+        return reinterpret_cast<EncodeTiledFn>(f);
+    }();
+    return fn;
+}
+
+// bf16 tensor [d2][d1][d0] (d0 contiguous), box [1][box1][64], 128-byte swizzle
+int make_tmap_bf16_3d(CUtensorMap* m, const void* ptr, uint64_t d0, uint64_t d1, uint64_t d2, uint32_t box1) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return fail(GIMBAL_ERR_CUDA, "cuTensorMapEncodeTiled not available");
+    cuuint64_t dims[3] = {d0, d1, d2};
+    cuuint64_t strides[2] = {d0 * 2, d0 * d1 * 2};
+    cuuint32_t box[3] = {64, box1, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(ptr), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(GIMBAL_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+    return GIMBAL_OK;
+}
+
+GateParams gate_params(const gimbal_router_cfg* c) {
+    GateParams g;
+    g.k = c->k; g.score_fn = c->score_fn; g.renorm = c->renorm; g.n_groups = c->n_groups;
+    g.topk_groups = c->topk_groups; g.topn = c->group_score_topn; g.routed_scale = c->routed_scale;
+    return g;
+}
+
+
+}  // namespace gimbal

@@ -1,0 +1,4 @@
+#include "route_launch.cuh"
+namespace gimbal {
+GIMBAL_DEFINE_E(64)
+}

@@ -1,0 +1,82 @@
+// Launchers of the router GEMM and the standalone gating kernel, instantiated once per
+// expert count in route_e*.cu so that the translation units compile in parallel.
+#pragma once
+#include "host_common.h"
+#include "router_gemm.cuh"
+
+namespace gimbal {
+
+template <int N, int kCG>
+int launch_gemm_t(const RouteArgs& a) {
+    const gimbal_router_cfg* c = a.cfg;
+    CUtensorMap ta, tb;
+    int rc = make_tmap_bf16_3d(&ta, a.hidden, (uint64_t)c->H, (uint64_t)a.T, (uint64_t)a.n_layers, kBlockM);
+    if (rc) return rc;
+    rc = make_tmap_bf16_3d(&tb, a.w_router, (uint64_t)c->H, (uint64_t)c->E, (uint64_t)c->L, N / kCG);
+    if (rc) return rc;
+    GemmParams p{};
+    p.n_layers = a.n_layers; p.layer0 = a.layer0; p.T = a.T; p.H = c->H; p.S = c->S;
+    p.m_tiles = (a.T + kBlockM * kCG - 1) / (kBlockM * kCG);
+    p.stages = gemm_pick_stages<N, kCG>(c->S);
+    if (p.stages < 2) return fail(GIMBAL_ERR_UNSUPPORTED, "router GEMM: not enough shared memory for E=%d S=%d", N, c->S);
+    p.src_logit_bias = a.src_logit_bias; p.src_offsets = a.src_offsets; p.logits = a.logits;
+    p.do_gate = a.fuse_gate; p.select_bias = a.select_bias; p.topk_ids = a.topk_ids; p.topk_w = a.topk_w;
+    p.A_step = a.A_step; p.gp = gate_params(c);
+    const size_t smem = gemm_smem_bytes<N, kCG>(c->S, p.stages);
+    auto kern = router_gemm_kernel<N, kCG, GIMBAL_MAX_TOPK>;
+    CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int sms = device_info().sms;
+    const int n_tiles = p.n_layers * p.m_tiles;
+    int pairs = sms / kCG;
+    if (pairs > n_tiles) pairs = n_tiles;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(pairs * kCG);
+    cfg.blockDim = dim3(kGemmThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = a.stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = kCG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, ta, tb, p));
+    LAUNCH_CHECK("router_gemm_kernel");
+    return GIMBAL_OK;
+}
+
+template <int N>
+int launch_gemm_n(const RouteArgs& a) {
+    return a.cta_group == 2 ? launch_gemm_t<N, 2>(a) : launch_gemm_t<N, 1>(a);
+}
+
+
+// ---- standalone gating ---------------------------------------------------------------------
+template <int E>
+int launch_gate_t(const RouteArgs& a) {
+    constexpr int kWarps = 4;
+    GateKernelParams p{};
+    p.logits = a.logits; p.select_bias = a.select_bias; p.src_offsets = a.src_offsets;
+    p.topk_ids = a.topk_ids; p.topk_w = a.topk_w; p.A_step = a.A_step;
+    p.layer0 = a.layer0; p.T = a.T; p.S = a.cfg->S; p.gp = gate_params(a.cfg);
+    const size_t smem = gate_smem_bytes<E, GIMBAL_MAX_TOPK, kWarps>(a.cfg->S);
+    if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "gating: E=%d S=%d needs %zu B of shared memory", E, a.cfg->S, smem);
+    dim3 grid((a.T + kWarps * 32 - 1) / (kWarps * 32), a.n_layers);
+    if (a.topk_w) {
+        auto kern = gate_hist_kernel<E, GIMBAL_MAX_TOPK, kWarps, true>;
+        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<grid, kWarps * 32, smem, a.stream>>>(p);
+    } else {
+        auto kern = gate_hist_kernel<E, GIMBAL_MAX_TOPK, kWarps, false>;
+        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<grid, kWarps * 32, smem, a.stream>>>(p);
+    }
+    LAUNCH_CHECK("gate_hist_kernel");
+    return GIMBAL_OK;
+}
+
+
+
+#define GIMBAL_DEFINE_E(E)                                                     \
+    int launch_gemm_e##E(const RouteArgs& a) { return launch_gemm_n<E>(a); }   \
+    int launch_gate_e##E(const RouteArgs& a) { return launch_gate_t<E>(a); }
+
+}  // namespace gimbal

@@ -1,0 +1,308 @@
+// a1: router GEMM  logits[i,t,e] = sum_h hidden[i,t,h] * W[layer0+i,e,h]  (+ src_logit_bias),
+// bf16 operands, fp32 accumulation in TMEM (BASELINE.json north_star (2)).
+//
+// Persistent, warp-specialised tcgen05 kernel over all (layer, 128-token tile) pairs of a step:
+//   warp 0      TMA producer: hidden tile [128 x 64] + W tile [N/kCG x 64] per k-block into a
+//               kStages-deep shared-memory ring (128-byte swizzle), mbarrier full/empty
+//   warp 1      MMA issuer (pair leader only): one elected lane issues tcgen05.mma
+//               (M = 128*kCG, N = E, K = 16) x 4 per k-block, commits to the ring's empty
+//               barriers and, per tile, to the TMEM-full barrier
+//   warp 2      TMEM allocator (2 accumulator stages of N fp32 columns)
+//   warps 4..7  epilogue: tcgen05.ld 32 lanes x 32 columns -> registers (thread = token row)
+//               -> + bias -> logits to HBM and/or fused gating + histogram (a2, a3), then
+//               release the accumulator stage
+// kCG == 2 pairs two SMs (cta_group::2): each CTA loads its own 128 hidden rows and HALF of
+// the W tile, so W traffic out of L2 halves; the leader issues one M=256 MMA for both.
+#pragma once
+#include "gating.cuh"
+#include "ptx.cuh"
+
+namespace gimbal { constexpr size_t kGemmSmemLimit = 227 * 1024; }
+
+namespace gimbal {
+
+struct GemmParams {
+    int n_layers, layer0, T, H, S;
+    int m_tiles;                    // ceil(T / (128*kCG))
+    int stages;                     // depth of the shared-memory ring (host: gemm_pick_stages)
+    const float* src_logit_bias;    // [L,S,E] | nullptr
+    const int32_t* src_offsets;     // [S+1]
+    float* logits;                  // [n_layers,T,E] | nullptr
+    // fused gating (do_gate != 0)
+    int do_gate;
+    const float* select_bias;       // [L,E] | nullptr
+    int32_t* topk_ids;
+    float* topk_w;
+    int32_t* A_step;                // [L,S,E]
+    GateParams gp;
+};
+
+constexpr int kGemmThreads = 256;
+constexpr int kBlockM = 128;
+constexpr int kBlockK = 64;         // 64 bf16 = 128 B = one swizzle row
+
+template <int N, int kCG>
+constexpr int gemm_stage_bytes() { return kBlockM * kBlockK * 2 + (N / kCG) * kBlockK * 2; }
+
+constexpr int kGemmAuxBytes = 1024;  // barriers + tmem pointer (<= 12 stages)
+constexpr int kGemmMaxStages = 12;
+
+// bytes after the ring: [aux][select_bias N f32][src_offsets S+1 (padded)][hist S*N i32]
+template <int N>
+constexpr size_t gemm_tail_bytes(int S) {
+    return kGemmAuxBytes + sizeof(float) * N + sizeof(int32_t) * (size_t)((S + 1 + 3) & ~3) + sizeof(int32_t) * (size_t)S * N;
+}
+template <int N, int kCG>
+inline int gemm_pick_stages(int S) {
+    const long avail = (long)kGemmSmemLimit - 1024 - (long)gemm_tail_bytes<N>(S);
+    long s = avail / gemm_stage_bytes<N, kCG>();
+    if (s > kGemmMaxStages) s = kGemmMaxStages;
+    return (int)s;
+}
+template <int N, int kCG>
+inline size_t gemm_smem_bytes(int S, int stages) {
+    return 1024 + (size_t)stages * gemm_stage_bytes<N, kCG>() + gemm_tail_bytes<N>(S);
+}
+
+template <int N>
+struct TmemRowSrc {
+    uint32_t taddr;                 // lane base | column base of this accumulator stage
+    const float* bias;              // src_logit_bias row for this token (global) | nullptr
+    static constexpr int CH = N < 32 ? N : 32;
+    __device__ __forceinline__ void load(int c, float (&v)[CH]) {
+        if constexpr (CH == 32) {
+            uint32_t r[32];
+            ptx::tmem_ld_32x32b_x32(taddr + c * 32, r);
+            ptx::tmem_ld_wait();
+#pragma unroll
+            for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+        } else {
+            uint32_t r[16];
+            ptx::tmem_ld_32x32b_x16(taddr + c * 16, r);
+            ptx::tmem_ld_wait();
+#pragma unroll
+            for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+        }
+        if (bias) {
+#pragma unroll
+            for (int i = 0; i < CH; i += 4) {
+                const float4 b = __ldg(reinterpret_cast<const float4*>(bias + c * CH + i));
+                v[i] = __fadd_rn(v[i], b.x); v[i + 1] = __fadd_rn(v[i + 1], b.y);
+                v[i + 2] = __fadd_rn(v[i + 2], b.z); v[i + 3] = __fadd_rn(v[i + 3], b.w);
+            }
+        }
+    }
+};
+
+template <int N, int kCG, int KMAX>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b, const GemmParams p) {
+    const int kStages = p.stages;
+    constexpr int kABytes = kBlockM * kBlockK * 2;
+    constexpr int kBBytes = (N / kCG) * kBlockK * 2;
+    constexpr int kStageBytes = kABytes + kBBytes;
+    constexpr int kAccCols = N < 32 ? 32 : N;           // TMEM columns per accumulator stage
+    constexpr int kTmemCols = 2 * kAccCols < 32 ? 32 : 2 * kAccCols;
+    constexpr uint32_t kIdesc = ptx::make_idesc_bf16_f32(128 * kCG, N);
+    static_assert(kTmemCols <= 512, "TMEM");
+
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t raw_addr = ptx::smem_u32(smem_raw);
+    const uint32_t base = (raw_addr + 1023u) & ~1023u;
+    unsigned char* base_ptr = smem_raw + (base - raw_addr);
+    // barriers
+    const uint32_t aux = base + kStages * kStageBytes;
+    const uint32_t full_bar = aux;                       // kStages x 8
+    const uint32_t empty_bar = aux + 8 * kStages;        // kStages x 8
+    const uint32_t tfull_bar = aux + 16 * kStages;       // 2 x 8
+    const uint32_t tempty_bar = tfull_bar + 16;          // 2 x 8
+    const uint32_t tmem_slot = tempty_bar + 16;
+    uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(base_ptr + kStages * kStageBytes + 16 * kStages + 32);
+    float* sb_s = reinterpret_cast<float*>(base_ptr + kStages * kStageBytes + kGemmAuxBytes);
+    int32_t* off_s = reinterpret_cast<int32_t*>(sb_s + N);
+    int32_t* hist = off_s + ((p.S + 1 + 3) & ~3);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t cta_rank = (kCG == 2) ? ptx::cluster_ctarank() : 0u;
+    const bool leader = cta_rank == 0;
+    const int pair = blockIdx.x / kCG, n_pairs = gridDim.x / kCG;
+    const int n_tiles = p.n_layers * p.m_tiles;
+    const int num_kb = (p.H + kBlockK - 1) / kBlockK;
+
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tmap(&tmap_a);
+        ptx::prefetch_tmap(&tmap_b);
+    }
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < kStages; ++s) {
+            ptx::mbar_init(full_bar + 8 * s, 1);
+            ptx::mbar_init(empty_bar + 8 * s, 1);
+        }
+        for (int a = 0; a < 2; ++a) {
+            ptx::mbar_init(tfull_bar + 8 * a, 1);
+            ptx::mbar_init(tempty_bar + 8 * a, 4 * kCG);   // one arrive per epilogue warp per CTA
+        }
+        ptx::fence_barrier_init();
+    }
+    if (warp == 2) {
+        ptx::tmem_alloc<kCG>(tmem_slot, kTmemCols);
+        ptx::tmem_relinquish<kCG>();
+    }
+    for (int i = threadIdx.x; i <= p.S; i += kGemmThreads) off_s[i] = p.src_offsets[i];
+    ptx::tc_fence_before();
+    if constexpr (kCG == 2) ptx::cluster_sync(); else __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ================= TMA producer =================
+        if (lane == 0) {
+            const uint64_t pol_a = ptx::policy_evict_first();   // hidden is read exactly once
+            const uint64_t pol_b = ptx::policy_evict_last();    // W[l] is re-read by every tile of the layer
+            const uint32_t full_leader = (kCG == 2) ? ptx::mapa(full_bar, 0) : full_bar;
+            int stage = 0; uint32_t phase = 0;
+            for (int tile = pair; tile < n_tiles; tile += n_pairs) {
+                const int li = tile / p.m_tiles, mt = tile % p.m_tiles;
+                const int m0 = (mt * kCG + (int)cta_rank) * kBlockM;
+                const int n0 = (int)cta_rank * (N / kCG);
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    ptx::mbar_wait(empty_bar + 8 * stage, phase ^ 1);
+                    if (leader) ptx::mbar_arrive_expect_tx(full_bar + 8 * stage, kCG * kStageBytes);
+                    const uint32_t sa = base + stage * kStageBytes;
+                    const uint32_t fb = (kCG == 2) ? full_leader + 8 * stage : full_bar + 8 * stage;
+                    ptx::tma_load_3d<kCG>(sa, &tmap_a, fb, kb * kBlockK, m0, li, pol_a);
+                    ptx::tma_load_3d<kCG>(sa + kABytes, &tmap_b, fb, kb * kBlockK, n0, p.layer0 + li, pol_b);
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ================= MMA issuer (leader CTA of the pair) =================
+        if (leader) {
+            int stage = 0; uint32_t phase = 0;
+            int it = 0;
+            for (int tile = pair; tile < n_tiles; tile += n_pairs, ++it) {
+                const int as = it & 1;
+                const uint32_t aphase = (it >> 1) & 1;
+                if (kCG == 2) ptx::mbar_wait_cluster(tempty_bar + 8 * as, aphase ^ 1);
+                else ptx::mbar_wait(tempty_bar + 8 * as, aphase ^ 1);
+                ptx::tc_fence_after();
+                const uint32_t d_tmem = tmem_base + as * kAccCols;
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    ptx::mbar_wait(full_bar + 8 * stage, phase);
+                    ptx::tc_fence_after();
+                    if (lane == 0) {
+                        const uint32_t sa = base + stage * kStageBytes;
+                        const uint64_t da = ptx::make_sw128_kmajor_desc(sa);
+                        const uint64_t db = ptx::make_sw128_kmajor_desc(sa + kABytes);
+#pragma unroll
+                        for (int k = 0; k < kBlockK / 16; ++k) {
+                            // +32 B per K=16 step inside the 128-byte swizzle row (>>4 = 2)
+                            ptx::umma_bf16<kCG>(d_tmem, da + 2 * k, db + 2 * k, kIdesc, (kb | k) != 0);
+                        }
+                        ptx::umma_commit<kCG>(empty_bar + 8 * stage);          // frees the smem slot (both CTAs)
+                        if (kb == num_kb - 1) ptx::umma_commit<kCG>(tfull_bar + 8 * as);   // accumulator ready
+                    }
+                    __syncwarp();
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp >= 4) {
+        // ================= epilogue: TMEM -> registers -> logits / gating =================
+        const int q = warp - 4;                       // TMEM lane quadrant (== warp % 4)
+        const int ep_tid = threadIdx.x - 128;
+        const uint32_t tempty_leader = (kCG == 2) ? ptx::mapa(tempty_bar, 0) : tempty_bar;
+        int it = 0;
+        int cur_layer = -1;
+        for (int tile = pair; tile < n_tiles; tile += n_pairs, ++it) {
+            const int as = it & 1;
+            const uint32_t aphase = (it >> 1) & 1;
+            const int li = tile / p.m_tiles, mt = tile % p.m_tiles;
+            const int layer = p.layer0 + li;
+            const int m0 = (mt * kCG + (int)cta_rank) * kBlockM;
+            const int t = m0 + q * 32 + lane;
+            if (p.do_gate && layer != cur_layer) {
+                // new layer: flush the histogram of the previous one, load this layer's select bias
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                if (cur_layer >= 0) {
+                    int32_t* dst = p.A_step + (size_t)cur_layer * p.S * N;
+                    for (int i = ep_tid; i < p.S * N; i += 128) {
+                        const int32_t c = hist[i];
+                        if (c) atomicAdd(dst + i, c);
+                    }
+                }
+                for (int i = ep_tid; i < p.S * N; i += 128) hist[i] = 0;
+                if (p.select_bias)
+                    for (int i = ep_tid; i < N; i += 128) sb_s[i] = p.select_bias[(size_t)layer * N + i];
+                cur_layer = layer;
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+            }
+            ptx::mbar_wait(tfull_bar + 8 * as, aphase);
+            ptx::tc_fence_after();
+            const uint32_t taddr = tmem_base + as * kAccCols + ((uint32_t)(q * 32) << 16);
+            const int s = find_source(off_s, p.S, min(t, p.T - 1));
+            const float* bias = p.src_logit_bias ? p.src_logit_bias + ((size_t)layer * p.S + s) * N : nullptr;
+            TmemRowSrc<N> src{taddr, bias};
+            if (p.logits) {
+                constexpr int CH = TmemRowSrc<N>::CH;
+                float v[CH];
+                float* orow = p.logits + ((size_t)li * p.T + t) * N;
+#pragma unroll
+                for (int c = 0; c < N / CH; ++c) {
+                    src.load(c, v);
+                    if (t < p.T) {
+#pragma unroll
+                        for (int i = 0; i < CH; i += 4)
+                            *reinterpret_cast<float4*>(orow + c * CH + i) = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+                    }
+                }
+            }
+            if (p.do_gate) {
+                int32_t ids[KMAX];
+                float w[KMAX];
+                if (p.topk_w) gate_row<N, KMAX, true>(p.gp, p.select_bias ? sb_s : nullptr, src, ids, w);
+                else gate_row<N, KMAX, false>(p.gp, p.select_bias ? sb_s : nullptr, src, ids, w);
+                if (t < p.T) {
+#pragma unroll
+                    for (int j = 0; j < KMAX; ++j)
+                        if (j < p.gp.k) atomicAdd(&hist[s * N + ids[j]], 1);
+                    if (p.topk_ids) {
+                        int32_t* o = p.topk_ids + ((size_t)li * p.T + t) * p.gp.k;
+#pragma unroll
+                        for (int j = 0; j < KMAX; ++j)
+                            if (j < p.gp.k) o[j] = ids[j];
+                    }
+                    if (p.topk_w) {
+                        float* o = p.topk_w + ((size_t)li * p.T + t) * p.gp.k;
+#pragma unroll
+                        for (int j = 0; j < KMAX; ++j)
+                            if (j < p.gp.k) o[j] = w[j];
+                    }
+                }
+            }
+            // release this accumulator stage to the MMA issuer
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+                if (kCG == 2) ptx::mbar_arrive_cluster(tempty_leader + 8 * as);
+                else ptx::mbar_arrive(tempty_bar + 8 * as);
+            }
+        }
+        if (p.do_gate && cur_layer >= 0) {
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            int32_t* dst = p.A_step + (size_t)cur_layer * p.S * N;
+            for (int i = ep_tid; i < p.S * N; i += 128) {
+                const int32_t c = hist[i];
+                if (c) atomicAdd(dst + i, c);
+            }
+        }
+    }
+
+    // ================= teardown =================
+    ptx::tc_fence_before();
+    if constexpr (kCG == 2) ptx::cluster_sync(); else __syncthreads();
+    if (warp == 2) ptx::tmem_dealloc<kCG>(tmem_base, kTmemCols);
+}
+
+}  // namespace gimbal

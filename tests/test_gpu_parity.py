@@ -1,0 +1,440 @@
+"""GPU parity tests: the CUDA path (through the C-ABI binding) against the CPU oracle,
+element by element on the same seeded inputs.
+
+Bars (BASELINE.json north_star): integer / index work bit-exact; router logits within 1e-2
+relative (bf16 inputs, fp32 accumulation); fp32 objectives within 1e-5 relative (relative to
+the magnitude of the terms that were added when a result is a cancelling sum, R13).
+
+Order matters on a fresh box: placement and gating kernels first, the tcgen05 GEMM last.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2606_15177_b200 as g
+from tests.util import bf16_bits, to_np, ws_tensor
+from workloads import gen, get_workload, scaled
+from workloads.configs import MODE_EMA, MODE_WINDOW, SIGMOID
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+SHAPES = {                      # name -> (L, T, P) scaled so the oracle finishes in seconds
+    "tiny": (1, 1000, 64),
+    "v2lite": (3, 1500, 96),
+    "qwen3": (2, 1300, 64),
+    "v3": (2, 1100, 48),
+    "decode": (2, 256, 64),
+}
+
+
+def _wl(name):
+    L, T, P = SHAPES[name]
+    return scaled(get_workload(name), L=L, T=T, P=P)
+
+
+# ------------------------------------------------------------------------------------------
+# placement side (a6, a7)
+# ------------------------------------------------------------------------------------------
+def _placement_instance(name, seed=0, counts="i32", table_M=False, seeded_D=False):
+    w = _wl(name)
+    r = w.router
+    rng = np.random.default_rng(100 + seed)
+    # counts shaped like a skewed routing profile; B lives on another scale than A
+    pop = rng.zipf(1.3, size=(r.L, r.E)).clip(1, 500).astype(np.float64)
+    A = (rng.random((r.L, r.S, r.E)) * pop[:, None, :] * 40).astype(np.int64)
+    B = A.sum(1) * rng.integers(50, 150, (r.L, r.E))
+    if counts == "f32":
+        A_t = torch.from_numpy((A * 0.37).astype(np.float32)).to(DEV)
+        B_t = torch.from_numpy((B * 0.37).astype(np.float32)).to(DEV)
+    else:
+        A_t = torch.from_numpy(A.astype(np.int32)).to(DEV)
+        B_t = torch.from_numpy(B.astype(np.int32)).to(DEV)
+    D = gen.comm_cost_D(w, "seeded" if seeded_D else "binary", DEV)
+    M = gen.mig_cost_M(w, DEV) if table_M else None
+    prev = gen.prev_placement(w, to_np(B_t), DEV)
+    cfg = g.PlacementCfg(L=r.L, E=r.E, G=w.G, slots_per_rank=w.slots_per_rank, S=r.S,
+                         counts_dtype=g.COUNTS_F32 if counts == "f32" else g.COUNTS_I32)
+    return w, cfg, A_t, B_t, D, M, prev
+
+
+def _oracle_kw(cfg):
+    return dict(G=cfg.G, sp=cfg.slots_per_rank, weights=(cfg.alpha, cfg.beta, cfg.gamma))
+
+
+def _check_objective(out, ref, tol=1e-5):
+    """out, ref [P,5]: every column is a sum of same-signed terms except J's mix, all >= 0."""
+    assert np.array_equal(np.isnan(out), np.isnan(ref))
+    ok = ~np.isnan(ref[:, 0])
+    scale = np.abs(ref[ok]) + 1e-30
+    err = np.abs(out[ok] - ref[ok]) / scale
+    # C_load is a sum of squares of exact differences; tiny absolute values can sit below fp32 resolution of J
+    assert err[:, [0, 2, 3, 4]].max() <= tol, err.max(0)
+    load_scale = np.maximum(np.abs(ref[ok, 1]), 1e-6 * np.abs(ref[ok, 4]) ** 2)
+    assert (np.abs(out[ok, 1] - ref[ok, 1]) / load_scale).max() <= tol
+
+
+@pytest.mark.parametrize("name,counts,table_M,seeded_D", [
+    ("tiny", "i32", False, False), ("v2lite", "f32", True, True), ("qwen3", "i32", False, True),
+    ("v3", "i32", False, False), ("v3", "f32", True, True), ("decode", "f32", False, False), ("decode", "i32", True, True),
+])
+def test_eval_placements_parity(name, counts, table_M, seeded_D):
+    w, cfg, A, B, D, M, prev = _placement_instance(name, 0, counts, table_M, seeded_D)
+    cands = gen.candidates(w, prev, w.P, DEV)
+    out = torch.full((w.P, 5), -1.0, device=DEV)
+    argmin = torch.full((1,), -7, dtype=torch.int32, device=DEV)
+    ws = ws_tensor(g.eval_placements_workspace_bytes(cfg, w.P))
+    g.eval_placements(cfg, cands, A, B, D, prev, out, M=M, M_scalar=1.25, argmin=argmin, workspace=ws)
+    torch.cuda.synchronize()
+    ref = oracle.objective_batch(to_np(cands), to_np(prev), to_np(A), to_np(B), to_np(D), to_np(M), 1.25, **_oracle_kw(cfg))
+    o = to_np(out).astype(np.float64)
+    _check_objective(o, ref)
+    assert o[0, 3] == 0.0                                   # candidate 0 is x0: C_mig = 0
+    # argmin: lowest index among the minimisers of the GPU's own J; its oracle J is the oracle minimum (to tolerance)
+    am = int(argmin.item())
+    assert am == int(np.nanargmin(to_np(out)[:, 0]))
+    assert ref[am, 0] <= np.nanmin(ref[:, 0]) * (1 + 2e-5)
+
+
+def test_eval_placements_invalid_candidates_and_edges():
+    w, cfg, A, B, D, M, prev = _placement_instance("v3", 1)
+    P = 40
+    cands = gen.candidates(w, prev, P, DEV).clone()
+    NS, sp = w.NS, w.slots_per_rank
+    cands[3, 0, 5] = 300                                   # id out of range
+    cands[4, 1, 7] = -2
+    c5 = cands[5, 0].clone(); c5[0] = c5[1]; cands[5, 0] = c5            # expert twice on a rank (and one missing)
+    # a co-located duplicate that keeps the multiset: exchange so that both copies of a replicated expert share a rank
+    row = to_np(cands[6, 1]).copy()
+    vals, cnt = np.unique(row, return_counts=True)
+    e = vals[cnt == 2][0]
+    j0, j1 = np.nonzero(row == e)[0]
+    tgt = (j0 // sp) * sp + ((j0 % sp) + 1) % sp           # another slot on j0's rank
+    row[j1], row[tgt] = row[tgt], row[j1]
+    cands[6, 1] = torch.from_numpy(row).to(DEV)
+    out = torch.empty(P, 5, device=DEV)
+    ws = ws_tensor(g.eval_placements_workspace_bytes(cfg, P))
+    g.eval_placements(cfg, cands, A, B, D, prev, out, workspace=ws)
+    ref = oracle.objective_batch(to_np(cands), to_np(prev), to_np(A), to_np(B), to_np(D), None, 1.0, **_oracle_kw(cfg))
+    o = to_np(out).astype(np.float64)
+    assert np.isnan(ref[[3, 4, 5, 6]]).all() and np.isnan(o[[3, 4, 5, 6]]).all()
+    _check_objective(o, ref)
+    # P = 0 is a no-op; P = 1 works
+    g.eval_placements(cfg, cands[:0], A, B, D, prev, out[:0], workspace=ws)
+    g.eval_placements(cfg, cands[:1], A, B, D, prev, out[:1], workspace=ws)
+    np.testing.assert_allclose(to_np(out[0]).astype(np.float64), ref[0], rtol=1e-5)
+    # GPU contract (R12): candidates place the same expert copies as x0 -> another multiset is NaN
+    c = cands[:1].clone()
+    r0 = to_np(c[0, 0]).copy()
+    vals, cnt = np.unique(r0, return_counts=True)
+    single = vals[cnt == 1][0]; dbl = vals[cnt == 2][0]
+    r0[np.nonzero(r0 == dbl)[0][0]] = single               # drops a replica of `dbl`, adds one of `single`
+    c[0, 0] = torch.from_numpy(r0).to(DEV)
+    g.eval_placements(cfg, c, A, B, D, prev, out[:1], workspace=ws)
+    assert torch.isnan(out[0]).all()
+    # an invalid x0 poisons everything
+    bad_prev = prev.clone(); bad_prev[0, 0] = bad_prev[0, 1]
+    g.eval_placements(cfg, cands[:4], A, B, D, bad_prev, out[:4], workspace=ws)
+    assert torch.isnan(out[:4]).all()
+
+
+def _delta_scales(cfg, moves, cur, A, B, D, M, M_scalar):
+    """|terms| that a delta is made of (tolerance base, R13)."""
+    L, E, G, sp = cfg.L, cfg.E, cfg.G, cfg.slots_per_rank
+    A = A.astype(np.float64); B = B.astype(np.float64); D = D.astype(np.float64)
+    r = np.stack([np.bincount(cur[l], minlength=E) for l in range(L)]).astype(np.float64)
+    w = B / r
+    Lg = np.stack([[w[l, cur[l, gidx * sp:(gidx + 1) * sp]].sum() for gidx in range(G)] for l in range(L)])
+    c = np.einsum("lse,sg->leg", A, D) / r[:, :, None]
+    sc = np.zeros((len(moves), 5))
+    for i, (l, a, b) in enumerate(moves):
+        e1, e2, g1, g2 = cur[l, a], cur[l, b], a // sp, b // sp
+        dl = w[l, e2] - w[l, e1]
+        sc[i, 1] = abs(2 * dl * (Lg[l, g1] - Lg[l, g2])) + 2 * dl * dl
+        sc[i, 2] = c[l, e1, g1] + c[l, e1, g2] + c[l, e2, g1] + c[l, e2, g2]
+        sc[i, 3] = 4 * (M_scalar if M is None else M[l].max())
+        sc[i, 4] = Lg[l].max()
+        sc[i, 0] = cfg.alpha * sc[i, 2] + cfg.beta * sc[i, 1] + cfg.gamma * sc[i, 3]
+    return sc
+
+
+def _check_deltas(cfg, d, ref, moves, cur, A, B, D, M, M_scalar, tol=1e-5):
+    assert np.array_equal(np.isnan(d), np.isnan(ref))
+    ok = ~np.isnan(ref[:, 0])
+    sc = _delta_scales(cfg, moves[ok], cur, A, B, D, M, M_scalar)
+    err = np.abs(d[ok] - ref[ok])
+    assert np.all(err <= tol * sc + 1e-30), (err / (sc + 1e-30)).max(0)
+
+
+@pytest.mark.parametrize("name,counts,table_M", [("tiny", "i32", False), ("v2lite", "f32", True), ("v3", "i32", False),
+                                                   ("v3", "f32", True), ("decode", "i32", False)])
+def test_eval_moves_parity(name, counts, table_M):
+    w, cfg, A, B, D, M, prev = _placement_instance(name, 2, counts, table_M, True)
+    cur = gen.candidates(w, prev, 4, DEV)[2].contiguous()          # a few transpositions away from x0
+    kw = _oracle_kw(cfg)
+    An, Bn, Dn, Mn, curn, prevn = to_np(A), to_np(B), to_np(D), to_np(M), to_np(cur), to_np(prev)
+    ws = ws_tensor(g.eval_moves_workspace_bytes(cfg))
+    # explicit list
+    moves = gen.explicit_moves(w, 3000, DEV)
+    delta = torch.empty(3000, 5, device=DEV)
+    best = torch.empty(cfg.L, dtype=torch.int32, device=DEV)
+    g.eval_moves(cfg, cur, prev, A, B, D, delta, moves=moves, M=M, M_scalar=0.75, best_per_layer=best, workspace=ws)
+    mv = to_np(moves)
+    ref = oracle.move_deltas(curn, prevn, mv, An, Bn, Dn, Mn, 0.75, **kw)
+    d = to_np(delta).astype(np.float64)
+    _check_deltas(cfg, d, ref, mv, curn, An, Bn, Dn, Mn, 0.75)
+    for l in range(cfg.L):                                          # lowest dJ of the layer, lowest index on ties
+        idx = np.nonzero((mv[:, 0] == l) & ~np.isnan(d[:, 0]))[0]
+        dj = to_np(delta)[idx, 0]
+        assert int(best[l].item()) == int(idx[np.argmin(dj)])
+    # implicit whole neighbourhood in canonical order
+    allmv = oracle.all_pair_moves(cfg.L, cfg.NS)
+    n = allmv.shape[0]
+    delta = torch.empty(n, 5, device=DEV)
+    g.eval_moves(cfg, cur, prev, A, B, D, delta, M=M, M_scalar=0.75, best_per_layer=best, workspace=ws)
+    d = to_np(delta).astype(np.float64)
+    pick = np.unique(np.concatenate([np.arange(min(n, 300)), np.arange(max(0, n - 300), n),
+                                     np.random.default_rng(5).integers(0, n, 3000)]))
+    ref = oracle.move_deltas(curn, prevn, allmv[pick], An, Bn, Dn, Mn, 0.75, **kw)
+    _check_deltas(cfg, d[pick], ref, allmv[pick], curn, An, Bn, Dn, Mn, 0.75)
+    per = n // cfg.L
+    for l in range(cfg.L):
+        seg = to_np(delta)[l * per:(l + 1) * per, 0]
+        assert int(best[l].item()) == l * per + int(np.nanargmin(seg))
+    # swap deltas equal full re-evaluation through the batched objective as well (BASELINE.json invariant)
+    some = pick[~np.isnan(d[pick, 0])][:32]
+    cands = cur.unsqueeze(0).repeat(len(some) + 1, 1, 1).contiguous()
+    for i, m in enumerate(some):
+        l, a, b = allmv[m]
+        cands[i + 1, l, a], cands[i + 1, l, b] = cur[l, b], cur[l, a]
+    out = torch.empty(len(some) + 1, 5, device=DEV)
+    ws2 = ws_tensor(g.eval_placements_workspace_bytes(cfg, len(some) + 1))
+    g.eval_placements(cfg, cands, A, B, D, prev, out, M=M, M_scalar=0.75, workspace=ws2)
+    o = to_np(out).astype(np.float64)
+    full = o[1:] - o[0]
+    for j in (1, 2, 3, 4):
+        np.testing.assert_allclose(full[:, j], d[some, j], rtol=0, atol=2e-5 * np.abs(o[:, j]).max())
+
+
+def test_eval_moves_invalid_and_zero_moves():
+    w, cfg, A, B, D, M, prev = _placement_instance("v3", 3)
+    cur = prev.clone()
+    curn = to_np(cur)
+    sp = cfg.slots_per_rank
+    row = curn[0]
+    vals, cnt = np.unique(row, return_counts=True)
+    e = vals[cnt == 2][0]
+    j0, j1 = np.nonzero(row == e)[0]
+    other = (j0 // sp) * sp + ((j0 % sp) + 1) % sp            # a different expert on j0's rank
+    moves = torch.tensor([[0, j0, j1],                        # two replicas of one expert: zeros
+                          [0, other, j1],                     # would co-locate both copies of e on j0's rank: NaN
+                          [0, j0, other],                     # same rank: zeros
+                          [1, 0, cfg.NS - 1]], dtype=torch.int32, device=DEV)
+    delta = torch.empty(4, 5, device=DEV)
+    ws = ws_tensor(g.eval_moves_workspace_bytes(cfg))
+    g.eval_moves(cfg, cur, prev, A, B, D, delta, moves=moves, workspace=ws)
+    d = to_np(delta)
+    ref = oracle.move_deltas(curn, to_np(prev), to_np(moves), to_np(A), to_np(B), to_np(D), None, 1.0, **_oracle_kw(cfg))
+    assert np.all(d[0] == 0) and np.all(d[2] == 0) and np.isnan(d[1]).all()
+    assert np.array_equal(np.isnan(d), np.isnan(ref))
+    # a swap applied twice returns to the start: delta(back) = -delta(forth)
+    nxt = cur.clone(); nxt[1, 0], nxt[1, cfg.NS - 1] = cur[1, cfg.NS - 1], cur[1, 0]
+    back = torch.empty(1, 5, device=DEV)
+    g.eval_moves(cfg, nxt, prev, A, B, D, back, moves=moves[3:4], workspace=ws)
+    if not np.isnan(d[3]).any():
+        np.testing.assert_allclose(to_np(back)[0, 1:4], -d[3, 1:4], rtol=1e-5, atol=1e-3)
+
+
+# ------------------------------------------------------------------------------------------
+# stats side (a1..a5)
+# ------------------------------------------------------------------------------------------
+def _router_inputs(w, step=0):
+    hidden = gen.hidden_all(w, step, DEV)
+    W = gen.w_router(w, DEV)
+    slb = gen.src_logit_bias(w, step, DEV)
+    sb = gen.select_bias(w, DEV)
+    off = gen.src_offsets(w, step, w.T, DEV)
+    return hidden, W, slb, sb, off
+
+
+def _synthetic_logits(w, seed):
+    """fp32 logits with the workload's skew plus edge rows: exact ties, NaN, -inf, -0."""
+    r = w.router
+    gen_ = torch.Generator(device=DEV); gen_.manual_seed(seed)
+    x = torch.randn(r.L, w.T, r.E, generator=gen_, device=DEV) * 1.7
+    off = gen.src_offsets(w, 0, w.T, DEV)
+    slb = gen.src_logit_bias(w, 0, DEV)
+    src = torch.repeat_interleave(torch.arange(r.S, device=DEV), (off[1:] - off[:-1]).long())
+    x = x + slb[:, src, :]
+    x[:, 0::7] = torch.round(x[:, 0::7] * 2) / 2            # many exact ties
+    x[:, 5, :] = 0.25                                       # all equal
+    x[:, 6, :] = float("-inf")
+    x[:, 7, 3] = float("nan")
+    x[:, 8, :4] = torch.tensor([0.0, -0.0, 0.0, -0.0], device=DEV)
+    x[:, 9, 1] = float("inf")
+    return x.contiguous(), off
+
+
+@pytest.mark.parametrize("name", list(SHAPES))
+def test_gating_and_histogram_bit_exact_on_given_logits(name):
+    w = _wl(name)
+    r = w.router
+    cfg = g.RouterCfg.from_workload(r)
+    x, off = _synthetic_logits(w, 11)
+    sb = gen.select_bias(w, DEV)
+    st = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+    ids = torch.full((r.L, w.T, r.k), -9, dtype=torch.int32, device=DEV)
+    wts = torch.full((r.L, w.T, r.k), -9.0, device=DEV)
+    ws = ws_tensor(g.route_stats_workspace_bytes(cfg, r.L, w.T))
+    g.route_stats(cfg, st, T=w.T, select_bias=sb, src_offsets=off, logits_mode=g.LOGITS_IN, logits=x, topk_ids=ids, topk_w=wts,
+                  workspace=ws)
+    torch.cuda.synchronize()
+    xn, offn = to_np(x), to_np(off)
+    for l in range(r.L):
+        rid, rw = oracle.gate(xn[l], r, None if sb is None else to_np(sb)[l], tier=1)
+        np.testing.assert_array_equal(to_np(ids[l]), rid)                      # bit-exact ids, best first
+        finite = np.isfinite(rw).all(1)
+        np.testing.assert_allclose(to_np(wts[l])[finite], rw[finite], rtol=1e-5, atol=1e-30)
+        C = oracle.counts(rid, offn, r.S, r.E)
+        np.testing.assert_array_equal(to_np(st.A_step[l]), C)                  # bit-exact counts
+        np.testing.assert_array_equal(C.sum(1), np.diff(offn) * r.k)           # row sums = tokens x k
+        if r.n_groups > 1:
+            assert all(len(set((row // 32).tolist())) <= r.topk_groups for row in to_np(ids[l]))
+    # without the optional outputs the counts are the same
+    st2 = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+    g.route_stats(cfg, st2, T=w.T, select_bias=sb, src_offsets=off, logits_mode=g.LOGITS_IN, logits=x, workspace=ws)
+    assert torch.equal(st2.A_step, st.A_step)
+
+
+@pytest.mark.parametrize("name,mode", [("v2lite", MODE_EMA), ("qwen3", MODE_WINDOW), ("v3", MODE_WINDOW), ("decode", MODE_EMA)])
+def test_update_load_and_pressure_over_steps(name, mode):
+    w = _wl(name)
+    r = w.router
+    cfg = g.RouterCfg.from_workload(r)
+    window_len, decay, steps = 3, 0.9, 7
+    st = g.StatsState(cfg, mode, window_len=window_len, ema_decay=decay)
+    rng = np.random.default_rng(3)
+    Bsyn = rng.integers(1, 1000, (r.L, r.E))
+    place = gen.prev_placement(w, Bsyn, DEV)
+    dp = gen.dp_of_rank(w, DEV)
+    sb = gen.select_bias(w, DEV)
+    ws = ws_tensor(g.route_stats_workspace_bytes(cfg, r.L, w.T))
+    A_win = np.zeros((r.L, r.S, r.E), np.int64); A_pub = np.zeros_like(A_win); A_ema = np.zeros((r.L, r.S, r.E))
+    for step in range(steps):
+        x, off = _synthetic_logits(w, 100 + step)
+        g.route_stats(cfg, st, T=w.T, select_bias=sb, src_offsets=off, logits_mode=g.LOGITS_IN, logits=x,
+                      cur_placement=place, dp_of_rank=dp, G=w.G, slots_per_rank=w.slots_per_rank, workspace=ws)
+        torch.cuda.synchronize()
+        Cs = np.stack([oracle.counts(oracle.gate(to_np(x[l]), r, None if sb is None else to_np(sb)[l], 1)[0], to_np(off), r.S, r.E)
+                       for l in range(r.L)])
+        np.testing.assert_array_equal(to_np(st.A_step), Cs)
+        if mode == MODE_WINDOW:
+            live = A_win + Cs                                   # profile after accumulation, before any reset
+            pub = oracle.update_window(A_win, Cs, A_pub, step, window_len)
+            np.testing.assert_array_equal(to_np(st.A_win), A_win)
+            np.testing.assert_array_equal(to_np(st.A_pub), A_pub)
+            assert pub == ((step + 1) % window_len == 0)
+            d = oracle.derived(live.astype(np.float64), to_np(place), to_np(dp), w.G, w.slots_per_rank)
+            np.testing.assert_array_equal(to_np(st.B), d["B"].astype(np.int64))
+            if pub:
+                np.testing.assert_array_equal(to_np(st.B_pub), d["B"].astype(np.int64))
+        else:
+            oracle.update_ema(A_ema, Cs, decay)
+            np.testing.assert_allclose(to_np(st.A_ema), A_ema, rtol=1e-5)
+            d = oracle.derived(A_ema, to_np(place), to_np(dp), w.G, w.slots_per_rank)
+            np.testing.assert_allclose(to_np(st.B), d["B"], rtol=1e-5)
+        np.testing.assert_allclose(to_np(st.pressure_raw), d["pressure_raw"], rtol=1e-5)
+        np.testing.assert_allclose(to_np(st.pressure_rel), d["pressure_rel"], rtol=1e-5)
+        np.testing.assert_allclose(to_np(st.pressure_raw).sum(), d["B"].sum(), rtol=1e-5)
+        assert int(st.step_counter.item()) == step + 1 and int(st.status.item()) == 0
+
+
+def _logit_err(gl, rl):
+    """|g - r| <= tol * max(|r|, rms(row r)); returns the max of err / that scale."""
+    rms = np.sqrt((rl.astype(np.float64) ** 2).mean(-1, keepdims=True))
+    return float((np.abs(gl.astype(np.float64) - rl) / np.maximum(np.abs(rl), rms)).max())
+
+
+@pytest.mark.parametrize("cta_group", [1, 2])
+@pytest.mark.parametrize("name", list(SHAPES))
+def test_router_gemm_logits_and_full_path(name, cta_group, monkeypatch):
+    """a1 against the fp64 oracle, then the fused path against (logits OUT -> gating IN)."""
+    monkeypatch.setenv("GIMBAL_CTA_GROUP", str(cta_group))
+    w = _wl(name)
+    r = w.router
+    cfg = g.RouterCfg.from_workload(r)
+    hidden, W, slb, sb, off = _router_inputs(w)
+    ws = ws_tensor(g.route_stats_workspace_bytes(cfg, r.L, w.T))
+    st = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+    logits = torch.full((r.L, w.T, r.E), 7.0, device=DEV)
+    ids = torch.full((r.L, w.T, r.k), -9, dtype=torch.int32, device=DEV)
+    wts = torch.zeros(r.L, w.T, r.k, device=DEV)
+    g.route_stats(cfg, st, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off,
+                  logits_mode=g.LOGITS_OUT, logits=logits, topk_ids=ids, topk_w=wts, workspace=ws)
+    torch.cuda.synchronize()
+    hb, wb, offn = bf16_bits(hidden), bf16_bits(W), to_np(off)
+    flips = 0
+    for l in range(r.L):
+        l64, l32 = oracle.router_logits(hb[l], wb[l], to_np(slb)[l], offn)
+        assert _logit_err(to_np(logits[l]), l64) < 1e-2                         # the stated bar
+        assert _logit_err(to_np(logits[l]), l64) < 2e-4                         # what fp32 accumulation should give
+        # same logits -> same ids / counts, bit-exact
+        rid, rw = oracle.gate(to_np(logits[l]), r, None if sb is None else to_np(sb)[l], 1)
+        np.testing.assert_array_equal(to_np(ids[l]), rid)
+        np.testing.assert_allclose(to_np(wts[l]), rw, rtol=1e-5)
+        np.testing.assert_array_equal(to_np(st.A_step[l]), oracle.counts(rid, offn, r.S, r.E))
+        # end to end (oracle logits in fp64 -> fp32): report the flip rate
+        eid, _ = oracle.gate(l32, r, None if sb is None else to_np(sb)[l], 1)
+        flips += int((np.sort(eid, 1) != np.sort(to_np(ids[l]), 1)).any(1).sum())
+    rate = flips / (r.L * w.T)
+    print(f"[{name} cg{cta_group}] end-to-end top-k flip rate {rate:.2e}")
+    assert rate < 5e-3
+    # fused, logits never written: identical integers
+    st2 = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+    ids2 = torch.full_like(ids, -9)
+    g.route_stats(cfg, st2, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off,
+                  logits_mode=g.LOGITS_NONE, topk_ids=ids2, workspace=ws)
+    assert torch.equal(ids2, ids) and torch.equal(st2.A_step, st.A_step)
+    # unfused two-kernel path (GEMM -> logits -> gating kernel): identical integers again
+    monkeypatch.setenv("GIMBAL_FUSE_GATE", "0")
+    st3 = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+    ids3 = torch.full_like(ids, -9)
+    logits3 = torch.empty_like(logits)
+    g.route_stats(cfg, st3, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off,
+                  logits_mode=g.LOGITS_OUT, logits=logits3, topk_ids=ids3, workspace=ws)
+    assert torch.equal(logits3, logits) and torch.equal(ids3, ids) and torch.equal(st3.A_step, st.A_step)
+    # layer slices give the same result as one call
+    if r.L > 1:
+        monkeypatch.setenv("GIMBAL_FUSE_GATE", "1")
+        st4 = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+        for l in range(r.L):
+            g.route_stats(cfg, st4, T=w.T, hidden=hidden[l:l + 1], w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off,
+                          layer0=l, n_layers=1, workspace=ws)
+        assert torch.equal(st4.A_step, st.A_step) and int(st4.step_counter.item()) == 1
+
+
+def test_gemm_special_cases():
+    """one-hot W rows return columns of hidden exactly; all-ones give H; T smaller than a tile."""
+    cfg = g.RouterCfg(L=1, H=256, E=16, k=2, S=1)
+    T = 37
+    hidden = torch.randn(1, T, 256, device=DEV).to(torch.bfloat16)
+    W = torch.zeros(1, 16, 256, device=DEV, dtype=torch.bfloat16)
+    cols = [7, 0, 255, 64, 63, 128, 1, 2, 3, 4, 5, 6, 8, 9, 10, 11]
+    for e, c in enumerate(cols):
+        W[0, e, c] = 1.0
+    off = torch.tensor([0, T], dtype=torch.int32, device=DEV)
+    st = g.StatsState(cfg, MODE_WINDOW)
+    logits = torch.empty(1, T, 16, device=DEV)
+    ws = ws_tensor(g.route_stats_workspace_bytes(cfg, 1, T))
+    for cg in ("1", "2"):
+        os.environ["GIMBAL_CTA_GROUP"] = cg
+        logits.fill_(-1)
+        g.route_stats(cfg, st, T=T, hidden=hidden, w_router=W, src_offsets=off, logits_mode=g.LOGITS_OUT, logits=logits, workspace=ws)
+        assert torch.equal(logits[0], hidden[0][:, cols].float())
+        g.route_stats(cfg, st, T=T, hidden=torch.ones_like(hidden), w_router=torch.ones_like(W), src_offsets=off,
+                      logits_mode=g.LOGITS_OUT, logits=logits, workspace=ws)
+        assert torch.all(logits == 256.0)
+    os.environ.pop("GIMBAL_CTA_GROUP")

@@ -1,0 +1,82 @@
+"""CPU-only checks of the C-ABI boundary: the library loads, exports every symbol that
+include/gimbal.h declares, validates arguments on the host, and refuses to compute without a
+GPU (no CPU fallback)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+import torch
+
+import paper_2606_15177_b200 as g
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    src = open(os.path.join(ROOT, "include", "gimbal.h")).read()
+    return sorted(set(re.findall(r"GIMBAL_API\s+[\w\s\*]+?\b(gimbal_\w+)\s*\(", src)))
+
+
+def test_build_is_current_and_loads():
+    from paper_2606_15177_b200 import build
+    build.build()
+    assert g.lib().gimbal_version() >= 100
+
+
+def test_every_declared_symbol_is_exported():
+    decl = _declared_symbols()
+    assert len(decl) >= 12
+    assert sorted(decl) == sorted(g.EXPORTED_SYMBOLS)
+    for name in decl:
+        assert hasattr(g.lib(), name), name
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2606_15177_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt and "gimbal_oracle" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2606_15177_b200" not in txt and "from paper_2606_15177_b200" not in txt and "csrc" not in txt.replace("under paper_2606_15177_b200/csrc", ""), f
+
+
+def test_host_side_validation():
+    cfg = g.RouterCfg(L=2, H=256, E=48, k=2, S=2)            # E not supported
+    c = cfg.c()
+    st = g.binding._StatsState()
+    rc = g.lib().gimbal_route_stats(C.byref(c), 0, 2, 16, None, None, None, None, None, 0, None, None, None, None, None, 0, 0,
+                                    C.byref(st), None, C.c_size_t(0), None)
+    assert rc == -2 and "E=48" in g.last_error()
+    cfg = g.RouterCfg(L=2, H=250, E=64, k=2, S=2)
+    c = cfg.c()
+    rc = g.lib().gimbal_route_stats(C.byref(c), 0, 2, 16, None, None, None, None, None, 0, None, None, None, None, None, 0, 0,
+                                    C.byref(st), None, C.c_size_t(0), None)
+    assert rc == -2 and "multiple of 64" in g.last_error()
+    cfg = g.RouterCfg(L=2, H=256, E=64, k=2, S=2)
+    c = cfg.c()
+    rc = g.lib().gimbal_route_stats(C.byref(c), 0, 3, 16, None, None, None, None, None, 0, None, None, None, None, None, 0, 0,
+                                    C.byref(st), None, C.c_size_t(0), None)
+    assert rc == -1 and "layer range" in g.last_error()
+    pc = g.PlacementCfg(L=1, E=16, G=3, slots_per_rank=6, S=2).c()
+    rc = g.lib().gimbal_eval_placements(C.byref(pc), 1, None, None, None, None, None, C.c_float(1.0), None, None, None, None,
+                                        C.c_size_t(0), None)
+    assert rc == -2 and "power of two" in g.last_error()
+    assert g.eval_placements_workspace_bytes(g.PlacementCfg(L=58, E=256, G=32, slots_per_rank=9, S=16), 4096) > 58 * 256 * 32 * 8
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU behaviour")
+def test_no_cpu_fallback_without_gpu():
+    cfg = g.RouterCfg(L=1, H=256, E=16, k=2, S=2)
+    c = cfg.c()
+    st = g.binding._StatsState()
+    one = C.c_void_p(16)          # fake non-NULL, 16-byte aligned "device" pointers: never dereferenced on the host
+    st.A_step = st.A_win = st.A_pub = st.B_pub = st.B = st.step_counter = 16
+    st.mode, st.window_len = 0, 1
+    rc = g.lib().gimbal_route_stats(C.byref(c), 0, 1, 16, one, one, None, None, one, 0, None, None, None, None, None, 0, 0,
+                                    C.byref(st), one, C.c_size_t(1 << 20), None)
+    assert rc == -2 and "CUDA" in g.last_error()
