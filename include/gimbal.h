@@ -242,6 +242,17 @@ GIMBAL_API int gimbal_eval_moves(const gimbal_placement_cfg *cfg, const int16_t 
 /* Counters for bench.py: kernels launched by this library since load. */
 GIMBAL_API int64_t gimbal_launch_count(void);
 
+/* Measurement hooks for bench.py.  With timing enabled the library records a pair of CUDA
+ * events on the caller's stream around each launch of its four main kernels (never enable
+ * this while capturing a CUDA graph).  gimbal_kernel_elapsed_ms() waits for the most recent
+ * launch of kernel `which` to finish and returns its device time in milliseconds.           */
+#define GIMBAL_KERNEL_ROUTER 0 /* router GEMM (+ fused gating / histogram)  a1-a3 */
+#define GIMBAL_KERNEL_GATE 1   /* standalone gating + histogram              a2-a3 */
+#define GIMBAL_KERNEL_SCORE 2  /* placement scoring                          a6    */
+#define GIMBAL_KERNEL_MOVES 3  /* move deltas                                a7    */
+GIMBAL_API int gimbal_kernel_timing(int enable);
+GIMBAL_API int gimbal_kernel_elapsed_ms(int which, float *ms);
+
 #ifdef __cplusplus
 }
 #endif

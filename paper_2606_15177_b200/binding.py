@@ -20,7 +20,9 @@ EXPORTED_SYMBOLS = [
     "gimbal_route_stats_host",
     "gimbal_eval_placements_workspace_bytes", "gimbal_eval_placements", "gimbal_eval_placements_host",
     "gimbal_eval_moves_workspace_bytes", "gimbal_eval_moves",
+    "gimbal_kernel_timing", "gimbal_kernel_elapsed_ms",
 ]
+KERNEL_ROUTER, KERNEL_GATE, KERNEL_SCORE, KERNEL_MOVES = 0, 1, 2, 3
 
 
 class GimbalError(RuntimeError):
@@ -80,6 +82,16 @@ def last_error() -> str:
 
 def launch_count() -> int:
     return int(lib().gimbal_launch_count())
+
+
+def kernel_timing(enable: bool) -> None:
+    _check(lib().gimbal_kernel_timing(C.c_int(1 if enable else 0)), "gimbal_kernel_timing")
+
+
+def kernel_elapsed_ms(which: int) -> float:
+    ms = C.c_float(0.0)
+    _check(lib().gimbal_kernel_elapsed_ms(C.c_int(which), C.byref(ms)), "gimbal_kernel_elapsed_ms")
+    return float(ms.value)
 
 
 def _check(rc: int, what: str):

@@ -16,6 +16,8 @@
 using namespace gimbal;
 
 namespace gimbal {
+int ktime_enable(int on);
+int ktime_elapsed(int which, float* ms);
 int64_t launches();
 void copy_last_error(char* buf, size_t n);
 }
@@ -135,7 +137,7 @@ static size_t place_ws_carve(const gimbal_placement_cfg* c, int P, void* ws, Pla
     const size_t LE = (size_t)c->L * c->E;
     w.t.wc = cv.take<float2>(LE * GP);
     w.t.m = cv.take<float>(LE * GP);
-    w.t.w_e = cv.take<float>(LE);
+    w.t.w_e = cv.take<double>(LE);
     w.t.hsum = cv.take<uint32_t>(c->L);
     w.t.base_mig = cv.take<float>(c->L);
     w.t.sumB = cv.take<double>(c->L);
@@ -144,8 +146,8 @@ static size_t place_ws_carve(const gimbal_placement_cfg* c, int P, void* ws, Pla
     w.t.bad = cv.take<int32_t>(64);
     w.partial = cv.take<float4>((size_t)P * c->L);
     w.best = cv.take<unsigned long long>(c->L + 1);
-    w.mp.Lg = cv.take<float>((size_t)c->L * c->G);
-    w.mp.top = cv.take<float>((size_t)c->L * 4);
+    w.mp.Lg = cv.take<double>((size_t)c->L * c->G);
+    w.mp.top = cv.take<double>((size_t)c->L * 4);
     w.mp.top_g = cv.take<int32_t>((size_t)c->L * 4);
     w.mp.cmask = cv.take<uint64_t>(LE);
     w.mp.bad = cv.take<int32_t>(64);
@@ -168,7 +170,9 @@ template <int SP>
 static int launch_score(const ScoreParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
     auto kern = place_score_kernel<SP>;
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ktime_begin(GIMBAL_KERNEL_SCORE, stream);
     kern<<<grid, kScoreThreads, smem, stream>>>(sp);
+    ktime_end(GIMBAL_KERNEL_SCORE, stream);
     LAUNCH_CHECK("place_score_kernel");
     return GIMBAL_OK;
 }
@@ -185,6 +189,10 @@ void gimbal_last_error(char* buf, size_t n) {
 }
 
 int64_t gimbal_launch_count(void) { return gimbal::launches(); }
+
+int gimbal_kernel_timing(int enable) { return gimbal::ktime_enable(enable); }
+
+int gimbal_kernel_elapsed_ms(int which, float* ms) { return gimbal::ktime_elapsed(which, ms); }
 
 size_t gimbal_route_stats_workspace_bytes(const gimbal_router_cfg* cfg, int n_layers, int T) {
     (void)n_layers; (void)T;
@@ -458,7 +466,9 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
         mp.alpha = cfg->alpha; mp.beta = cfg->beta; mp.gamma = cfg->gamma; mp.M_scalar = M_scalar; mp.has_M = M != nullptr;
         mp.t = w.t; mp.mp = w.mp; mp.delta = delta; mp.best = best_per_layer ? w.best : nullptr;
         const long long blocks = (n_moves + 255) / 256;
+        ktime_begin(GIMBAL_KERNEL_MOVES, stream);
         move_delta_kernel<<<(unsigned)blocks, 256, 0, stream>>>(mp);
+        ktime_end(GIMBAL_KERNEL_MOVES, stream);
         LAUNCH_CHECK("move_delta_kernel");
     }
     if (best_per_layer) {

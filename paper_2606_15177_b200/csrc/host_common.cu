@@ -21,6 +21,29 @@ int fail(int code, const char* fmt, ...) {
     return code;
 }
 void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+
+static bool g_ktime_on = false;
+static cudaEvent_t g_kev[4][2];
+static bool g_kev_made = false, g_kev_rec[4] = {false, false, false, false};
+int ktime_enable(int on) {
+    if (on && !g_kev_made) {
+        for (int i = 0; i < 4; ++i)
+            for (int j = 0; j < 2; ++j)
+                if (cudaEventCreate(&g_kev[i][j]) != cudaSuccess) return fail(GIMBAL_ERR_CUDA, "cudaEventCreate failed");
+        g_kev_made = true;
+    }
+    g_ktime_on = on != 0;
+    return GIMBAL_OK;
+}
+void ktime_begin(int which, cudaStream_t s) { if (g_ktime_on) cudaEventRecord(g_kev[which][0], s); }
+void ktime_end(int which, cudaStream_t s) { if (g_ktime_on) { cudaEventRecord(g_kev[which][1], s); g_kev_rec[which] = true; } }
+int ktime_elapsed(int which, float* ms) {
+    if (which < 0 || which > 3 || !ms) return fail(GIMBAL_ERR_INVALID_ARG, "kernel id %d", which);
+    if (!g_kev_made || !g_kev_rec[which]) return fail(GIMBAL_ERR_INVALID_ARG, "kernel %d was not timed", which);
+    if (cudaEventSynchronize(g_kev[which][1]) != cudaSuccess) return fail(GIMBAL_ERR_CUDA, "cudaEventSynchronize failed");
+    if (cudaEventElapsedTime(ms, g_kev[which][0], g_kev[which][1]) != cudaSuccess) return fail(GIMBAL_ERR_CUDA, "cudaEventElapsedTime failed");
+    return GIMBAL_OK;
+}
 int64_t launches() { return g_launches.load(); }
 void copy_last_error(char* buf, size_t n) {
     std::lock_guard<std::mutex> lk(g_err_mu);

@@ -12,6 +12,9 @@ namespace gimbal {
 
 int fail(int code, const char* fmt, ...);
 void count_launch();
+// optional CUDA-event brackets around the main kernels (gimbal_kernel_timing)
+void ktime_begin(int which, cudaStream_t s);
+void ktime_end(int which, cudaStream_t s);
 
 #define CUDA_TRY(expr)                                                                         \
     do {                                                                                       \

@@ -6,8 +6,9 @@
 //     c  = sum_s A[l,s,e] D[s,g] / r[l,e]                    (communication,     PAPER.md:244)
 //     m  = M[l,e,g]                                          (migration,         PAPER.md:248)
 // with the sign bit of c carrying "x0 already hosts e on g" (c >= 0 because A, D >= 0).
-// C_mig = sum |x - x0| M = (sum over x0's cells of M) + sum over candidate slots of (+M if the
-// cell is new, -M if x0 has it) for binary x.  r[l,e] is taken from x0: candidates place the
+// C_mig = sum |x - x0| M = (M over the candidate's cells that x0 lacks) + (M over x0's cells -
+// M over the cells both have) for binary x; exact for a scalar M, and with an M table the
+// rounding is relative to sum of M over x0's cells.  r[l,e] is taken from x0: candidates place the
 // same expert copies as x0 (R12); a candidate with another multiset of experts,
 // an id out of range or an expert twice on one rank gets NaN.
 //
@@ -29,7 +30,7 @@ constexpr int kMaxG = 64;
 struct PlaceTables {
     float2* wc;        // [L][E][GP]  {w, c with sign bit = member of x0}
     float* m;          // [L][E][GP]  M[l,e,g] (only when an M table is given)
-    float* w_e;        // [L][E]      w
+    double* w_e;       // [L][E]      w in double (move deltas subtract nearly equal loads)
     uint32_t* hsum;    // [L]         multiset hash of x0's slot contents
     float* base_mig;   // [L]         sum over x0's cells of M
     double* sumB;      // [L]         sum_e B[l,e]
@@ -91,9 +92,7 @@ __global__ void __launch_bounds__(256) place_tables_kernel(const TableParams p) 
         const double b = p.counts_f32 ? (double)reinterpret_cast<const float*>(p.B)[(size_t)l * p.E + e]
                                       : (double)reinterpret_cast<const int32_t*>(p.B)[(size_t)l * p.E + e];
         atomicAdd(&sb_s, b);
-        const float inv = 1.0f / (float)max(r_s[e], 1);
-        const float w = (float)b * inv;
-        p.t.w_e[(size_t)l * p.E + e] = w;
+        p.t.w_e[(size_t)l * p.E + e] = b / (double)max(r_s[e], 1);
         p.t.r[(size_t)l * p.E + e] = r_s[e];
         p.t.pmask[(size_t)l * p.E + e] = pm_s[e];
     }
@@ -110,7 +109,7 @@ __global__ void __launch_bounds__(256) place_tables_kernel(const TableParams p) 
         const float inv = 1.0f / (float)max(r_s[e], 1);
         c = fabsf(c * inv);
         const bool member = (pm_s[e] >> g) & 1ull;
-        const float w = p.t.w_e[(size_t)l * p.E + e];
+        const float w = (float)p.t.w_e[(size_t)l * p.E + e];
         p.t.wc[((size_t)l * p.E + e) * GP + gp] = make_float2(w, member ? -c : c);   // -0.0f keeps the flag when c == 0
         if (p.M) p.t.m[((size_t)l * p.E + e) * GP + gp] = p.M[((size_t)l * p.E + e) * p.G + g];
     }
@@ -188,7 +187,7 @@ __global__ void __launch_bounds__(kScoreThreads, 1) place_score_kernel(const Sco
     for (int pc = p_begin + warp * upw; pc < p_end; pc += (kScoreThreads / 32) * upw) {
         const int cand = pc + sub;
         const bool active = cand < p_end;
-        float sq = 0.0f, comm = 0.0f, mig = 0.0f, mx = -CUDART_INF_F;
+        float sq = 0.0f, comm = 0.0f, mig_in = 0.0f, mig_kept = 0.0f, mx = -CUDART_INF_F;
         uint32_t hs = 0;
         int bad = 0;
         if (active) {
@@ -210,7 +209,7 @@ __global__ void __launch_bounds__(kScoreThreads, 1) place_score_kernel(const Sco
                         comm += fabsf(wc.y);
                         const bool member = __float_as_int(wc.y) < 0;
                         const float mm = p.has_M ? m_s[idx] : p.M_scalar;
-                        mig += member ? -mm : mm;
+                        if (member) mig_kept += mm; else mig_in += mm;     // retained / entering cell of x0
                     }
                 }
                 if (check_dup) {
@@ -230,14 +229,16 @@ __global__ void __launch_bounds__(kScoreThreads, 1) place_score_kernel(const Sco
         for (int o = seg >> 1; o > 0; o >>= 1) {
             sq += __shfl_xor_sync(0xffffffffu, sq, o);
             comm += __shfl_xor_sync(0xffffffffu, comm, o);
-            mig += __shfl_xor_sync(0xffffffffu, mig, o);
+            mig_in += __shfl_xor_sync(0xffffffffu, mig_in, o);
+            mig_kept += __shfl_xor_sync(0xffffffffu, mig_kept, o);
             mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
             hs += __shfl_xor_sync(0xffffffffu, hs, o);
             bad |= __shfl_xor_sync(0xffffffffu, bad, o);
         }
         if (active && g0 == 0) {
             if (hs != want_hash) bad = 1;
-            float4 out = make_float4(sq, comm, base_mig + mig, mx);
+            // C_mig = entering cells + (x0's cells - retained cells); exact for a scalar M
+            float4 out = make_float4(sq, comm, mig_in + (base_mig - mig_kept), mx);
             if (bad) out.x = CUDART_NAN_F;
             p.partial[(size_t)cand * p.L + l] = out;
         }
@@ -303,8 +304,8 @@ __global__ void fill_u64_kernel(unsigned long long* p, unsigned long long v, int
 // each expert; then one thread per move evaluates the closed-form deltas.
 // ------------------------------------------------------------------------------------------
 struct MovePrep {
-    float* Lg;          // [L][G]
-    float* top;         // [L][4]  three largest rank loads (value) ...
+    double* Lg;         // [L][G]
+    double* top;        // [L][4]  three largest rank loads (value) ...
     int32_t* top_g;     // [L][4]  ... and their ranks
     uint64_t* cmask;    // [L][E]  bit g: cur hosts e on g
     int32_t* bad;       // [1]
@@ -320,7 +321,7 @@ struct MovePrepParams {
 __global__ void __launch_bounds__(256) move_prep_kernel(const MovePrepParams p) {
     __shared__ unsigned long long cm_s[kMaxE];
     __shared__ int cnt_s[kMaxE];
-    __shared__ float lg_s[kMaxG];
+    __shared__ double lg_s[kMaxG];
     __shared__ int bad_s;
     const int l = blockIdx.x, tid = threadIdx.x, NS = p.G * p.sp;
     const int16_t* cu = p.cur + (size_t)l * NS;
@@ -339,7 +340,7 @@ __global__ void __launch_bounds__(256) move_prep_kernel(const MovePrepParams p) 
         p.mp.cmask[(size_t)l * p.E + e] = cm_s[e];
     }
     if (tid < p.G) {
-        float lg = 0.0f;
+        double lg = 0.0;
         for (int j = 0; j < p.sp; ++j) {
             const int e = cu[tid * p.sp + j];
             if (e >= 0 && e < p.E) lg += p.t.w_e[(size_t)l * p.E + e];
@@ -349,10 +350,10 @@ __global__ void __launch_bounds__(256) move_prep_kernel(const MovePrepParams p) 
     }
     __syncthreads();
     if (tid == 0) {
-        float v[3] = {-CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F};
+        double v[3] = {-CUDART_INF, -CUDART_INF, -CUDART_INF};
         int gi[3] = {-1, -1, -1};
         for (int g = 0; g < p.G; ++g) {
-            const float x = lg_s[g];
+            const double x = lg_s[g];
             if (x > v[0]) { v[2] = v[1]; gi[2] = gi[1]; v[1] = v[0]; gi[1] = gi[0]; v[0] = x; gi[0] = g; }
             else if (x > v[1]) { v[2] = v[1]; gi[2] = gi[1]; v[1] = x; gi[1] = g; }
             else if (x > v[2]) { v[2] = x; gi[2] = g; }
@@ -408,10 +409,11 @@ __global__ void __launch_bounds__(256) move_delta_kernel(const MoveParams p) {
             else {
                 const float2* wc = p.t.wc + (size_t)l * p.E * GP;
                 const float2 t11 = wc[e1 * GP + g1], t12 = wc[e1 * GP + g2], t21 = wc[e2 * GP + g1], t22 = wc[e2 * GP + g2];
-                const float w1 = t11.x, w2 = t22.x;
-                const float L1 = p.mp.Lg[(size_t)l * p.G + g1], L2 = p.mp.Lg[(size_t)l * p.G + g2];
-                const float dl = w2 - w1;                                     // moved onto g1
-                dload = 2.0f * dl * (L1 - L2) + 2.0f * dl * dl;               // the mean cancels
+                // loads in double: L1 - L2 and w2 - w1 subtract nearly equal numbers that can exceed 2^24
+                const double w1 = p.t.w_e[(size_t)l * p.E + e1], w2 = p.t.w_e[(size_t)l * p.E + e2];
+                const double L1 = p.mp.Lg[(size_t)l * p.G + g1], L2 = p.mp.Lg[(size_t)l * p.G + g2];
+                const double dl = w2 - w1;                                    // moved onto g1
+                dload = (float)(2.0 * dl * (L1 - L2) + 2.0 * dl * dl);        // the mean cancels
                 dcomm = (fabsf(t12.y) - fabsf(t11.y)) + (fabsf(t21.y) - fabsf(t22.y));
                 const float* mt = p.t.m + (size_t)l * p.E * GP;
                 const float m11 = p.has_M ? mt[e1 * GP + g1] : p.M_scalar, m12 = p.has_M ? mt[e1 * GP + g2] : p.M_scalar;
@@ -419,13 +421,13 @@ __global__ void __launch_bounds__(256) move_delta_kernel(const MoveParams p) {
                 // leaving a cell x0 has: +M, leaving a cell x0 lacks: -M; entering: the opposite
                 dmig = (__float_as_int(t11.y) < 0 ? m11 : -m11) + (__float_as_int(t12.y) < 0 ? -m12 : m12) +
                        (__float_as_int(t22.y) < 0 ? m22 : -m22) + (__float_as_int(t21.y) < 0 ? -m21 : m21);
-                const float n1 = L1 + dl, n2 = L2 - dl;
-                float rest = -CUDART_INF_F;
+                const double n1 = L1 + dl, n2 = L2 - dl;
+                double rest = -CUDART_INF;
                 for (int q = 0; q < 3; ++q) {
                     const int tg = p.mp.top_g[l * 4 + q];
                     if (tg >= 0 && tg != g1 && tg != g2) { rest = p.mp.top[l * 4 + q]; break; }
                 }
-                dmax = fmaxf(fmaxf(n1, n2), rest) - p.mp.top[l * 4];
+                dmax = (float)(fmax(fmax(n1, n2), rest) - p.mp.top[l * 4]);
                 dJ = p.alpha * dcomm + p.beta * dload + p.gamma * dmig;
             }
         }

@@ -38,7 +38,9 @@ int launch_gemm_t(const RouteArgs& a) {
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = kCG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
+    ktime_begin(GIMBAL_KERNEL_ROUTER, a.stream);
     CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, ta, tb, p));
+    ktime_end(GIMBAL_KERNEL_ROUTER, a.stream);
     LAUNCH_CHECK("router_gemm_kernel");
     return GIMBAL_OK;
 }
@@ -60,6 +62,7 @@ int launch_gate_t(const RouteArgs& a) {
     const size_t smem = gate_smem_bytes<E, GIMBAL_MAX_TOPK, kWarps>(a.cfg->S);
     if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "gating: E=%d S=%d needs %zu B of shared memory", E, a.cfg->S, smem);
     dim3 grid((a.T + kWarps * 32 - 1) / (kWarps * 32), a.n_layers);
+    ktime_begin(GIMBAL_KERNEL_GATE, a.stream);
     if (a.topk_w) {
         auto kern = gate_hist_kernel<E, GIMBAL_MAX_TOPK, kWarps, true>;
         CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -69,6 +72,7 @@ int launch_gate_t(const RouteArgs& a) {
         CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         kern<<<grid, kWarps * 32, smem, a.stream>>>(p);
     }
+    ktime_end(GIMBAL_KERNEL_GATE, a.stream);
     LAUNCH_CHECK("gate_hist_kernel");
     return GIMBAL_OK;
 }
