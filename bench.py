@@ -58,7 +58,7 @@ class ClockSampler:
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "20",
                                           "-i", str(self.gpu)], stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
@@ -291,7 +291,10 @@ def run_ours(args, w):
     e2e = None
     import psutil
     fits = hidden.numel() * 2 * world < 0.6 * psutil.virtual_memory().total
-    if not fits:
+    if args.no_e2e:
+        fits = False
+        e2e = dict(value=None, unit="routed tokens/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0, error="skipped (--no-e2e)")
+    elif not fits:
         e2e = dict(value=None, unit="routed tokens/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0,
                    error="pinned host copies of the hidden states of all ranks do not fit host RAM")
     else:
@@ -372,13 +375,17 @@ def run_e2e(g, w, cfg, pc, st, hidden, off, cands, W, sb, slb, cur, dp, D, prev,
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="v3", choices=["tiny", "v2lite", "qwen3", "v3", "decode"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    ap.add_argument("--layers", type=int, default=0, help="profiling only: run the first N MoE layers (named in config.workload)")
     args = ap.parse_args()
     w = get_workload(args.workload)
+    if args.layers > 0:
+        w = scaled(w, L=args.layers)
     if args.impl == "reference":
         run_reference(args, w)
     else:

@@ -6,7 +6,7 @@
 
 namespace gimbal {
 
-template <int N, int kCG>
+template <int N, int kCG, bool kSig>
 int launch_gemm_t(const RouteArgs& a) {
     const gimbal_router_cfg* c = a.cfg;
     CUtensorMap ta, tb;
@@ -23,7 +23,7 @@ int launch_gemm_t(const RouteArgs& a) {
     p.do_gate = a.fuse_gate; p.select_bias = a.select_bias; p.topk_ids = a.topk_ids; p.topk_w = a.topk_w;
     p.A_step = a.A_step; p.gp = gate_params(c);
     const size_t smem = gemm_smem_bytes<N, kCG>(c->S, p.stages);
-    auto kern = router_gemm_kernel<N, kCG, GIMBAL_MAX_TOPK>;
+    auto kern = router_gemm_kernel<N, kCG, kSig>;
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int sms = device_info().sms;
     const int n_tiles = p.n_layers * p.m_tiles;
@@ -47,11 +47,22 @@ int launch_gemm_t(const RouteArgs& a) {
 
 template <int N>
 int launch_gemm_n(const RouteArgs& a) {
-    return a.cta_group == 2 ? launch_gemm_t<N, 2>(a) : launch_gemm_t<N, 1>(a);
+    const bool sig = a.cfg->score_fn == GIMBAL_SCORE_SIGMOID;
+    if (a.cta_group == 2) return sig ? launch_gemm_t<N, 2, true>(a) : launch_gemm_t<N, 2, false>(a);
+    return sig ? launch_gemm_t<N, 1, true>(a) : launch_gemm_t<N, 1, false>(a);
 }
 
 
 // ---- standalone gating ---------------------------------------------------------------------
+template <int E, bool kSig, bool kOut>
+int launch_gate_v(const GateKernelParams& p, dim3 grid, size_t smem, cudaStream_t stream) {
+    constexpr int kWarps = 4;
+    auto kern = gate_hist_kernel<E, kSig, kOut, kWarps>;
+    CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<grid, kWarps * 32, smem, stream>>>(p);
+    return GIMBAL_OK;
+}
+
 template <int E>
 int launch_gate_t(const RouteArgs& a) {
     constexpr int kWarps = 4;
@@ -59,25 +70,19 @@ int launch_gate_t(const RouteArgs& a) {
     p.logits = a.logits; p.select_bias = a.select_bias; p.src_offsets = a.src_offsets;
     p.topk_ids = a.topk_ids; p.topk_w = a.topk_w; p.A_step = a.A_step;
     p.layer0 = a.layer0; p.T = a.T; p.S = a.cfg->S; p.gp = gate_params(a.cfg);
-    const size_t smem = gate_smem_bytes<E, GIMBAL_MAX_TOPK, kWarps>(a.cfg->S);
+    const size_t smem = gate_smem_bytes<E, kWarps>(a.cfg->S);
     if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "gating: E=%d S=%d needs %zu B of shared memory", E, a.cfg->S, smem);
     dim3 grid((a.T + kWarps * 32 - 1) / (kWarps * 32), a.n_layers);
+    const bool sig = a.cfg->score_fn == GIMBAL_SCORE_SIGMOID, out = a.topk_ids || a.topk_w;
     ktime_begin(GIMBAL_KERNEL_GATE, a.stream);
-    if (a.topk_w) {
-        auto kern = gate_hist_kernel<E, GIMBAL_MAX_TOPK, kWarps, true>;
-        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kern<<<grid, kWarps * 32, smem, a.stream>>>(p);
-    } else {
-        auto kern = gate_hist_kernel<E, GIMBAL_MAX_TOPK, kWarps, false>;
-        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kern<<<grid, kWarps * 32, smem, a.stream>>>(p);
-    }
+    int rc;
+    if (sig) rc = out ? launch_gate_v<E, true, true>(p, grid, smem, a.stream) : launch_gate_v<E, true, false>(p, grid, smem, a.stream);
+    else rc = out ? launch_gate_v<E, false, true>(p, grid, smem, a.stream) : launch_gate_v<E, false, false>(p, grid, smem, a.stream);
+    if (rc) return rc;
     ktime_end(GIMBAL_KERNEL_GATE, a.stream);
     LAUNCH_CHECK("gate_hist_kernel");
     return GIMBAL_OK;
 }
-
-
 
 #define GIMBAL_DEFINE_E(E)                                                     \
     int launch_gemm_e##E(const RouteArgs& a) { return launch_gemm_n<E>(a); }   \

@@ -69,20 +69,16 @@ struct TmemRowSrc {
     uint32_t taddr;                 // lane base | column base of this accumulator stage
     const float* bias;              // src_logit_bias row for this token (global) | nullptr
     static constexpr int CH = N < 32 ? N : 32;
+    __device__ __forceinline__ void load_raw(int c, uint32_t (&r)[CH]) {
+        if constexpr (CH == 32) ptx::tmem_ld_32x32b_x32(taddr + c * 32, r);
+        else ptx::tmem_ld_32x32b_x16(taddr + c * 16, r);
+        ptx::tmem_ld_wait();
+    }
     __device__ __forceinline__ void load(int c, float (&v)[CH]) {
-        if constexpr (CH == 32) {
-            uint32_t r[32];
-            ptx::tmem_ld_32x32b_x32(taddr + c * 32, r);
-            ptx::tmem_ld_wait();
+        uint32_t r[CH];
+        load_raw(c, r);
 #pragma unroll
-            for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
-        } else {
-            uint32_t r[16];
-            ptx::tmem_ld_32x32b_x16(taddr + c * 16, r);
-            ptx::tmem_ld_wait();
-#pragma unroll
-            for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
-        }
+        for (int i = 0; i < CH; ++i) v[i] = __uint_as_float(r[i]);
         if (bias) {
 #pragma unroll
             for (int i = 0; i < CH; i += 4) {
@@ -92,9 +88,25 @@ struct TmemRowSrc {
             }
         }
     }
+    // order keys overwrite the accumulator columns of this row (the MMA issuer only gets the
+    // stage back after the row is done)
+    __device__ __forceinline__ void store_keys(int c, const int32_t (&o)[CH]) {
+        uint32_t r[CH];
+#pragma unroll
+        for (int i = 0; i < CH; ++i) r[i] = (uint32_t)o[i];
+        if constexpr (CH == 32) ptx::tmem_st_32x32b_x32(taddr + c * 32, r);
+        else ptx::tmem_st_32x32b_x16(taddr + c * 16, r);
+        ptx::tmem_st_wait();
+    }
+    __device__ __forceinline__ void load_keys(int c, int32_t (&o)[CH]) {
+        uint32_t r[CH];
+        load_raw(c, r);
+#pragma unroll
+        for (int i = 0; i < CH; ++i) o[i] = (int32_t)r[i];
+    }
 };
 
-template <int N, int kCG, int KMAX>
+template <int N, int kCG, bool kSig>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b, const GemmParams p) {
     const int kStages = p.stages;
@@ -233,8 +245,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
                     }
                 }
                 for (int i = ep_tid; i < p.S * N; i += 128) hist[i] = 0;
-                if (p.select_bias)
-                    for (int i = ep_tid; i < N; i += 128) sb_s[i] = p.select_bias[(size_t)layer * N + i];
+                for (int i = ep_tid; i < N; i += 128) sb_s[i] = p.select_bias ? p.select_bias[(size_t)layer * N + i] : 0.0f;
                 cur_layer = layer;
                 asm volatile("bar.sync 1, 128;" ::: "memory");
             }
@@ -259,26 +270,25 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
                 }
             }
             if (p.do_gate) {
-                int32_t ids[KMAX];
-                float w[KMAX];
-                if (p.topk_w) gate_row<N, KMAX, true>(p.gp, p.select_bias ? sb_s : nullptr, src, ids, w);
-                else gate_row<N, KMAX, false>(p.gp, p.select_bias ? sb_s : nullptr, src, ids, w);
-                if (t < p.T) {
-#pragma unroll
-                    for (int j = 0; j < KMAX; ++j)
-                        if (j < p.gp.k) atomicAdd(&hist[s * N + ids[j]], 1);
-                    if (p.topk_ids) {
+                int32_t ids[kTopK];
+                float w[kTopK];
+                const bool valid = t < p.T;
+                if (p.topk_ids || p.topk_w) {
+                    gate_row<N, kSig, true>(p.gp, sb_s, src, valid, hist + s * N, ids, w);
+                    if (valid && p.topk_ids) {
                         int32_t* o = p.topk_ids + ((size_t)li * p.T + t) * p.gp.k;
 #pragma unroll
-                        for (int j = 0; j < KMAX; ++j)
+                        for (int j = 0; j < kTopK; ++j)
                             if (j < p.gp.k) o[j] = ids[j];
                     }
-                    if (p.topk_w) {
+                    if (valid && p.topk_w) {
                         float* o = p.topk_w + ((size_t)li * p.T + t) * p.gp.k;
 #pragma unroll
-                        for (int j = 0; j < KMAX; ++j)
+                        for (int j = 0; j < kTopK; ++j)
                             if (j < p.gp.k) o[j] = w[j];
                     }
+                } else {
+                    gate_row<N, kSig, false>(p.gp, sb_s, src, valid, hist + s * N, ids, w);
                 }
             }
             // release this accumulator stage to the MMA issuer
