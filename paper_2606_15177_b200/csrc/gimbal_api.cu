@@ -166,15 +166,21 @@ static int launch_tables(const gimbal_placement_cfg* c, const void* A, const voi
     return GIMBAL_OK;
 }
 
-template <int SP>
-static int launch_score(const ScoreParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
-    auto kern = place_score_kernel<SP>;
+template <int SP, bool kDup, bool kHasM>
+static int launch_score_v(const ScoreParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
+    auto kern = place_score_kernel<SP, kDup, kHasM>;
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ktime_begin(GIMBAL_KERNEL_SCORE, stream);
     kern<<<grid, kScoreThreads, smem, stream>>>(sp);
     ktime_end(GIMBAL_KERNEL_SCORE, stream);
     LAUNCH_CHECK("place_score_kernel");
     return GIMBAL_OK;
+}
+
+template <int SP>
+static int launch_score(const ScoreParams& sp, bool dup, dim3 grid, size_t smem, cudaStream_t stream) {
+    if (sp.has_M) return dup ? launch_score_v<SP, true, true>(sp, grid, smem, stream) : launch_score_v<SP, false, true>(sp, grid, smem, stream);
+    return dup ? launch_score_v<SP, true, false>(sp, grid, smem, stream) : launch_score_v<SP, false, false>(sp, grid, smem, stream);
 }
 
 }  // namespace
@@ -381,19 +387,24 @@ int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const int16_t
         ScoreParams sp{};
         sp.P = P; sp.L = cfg->L; sp.E = cfg->E; sp.G = cfg->G; sp.sp = cfg->slots_per_rank; sp.M_scalar = M_scalar; sp.has_M = M != nullptr;
         sp.cand = candidates; sp.t = w.t; sp.partial = w.partial;
+        // one wave: two resident blocks per SM (one when the table needs more than half the shared memory)
         const int sms = device_info().sms;
-        int nchunk = (2 * sms + cfg->L - 1) / cfg->L;
+        const int per_sm = 2 * smem + 2048 <= kSmemLimit ? 2 : 1;
+        int nchunk = per_sm * sms / cfg->L;
         const int units_per_pass = (kScoreThreads / 32) * (cfg->G < 32 ? 32 / cfg->G : 1);
         int max_chunks = (P + units_per_pass - 1) / units_per_pass;
         if (nchunk > max_chunks) nchunk = max_chunks;
         if (nchunk < 1) nchunk = 1;
         sp.chunk = (P + nchunk - 1) / nchunk;
         dim3 grid((P + sp.chunk - 1) / sp.chunk, cfg->L);
-        switch (cfg->slots_per_rank) {
-            case 4: rc = launch_score<4>(sp, grid, smem, stream); break;
-            case 8: rc = launch_score<8>(sp, grid, smem, stream); break;
-            case 9: rc = launch_score<9>(sp, grid, smem, stream); break;
-            default: rc = launch_score<0>(sp, grid, smem, stream); break;
+        const bool dup = cfg->G * cfg->slots_per_rank > cfg->E;
+        const int NS = cfg->G * cfg->slots_per_rank;
+        const int spk = (cfg->G >= 2 && NS % 2 == 0) ? cfg->slots_per_rank : 0;   // packed-word loads need aligned rows
+        switch (spk) {
+            case 4: rc = launch_score<4>(sp, dup, grid, smem, stream); break;
+            case 8: rc = launch_score<8>(sp, dup, grid, smem, stream); break;
+            case 9: rc = launch_score<9>(sp, dup, grid, smem, stream); break;
+            default: rc = launch_score<0>(sp, dup, grid, smem, stream); break;
         }
         if (rc) return rc;
         FinalizeParams fp{};
@@ -460,7 +471,24 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
         fill_u64_kernel<<<(cfg->L + 255) / 256, 256, 0, stream>>>(w.best, ~0ull, cfg->L);
         LAUNCH_CHECK("fill_u64_kernel");
     }
-    if (n_moves > 0) {
+    if (n_moves > 0 && !moves) {
+        // implicit neighbourhood: blocks of ~2048 pair indices of one layer, tables staged in shared memory
+        MoveAllParams ap{};
+        ap.L = cfg->L; ap.E = cfg->E; ap.G = cfg->G; ap.sp = cfg->slots_per_rank; ap.has_M = M != nullptr;
+        ap.alpha = cfg->alpha; ap.beta = cfg->beta; ap.gamma = cfg->gamma; ap.M_scalar = M_scalar;
+        ap.cur = cur; ap.t = w.t; ap.mp = w.mp; ap.delta = delta; ap.best = best_per_layer ? w.best : nullptr;
+        const long long npairs = NS * (NS - 1) / 2;
+        int bpl = (int)((npairs + 2047) / 2048);
+        ap.pairs_per_block = (int)(((npairs + bpl - 1) / bpl + kMoveAllThreads - 1) / kMoveAllThreads) * kMoveAllThreads;
+        bpl = (int)((npairs + ap.pairs_per_block - 1) / ap.pairs_per_block);
+        const size_t smem = move_all_smem_bytes((int)NS, cfg->G, ap.has_M);
+        if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "move neighbourhood: NS=%lld G=%d needs %zu B of shared memory", NS, cfg->G, smem);
+        CUDA_TRY(cudaFuncSetAttribute(move_all_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ktime_begin(GIMBAL_KERNEL_MOVES, stream);
+        move_all_kernel<<<dim3(bpl, cfg->L), kMoveAllThreads, smem, stream>>>(ap);
+        ktime_end(GIMBAL_KERNEL_MOVES, stream);
+        LAUNCH_CHECK("move_all_kernel");
+    } else if (n_moves > 0) {
         MoveParams mp{};
         mp.L = cfg->L; mp.E = cfg->E; mp.G = cfg->G; mp.sp = cfg->slots_per_rank; mp.n_moves = n_moves; mp.moves = moves; mp.cur = cur;
         mp.alpha = cfg->alpha; mp.beta = cfg->beta; mp.gamma = cfg->gamma; mp.M_scalar = M_scalar; mp.has_M = M != nullptr;

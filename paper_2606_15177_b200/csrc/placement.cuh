@@ -41,10 +41,10 @@ struct PlaceTables {
 
 __host__ __device__ inline int place_gp(int G) { return G < 32 ? 32 : G; }
 
+// multiset checksum term of one slot: two integer multiply-adds in the scoring loop; injective on [0, 256)
 __device__ __forceinline__ uint32_t slot_hash(uint32_t e) {
-    uint32_t h = (e + 1u) * 0x9E3779B1u;
-    h ^= h >> 15;
-    return h * 0x85EBCA77u;
+    const uint32_t t = e * 0x9E3779B1u + 0x7F4A7C15u;
+    return t * t;
 }
 
 struct TableParams {
@@ -133,30 +133,56 @@ struct ScoreParams {
 
 constexpr int kScoreThreads = 512;
 
+// The slots of one rank as 16-bit ids packed two per word, SP = slots per rank (0: runtime sp,
+// scalar loads).  `row` points at the first slot of the candidate's layer row, g is the rank.
 template <int SP>
-__device__ __forceinline__ void load_slots(const int16_t* g, int sp, int (&e)[16]) {
-    // this lane's SP consecutive int16 slots
-    if constexpr (SP == 8) {
-        const uint4 q = __ldcs(reinterpret_cast<const uint4*>(g));
-        e[0] = (int16_t)(q.x & 0xffff); e[1] = (int16_t)(q.x >> 16); e[2] = (int16_t)(q.y & 0xffff); e[3] = (int16_t)(q.y >> 16);
-        e[4] = (int16_t)(q.z & 0xffff); e[5] = (int16_t)(q.z >> 16); e[6] = (int16_t)(q.w & 0xffff); e[7] = (int16_t)(q.w >> 16);
-    } else if constexpr (SP == 4) {
-        const uint2 q = __ldcs(reinterpret_cast<const uint2*>(g));
-        e[0] = (int16_t)(q.x & 0xffff); e[1] = (int16_t)(q.x >> 16); e[2] = (int16_t)(q.y & 0xffff); e[3] = (int16_t)(q.y >> 16);
-    } else {
+struct RankSlots {
+    static constexpr int NW = SP == 0 ? 8 : (SP + 1) / 2;   // words fetched
+    uint32_t w[NW];
+    __device__ __forceinline__ void load(const int16_t* row, int g, int sp) {
+        if constexpr (SP == 8) {
+            const uint4 q = __ldcs(reinterpret_cast<const uint4*>(row + g * 8));
+            w[0] = q.x; w[1] = q.y; w[2] = q.z; w[3] = q.w;
+        } else if constexpr (SP == 4) {
+            const uint2 q = __ldcs(reinterpret_cast<const uint2*>(row + g * 4));
+            w[0] = q.x; w[1] = q.y;
+        } else if constexpr (SP == 0) {
 #pragma unroll
-        for (int j = 0; j < 16; ++j)
-            if (j < sp) e[j] = __ldcs(g + j);
+            for (int j = 0; j < 8; ++j) {
+                const uint32_t lo = 2 * j < sp ? (uint16_t)__ldcs(row + g * sp + 2 * j) : 0xffffu;
+                const uint32_t hi = 2 * j + 1 < sp ? (uint16_t)__ldcs(row + g * sp + 2 * j + 1) : 0xffffu;
+                w[j] = lo | (hi << 16);
+            }
+        } else {
+            // odd SP: the rank's slots start on a word boundary for even g and in the middle of a
+            // word for odd g; fetch the NW aligned words that cover them (rows are 4-byte aligned
+            // because NS * 2 is)
+            const uint32_t* base = reinterpret_cast<const uint32_t*>(row) + ((g * SP) >> 1);
+#pragma unroll
+            for (int j = 0; j < NW; ++j) w[j] = __ldcs(base + j);
+        }
     }
-}
+    // id of slot j of the rank (g only matters for odd SP)
+    __device__ __forceinline__ uint32_t id(int j, int g) const {
+        if constexpr (SP == 0 || SP % 2 == 0) {
+            return (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu);
+        } else {
+            // odd g: slot j sits at half-word j + 1 of the fetched words
+            const uint32_t even = (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu);
+            const uint32_t odd = ((j + 1) & 1) ? (w[(j + 1) >> 1] >> 16) : (w[(j + 1) >> 1] & 0xffffu);
+            return (g & 1) ? odd : even;
+        }
+    }
+};
 
-// SP: compile-time slots per rank (0 = generic, runtime p.sp <= 16)
-template <int SP>
-__global__ void __launch_bounds__(kScoreThreads, 1) place_score_kernel(const ScoreParams p) {
+// SP: compile-time slots per rank (0 = generic, runtime p.sp <= 16); kDup: NS > E, so a rank can
+// hold the same expert twice and the per-rank duplicate check is needed; kHasM: M table.
+template <int SP, bool kDup, bool kHasM>
+__global__ void __launch_bounds__(kScoreThreads, SP == 0 ? 1 : 2) place_score_kernel(const ScoreParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int GP = place_gp(p.G);
     float2* wc_s = reinterpret_cast<float2*>(smem_raw);                       // [E][GP]
-    float* m_s = reinterpret_cast<float*>(smem_raw + sizeof(float2) * (size_t)p.E * GP);   // [E][GP] (has_M)
+    float* m_s = reinterpret_cast<float*>(smem_raw + sizeof(float2) * (size_t)p.E * GP);   // [E][GP] (kHasM)
     const int l = blockIdx.y;
     const int NS = p.G * p.sp;
     const int sp = SP > 0 ? SP : p.sp;
@@ -164,7 +190,7 @@ __global__ void __launch_bounds__(kScoreThreads, 1) place_score_kernel(const Sco
         const uint4* src = reinterpret_cast<const uint4*>(p.t.wc + (size_t)l * p.E * GP);
         uint4* dst = reinterpret_cast<uint4*>(wc_s);
         for (int i = threadIdx.x; i < p.E * GP / 2; i += kScoreThreads) dst[i] = src[i];
-        if (p.has_M) {
+        if constexpr (kHasM) {
             const uint4* ms = reinterpret_cast<const uint4*>(p.t.m + (size_t)l * p.E * GP);
             uint4* md = reinterpret_cast<uint4*>(m_s);
             for (int i = threadIdx.x; i < p.E * GP / 4; i += kScoreThreads) md[i] = ms[i];
@@ -173,75 +199,97 @@ __global__ void __launch_bounds__(kScoreThreads, 1) place_score_kernel(const Sco
     __syncthreads();
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int upw = p.G < 32 ? 32 / p.G : 1;            // (candidate, layer) units per warp
+    const int seg = p.G < 32 ? p.G : 32;                // lanes of one (candidate, layer) unit
+    const int upw = 32 / seg;                           // units per warp
     const int rpl = p.G > 32 ? p.G / 32 : 1;            // ranks per lane
-    const int sub = p.G < 32 ? lane / p.G : 0;
-    const int g0 = p.G < 32 ? lane % p.G : lane;
+    const int sub = lane / seg;
+    const int g0 = lane % seg;
+    const uint32_t seg_mask = seg == 32 ? 0xffffffffu : (((1u << seg) - 1u) << (sub * seg));
     const double Gd = (double)p.G;
     const double sumB = p.t.sumB[l];
     const uint32_t want_hash = p.t.hsum[l];
     const float base_mig = p.t.base_mig[l];
-    const bool check_dup = NS > p.E;                    // with NS == E the multiset check already implies it
+    const uint32_t emax = (uint32_t)p.E - 1u;
+    const int col = p.G < 32 ? lane : g0;               // table column of this lane (rank g0 + 32*rr -> col + 32*rr)
 
     const int p_begin = blockIdx.x * p.chunk, p_end = min(p.P, p_begin + p.chunk);
-    for (int pc = p_begin + warp * upw; pc < p_end; pc += (kScoreThreads / 32) * upw) {
+    const int stride = (kScoreThreads / 32) * upw;
+    RankSlots<SP> cur, nxt;
+    int pc = p_begin + warp * upw;
+    if (pc + sub < p_end && rpl == 1) cur.load(p.cand + ((size_t)(pc + sub) * p.L + l) * NS, g0, sp);
+    for (; pc < p_end; pc += stride) {
         const int cand = pc + sub;
         const bool active = cand < p_end;
-        float sq = 0.0f, comm = 0.0f, mig_in = 0.0f, mig_kept = 0.0f, mx = -CUDART_INF_F;
-        uint32_t hs = 0;
-        int bad = 0;
+        if (rpl == 1 && cand + stride < p_end) nxt.load(p.cand + ((size_t)(cand + stride) * p.L + l) * NS, g0, sp);
+        float sq = 0.0f, comm = 0.0f, mig_in = 0.0f, mig_kept = 0.0f, mx = 0.0f;
+        uint32_t hs = 0, orall = 0, kept = 0;
+        bool dup = false;
         if (active) {
-            const int16_t* row = p.cand + ((size_t)cand * p.L + l) * NS;
             for (int rr = 0; rr < rpl; ++rr) {
                 const int g = g0 + rr * 32;
-                int e[16];
-                load_slots<SP>(row + g * sp, sp, e);
+                if (rpl > 1) cur.load(p.cand + ((size_t)cand * p.L + l) * NS, g, sp);
+                uint32_t e[SP == 0 ? 16 : SP];
                 float lg = 0.0f;
 #pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    if (j < sp) {
-                        int x = e[j];
-                        if ((unsigned)x >= (unsigned)p.E) { bad = 1; x = 0; }
-                        hs += slot_hash((uint32_t)x);
-                        const int idx = x * GP + (p.G < 32 ? lane : g);
+                for (int j = 0; j < (SP == 0 ? 16 : SP); ++j) {
+                    if (SP != 0 || j < sp) {
+                        const uint32_t raw = cur.id(j, g);
+                        orall |= raw > emax ? 1u : 0u;
+                        const uint32_t x = min(raw, emax);
+                        e[j] = x;
+                        hs += slot_hash(x);
+                        const int idx = x * GP + col + rr * 32;
                         const float2 wc = wc_s[idx];
                         lg += wc.x;
                         comm += fabsf(wc.y);
-                        const bool member = __float_as_int(wc.y) < 0;
-                        const float mm = p.has_M ? m_s[idx] : p.M_scalar;
-                        if (member) mig_kept += mm; else mig_in += mm;     // retained / entering cell of x0
-                    }
+                        const uint32_t member = __float_as_uint(wc.y) >> 31;
+                        kept += member;
+                        if constexpr (kHasM) {
+                            const float mm = m_s[idx];
+                            if (member) mig_kept += mm; else mig_in += mm;     // retained / entering cell of x0
+                        }
+                    } else e[j] = 0xffff0000u + j;
                 }
-                if (check_dup) {
+                if constexpr (kDup) {
 #pragma unroll
-                    for (int a = 0; a < 16; ++a)
+                    for (int a = 0; a < (SP == 0 ? 16 : SP); ++a)
 #pragma unroll
-                        for (int b = a + 1; b < 16; ++b)
-                            if (b < sp) bad |= (e[a] == e[b]);
+                        for (int b = a + 1; b < (SP == 0 ? 16 : SP); ++b) dup |= (e[a] == e[b]);
                 }
                 const float d = (float)((double)lg * Gd - sumB);  // G*L_g - sum_g L_g, exact difference for integer counts
                 sq = __fmaf_rn(d, d, sq);
                 mx = fmaxf(mx, lg);
             }
         }
-        // reduce over the lanes of this unit (segments of min(G,32) lanes)
-        const int seg = p.G < 32 ? p.G : 32;
-        for (int o = seg >> 1; o > 0; o >>= 1) {
-            sq += __shfl_xor_sync(0xffffffffu, sq, o);
-            comm += __shfl_xor_sync(0xffffffffu, comm, o);
-            mig_in += __shfl_xor_sync(0xffffffffu, mig_in, o);
-            mig_kept += __shfl_xor_sync(0xffffffffu, mig_kept, o);
-            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-            hs += __shfl_xor_sync(0xffffffffu, hs, o);
-            bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+        // reduce over the `seg` lanes of this unit: integers with redux, the two float sums with a
+        // transposed butterfly (first step folds both values into one register)
+        hs = __reduce_add_sync(seg_mask, hs);
+        kept = __reduce_add_sync(seg_mask, kept);
+        const uint32_t bad = __reduce_or_sync(seg_mask, orall | (dup ? 1u : 0u));
+        const float mxa = __uint_as_float(__reduce_max_sync(seg_mask, __float_as_uint(mx)));   // loads are >= 0
+        float commt = comm;
+        if (seg > 1) {
+            const int h = seg >> 1;
+            const bool up = (lane & h) != 0;
+            float v = (up ? comm : sq) + __shfl_xor_sync(0xffffffffu, up ? sq : comm, h);
+            for (int o = h >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            commt = __shfl_sync(0xffffffffu, v, sub * seg + h);
+            sq = v;                                                                  // valid on unit lanes with bit h clear
+        }
+        if constexpr (kHasM) {
+            for (int o = seg >> 1; o > 0; o >>= 1) {
+                mig_in += __shfl_xor_sync(0xffffffffu, mig_in, o);
+                mig_kept += __shfl_xor_sync(0xffffffffu, mig_kept, o);
+            }
         }
         if (active && g0 == 0) {
-            if (hs != want_hash) bad = 1;
             // C_mig = entering cells + (x0's cells - retained cells); exact for a scalar M
-            float4 out = make_float4(sq, comm, mig_in + (base_mig - mig_kept), mx);
-            if (bad) out.x = CUDART_NAN_F;
+            const float mig = kHasM ? mig_in + (base_mig - mig_kept) : p.M_scalar * (float)(2 * (NS - (int)kept));
+            float4 out = make_float4(sq, commt, mig, mxa);
+            if (bad || hs != want_hash) out.x = CUDART_NAN_F;
             p.partial[(size_t)cand * p.L + l] = out;
         }
+        if (rpl == 1) cur = nxt;
     }
 }
 
@@ -434,9 +482,154 @@ __global__ void __launch_bounds__(256) move_delta_kernel(const MoveParams p) {
     }
     if (nan) dJ = dload = dcomm = dmig = dmax = CUDART_NAN_F;
     out[0] = dJ; out[1] = dload; out[2] = dcomm; out[3] = dmig; out[4] = dmax;
-    if (p.best && !nan) {
-        const unsigned long long key = ((unsigned long long)ordered_u32(dJ + 0.0f) << 32) | (unsigned long long)(uint32_t)(i & 0xffffffffll);
-        atomicMin(p.best + l, key);
+    if (p.best) {
+        unsigned long long key = nan ? ~0ull : ((unsigned long long)ordered_u32(dJ + 0.0f) << 32) | (unsigned long long)(uint32_t)(i & 0xffffffffll);
+        const unsigned act = __activemask();
+        const int l0 = __shfl_sync(act, l, __ffs(act) - 1);
+        if (act == 0xffffffffu && __all_sync(act, l == l0)) {      // one atomic per warp instead of 32 on one address
+            for (int o = 16; o > 0; o >>= 1) {
+                const unsigned long long other = __shfl_xor_sync(0xffffffffu, key, o);
+                key = other < key ? other : key;
+            }
+            if ((threadIdx.x & 31) == 0 && key != ~0ull) atomicMin(p.best + l, key);
+        } else if (key != ~0ull) {
+            atomicMin(p.best + l, key);
+        }
+    }
+}
+
+// The whole neighbourhood of `cur` in canonical order (l, a < b): one block per (layer, range of
+// pair indices).  The layer's per-slot rows -- communication cost of the slot's expert on every
+// rank (sign = x0 hosts it there), its load share, the ranks hosting it -- are staged in shared
+// memory (pitch G+1: lanes walk b, so rows fall in distinct banks); a warp's 32 results are
+// staged too and leave as five fully coalesced 128-byte stores.
+constexpr int kMoveAllThreads = 256;
+
+__host__ __device__ inline size_t move_all_smem_bytes(int NS, int G, int has_M) {
+    size_t b = sizeof(float) * (size_t)NS * (G + 1) * (has_M ? 2 : 1);   // Cs (+ Ms)
+    b = (b + 15) & ~size_t(15);
+    b += sizeof(double) * NS + sizeof(unsigned long long) * NS + sizeof(int2) * NS;   // w, cmask, (e, g)
+    b += sizeof(double) * 64;                                                       // Lg
+    b += sizeof(float) * (kMoveAllThreads / 32) * 160;                              // output staging
+    b += sizeof(unsigned long long) * (kMoveAllThreads / 32);                       // block argmin
+    return b;
+}
+
+struct MoveAllParams {
+    int L, E, G, sp, has_M;
+    int pairs_per_block;
+    float alpha, beta, gamma, M_scalar;
+    const int16_t* cur;
+    PlaceTables t;
+    MovePrep mp;
+    float* delta;                       // [L * NS*(NS-1)/2, 5]
+    unsigned long long* best;           // [L] | nullptr
+};
+
+__global__ void __launch_bounds__(kMoveAllThreads) move_all_kernel(const MoveAllParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int NS = p.G * p.sp, GP = place_gp(p.G), PITCH = p.G + 1;
+    const int l = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    float* Cs = reinterpret_cast<float*>(smem_raw);
+    float* Ms = Cs + (size_t)NS * PITCH;
+    size_t off = sizeof(float) * (size_t)NS * PITCH * (p.has_M ? 2 : 1);
+    off = (off + 15) & ~size_t(15);
+    double* ws = reinterpret_cast<double*>(smem_raw + off); off += sizeof(double) * NS;
+    unsigned long long* cms = reinterpret_cast<unsigned long long*>(smem_raw + off); off += sizeof(unsigned long long) * NS;
+    int2* eg = reinterpret_cast<int2*>(smem_raw + off); off += sizeof(int2) * NS;
+    double* Lgs = reinterpret_cast<double*>(smem_raw + off); off += sizeof(double) * 64;
+    float* stage = reinterpret_cast<float*>(smem_raw + off) + warp * 160; off += sizeof(float) * (kMoveAllThreads / 32) * 160;
+    unsigned long long* bests = reinterpret_cast<unsigned long long*>(smem_raw + off);
+
+    const int npairs = NS * (NS - 1) / 2;
+    const bool poisoned = (*p.mp.bad != 0) || (*p.t.bad != 0);
+    const int16_t* cu = p.cur + (size_t)l * NS;
+    for (int j = tid; j < NS; j += kMoveAllThreads) {
+        int e = cu[j];
+        if (e < 0 || e >= p.E) e = 0;                                  // flagged by move_prep_kernel
+        eg[j] = make_int2(e, j / p.sp);
+        ws[j] = p.t.w_e[(size_t)l * p.E + e];
+        cms[j] = p.mp.cmask[(size_t)l * p.E + e];
+    }
+    if (tid < p.G) Lgs[tid] = p.mp.Lg[(size_t)l * p.G + tid];
+    __syncthreads();
+    for (int i = tid; i < NS * p.G; i += kMoveAllThreads) {
+        const int j = i / p.G, g = i - j * p.G;
+        const size_t src = ((size_t)l * p.E + eg[j].x) * GP + g;
+        Cs[j * PITCH + g] = p.t.wc[src].y;
+        if (p.has_M) Ms[j * PITCH + g] = p.t.m[src];
+    }
+    __syncthreads();
+    double top[3]; int top_g[3];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) { top[q] = p.mp.top[l * 4 + q]; top_g[q] = p.mp.top_g[l * 4 + q]; }
+
+    const int r_begin = blockIdx.x * p.pairs_per_block, r_end = min(npairs, r_begin + p.pairs_per_block);
+    const float two_ns_1 = 2.0f * NS - 1.0f;
+    unsigned long long best = ~0ull;
+    for (int rb = r_begin + warp * 32; rb < r_end; rb += kMoveAllThreads) {
+        const int r = rb + lane;
+        float dJ = 0.0f, dload = 0.0f, dcomm = 0.0f, dmig = 0.0f, dmax = 0.0f;
+        bool nan = poisoned;
+        if (r < r_end && !nan) {
+            // canonical order: a outer, b inner, a < b.  Row a starts at a*NS - a*(a+1)/2.
+            int a = (int)((two_ns_1 - sqrtf(two_ns_1 * two_ns_1 - 8.0f * (float)r)) * 0.5f);
+            a = max(0, min(a, NS - 2));
+            while (a * NS - a * (a + 1) / 2 > r) --a;
+            while ((a + 1) * NS - (a + 1) * (a + 2) / 2 <= r) ++a;
+            const int b = r - (a * NS - a * (a + 1) / 2) + a + 1;
+            const int2 s1 = eg[a], s2 = eg[b];
+            const int e1 = s1.x, e2 = s2.x, g1 = s1.y, g2 = s2.y;
+            if (g1 != g2 && e1 != e2) {
+                if (((cms[a] >> g2) & 1ull) || ((cms[b] >> g1) & 1ull)) nan = true;      // second copy on a rank
+                else {
+                    const float t11 = Cs[a * PITCH + g1], t12 = Cs[a * PITCH + g2], t21 = Cs[b * PITCH + g1], t22 = Cs[b * PITCH + g2];
+                    // loads in double: L1 - L2 and w2 - w1 subtract nearly equal numbers that can exceed 2^24
+                    const double L1 = Lgs[g1], L2 = Lgs[g2];
+                    const double dl = ws[b] - ws[a];                              // moved onto g1
+                    dload = (float)(2.0 * dl * (L1 - L2) + 2.0 * dl * dl);        // the mean cancels
+                    dcomm = (fabsf(t12) - fabsf(t11)) + (fabsf(t21) - fabsf(t22));
+                    const float m11 = p.has_M ? Ms[a * PITCH + g1] : p.M_scalar, m12 = p.has_M ? Ms[a * PITCH + g2] : p.M_scalar;
+                    const float m21 = p.has_M ? Ms[b * PITCH + g1] : p.M_scalar, m22 = p.has_M ? Ms[b * PITCH + g2] : p.M_scalar;
+                    // leaving a cell x0 has: +M, leaving a cell x0 lacks: -M; entering: the opposite
+                    dmig = (__float_as_int(t11) < 0 ? m11 : -m11) + (__float_as_int(t12) < 0 ? -m12 : m12) +
+                           (__float_as_int(t22) < 0 ? m22 : -m22) + (__float_as_int(t21) < 0 ? -m21 : m21);
+                    const double n1 = L1 + dl, n2 = L2 - dl;
+                    double rest = -CUDART_INF;
+#pragma unroll
+                    for (int q = 2; q >= 0; --q)
+                        if (top_g[q] >= 0 && top_g[q] != g1 && top_g[q] != g2) rest = top[q];
+                    dmax = (float)(fmax(fmax(n1, n2), rest) - top[0]);
+                    dJ = p.alpha * dcomm + p.beta * dload + p.gamma * dmig;
+                }
+            }
+        }
+        if (nan) dJ = dload = dcomm = dmig = dmax = CUDART_NAN_F;
+        if (r < r_end && !nan && p.best) {
+            const unsigned long long key = ((unsigned long long)ordered_u32(dJ + 0.0f) << 32) | (unsigned long long)(uint32_t)(l * npairs + r);
+            best = key < best ? key : best;
+        }
+        // stage the warp's 32 x 5 results, then write them as contiguous words
+        stage[lane * 5 + 0] = dJ; stage[lane * 5 + 1] = dload; stage[lane * 5 + 2] = dcomm; stage[lane * 5 + 3] = dmig; stage[lane * 5 + 4] = dmax;
+        __syncwarp();
+        const int n_out = min(32, r_end - rb) * 5;
+        float* out = p.delta + ((size_t)l * npairs + rb) * 5;
+#pragma unroll
+        for (int q = 0; q < 5; ++q)
+            if (q * 32 + lane < n_out) __stcs(out + q * 32 + lane, stage[q * 32 + lane]);
+        __syncwarp();
+    }
+    if (p.best) {
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long other = __shfl_xor_sync(0xffffffffu, best, o);
+            best = other < best ? other : best;
+        }
+        if (lane == 0) bests[warp] = best;
+        __syncthreads();
+        if (tid == 0) {
+            for (int w = 1; w < kMoveAllThreads / 32; ++w) best = bests[w] < best ? bests[w] : best;
+            if (best != ~0ull) atomicMin(p.best + l, best);
+        }
     }
 }
 
