@@ -177,10 +177,26 @@ static int launch_score_v(const ScoreParams& sp, dim3 grid, size_t smem, cudaStr
     return GIMBAL_OK;
 }
 
-template <int SP>
-static int launch_score(const ScoreParams& sp, bool dup, dim3 grid, size_t smem, cudaStream_t stream) {
-    if (sp.has_M) return dup ? launch_score_v<SP, true, true>(sp, grid, smem, stream) : launch_score_v<SP, false, true>(sp, grid, smem, stream);
-    return dup ? launch_score_v<SP, true, false>(sp, grid, smem, stream) : launch_score_v<SP, false, false>(sp, grid, smem, stream);
+static int launch_score_generic(const ScoreParams& sp, bool dup, dim3 grid, size_t smem, cudaStream_t stream) {
+    if (sp.has_M) return dup ? launch_score_v<0, true, true>(sp, grid, smem, stream) : launch_score_v<0, false, true>(sp, grid, smem, stream);
+    return dup ? launch_score_v<0, true, false>(sp, grid, smem, stream) : launch_score_v<0, false, false>(sp, grid, smem, stream);
+}
+
+template <int SP, int G, bool kDup, bool kHasM>
+static int launch_score_fast_v(const ScoreParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
+    auto kern = place_score_fast_kernel<SP, G, kDup, kHasM>;
+    CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ktime_begin(GIMBAL_KERNEL_SCORE, stream);
+    kern<<<grid, kScoreThreads, smem, stream>>>(sp);
+    ktime_end(GIMBAL_KERNEL_SCORE, stream);
+    LAUNCH_CHECK("place_score_fast_kernel");
+    return GIMBAL_OK;
+}
+
+template <int SP, int G>
+static int launch_score_fast(const ScoreParams& sp, bool dup, dim3 grid, size_t smem, cudaStream_t stream) {
+    if (sp.has_M) return dup ? launch_score_fast_v<SP, G, true, true>(sp, grid, smem, stream) : launch_score_fast_v<SP, G, false, true>(sp, grid, smem, stream);
+    return dup ? launch_score_fast_v<SP, G, true, false>(sp, grid, smem, stream) : launch_score_fast_v<SP, G, false, false>(sp, grid, smem, stream);
 }
 
 }  // namespace
@@ -398,13 +414,17 @@ int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const int16_t
         sp.chunk = (P + nchunk - 1) / nchunk;
         dim3 grid((P + sp.chunk - 1) / sp.chunk, cfg->L);
         const bool dup = cfg->G * cfg->slots_per_rank > cfg->E;
-        const int NS = cfg->G * cfg->slots_per_rank;
-        const int spk = (cfg->G >= 2 && NS % 2 == 0) ? cfg->slots_per_rank : 0;   // packed-word loads need aligned rows
-        switch (spk) {
-            case 4: rc = launch_score<4>(sp, dup, grid, smem, stream); break;
-            case 8: rc = launch_score<8>(sp, dup, grid, smem, stream); break;
-            case 9: rc = launch_score<9>(sp, dup, grid, smem, stream); break;
-            default: rc = launch_score<0>(sp, dup, grid, smem, stream); break;
+        // the five configuration shapes have specialised kernels (E must be a power of two there)
+        const bool pow2E = (cfg->E & (cfg->E - 1)) == 0;
+        const char* force = getenv("GIMBAL_SCORE_GENERIC");     // tests: run the generic kernel on a specialised shape
+        const int key = (pow2E && !(force && atoi(force))) ? cfg->slots_per_rank * 100 + cfg->G : 0;
+        switch (key) {
+            case 932: rc = launch_score_fast<9, 32>(sp, dup, grid, smem, stream); break;
+            case 816: rc = launch_score_fast<8, 16>(sp, dup, grid, smem, stream); break;
+            case 808: rc = launch_score_fast<8, 8>(sp, dup, grid, smem, stream); break;
+            case 464: rc = launch_score_fast<4, 64>(sp, dup, grid, smem, stream); break;
+            case 404: rc = launch_score_fast<4, 4>(sp, dup, grid, smem, stream); break;
+            default: rc = launch_score_generic(sp, dup, grid, smem, stream); break;
         }
         if (rc) return rc;
         FinalizeParams fp{};

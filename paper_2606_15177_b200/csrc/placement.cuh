@@ -293,6 +293,157 @@ __global__ void __launch_bounds__(kScoreThreads, SP == 0 ? 1 : 2) place_score_ke
     }
 }
 
+// Specialised scoring kernel for compile-time (slots per rank, ranks) and a power-of-two E:
+// ids are fetched as aligned 32-bit words (two per word), the range check is one OR per word,
+// the cross-lane reductions are fully unrolled.  Same results, bit for bit, as the generic kernel.
+template <int SP, int G, bool kDup, bool kHasM>
+__global__ void __launch_bounds__(kScoreThreads, 2) place_score_fast_kernel(const ScoreParams p) {
+    constexpr int GP = G < 32 ? 32 : G;
+    constexpr int SEG = G < 32 ? G : 32, UPW = 32 / SEG, RPL = G > 32 ? G / 32 : 1;
+    constexpr int NS = G * SP;
+    constexpr int NW = (SP + 1) / 2;                    // words holding one rank's ids
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2* wc_s = reinterpret_cast<float2*>(smem_raw);                       // [E][GP]
+    float* m_s = reinterpret_cast<float*>(smem_raw + sizeof(float2) * (size_t)p.E * GP);   // [E][GP] (kHasM)
+    const int l = blockIdx.y;
+    {
+        const uint4* src = reinterpret_cast<const uint4*>(p.t.wc + (size_t)l * p.E * GP);
+        uint4* dst = reinterpret_cast<uint4*>(wc_s);
+        for (int i = threadIdx.x; i < p.E * GP / 2; i += kScoreThreads) dst[i] = src[i];
+        if constexpr (kHasM) {
+            const uint4* ms = reinterpret_cast<const uint4*>(p.t.m + (size_t)l * p.E * GP);
+            uint4* md = reinterpret_cast<uint4*>(m_s);
+            for (int i = threadIdx.x; i < p.E * GP / 4; i += kScoreThreads) md[i] = ms[i];
+        }
+    }
+    __syncthreads();
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int sub = lane / SEG, g0 = lane % SEG;
+    const uint32_t seg_mask = SEG == 32 ? 0xffffffffu : (((1u << SEG) - 1u) << (sub * SEG));
+    const double Gd = (double)G;
+    const double sumB = p.t.sumB[l];
+    const uint32_t want_hash = p.t.hsum[l];
+    const float base_mig = p.t.base_mig[l];
+    const uint32_t emask = (uint32_t)p.E - 1u;
+    const uint32_t okbits = emask | (emask << 16);
+    const int col = G < 32 ? lane : g0;                 // table column of rank g0 (+32 for the lane's second rank)
+
+    const int p_begin = blockIdx.x * p.chunk, p_end = min(p.P, p_begin + p.chunk);
+    constexpr int kStride = (kScoreThreads / 32) * UPW;
+    const size_t step_words = (size_t)kStride * p.L * NS / 2;
+    int cand = p_begin + warp * UPW + sub;
+    const uint32_t* rowp = reinterpret_cast<const uint32_t*>(p.cand + ((size_t)cand * p.L + l) * NS);
+    uint32_t cur[RPL][NW], nxt[RPL][NW];
+    auto fetch = [&](const uint32_t* row, uint32_t (&w)[RPL][NW]) {
+#pragma unroll
+        for (int rr = 0; rr < RPL; ++rr) {
+            const int g = g0 + rr * 32;
+            if constexpr (SP % 8 == 0) {
+#pragma unroll
+                for (int q = 0; q < SP / 8; ++q) {
+                    const uint4 v = __ldcs(reinterpret_cast<const uint4*>(row + g * (SP / 2)) + q);
+                    w[rr][4 * q] = v.x; w[rr][4 * q + 1] = v.y; w[rr][4 * q + 2] = v.z; w[rr][4 * q + 3] = v.w;
+                }
+            } else if constexpr (SP % 4 == 0) {
+#pragma unroll
+                for (int q = 0; q < SP / 4; ++q) {
+                    const uint2 v = __ldcs(reinterpret_cast<const uint2*>(row + g * (SP / 2)) + q);
+                    w[rr][2 * q] = v.x; w[rr][2 * q + 1] = v.y;
+                }
+            } else {
+#pragma unroll
+                for (int j = 0; j < NW; ++j) w[rr][j] = __ldcs(row + ((g * SP) >> 1) + j);
+            }
+        }
+    };
+    if (cand < p_end) fetch(rowp, cur);
+    for (int pc = p_begin + warp * UPW; pc < p_end; pc += kStride, cand += kStride) {
+        const bool active = cand < p_end;
+        rowp += step_words;
+        if (cand + kStride < p_end) fetch(rowp, nxt);
+        float sq = 0.0f, comm = 0.0f, mig_in = 0.0f, mig_kept = 0.0f, mx = 0.0f;
+        uint32_t hs = 0, orall = 0, kept = 0;
+        bool dup = false;
+        if (active) {
+#pragma unroll
+            for (int rr = 0; rr < RPL; ++rr) {
+                uint32_t w[NW];
+#pragma unroll
+                for (int j = 0; j < NW; ++j) w[j] = cur[rr][j];
+                if constexpr (SP % 2 == 1) {
+                    // odd ranks start in the upper half of their first word: realign
+                    const uint32_t sh = ((g0 + rr * 32) & 1) * 16;
+#pragma unroll
+                    for (int j = 0; j + 1 < NW; ++j) w[j] = __funnelshift_r(w[j], w[j + 1], sh);
+                    w[NW - 1] = (w[NW - 1] >> sh) & 0xffffu;
+                }
+                uint32_t e[SP];
+                float lg = 0.0f;
+#pragma unroll
+                for (int j = 0; j < NW; ++j) orall |= w[j];
+#pragma unroll
+                for (int j = 0; j < SP; ++j) {
+                    const uint32_t x = ((j & 1) ? (w[j >> 1] >> 16) : w[j >> 1]) & emask;
+                    e[j] = x;
+                    hs += slot_hash(x);
+                    const int idx = x * GP + col + rr * 32;
+                    const float2 wc = wc_s[idx];
+                    lg += wc.x;
+                    comm += fabsf(wc.y);
+                    const uint32_t member = __float_as_uint(wc.y) >> 31;
+                    kept += member;
+                    if constexpr (kHasM) {
+                        const float mm = m_s[idx];
+                        if (member) mig_kept += mm; else mig_in += mm;     // retained / entering cell of x0
+                    }
+                }
+                if constexpr (kDup) {
+#pragma unroll
+                    for (int a = 0; a < SP; ++a)
+#pragma unroll
+                        for (int b = a + 1; b < SP; ++b) dup |= (e[a] == e[b]);
+                }
+                const float d = (float)((double)lg * Gd - sumB);  // G*L_g - sum_g L_g, exact difference for integer counts
+                sq = __fmaf_rn(d, d, sq);
+                mx = fmaxf(mx, lg);
+            }
+        }
+        const uint32_t flags = ((orall & ~okbits) ? 1u : 0u) | (dup ? 1u : 0u);
+        hs = __reduce_add_sync(seg_mask, hs);
+        kept = __reduce_add_sync(seg_mask, kept);
+        const uint32_t bad = __reduce_or_sync(seg_mask, flags);
+        const float mxa = __uint_as_float(__reduce_max_sync(seg_mask, __float_as_uint(mx)));   // loads are >= 0
+        float commt = comm;
+        if constexpr (SEG > 1) {
+            constexpr int h = SEG >> 1;
+            const bool up = (lane & h) != 0;
+            float v = (up ? comm : sq) + __shfl_xor_sync(0xffffffffu, up ? sq : comm, h);
+#pragma unroll
+            for (int o = h >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            commt = __shfl_sync(0xffffffffu, v, sub * SEG + h);
+            sq = v;                                                                  // valid on unit lanes with bit h clear
+        }
+        if constexpr (kHasM) {
+#pragma unroll
+            for (int o = SEG >> 1; o > 0; o >>= 1) {
+                mig_in += __shfl_xor_sync(0xffffffffu, mig_in, o);
+                mig_kept += __shfl_xor_sync(0xffffffffu, mig_kept, o);
+            }
+        }
+        if (active && g0 == 0) {
+            const float mig = kHasM ? mig_in + (base_mig - mig_kept) : p.M_scalar * (float)(2 * (NS - (int)kept));
+            float4 out = make_float4(sq, commt, mig, mxa);
+            if (bad || hs != want_hash) out.x = CUDART_NAN_F;
+            p.partial[(size_t)cand * p.L + l] = out;
+        }
+#pragma unroll
+        for (int rr = 0; rr < RPL; ++rr)
+#pragma unroll
+            for (int j = 0; j < NW; ++j) cur[rr][j] = nxt[rr][j];
+    }
+}
+
 struct FinalizeParams {
     int P, L, G;
     float alpha, beta, gamma;

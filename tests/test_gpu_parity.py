@@ -94,7 +94,9 @@ def _check_objective(out, ref, tol=1e-5, mig_scale=0.0):
     ("tiny", "i32", False, False), ("v2lite", "f32", True, True), ("qwen3", "i32", False, True),
     ("v3", "i32", False, False), ("v3", "f32", True, True), ("decode", "f32", False, False), ("decode", "i32", True, True),
 ])
-def test_eval_placements_parity(name, counts, table_M, seeded_D):
+@pytest.mark.parametrize("generic", [0, 1])
+def test_eval_placements_parity(name, counts, table_M, seeded_D, generic, monkeypatch):
+    monkeypatch.setenv("GIMBAL_SCORE_GENERIC", str(generic))      # specialised and generic scoring kernels
     w, cfg, A, B, D, M, prev = _placement_instance(name, 0, counts, table_M, seeded_D)
     cands = gen.candidates(w, prev, w.P, DEV)
     out = torch.full((w.P, 5), -1.0, device=DEV)
@@ -113,7 +115,9 @@ def test_eval_placements_parity(name, counts, table_M, seeded_D):
     assert ref[am, 0] <= np.nanmin(ref[:, 0]) * (1 + 2e-5)
 
 
-def test_eval_placements_invalid_candidates_and_edges():
+@pytest.mark.parametrize("generic", [0, 1])
+def test_eval_placements_invalid_candidates_and_edges(generic, monkeypatch):
+    monkeypatch.setenv("GIMBAL_SCORE_GENERIC", str(generic))
     w, cfg, A, B, D, M, prev = _placement_instance("v3", 1)
     P = 40
     cands = gen.candidates(w, prev, P, DEV).clone()
