@@ -93,7 +93,7 @@ class ClockSampler:
 # --------------------------------------------------------------------------------------------
 # oracle timing (cpu_baseline / --impl reference)
 # --------------------------------------------------------------------------------------------
-def oracle_step_time(w, sample_tokens, sample_layers, sample_P, sample_moves, inputs=None):
+def oracle_step_time(w, sample_tokens, sample_layers, sample_P, sample_moves, place_layers=None):
     """Times the CPU oracle, as it stands, on a bounded sample of the workload and extrapolates
     to one full step.  Returns (seconds per full step, description, threads)."""
     import oracle
@@ -112,9 +112,10 @@ def oracle_step_time(w, sample_tokens, sample_layers, sample_P, sample_moves, in
     t_stats = time.perf_counter() - t0
     tok_layers_per_s = sample_tokens * sample_layers / t_stats
     # placement side on a profile of the right shape
-    A_full = np.repeat(res["C"][:1], sample_layers, 0).astype(np.float64)
+    place_layers = sample_layers if place_layers is None else place_layers
+    A_full = np.repeat(res["C"][:1], place_layers, 0).astype(np.float64)
     B_full = A_full.sum(1)
-    wl = scaled(w, L=sample_layers, P=sample_P)
+    wl = scaled(w, L=place_layers, P=sample_P)
     prev = gen.prev_placement(wl, B_full, "cpu")
     cands = gen.candidates(wl, prev, sample_P, "cpu").numpy()
     D = gen.comm_cost_D(wl, "binary", "cpu").numpy()
@@ -123,7 +124,7 @@ def oracle_step_time(w, sample_tokens, sample_layers, sample_P, sample_moves, in
     oracle.derived(A_full, prev.numpy(), dp, w.G, w.slots_per_rank)
     oracle.objective_batch(cands, prev.numpy(), A_full, B_full, D, None, 1.0, G=w.G, sp=w.slots_per_rank)
     t_obj = time.perf_counter() - t0
-    cand_layers_per_s = sample_P * sample_layers / t_obj
+    cand_layers_per_s = sample_P * place_layers / t_obj
     moves = gen.explicit_moves(wl, sample_moves, "cpu").numpy()
     t0 = time.perf_counter()
     oracle.move_deltas(prev.numpy(), prev.numpy(), moves, A_full, B_full, D, None, 1.0, G=w.G, sp=w.slots_per_rank)
@@ -132,17 +133,40 @@ def oracle_step_time(w, sample_tokens, sample_layers, sample_P, sample_moves, in
     n_moves = r.L * w.NS * (w.NS - 1) // 2
     step_s = w.T * r.L / tok_layers_per_s + w.P * r.L / cand_layers_per_s + n_moves / moves_per_s
     desc = (f"oracle as it stands: a1-a5 on {sample_tokens} tokens x {sample_layers} layers ({t_stats:.1f}s, "
-            f"{tok_layers_per_s:.0f} token-layers/s), a6 on {sample_P} candidates x {sample_layers} layers ({t_obj:.1f}s, "
+            f"{tok_layers_per_s:.0f} token-layers/s), a6 on {sample_P} candidates x {place_layers} layers ({t_obj:.1f}s, "
             f"{cand_layers_per_s:.0f} candidate-layers/s), a7 on {sample_moves} moves ({t_mv:.1f}s, {moves_per_s:.0f} moves/s); "
             f"extrapolated to one full step (T={w.T}, L={r.L}, P={w.P}, {n_moves} moves)")
     return step_s, desc, oracle.num_threads(), dict(token_layers_per_s=tok_layers_per_s, candidate_layers_per_s=cand_layers_per_s,
                                                      moves_per_s=moves_per_s)
 
 
-SAMPLES = {   # workload -> (tokens, layers, candidates, moves) of the oracle sample (~10-30 s of CPU work)
-    "tiny": (4096, 1, 64, 120), "v2lite": (8192, 2, 64, 4000), "qwen3": (8192, 2, 32, 4000),
-    "v3": (4096, 2, 16, 2000), "decode": (256, 8, 16, 2000),
+SAMPLES = {   # workload -> (tokens, layers, candidates, moves, placement layers) of the oracle sample (~10-30 s of CPU work)
+    "tiny": (4096, 1, 64, 120, 1), "v2lite": (16384, 26, 1024, 100000, 26), "qwen3": (32768, 8, 512, 100000, 48),
+    "v3": (16384, 4, 1024, 100000, 58), "decode": (256, 58, 1024, 100000, 58),
 }
+
+
+def _sample(w, scale: float = 1.0):
+    """scale < 1 shrinks the sample (reference arm: K + W samples must end within a few minutes)."""
+    tok, lay, P, mv, pl = SAMPLES[w.name]
+    tok, P, mv = max(256, int(tok * scale)), max(16, int(P * scale)), max(120, int(mv * scale))
+    return min(tok, w.T), min(lay, w.router.L), min(P, w.P), mv, min(pl, w.router.L)
+
+
+# --------------------------------------------------------------------------------------------
+# N > 1: independent replicas (DESIGN.md section 2); the only cross-rank step is the max of the timings
+# --------------------------------------------------------------------------------------------
+def max_over_ranks(ms: float, device="cpu") -> float:
+    """Slowest rank's time (torch.distributed must be initialised; works on gloo and nccl)."""
+    import torch.distributed as td
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    td.all_reduce(t, op=td.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_value(tokens_per_rank: int, world: int, ms_per_step: float) -> float:
+    """Whole-job routed tokens/s of `world` replicas that each process tokens_per_rank per step."""
+    return world * tokens_per_rank / (ms_per_step * 1e-3)
 
 
 # --------------------------------------------------------------------------------------------
@@ -150,10 +174,10 @@ def run_reference(args, w):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    tok, lay, P, mv = SAMPLES[w.name]
     times, desc, threads = [], "", 1
+    scale = min(1.0, 8.0 / (args.warmup + args.steps))         # a full sample is ~15 s; keep the whole run near 2 minutes
     for i in range(args.warmup + args.steps):
-        s, desc, threads, _ = oracle_step_time(w, tok, lay, P, mv)
+        s, desc, threads, _ = oracle_step_time(w, *_sample(w, scale))
         if i >= args.warmup:
             times.append(s)
     step_s = sum(times) / len(times)
@@ -258,11 +282,9 @@ def run_ours(args, w):
     clocks = sampler.stop()
     total_ms = sum(a.elapsed_time(b) for a, b in ev)
     if dist:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        td.all_reduce(t, op=td.ReduceOp.MAX)
-        total_ms = float(t.item())
+        total_ms = max_over_ranks(total_ms, dev)
     ms_per_step = total_ms / args.steps
-    value = world * w.T / (ms_per_step * 1e-3)
+    value = replica_value(w.T, world, ms_per_step)
 
     # ---- roofline of the dominant kernel (router GEMM with fused gating + histogram) -------------------
     gemm_ms = statistics.mean(k_router)
@@ -303,16 +325,13 @@ def run_ours(args, w):
         except Exception as ex:  # report, never fake
             e2e = dict(value=None, unit="routed tokens/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0, error=str(ex)[:300])
     if dist and fits:
-        t = torch.tensor([e2e["ms_per_step"]], device=dev, dtype=torch.float64)
-        td.all_reduce(t, op=td.ReduceOp.MAX)
-        e2e["ms_per_step"] = float(t.item())
-        e2e["value"] = world * w.T / (e2e["ms_per_step"] * 1e-3)
+        e2e["ms_per_step"] = max_over_ranks(e2e["ms_per_step"], dev)
+        e2e["value"] = replica_value(w.T, world, e2e["ms_per_step"])
 
     if rank == 0:
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
-            tok, lay, P_s, mv = SAMPLES[w.name]
-            s, desc, threads, rates = oracle_step_time(w, tok, lay, P_s, mv)
+            s, desc, threads, rates = oracle_step_time(w, *_sample(w))
             cpu = dict(value=w.T / s, unit="routed tokens/s", cores=threads, kind="oracle", sample=desc, **rates)
         line = dict(metric=METRIC, value=value, unit="routed tokens/s", n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
                     ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16",
