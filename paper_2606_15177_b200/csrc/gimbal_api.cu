@@ -151,6 +151,12 @@ static size_t place_ws_carve(const gimbal_placement_cfg* c, int P, void* ws, Pla
     w.mp.top_g = cv.take<int32_t>((size_t)c->L * 4);
     w.mp.cmask = cv.take<uint64_t>(LE);
     w.mp.bad = cv.take<int32_t>(64);
+    const size_t NSl = (size_t)c->L * c->G * c->slots_per_rank;
+    w.mp.slotC = cv.take<float>(NSl * c->G);
+    w.mp.slotM = cv.take<float>(NSl * c->G);
+    w.mp.slot_w = cv.take<double>(NSl);
+    w.mp.slot_cm = cv.take<uint64_t>(NSl);
+    w.mp.slot_eg = cv.take<int2>(NSl);
     if (out) *out = w;
     return cv.off + 256;
 }
@@ -491,16 +497,26 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
         fill_u64_kernel<<<(cfg->L + 255) / 256, 256, 0, stream>>>(w.best, ~0ull, cfg->L);
         LAUNCH_CHECK("fill_u64_kernel");
     }
-    if (n_moves > 0 && !moves) {
+    if (n_moves > 0 && !moves && cfg->G >= 4) {
         // implicit neighbourhood: blocks of ~2048 pair indices of one layer, tables staged in shared memory
         MoveAllParams ap{};
         ap.L = cfg->L; ap.E = cfg->E; ap.G = cfg->G; ap.sp = cfg->slots_per_rank; ap.has_M = M != nullptr;
         ap.alpha = cfg->alpha; ap.beta = cfg->beta; ap.gamma = cfg->gamma; ap.M_scalar = M_scalar;
         ap.cur = cur; ap.t = w.t; ap.mp = w.mp; ap.delta = delta; ap.best = best_per_layer ? w.best : nullptr;
-        const long long npairs = NS * (NS - 1) / 2;
-        int bpl = (int)((npairs + 2047) / 2048);
-        ap.pairs_per_block = (int)(((npairs + bpl - 1) / bpl + kMoveAllThreads - 1) / kMoveAllThreads) * kMoveAllThreads;
-        bpl = (int)((npairs + ap.pairs_per_block - 1) / ap.pairs_per_block);
+        int lg = 0;
+        while ((1 << lg) < cfg->G) ++lg;
+        ap.lgG = lg;
+        // a warp task = the row pair {a, NS-2-a} (NS-1 moves); 16 tasks (~4600 moves at NS = 288) per block
+        const int n_tasks = (int)(NS / 2);
+        ap.tasks_per_block = 2 * (kMoveAllThreads / 32);
+        const int bpl = (n_tasks + ap.tasks_per_block - 1) / ap.tasks_per_block;
+        {
+            MoveSlotsParams sl{};
+            sl.L = cfg->L; sl.E = cfg->E; sl.G = cfg->G; sl.sp = cfg->slots_per_rank; sl.lgG = lg; sl.has_M = ap.has_M;
+            sl.cur = cur; sl.t = w.t; sl.mp = w.mp;
+            move_slots_kernel<<<dim3((unsigned)((NS * cfg->G + 255) / 256), cfg->L), 256, 0, stream>>>(sl);
+            LAUNCH_CHECK("move_slots_kernel");
+        }
         const size_t smem = move_all_smem_bytes((int)NS, cfg->G, ap.has_M);
         if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "move neighbourhood: NS=%lld G=%d needs %zu B of shared memory", NS, cfg->G, smem);
         CUDA_TRY(cudaFuncSetAttribute(move_all_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -508,6 +508,12 @@ struct MovePrep {
     int32_t* top_g;     // [L][4]  ... and their ranks
     uint64_t* cmask;    // [L][E]  bit g: cur hosts e on g
     int32_t* bad;       // [1]
+    // per-slot rows of `cur` for the all-pairs kernel (move_slots_kernel)
+    float* slotC;       // [L][NS][G]  c (sign = x0 hosts it) of the slot's expert on every rank
+    float* slotM;       // [L][NS][G]  M of the slot's expert on every rank (M table only)
+    double* slot_w;     // [L][NS]     load share of the slot's expert
+    uint64_t* slot_cm;  // [L][NS]     ranks hosting the slot's expert in cur
+    int2* slot_eg;      // [L][NS]     {expert, rank} of the slot
 };
 
 struct MovePrepParams {
@@ -666,9 +672,35 @@ __host__ __device__ inline size_t move_all_smem_bytes(int NS, int G, int has_M) 
     return b;
 }
 
+struct MoveSlotsParams {
+    int L, E, G, sp, lgG, has_M;
+    const int16_t* cur;
+    PlaceTables t;
+    MovePrep mp;
+};
+
+// one thread per (slot, rank) cell of a layer: the layer's tables re-indexed by slot
+__global__ void __launch_bounds__(256) move_slots_kernel(const MoveSlotsParams p) {
+    const int NS = p.G * p.sp, GP = place_gp(p.G);
+    const int l = blockIdx.y, i = blockIdx.x * 256 + threadIdx.x;
+    if (i >= NS * p.G) return;
+    const int j = i >> p.lgG, g = i & (p.G - 1);
+    int e = p.cur[(size_t)l * NS + j];
+    if (e < 0 || e >= p.E) e = 0;                                      // flagged by move_prep_kernel
+    const size_t src = ((size_t)l * p.E + e) * GP + g, dst = ((size_t)l * NS + j) * p.G + g;
+    p.mp.slotC[dst] = p.t.wc[src].y;
+    if (p.has_M) p.mp.slotM[dst] = p.t.m[src];
+    if (g == 0) {
+        p.mp.slot_w[(size_t)l * NS + j] = p.t.w_e[(size_t)l * p.E + e];
+        p.mp.slot_cm[(size_t)l * NS + j] = p.mp.cmask[(size_t)l * p.E + e];
+        p.mp.slot_eg[(size_t)l * NS + j] = make_int2(e, j / p.sp);
+    }
+}
+
 struct MoveAllParams {
     int L, E, G, sp, has_M;
-    int pairs_per_block;
+    int lgG;                            // log2(G)
+    int tasks_per_block;                // warp tasks (a row pair) per block
     float alpha, beta, gamma, M_scalar;
     const int16_t* cur;
     PlaceTables t;
@@ -677,6 +709,10 @@ struct MoveAllParams {
     unsigned long long* best;           // [L] | nullptr
 };
 
+// Work split: row a of the pair triangle (all b > a) has NS-1-a moves, so a warp task is the row
+// pair {a, NS-2-a} -- NS-1 moves whatever a is.  Inside a row the lanes walk b: everything that
+// depends on a (expert, rank, load, its table row) is warp-uniform, and the results of 32
+// consecutive b are contiguous in `delta`.
 __global__ void __launch_bounds__(kMoveAllThreads) move_all_kernel(const MoveAllParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int NS = p.G * p.sp, GP = place_gp(p.G), PITCH = p.G + 1;
@@ -694,81 +730,94 @@ __global__ void __launch_bounds__(kMoveAllThreads) move_all_kernel(const MoveAll
 
     const int npairs = NS * (NS - 1) / 2;
     const bool poisoned = (*p.mp.bad != 0) || (*p.t.bad != 0);
-    const int16_t* cu = p.cur + (size_t)l * NS;
     for (int j = tid; j < NS; j += kMoveAllThreads) {
-        int e = cu[j];
-        if (e < 0 || e >= p.E) e = 0;                                  // flagged by move_prep_kernel
-        eg[j] = make_int2(e, j / p.sp);
-        ws[j] = p.t.w_e[(size_t)l * p.E + e];
-        cms[j] = p.mp.cmask[(size_t)l * p.E + e];
+        eg[j] = p.mp.slot_eg[(size_t)l * NS + j];
+        ws[j] = p.mp.slot_w[(size_t)l * NS + j];
+        cms[j] = p.mp.slot_cm[(size_t)l * NS + j];
     }
     if (tid < p.G) Lgs[tid] = p.mp.Lg[(size_t)l * p.G + tid];
-    __syncthreads();
-    for (int i = tid; i < NS * p.G; i += kMoveAllThreads) {
-        const int j = i / p.G, g = i - j * p.G;
-        const size_t src = ((size_t)l * p.E + eg[j].x) * GP + g;
-        Cs[j * PITCH + g] = p.t.wc[src].y;
-        if (p.has_M) Ms[j * PITCH + g] = p.t.m[src];
+    {   // coalesced 16-byte reads of the [NS][G] rows, written at pitch G+1
+        const float4* src = reinterpret_cast<const float4*>(p.mp.slotC + (size_t)l * NS * p.G);
+        const float4* srcm = reinterpret_cast<const float4*>(p.mp.slotM + (size_t)l * NS * p.G);
+        for (int i = tid; i < NS * p.G / 4; i += kMoveAllThreads) {
+            const int j = (i * 4) >> p.lgG, g = (i * 4) & (p.G - 1);
+            const float4 v = src[i];
+            float* d = Cs + j * PITCH + g;
+            d[0] = v.x; d[1] = v.y; d[2] = v.z; d[3] = v.w;
+            if (p.has_M) {
+                const float4 m = srcm[i];
+                float* dm = Ms + j * PITCH + g;
+                dm[0] = m.x; dm[1] = m.y; dm[2] = m.z; dm[3] = m.w;
+            }
+        }
     }
     __syncthreads();
     double top[3]; int top_g[3];
 #pragma unroll
     for (int q = 0; q < 3; ++q) { top[q] = p.mp.top[l * 4 + q]; top_g[q] = p.mp.top_g[l * 4 + q]; }
 
-    const int r_begin = blockIdx.x * p.pairs_per_block, r_end = min(npairs, r_begin + p.pairs_per_block);
-    const float two_ns_1 = 2.0f * NS - 1.0f;
+    // tasks: t in [0, ceil((NS-1)/2)) -> rows t and NS-2-t (the middle row of an even count once)
+    const int n_tasks = NS / 2;                                         // NS-1 rows: (NS-1+1)/2 pairs
+    const int t_begin = blockIdx.x * p.tasks_per_block, t_end = min(n_tasks, t_begin + p.tasks_per_block);
     unsigned long long best = ~0ull;
-    for (int rb = r_begin + warp * 32; rb < r_end; rb += kMoveAllThreads) {
-        const int r = rb + lane;
-        float dJ = 0.0f, dload = 0.0f, dcomm = 0.0f, dmig = 0.0f, dmax = 0.0f;
-        bool nan = poisoned;
-        if (r < r_end && !nan) {
-            // canonical order: a outer, b inner, a < b.  Row a starts at a*NS - a*(a+1)/2.
-            int a = (int)((two_ns_1 - sqrtf(two_ns_1 * two_ns_1 - 8.0f * (float)r)) * 0.5f);
-            a = max(0, min(a, NS - 2));
-            while (a * NS - a * (a + 1) / 2 > r) --a;
-            while ((a + 1) * NS - (a + 1) * (a + 2) / 2 <= r) ++a;
-            const int b = r - (a * NS - a * (a + 1) / 2) + a + 1;
-            const int2 s1 = eg[a], s2 = eg[b];
-            const int e1 = s1.x, e2 = s2.x, g1 = s1.y, g2 = s2.y;
-            if (g1 != g2 && e1 != e2) {
-                if (((cms[a] >> g2) & 1ull) || ((cms[b] >> g1) & 1ull)) nan = true;      // second copy on a rank
-                else {
-                    const float t11 = Cs[a * PITCH + g1], t12 = Cs[a * PITCH + g2], t21 = Cs[b * PITCH + g1], t22 = Cs[b * PITCH + g2];
-                    // loads in double: L1 - L2 and w2 - w1 subtract nearly equal numbers that can exceed 2^24
-                    const double L1 = Lgs[g1], L2 = Lgs[g2];
-                    const double dl = ws[b] - ws[a];                              // moved onto g1
-                    dload = (float)(2.0 * dl * (L1 - L2) + 2.0 * dl * dl);        // the mean cancels
-                    dcomm = (fabsf(t12) - fabsf(t11)) + (fabsf(t21) - fabsf(t22));
-                    const float m11 = p.has_M ? Ms[a * PITCH + g1] : p.M_scalar, m12 = p.has_M ? Ms[a * PITCH + g2] : p.M_scalar;
-                    const float m21 = p.has_M ? Ms[b * PITCH + g1] : p.M_scalar, m22 = p.has_M ? Ms[b * PITCH + g2] : p.M_scalar;
-                    // leaving a cell x0 has: +M, leaving a cell x0 lacks: -M; entering: the opposite
-                    dmig = (__float_as_int(t11) < 0 ? m11 : -m11) + (__float_as_int(t12) < 0 ? -m12 : m12) +
-                           (__float_as_int(t22) < 0 ? m22 : -m22) + (__float_as_int(t21) < 0 ? -m21 : m21);
-                    const double n1 = L1 + dl, n2 = L2 - dl;
-                    double rest = -CUDART_INF;
+    for (int task = t_begin + warp; task < t_end; task += kMoveAllThreads / 32) {
+        for (int half = 0; half < 2; ++half) {
+            const int a = half == 0 ? task : NS - 2 - task;
+            if (half == 1 && a <= task) break;                          // middle row already done
+            const int2 s1 = eg[a];
+            const int e1 = s1.x, g1 = s1.y;
+            const double w1 = ws[a], L1 = Lgs[g1];
+            const unsigned long long cm1 = cms[a];
+            const float t11 = Cs[a * PITCH + g1];
+            const float m11 = p.has_M ? Ms[a * PITCH + g1] : p.M_scalar;
+            const int row0 = a * NS - a * (a + 1) / 2 - a - 1;           // pair index of (a, b) = row0 + b
+            for (int bb = a + 1; bb < NS; bb += 32) {
+                const int b = bb + lane;
+                float dJ = 0.0f, dload = 0.0f, dcomm = 0.0f, dmig = 0.0f, dmax = 0.0f;
+                bool nan = poisoned;
+                if (b < NS && !nan) {
+                    const int2 s2 = eg[b];
+                    const int e2 = s2.x, g2 = s2.y;
+                    if (g1 != g2 && e1 != e2) {
+                        if (((cm1 >> g2) & 1ull) || ((cms[b] >> g1) & 1ull)) nan = true;      // second copy on a rank
+                        else {
+                            const float t12 = Cs[a * PITCH + g2], t21 = Cs[b * PITCH + g1], t22 = Cs[b * PITCH + g2];
+                            // loads in double: L1 - L2 and w2 - w1 subtract nearly equal numbers that can exceed 2^24
+                            const double L2 = Lgs[g2];
+                            const double dl = ws[b] - w1;                                 // moved onto g1
+                            dload = (float)(2.0 * dl * (L1 - L2) + 2.0 * dl * dl);        // the mean cancels
+                            dcomm = (fabsf(t12) - fabsf(t11)) + (fabsf(t21) - fabsf(t22));
+                            const float m12 = p.has_M ? Ms[a * PITCH + g2] : p.M_scalar;
+                            const float m21 = p.has_M ? Ms[b * PITCH + g1] : p.M_scalar, m22 = p.has_M ? Ms[b * PITCH + g2] : p.M_scalar;
+                            // leaving a cell x0 has: +M, leaving a cell x0 lacks: -M; entering: the opposite
+                            dmig = (__float_as_int(t11) < 0 ? m11 : -m11) + (__float_as_int(t12) < 0 ? -m12 : m12) +
+                                   (__float_as_int(t22) < 0 ? m22 : -m22) + (__float_as_int(t21) < 0 ? -m21 : m21);
+                            const double n1 = L1 + dl, n2 = L2 - dl;
+                            double rest = -CUDART_INF;
 #pragma unroll
-                    for (int q = 2; q >= 0; --q)
-                        if (top_g[q] >= 0 && top_g[q] != g1 && top_g[q] != g2) rest = top[q];
-                    dmax = (float)(fmax(fmax(n1, n2), rest) - top[0]);
-                    dJ = p.alpha * dcomm + p.beta * dload + p.gamma * dmig;
+                            for (int q = 2; q >= 0; --q)
+                                if (top_g[q] >= 0 && top_g[q] != g1 && top_g[q] != g2) rest = top[q];
+                            dmax = (float)(fmax(fmax(n1, n2), rest) - top[0]);
+                            dJ = p.alpha * dcomm + p.beta * dload + p.gamma * dmig;
+                        }
+                    }
                 }
+                if (nan) dJ = dload = dcomm = dmig = dmax = CUDART_NAN_F;
+                if (b < NS && !nan && p.best) {
+                    const unsigned long long key = ((unsigned long long)ordered_u32(dJ + 0.0f) << 32) | (unsigned long long)(uint32_t)(l * npairs + row0 + b);
+                    best = key < best ? key : best;
+                }
+                // stage the warp's 32 x 5 results, then write them as contiguous words
+                stage[lane * 5 + 0] = dJ; stage[lane * 5 + 1] = dload; stage[lane * 5 + 2] = dcomm; stage[lane * 5 + 3] = dmig; stage[lane * 5 + 4] = dmax;
+                __syncwarp();
+                const int n_out = min(32, NS - bb) * 5;
+                float* out = p.delta + ((size_t)l * npairs + row0 + bb) * 5;
+#pragma unroll
+                for (int q = 0; q < 5; ++q)
+                    if (q * 32 + lane < n_out) __stcs(out + q * 32 + lane, stage[q * 32 + lane]);
+                __syncwarp();
             }
         }
-        if (nan) dJ = dload = dcomm = dmig = dmax = CUDART_NAN_F;
-        if (r < r_end && !nan && p.best) {
-            const unsigned long long key = ((unsigned long long)ordered_u32(dJ + 0.0f) << 32) | (unsigned long long)(uint32_t)(l * npairs + r);
-            best = key < best ? key : best;
-        }
-        // stage the warp's 32 x 5 results, then write them as contiguous words
-        stage[lane * 5 + 0] = dJ; stage[lane * 5 + 1] = dload; stage[lane * 5 + 2] = dcomm; stage[lane * 5 + 3] = dmig; stage[lane * 5 + 4] = dmax;
-        __syncwarp();
-        const int n_out = min(32, r_end - rb) * 5;
-        float* out = p.delta + ((size_t)l * npairs + rb) * 5;
-#pragma unroll
-        for (int q = 0; q < 5; ++q)
-            if (q * 32 + lane < n_out) __stcs(out + q * 32 + lane, stage[q * 32 + lane]);
-        __syncwarp();
     }
     if (p.best) {
         for (int o = 16; o > 0; o >>= 1) {
