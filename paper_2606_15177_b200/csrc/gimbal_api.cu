@@ -167,7 +167,7 @@ static int launch_tables(const gimbal_placement_cfg* c, const void* A, const voi
     TableParams tp{};
     tp.L = c->L; tp.E = c->E; tp.G = c->G; tp.sp = c->slots_per_rank; tp.S = c->S; tp.counts_f32 = c->counts_dtype == GIMBAL_COUNTS_F32;
     tp.A = A; tp.B = B; tp.D = D; tp.M = M; tp.M_scalar = M_scalar; tp.prev = prev; tp.t = w.t;
-    place_tables_kernel<<<c->L, 256, 0, stream>>>(tp);
+    place_tables_kernel<<<dim3(c->L, kTableSplit), 256, 0, stream>>>(tp);
     LAUNCH_CHECK("place_tables_kernel");
     return GIMBAL_OK;
 }

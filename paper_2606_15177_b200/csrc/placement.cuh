@@ -54,22 +54,38 @@ struct TableParams {
     PlaceTables t;
 };
 
-// one block per layer, 256 threads
+// fixed-order block sum of one double per thread (256 threads): bit-reproducible
+__device__ __forceinline__ double block_sum_256(double v, double* red) {
+    red[threadIdx.x] = v;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    const double r = red[0];
+    __syncthreads();
+    return r;
+}
+
+constexpr int kTableSplit = 4;      // blocks per layer (the [E][G'] cells are split between them)
+
+// grid (L, kTableSplit), 256 threads.  Every block rebuilds the layer's replica counts / rank
+// masks of x0 (cheap); block y = 0 also writes the per-layer scalars.
 __global__ void __launch_bounds__(256) place_tables_kernel(const TableParams p) {
     __shared__ int r_s[kMaxE];
     __shared__ unsigned long long pm_s[kMaxE];
     __shared__ float D_s[64 * 64];
+    __shared__ double red_s[256];
     __shared__ int bad_s;
     __shared__ unsigned int hs_s;
-    __shared__ float bm_s;
-    __shared__ double sb_s;
     const int l = blockIdx.x, tid = threadIdx.x;
     const int NS = p.G * p.sp, GP = place_gp(p.G);
     const int16_t* pv = p.prev + (size_t)l * NS;
-    if (tid == 0) { bad_s = 0; hs_s = 0; sb_s = 0.0; }
+    if (tid == 0) { bad_s = 0; hs_s = 0; }
     for (int e = tid; e < p.E; e += 256) { r_s[e] = 0; pm_s[e] = 0ull; }
     for (int i = tid; i < p.S * p.G; i += 256) D_s[i] = p.D[i];
     __syncthreads();
+    double bm = 0.0;
     for (int j = tid; j < NS; j += 256) {
         const int e = pv[j], g = j / p.sp;
         if (e < 0 || e >= p.E) { bad_s = 1; continue; }
@@ -77,28 +93,33 @@ __global__ void __launch_bounds__(256) place_tables_kernel(const TableParams p) 
         const unsigned long long old = atomicOr(&pm_s[e], 1ull << g);
         if ((old >> g) & 1ull) bad_s = 1;                         // twice on one rank
         atomicAdd(&hs_s, slot_hash((uint32_t)e));
+        bm += p.M ? (double)p.M[((size_t)l * p.E + e) * p.G + g] : (double)p.M_scalar;
     }
-    if (tid == 0) {                                   // fixed order: bit-reproducible
-        double bm = 0.0;
-        for (int j = 0; j < NS; ++j) {
-            const int e = pv[j], g = j / p.sp;
-            if (e >= 0 && e < p.E) bm += p.M ? (double)p.M[((size_t)l * p.E + e) * p.G + g] : (double)p.M_scalar;
+    __syncthreads();
+    if (blockIdx.y == 0) {
+        const double bm_tot = block_sum_256(bm, red_s);
+        double sb = 0.0;
+        for (int e = tid; e < p.E; e += 256) {
+            if (r_s[e] < 1) bad_s = 1;
+            const double b = p.counts_f32 ? (double)reinterpret_cast<const float*>(p.B)[(size_t)l * p.E + e]
+                                          : (double)reinterpret_cast<const int32_t*>(p.B)[(size_t)l * p.E + e];
+            sb += b;
+            p.t.w_e[(size_t)l * p.E + e] = b / (double)max(r_s[e], 1);
+            p.t.r[(size_t)l * p.E + e] = r_s[e];
+            p.t.pmask[(size_t)l * p.E + e] = pm_s[e];
         }
-        bm_s = (float)bm;
+        const double sb_tot = block_sum_256(sb, red_s);
+        if (tid == 0) {
+            p.t.hsum[l] = hs_s;
+            p.t.base_mig[l] = (float)bm_tot;
+            p.t.sumB[l] = sb_tot;
+            if (bad_s) atomicOr(p.t.bad, 1);
+        }
     }
-    __syncthreads();
-    for (int e = tid; e < p.E; e += 256) {
-        if (r_s[e] < 1) bad_s = 1;
-        const double b = p.counts_f32 ? (double)reinterpret_cast<const float*>(p.B)[(size_t)l * p.E + e]
-                                      : (double)reinterpret_cast<const int32_t*>(p.B)[(size_t)l * p.E + e];
-        atomicAdd(&sb_s, b);
-        p.t.w_e[(size_t)l * p.E + e] = b / (double)max(r_s[e], 1);
-        p.t.r[(size_t)l * p.E + e] = r_s[e];
-        p.t.pmask[(size_t)l * p.E + e] = pm_s[e];
-    }
-    __syncthreads();
     // table entries; column gp of the table serves rank gp % G (replicated when G < 32)
-    for (int i = tid; i < p.E * GP; i += 256) {
+    const int cells = p.E * GP, per = (cells + kTableSplit - 1) / kTableSplit;
+    const int i_end = min(cells, (int)(blockIdx.y + 1) * per);
+    for (int i = blockIdx.y * per + tid; i < i_end; i += 256) {
         const int e = i / GP, gp = i % GP, g = gp % p.G;
         float c = 0.0f;
         for (int s = 0; s < p.S; ++s) {
@@ -106,18 +127,15 @@ __global__ void __launch_bounds__(256) place_tables_kernel(const TableParams p) 
                                          : (float)reinterpret_cast<const int32_t*>(p.A)[((size_t)l * p.S + s) * p.E + e];
             c = __fmaf_rn(a, D_s[s * p.G + g], c);
         }
-        const float inv = 1.0f / (float)max(r_s[e], 1);
+        const int re = max(r_s[e], 1);
+        const float inv = 1.0f / (float)re;
         c = fabsf(c * inv);
         const bool member = (pm_s[e] >> g) & 1ull;
-        const float w = (float)p.t.w_e[(size_t)l * p.E + e];
+        const double b = p.counts_f32 ? (double)reinterpret_cast<const float*>(p.B)[(size_t)l * p.E + e]
+                                      : (double)reinterpret_cast<const int32_t*>(p.B)[(size_t)l * p.E + e];
+        const float w = (float)(b / (double)re);
         p.t.wc[((size_t)l * p.E + e) * GP + gp] = make_float2(w, member ? -c : c);   // -0.0f keeps the flag when c == 0
         if (p.M) p.t.m[((size_t)l * p.E + e) * GP + gp] = p.M[((size_t)l * p.E + e) * p.G + g];
-    }
-    if (tid == 0) {
-        p.t.hsum[l] = hs_s;
-        p.t.base_mig[l] = bm_s;
-        p.t.sumB[l] = sb_s;
-        if (bad_s) atomicOr(p.t.bad, 1);
     }
 }
 
