@@ -35,6 +35,10 @@ from workloads import gen, get_workload, scaled  # noqa: E402
 from workloads.configs import MODE_WINDOW  # noqa: E402
 
 METRIC = "routed tokens/s (stats path + placement scoring, whole hot path)"
+# dram__bytes_read + dram__bytes_write of router_gemm_kernel per token-layer at the V3 shape, from the committed
+# `ncu --set full` capture profiles/r1_ncu_k1_router_gemm.txt: (5.661685e9 + 5.92e6) B over 65536 tokens x 6 layers
+# (algorithmic: 2*H = 14336 B).  The capture covers 6 of the 58 layers; traffic per launch scales it by T*L.
+NCU_DRAM_BYTES_PER_TOKEN_LAYER_V3 = (5.661685e9 + 5.92e6) / (65536 * 6)
 
 
 def _peaks():
@@ -292,7 +296,10 @@ def run_ours(args, w):
     bytes_hidden = 2.0 * w.T * r.H * r.L                      # 2*H bytes per token-layer, read exactly once
     tf = flops / (gemm_ms * 1e-3) / 1e12
     roofline = dict(bound="tensor", achieved=tf, peak=peaks["tf_sustained"], unit="TFLOP/s", frac=tf / peaks["tf_sustained"],
-                    traffic=None, kernel="router_gemm_kernel (a1 + fused a2/a3)", ms=gemm_ms, share_of_step=gemm_ms / ms_per_step,
+                    traffic=(NCU_DRAM_BYTES_PER_TOKEN_LAYER_V3 * w.T * r.L if w.name == "v3" else None),
+                    traffic_unit="bytes per launch (ncu dram read+write per token-layer x T x L, profiles/r1_ncu_k1_router_gemm.txt)",
+                    algorithmic_bytes=bytes_hidden, algorithmic_flops=flops,
+                    kernel="router_gemm_kernel (a1 + fused a2/a3)", ms=gemm_ms, share_of_step=gemm_ms / ms_per_step,
                     peak_source=peaks["source"] + ", sustained bf16 (kernel timed inside a long step)",
                     frac_of_burst_peak=tf / peaks["tf_burst"],
                     hbm=dict(achieved=bytes_hidden / (gemm_ms * 1e-3) / 1e9, peak=peaks["hbm"], unit="GB/s",
