@@ -258,6 +258,12 @@ def run_ours(args, w):
         g.eval_moves(pc, cur, prev, A_live, B_live, D, delta, best_per_layer=best, workspace=ws_p)
 
     g.kernel_timing(True)
+    # NEXT-1 (not part of the timed step): the greedy heuristic on the same profile, timed on its own
+    greedy_out = torch.empty_like(prev)
+    greedy_ms = []
+    for _ in range(4):
+        g.greedy_place(pc, A_live, B_live, D, prev, greedy_out)
+        greedy_ms.append(g.kernel_elapsed_ms(g.KERNEL_GREEDY))
     for _ in range(max(args.warmup, 3)):
         step()
     torch.cuda.synchronize()
@@ -308,6 +314,7 @@ def run_ours(args, w):
     score_ms, moves_ms = statistics.mean(k_score), statistics.mean(k_moves)
     cand_bytes = 2.0 * r.L * w.NS * w.P
     extra = dict(
+        greedy_place_kernel=dict(ms=min(greedy_ms[1:]), layers=r.L, note="NEXT-1, PAPER.md:260-268; outside the timed step"),
         placements_per_s=world * w.P / (score_ms * 1e-3), moves_per_s=world * n_moves / (moves_ms * 1e-3),
         place_score_kernel=dict(ms=score_ms, bound="hbm", achieved=cand_bytes / (score_ms * 1e-3) / 1e9, peak=peaks["hbm"],
                                 unit="GB/s", frac=cand_bytes / (score_ms * 1e-3) / 1e9 / peaks["hbm"],

@@ -239,6 +239,26 @@ GIMBAL_API int gimbal_eval_moves(const gimbal_placement_cfg *cfg, const int16_t 
                       float *delta, int32_t *best_per_layer,
                       void *workspace, size_t workspace_bytes, gimbal_stream_t stream);
 
+/* ---------------------------------------------------------------------------------------
+ * gimbal_greedy_place -- the online greedy placement heuristic (section
+ * 5.3; R17), every layer in parallel.  Items are the slot contents of x0 (`prev`);
+ * they are taken in order of hotness (B[l,e] + sum_s A[l,s,e]) / r (descending; expert index,
+ * then slot index break ties) and each goes to the feasible rank (free slot, not already
+ * holding that expert) with the lowest local score
+ *     S[l,e,g] = alpha * sum_s A[l,s,e] D[s,g] / r  +  beta * (load placed on g so far + B[l,e]/r)
+ *              + gamma * (M[l,e,g] if x0 does not host e on g, else 0)
+ * ties: a placement that avoids migration first, then the less-filled rank,
+ * then the lower rank index.  Scores are evaluated in IEEE double, one rounding per operation,
+ * so the resulting placement is a pure function of the inputs (bit-exact against the oracle).
+ *   out [L,NS] i16   slot -> expert; slot g*slots_per_rank + i = the i-th item given to rank g.
+ *                    A layer whose x0 is invalid, or where an item finds no feasible rank, is
+ *                    filled with -1 and bit 1 of `status` is set.
+ *   status [1] i32 inout | NULL
+ * Other arguments as in gimbal_eval_placements.  Needs no workspace.                       */
+GIMBAL_API int gimbal_greedy_place(const gimbal_placement_cfg *cfg, const void *A, const void *B, const float *D,
+                        const float *M, float M_scalar, const int16_t *prev, int16_t *out, int32_t *status,
+                        gimbal_stream_t stream);
+
 /* Counters for bench.py: kernels launched by this library since load. */
 GIMBAL_API int64_t gimbal_launch_count(void);
 
@@ -250,6 +270,7 @@ GIMBAL_API int64_t gimbal_launch_count(void);
 #define GIMBAL_KERNEL_GATE 1   /* standalone gating + histogram              a2-a3 */
 #define GIMBAL_KERNEL_SCORE 2  /* placement scoring                          a6    */
 #define GIMBAL_KERNEL_MOVES 3  /* move deltas                                a7    */
+#define GIMBAL_KERNEL_GREEDY 4 /* greedy placement heuristic                 NEXT-1 */
 GIMBAL_API int gimbal_kernel_timing(int enable);
 GIMBAL_API int gimbal_kernel_elapsed_ms(int which, float *ms);
 

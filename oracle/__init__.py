@@ -51,6 +51,7 @@ def lib():
         _lib.oracle_objective.restype = C.c_int
         _lib.oracle_derived.restype = C.c_int
         _lib.oracle_num_threads.restype = C.c_int
+        _lib.oracle_greedy_place.restype = C.c_int
     return _lib
 
 
@@ -198,6 +199,20 @@ def move_deltas(cur, prev, moves, A, B, D, M=None, M_scalar=1.0, *, G, sp, weigh
                              C.c_double(M_scalar), C.c_int(L), C.c_int(S), C.c_int(E), C.c_int(G), C.c_int(sp),
                              C.c_double(weights[0]), C.c_double(weights[1]), C.c_double(weights[2]), _p(out, C.c_double))
     return out
+
+
+# -- NEXT-1: greedy heuristic -----------------------------------------------------------
+def greedy_place(prev, A, B, D, M=None, M_scalar=1.0, *, G, sp, weights=(1.0, 0.0025, 1.0)):
+    """prev [L,NS] int16 -> (ok, placement [L,NS] int16) by the paper's online heuristic."""
+    A, B, D, M = _obj_args(A, B, D, M)
+    prev = _c(prev, np.int16)
+    L, S, E = A.shape
+    out = np.empty_like(prev)
+    ok = lib().oracle_greedy_place(_p(prev, C.c_int16), _p(A, C.c_double), _p(B, C.c_double), _p(D, C.c_double),
+                                   _p(M, C.c_double), C.c_double(M_scalar), C.c_int(L), C.c_int(S), C.c_int(E), C.c_int(G),
+                                   C.c_int(sp), C.c_double(weights[0]), C.c_double(weights[1]), C.c_double(weights[2]),
+                                   _p(out, C.c_int16))
+    return bool(ok), out
 
 
 # -- brute force ------------------------------------------------------------------------

@@ -485,6 +485,97 @@ int64_t oracle_bruteforce(const int16_t *prev /*[NS]*/, const double *A /*[S,E]*
     return total;
 }
 
+/* ------------------------------------------------------------------------------------ */
+/* NEXT-1  The online greedy placement heuristic (section 5.3), step by step
+ *     in the paper's order, one layer at a time (layers are independent):
+ *       1. "ranks experts by a hotness signal derived from aggregate expert load and
+ *          source-aware activation volume": hot[e] = (B[l,e] + sum_s A[l,s,e]) / r[l,e]
+ *          (R17); the items are the slot contents of x0 (an expert hosted by r ranks
+ *          is r items, each carrying 1/r of its tokens, R12), ordered by (hot descending,
+ *          expert ascending, slot index in x0 ascending).
+ *       2. "For each hot expert, ... enumerates feasible ranks that still have placement
+ *          capacity and computes a local placement score"
+ *              S[l,e,g] = alpha*Ccomm + beta*Cload + gamma*Cmig
+ *          with (R17)  Ccomm = sum_s A[l,s,e] D[s,g] / r   "communication cost if expert e is
+ *                              placed on rank g",
+ *                      Cload = Lcur[g] + B[l,e]/r           "the resulting rank-load": load
+ *                              already placed on g in this pass plus the item's,
+ *                      Cmig  = M[l,e,g] if x0 does not host e on g, else 0  "relative to the
+ *                              current placement".
+ *          A rank is feasible when it has a free slot and does not already hold this expert.
+ *       3. "assigns each expert to the feasible rank with the lowest score, breaking ties by
+ *          preferring placements that avoid migration and then by choosing less-filled ranks"
+ *          (PAPER.md:266-268); a last tie goes to the lowest rank index.
+ *     All arithmetic is IEEE double, one operation at a time, in the order written here
+ *     (S = ((alpha*Ccomm) + (beta*Cload)) + (gamma*Cmig), Ccomm summed over s ascending then
+ *     divided by r); the decision precision of the contract is this double arithmetic.
+ *     out[l, g*sp + i] = the i-th item assigned to rank g.  A layer whose x0 is invalid, or in
+ *     which an item finds no feasible rank, gets a row of -1 (return value 0); the other
+ *     layers are unaffected.                                                              */
+/* ------------------------------------------------------------------------------------ */
+int oracle_greedy_place(const int16_t *prev /*[L,NS]*/, const double *A /*[L,S,E]*/, const double *B /*[L,E]*/,
+                        const double *D /*[S,G]*/, const double *M /*[L,E,G] or NULL*/, double M_scalar,
+                        int L, int S, int E, int G, int sp, double alpha, double beta, double gamma,
+                        int16_t *out /*[L,NS]*/)
+{
+    const int NS = G * sp;
+    int ok = 1;
+    double *x0 = (double *)malloc(sizeof(double) * (size_t)E * G), *r = (double *)malloc(sizeof(double) * E);
+    double *hot = (double *)malloc(sizeof(double) * NS), *Lcur = (double *)malloc(sizeof(double) * G);
+    int *order = (int *)malloc(sizeof(int) * NS), *fill = (int *)malloc(sizeof(int) * G);
+    char *has = (char *)malloc((size_t)E * G);
+    for (int i = 0; i < L * NS; ++i) out[i] = -1;
+    for (int l = 0; l < L; ++l) {
+        const int16_t *pv = prev + (size_t)l * NS;
+        const double *Al = A + (size_t)l * S * E, *Bl = B + (size_t)l * E;
+        int lok = 1;
+        if (!build_x(pv, E, G, sp, x0, r)) { ok = 0; continue; }
+        /* 1. hotness ranking of the items (selection sort on the total order) */
+        for (int j = 0; j < NS; ++j) {
+            int e = pv[j];
+            double vol = 0.0;
+            for (int s = 0; s < S; ++s) vol += Al[(size_t)s * E + e];
+            hot[j] = (Bl[e] + vol) / r[e];
+            order[j] = j;
+        }
+        for (int i = 0; i < NS; ++i) {
+            int best = i;
+            for (int j = i + 1; j < NS; ++j) {
+                int a = order[j], b = order[best];
+                int before_ = hot[a] > hot[b] || (hot[a] == hot[b] && (pv[a] < pv[b] || (pv[a] == pv[b] && a < b)));
+                if (before_) best = j;
+            }
+            int t = order[i]; order[i] = order[best]; order[best] = t;
+        }
+        /* 2.-3. greedy assignment */
+        for (int g = 0; g < G; ++g) { Lcur[g] = 0.0; fill[g] = 0; }
+        memset(has, 0, (size_t)E * G);
+        for (int i = 0; i < NS && lok; ++i) {
+            int e = pv[order[i]];
+            double b = Bl[e] / r[e];
+            int bg = -1, bmig = 0, bfill = 0; double bs = 0.0;
+            for (int g = 0; g < G; ++g) {
+                if (fill[g] >= sp || has[(size_t)e * G + g]) continue;
+                double c = 0.0;
+                for (int s = 0; s < S; ++s) c += Al[(size_t)s * E + e] * D[(size_t)s * G + g];
+                c = c / r[e];
+                int mig = x0[(size_t)e * G + g] == 0.0;
+                double m = mig ? (M ? M[((size_t)l * E + e) * G + g] : M_scalar) : 0.0;
+                double load = Lcur[g] + b;
+                double sc = ((alpha * c) + (beta * load)) + (gamma * m);
+                int better = bg < 0 || sc < bs || (sc == bs && (mig < bmig || (mig == bmig && fill[g] < bfill)));
+                if (better) { bg = g; bs = sc; bmig = mig; bfill = fill[g]; }
+            }
+            if (bg < 0) { lok = 0; break; }
+            out[(size_t)l * NS + bg * sp + fill[bg]] = (int16_t)e;
+            fill[bg]++; has[(size_t)e * G + bg] = 1; Lcur[bg] += b;
+        }
+        if (!lok) { ok = 0; for (int j = 0; j < NS; ++j) out[(size_t)l * NS + j] = -1; }
+    }
+    free(x0); free(r); free(hot); free(Lcur); free(order); free(fill); free(has);
+    return ok;
+}
+
 /* threads the OpenMP loops above will use (reported as cpu_baseline.cores by bench.py) */
 #ifdef _OPENMP
 #include <omp.h>

@@ -19,10 +19,10 @@ EXPORTED_SYMBOLS = [
     "gimbal_route_stats_workspace_bytes", "gimbal_route_stats", "gimbal_route_stats_result_bytes",
     "gimbal_route_stats_host",
     "gimbal_eval_placements_workspace_bytes", "gimbal_eval_placements", "gimbal_eval_placements_host",
-    "gimbal_eval_moves_workspace_bytes", "gimbal_eval_moves",
+    "gimbal_eval_moves_workspace_bytes", "gimbal_eval_moves", "gimbal_greedy_place",
     "gimbal_kernel_timing", "gimbal_kernel_elapsed_ms",
 ]
-KERNEL_ROUTER, KERNEL_GATE, KERNEL_SCORE, KERNEL_MOVES = 0, 1, 2, 3
+KERNEL_ROUTER, KERNEL_GATE, KERNEL_SCORE, KERNEL_MOVES, KERNEL_GREEDY = 0, 1, 2, 3, 4
 
 
 class GimbalError(RuntimeError):
@@ -68,7 +68,7 @@ def lib():
                   "gimbal_eval_placements_workspace_bytes", "gimbal_eval_moves_workspace_bytes"):
             getattr(L, n).restype = C.c_size_t
         for n in ("gimbal_route_stats", "gimbal_route_stats_host", "gimbal_eval_placements",
-                  "gimbal_eval_placements_host", "gimbal_eval_moves"):
+                  "gimbal_eval_placements_host", "gimbal_eval_moves", "gimbal_greedy_place"):
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -273,3 +273,11 @@ def eval_moves(cfg: PlacementCfg, cur, prev, A, B, D, delta, *, moves=None, n_mo
                                  _ptr(D), _ptr(M), C.c_float(M_scalar), _ptr(delta), _ptr(best_per_layer), _ptr(workspace),
                                  C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream))
     _check(rc, "gimbal_eval_moves")
+
+
+def greedy_place(cfg: PlacementCfg, A, B, D, prev, out, *, M=None, M_scalar: float = 1.0, status=None, stream=None):
+    """gimbal_greedy_place (NEXT-1): the paper's online greedy heuristic, out [L,NS] int16 slot -> expert."""
+    c = cfg.c()
+    rc = lib().gimbal_greedy_place(C.byref(c), _ptr(A), _ptr(B), _ptr(D), _ptr(M), C.c_float(M_scalar), _ptr(prev), _ptr(out),
+                                   _ptr(status), _stream(stream))
+    _check(rc, "gimbal_greedy_place")

@@ -10,6 +10,7 @@
 #include <cstring>
 
 #include "host_common.h"
+#include "greedy.cuh"
 #include "placement.cuh"
 #include "stats_update.cuh"
 
@@ -539,6 +540,30 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
         best_to_index_kernel<<<(cfg->L + 255) / 256, 256, 0, stream>>>(w.best, best_per_layer, cfg->L);
         LAUNCH_CHECK("best_to_index_kernel");
     }
+    return GIMBAL_OK;
+}
+
+int gimbal_greedy_place(const gimbal_placement_cfg* cfg, const void* A, const void* B, const float* D, const float* M, float M_scalar,
+                        const int16_t* prev, int16_t* out, int32_t* status, gimbal_stream_t stream_) {
+    int rc = validate_place_cfg(cfg);
+    if (rc) return rc;
+    if (!A || !B || !D || !prev || !out) return fail(GIMBAL_ERR_INVALID_ARG, "NULL argument");
+    const int NS = cfg->G * cfg->slots_per_rank;
+    const size_t smem = greedy_smem_bytes(cfg->E, cfg->G, NS);
+    if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "greedy placement: E=%d G=%d needs %zu B of shared memory", cfg->E, cfg->G, smem);
+    rc = require_device();
+    if (rc) return rc;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    GreedyParams gp{};
+    gp.L = cfg->L; gp.E = cfg->E; gp.G = cfg->G; gp.sp = cfg->slots_per_rank; gp.S = cfg->S;
+    gp.counts_f32 = cfg->counts_dtype == GIMBAL_COUNTS_F32;
+    gp.A = A; gp.B = B; gp.D = D; gp.M = M; gp.M_scalar = M_scalar;
+    gp.alpha = cfg->alpha; gp.beta = cfg->beta; gp.gamma = cfg->gamma; gp.prev = prev; gp.out = out; gp.status = status;
+    CUDA_TRY(cudaFuncSetAttribute(greedy_place_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ktime_begin(GIMBAL_KERNEL_GREEDY, stream);
+    greedy_place_kernel<<<cfg->L, kGreedyThreads, smem, stream>>>(gp);
+    ktime_end(GIMBAL_KERNEL_GREEDY, stream);
+    LAUNCH_CHECK("greedy_place_kernel");
     return GIMBAL_OK;
 }
 

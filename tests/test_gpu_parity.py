@@ -456,3 +456,54 @@ def test_gemm_special_cases():
                       logits_mode=g.LOGITS_OUT, logits=logits, workspace=ws)
         assert torch.all(logits == 256.0)
     os.environ.pop("GIMBAL_CTA_GROUP")
+
+
+# ------------------------------------------------------------------------------------------
+# NEXT-1: greedy placement heuristic -- integer output, bit-exact
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,counts,table_M,seeded_D", [
+    ("tiny", "i32", False, False), ("v2lite", "f32", True, True), ("qwen3", "i32", False, True),
+    ("v3", "i32", False, False), ("v3", "f32", True, True), ("decode", "f32", False, False), ("decode", "i32", True, True),
+])
+def test_greedy_place_parity(name, counts, table_M, seeded_D):
+    w, cfg, A, B, D, M, prev = _placement_instance(name, 4, counts, table_M, seeded_D)
+    out = torch.full_like(prev, -7)
+    status = torch.zeros(1, dtype=torch.int32, device=DEV)
+    g.greedy_place(cfg, A, B, D, prev, out, M=M, M_scalar=1.25, status=status)
+    torch.cuda.synchronize()
+    # the cfg carries the weights as fp32: the oracle gets exactly those values
+    wts = tuple(float(np.float32(x)) for x in (cfg.alpha, cfg.beta, cfg.gamma))
+    ok, ref = oracle.greedy_place(to_np(prev), to_np(A), to_np(B), to_np(D), to_np(M), 1.25, G=cfg.G, sp=cfg.slots_per_rank, weights=wts)
+    np.testing.assert_array_equal(to_np(out), ref)                       # bit-exact placement, failed layers (-1) included
+    assert bool(status.item() & 2) == (not ok)
+    good = (ref >= 0).all(1)
+    assert good.any()
+    for l in np.nonzero(good)[0]:                                        # valid placement with x0's expert copies
+        assert sorted(ref[l].tolist()) == sorted(to_np(prev)[l].tolist())
+    # the result scores through a6 like any candidate (valid: no NaN)
+    if good.all():
+        cands = torch.stack([prev, out]).contiguous()
+        sc = torch.empty(2, 5, device=DEV)
+        ws = ws_tensor(g.eval_placements_workspace_bytes(cfg, 2))
+        g.eval_placements(cfg, cands, A, B, D, prev, sc, M=M, M_scalar=1.25, workspace=ws)
+        s = to_np(sc)
+        assert not np.isnan(s).any()
+
+
+def test_greedy_place_invalid_x0_and_other_weights():
+    w, cfg, A, B, D, M, prev = _placement_instance("v3", 5)
+    bad = prev.clone(); bad[1, 0] = bad[1, 1]
+    out = torch.zeros_like(prev)
+    status = torch.zeros(1, dtype=torch.int32, device=DEV)
+    g.greedy_place(cfg, A, B, D, bad, out, status=status)
+    ok, ref = oracle.greedy_place(to_np(bad), to_np(A), to_np(B), to_np(D), None, 1.0, G=cfg.G, sp=cfg.slots_per_rank,
+                                  weights=tuple(float(np.float32(x)) for x in (cfg.alpha, cfg.beta, cfg.gamma)))
+    assert not ok and (ref[1] == -1).all()
+    np.testing.assert_array_equal(to_np(out), ref)
+    assert int(status.item()) & 2
+    for wts in [(1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (0.0, 0.0, 0.0), (1.0, 0.0025, 1e9)]:
+        cfg2 = g.PlacementCfg(L=cfg.L, E=cfg.E, G=cfg.G, slots_per_rank=cfg.slots_per_rank, S=cfg.S, alpha=wts[0], beta=wts[1], gamma=wts[2])
+        g.greedy_place(cfg2, A, B, D, prev, out)
+        ok, ref = oracle.greedy_place(to_np(prev), to_np(A), to_np(B), to_np(D), None, 1.0, G=cfg.G, sp=cfg.slots_per_rank,
+                                      weights=tuple(float(np.float32(x)) for x in wts))
+        np.testing.assert_array_equal(to_np(out), ref)

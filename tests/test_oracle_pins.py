@@ -426,3 +426,115 @@ def test_bruteforce_tiny_config_full_enumeration():
     assert n == 63063000
     d = oracle.move_deltas(bp[None], prev, oracle.all_pair_moves(1, E), A, B, D, None, 1.0, G=G, sp=sp)
     assert d[:, 0].min() >= -1e-7
+
+
+# =========================================================================== NEXT-1 greedy heuristic
+def _valid_like(out, prev, G, sp):
+    for l in range(prev.shape[0]):
+        assert sorted(out[l].tolist()) == sorted(prev[l].tolist())            # same expert copies as x0
+        for g in range(G):
+            seg = out[l, g * sp:(g + 1) * sp].tolist()
+            assert len(set(seg)) == sp                                          # never twice on one rank
+
+
+def test_greedy_worked_examples():
+    gold = json.load(open(os.path.join(GOLD, "greedy_worked_examples.json")))
+    ins = gold["instance"]
+    A, B, D = np.array(ins["A"], float), np.array(ins["B"], float), np.array(ins["D"], float)
+    for c in gold["cases"]:
+        ok, out = oracle.greedy_place(np.array(c["prev"], np.int16), A, B, D, None, ins["M_scalar"], G=ins["G"],
+                                      sp=ins["slots_per_rank"], weights=tuple(c["weights"]))
+        assert ok, c["name"]
+        assert out.tolist() == c["out"], c["name"]
+
+
+def _greedy_instance(rng, L, S, E, G, sp, replicas=False):
+    NS = G * sp
+    A = rng.integers(0, 500, (L, S, E)).astype(float)
+    B = A.sum(1) * rng.integers(1, 4, (L, E))
+    D = rng.random((S, G)) * 2
+    prev = np.empty((L, NS), np.int16)
+    for l in range(L):
+        while True:
+            base = np.concatenate([np.arange(E), rng.choice(E, NS - E, replace=False)]) if replicas else np.arange(E)
+            row = rng.permutation(base)
+            if all(len(set(row[g * sp:(g + 1) * sp])) == sp for g in range(G)):
+                break
+        prev[l] = row
+    return A, B, D, prev
+
+
+def test_greedy_is_lpt_when_only_load_counts():
+    """alpha = gamma = 0: the heuristic is textbook LPT list scheduling with a slot capacity -- heaviest item
+    first onto the least-loaded rank that still has room (restated here with plain Python); equal loads (the
+    empty ranks at the start) fall to the paper's tie-break: avoid migration, then less-filled, then index."""
+    rng = np.random.default_rng(5)
+    L, S, E, G, sp = 3, 2, 24, 4, 6
+    A, B, D, prev = _greedy_instance(rng, L, S, E, G, sp)
+    B = (rng.permutation(E * L).reshape(L, E) + 1) * 1000.0 + rng.random((L, E))   # distinct loads -> no ties
+    A = np.zeros_like(A)                                                        # hotness = B
+    ok, out = oracle.greedy_place(prev, A, B, D, None, 1.0, G=G, sp=sp, weights=(0.0, 1.0, 0.0))
+    assert ok
+    for l in range(L):
+        loads, bins = [0.0] * G, [[] for _ in range(G)]
+        for e in np.argsort(-B[l], kind="stable"):
+            home = int(np.nonzero(prev[l] == e)[0][0]) // sp
+            g = min((g for g in range(G) if len(bins[g]) < sp), key=lambda g: (loads[g], g != home, len(bins[g]), g))
+            bins[g].append(int(e)); loads[g] += B[l, e]
+        assert out[l].tolist() == [e for b in bins for e in b]
+
+
+def test_greedy_invariants_and_tie_breaks():
+    rng = np.random.default_rng(6)
+    for replicas in (False, True):
+        L, S, E, G, sp = 2, 3, 16, 4, 5 if replicas else 4
+        for attempt in range(20):       # with replicas the last items can find every free rank already holding
+            A, B, D, prev = _greedy_instance(rng, L, S, E, G, sp, replicas)      # their expert: such a layer is -1
+            ok, out = oracle.greedy_place(prev, A, B, D, None, 1.0, G=G, sp=sp)
+            if ok:
+                break
+            assert ((out == -1).all(1) | (out >= 0).all(1)).all()
+        assert ok
+        _valid_like(out, prev, G, sp)
+        # a prohibitive migration cost keeps every expert on its rank (x0 itself is feasible)
+        ok, stay = oracle.greedy_place(prev, A, B, D, None, 1e12, G=G, sp=sp, weights=(1.0, 0.0025, 1.0))
+        assert ok
+        for l in range(L):
+            for g in range(G):
+                assert set(stay[l, g * sp:(g + 1) * sp]) == set(prev[l, g * sp:(g + 1) * sp])
+        # gamma = 0 and M irrelevant: same result whatever M is
+        o1 = oracle.greedy_place(prev, A, B, D, None, 1.0, G=G, sp=sp, weights=(1.0, 0.0025, 0.0))[1]
+        o2 = oracle.greedy_place(prev, A, B, D, None, 77.0, G=G, sp=sp, weights=(1.0, 0.0025, 0.0))[1]
+        assert np.array_equal(o1, o2)
+        # scaling all three weights by a power of two leaves every comparison, hence the placement, unchanged
+        o3 = oracle.greedy_place(prev, A, B, D, None, 1.0, G=G, sp=sp, weights=(4.0, 0.01, 4.0))[1]
+        o4 = oracle.greedy_place(prev, A, B, D, None, 1.0, G=G, sp=sp, weights=(1.0, 0.0025, 1.0))[1]
+        assert np.array_equal(o3, o4)
+    # invalid x0 (expert twice on a rank) -> that layer is -1, the other layer is still placed
+    bad = prev.copy(); bad[0, 1] = bad[0, 0]
+    ok, out = oracle.greedy_place(bad, A, B, D, None, 1.0, G=G, sp=sp)
+    assert not ok and (out[0] == -1).all() and (out[1] >= 0).all()
+
+
+def test_greedy_against_bruteforce_optimum_on_small_instances():
+    """With beta = 0 the local score is the marginal change of the (linear) objective alpha*C_comm + gamma*C_mig --
+    a moved expert costs M at the rank it enters AND at the rank it leaves (R10), so gamma_local = 2*gamma_J.
+    The heuristic is not optimal (capacity couples the choices), but its objective must lie between the
+    brute-force optimum and a typical random placement, much nearer the optimum."""
+    rng = np.random.default_rng(8)
+    gaps = []
+    for trial in range(12):
+        S, E, G, sp = 2, 8, 4, 2
+        A, B, D, prev = _greedy_instance(rng, 1, S, E, G, sp)
+        B = A.sum(1)
+        wJ, wloc = (1.0, 0.0, 25.0), (1.0, 0.0, 50.0)
+        ok, out = oracle.greedy_place(prev, A, B, D, None, 1.0, G=G, sp=sp, weights=wloc)
+        assert ok
+        Jg = oracle.objective(out, prev, A, B, D, None, 1.0, G=G, sp=sp, weights=wJ)[0]
+        n, Jopt, _ = oracle.bruteforce(prev[0], A[0], B[0], D, None, 1.0, G=G, sp=sp, weights=wJ)
+        Jrand = np.mean([oracle.objective(rng.permutation(E).astype(np.int16)[None], prev, A, B, D, None, 1.0, G=G, sp=sp,
+                                          weights=wJ)[0] for _ in range(50)])
+        assert n == math.factorial(E) // (math.factorial(sp) ** G)
+        assert Jopt <= Jg * (1 + 1e-12)
+        gaps.append((Jg - Jopt) / (Jrand - Jopt))
+    assert np.median(gaps) < 0.5, gaps      # typical instance: well inside the optimum's half of the range
