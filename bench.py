@@ -201,7 +201,8 @@ def _config(w, args):
                 parallelism="replicas only (no cross-GPU exchange on this path)",
                 l2="hidden states of one step (>> L2) stream through L2 between the placement kernels; an explicit 256 MiB flush runs "
                    "between timed steps, outside the timed events",
-                outputs="A_step/B/pressure (a3-a5), out[P,5]+argmin (a6), delta[n,5]+best_per_layer (a7); top-k ids not written")
+                outputs="A_step/B/pressure (a3-a5), out[P,5]+argmin (a6), delta[n,5]+best_per_layer (a7); top-k ids and weights "
+                        + ("written" if getattr(args, "with_ids", False) else "not written"))
 
 
 def run_ours(args, w):
@@ -251,8 +252,12 @@ def run_ours(args, w):
     # profile the placement side reads: this step's counts (window mode) or the EMA state
     A_live, B_live = (st.A_step if w.mode == MODE_WINDOW else st.A_ema), st.B
 
+    ids_out = torch.empty(r.L, w.T, r.k, dtype=torch.int32, device=dev) if args.with_ids else None
+    w_out = torch.empty(r.L, w.T, r.k, dtype=torch.float32, device=dev) if args.with_ids else None
+
     def step():
         g.route_stats(cfg, st, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off,
+                      topk_ids=ids_out, topk_w=w_out,
                       cur_placement=cur, dp_of_rank=dp, G=w.G, slots_per_rank=w.slots_per_rank, workspace=ws_r)
         g.eval_placements(pc, cands, A_live, B_live, D, prev, out, argmin=argmin, workspace=ws_p)
         g.eval_moves(pc, cur, prev, A_live, B_live, D, delta, best_per_layer=best, workspace=ws_p)
@@ -414,6 +419,7 @@ def main():
     ap.add_argument("--workload", default="v3", choices=["tiny", "v2lite", "qwen3", "v3", "decode"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    ap.add_argument("--with-ids", action="store_true", help="also write top-k ids and weights (a2 outputs) inside the timed step")
     ap.add_argument("--layers", type=int, default=0, help="profiling only: run the first N MoE layers (named in config.workload)")
     args = ap.parse_args()
     w = get_workload(args.workload)

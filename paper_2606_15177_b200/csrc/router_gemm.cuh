@@ -47,21 +47,23 @@ constexpr int gemm_stage_bytes() { return kBlockM * kBlockK * 2 + (N / kCG) * kB
 constexpr int kGemmAuxBytes = 1024;  // barriers + tmem pointer (<= 12 stages)
 constexpr int kGemmMaxStages = 12;
 
-// bytes after the ring: [aux][select_bias N f32][src_offsets S+1 (padded)][hist S*N i32]
+// bytes after the ring: [aux][select_bias N f32][src_offsets S+1 (padded)][hist S*N i32][selection list, when
+// ids / weights are written: kListWords x 128 epilogue threads]
 template <int N>
-constexpr size_t gemm_tail_bytes(int S) {
-    return kGemmAuxBytes + sizeof(float) * N + sizeof(int32_t) * (size_t)((S + 1 + 3) & ~3) + sizeof(int32_t) * (size_t)S * N;
+constexpr size_t gemm_tail_bytes(int S, bool out) {
+    return kGemmAuxBytes + sizeof(float) * N + sizeof(int32_t) * (size_t)((S + 1 + 3) & ~3) + sizeof(int32_t) * (size_t)S * N +
+           (out ? sizeof(int32_t) * (size_t)kListWords * 128 : 0);
 }
 template <int N, int kCG>
-inline int gemm_pick_stages(int S) {
-    const long avail = (long)kGemmSmemLimit - 1024 - (long)gemm_tail_bytes<N>(S);
+inline int gemm_pick_stages(int S, bool out) {
+    const long avail = (long)kGemmSmemLimit - 1024 - (long)gemm_tail_bytes<N>(S, out);
     long s = avail / gemm_stage_bytes<N, kCG>();
     if (s > kGemmMaxStages) s = kGemmMaxStages;
     return (int)s;
 }
 template <int N, int kCG>
-inline size_t gemm_smem_bytes(int S, int stages) {
-    return 1024 + (size_t)stages * gemm_stage_bytes<N, kCG>() + gemm_tail_bytes<N>(S);
+inline size_t gemm_smem_bytes(int S, int stages, bool out) {
+    return 1024 + (size_t)stages * gemm_stage_bytes<N, kCG>() + gemm_tail_bytes<N>(S, out);
 }
 
 template <int N>
@@ -133,6 +135,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
     float* sb_s = reinterpret_cast<float*>(base_ptr + kStages * kStageBytes + kGemmAuxBytes);
     int32_t* off_s = reinterpret_cast<int32_t*>(sb_s + N);
     int32_t* hist = off_s + ((p.S + 1 + 3) & ~3);
+    int32_t* list_s = hist + p.S * N;                    // [kListWords][128] (only when ids / weights are written)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t cta_rank = (kCG == 2) ? ptx::cluster_ctarank() : 0u;
@@ -274,7 +277,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
                 float w[kTopK];
                 const bool valid = t < p.T;
                 if (p.topk_ids || p.topk_w) {
-                    gate_row<N, kSig, true>(p.gp, sb_s, src, valid, hist + s * N, ids, w);
+                    gate_row<N, kSig, true>(p.gp, sb_s, src, valid, hist + s * N, list_s + ep_tid, 128, ids, w);
                     if (valid && p.topk_ids) {
                         int32_t* o = p.topk_ids + ((size_t)li * p.T + t) * p.gp.k;
 #pragma unroll
@@ -288,7 +291,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
                             if (j < p.gp.k) o[j] = w[j];
                     }
                 } else {
-                    gate_row<N, kSig, false>(p.gp, sb_s, src, valid, hist + s * N, ids, w);
+                    gate_row<N, kSig, false>(p.gp, sb_s, src, valid, hist + s * N, nullptr, 0, ids, w);
                 }
             }
             // release this accumulator stage to the MMA issuer
