@@ -125,6 +125,23 @@ typedef struct gimbal_placement_cfg {
     int32_t counts_dtype;
 } gimbal_placement_cfg;
 
+/* Expert mapping (NEXT-3; "fuse source counting with expert mapping"): the
+ * logical expert ids chosen by the router become PHYSICAL slot ids under a placement, in the
+ * same kernel that counts.  The slots hosting expert e, in ascending order, are s_0 < ... <
+ * s_{r-1}; token t (its index in the step's token list) is sent to s_{t mod r} -- the even split
+ * over replicas that the objective assumes (R12, R18); r = 1 in the paper.
+ *   rep_off   [L, E+1] i32   expert e of layer l owns rep_slots[l, rep_off[l,e] .. rep_off[l,e+1])
+ *   rep_slots [L, NS]  i16   slot ids grouped by expert, ascending inside a group
+ *       (both are written by gimbal_build_expert_map from a slot -> expert placement)
+ *   phys_ids  [n_layers, T, k] i32 out   slot id per (token, choice), in the order of topk_ids;
+ *       rank = slot / slots_per_rank; -1 if the placement does not host that expert            */
+typedef struct gimbal_expert_map {
+    const int32_t *rep_off;
+    const int16_t *rep_slots;
+    int32_t *phys_ids;
+    int32_t NS;
+} gimbal_expert_map;
+
 /* Library / device probe.  gimbal_version() never touches CUDA. */
 GIMBAL_API int gimbal_version(void);
 /* Writes the last CUDA / validation error string (NUL-terminated, truncated to n). */
@@ -152,6 +169,7 @@ GIMBAL_API void gimbal_last_error(char *buf, size_t n);
  *   cur_placement [L,NS] i16 | NULL,  dp_of_rank [G] i32 | NULL : needed for the pressure
  *                                      outputs only (both NULL: pressure is left untouched)
  *   G, slots_per_rank                  shape of cur_placement
+ *   map           | NULL               expert mapping: phys_ids written next to the counts
  * Errors: INVALID_ARG (NULL / shape / alignment), UNSUPPORTED (shape outside the compiled
  * range, no sm_100 device), WORKSPACE (workspace_bytes too small), CUDA.                  */
 GIMBAL_API size_t gimbal_route_stats_workspace_bytes(const gimbal_router_cfg *cfg, int n_layers, int T);
@@ -162,8 +180,13 @@ GIMBAL_API int gimbal_route_stats(const gimbal_router_cfg *cfg, int layer0, int 
                        const int32_t *src_offsets, int logits_mode, float *logits,
                        int32_t *topk_ids, float *topk_w,
                        const int16_t *cur_placement, const int32_t *dp_of_rank, int G, int slots_per_rank,
-                       gimbal_stats_state *state, void *workspace, size_t workspace_bytes,
-                       gimbal_stream_t stream);
+                       gimbal_stats_state *state, const gimbal_expert_map *map /* | NULL */,
+                       void *workspace, size_t workspace_bytes, gimbal_stream_t stream);
+
+/* Inverse of a slot -> expert placement [L,NS] for gimbal_expert_map: rep_off [L,E+1] and
+ * rep_slots [L,NS] (device, caller-owned).  Ids out of range set bit 0 of `status`.         */
+GIMBAL_API int gimbal_build_expert_map(int L, int E, int G, int slots_per_rank, const int16_t *placement,
+                            int32_t *rep_off, int16_t *rep_slots, int32_t *status, gimbal_stream_t stream);
 
 /* Same step with the per-step inputs in HOST memory: hidden_host [n_layers,T,H] bf16 and
  * src_offsets_host [S+1] are copied to the device staging buffers the caller provides

@@ -114,6 +114,16 @@ def counts(ids, src_offsets, S: int, E: int):
     return out
 
 
+def expert_map(ids, place):
+    """ids [T,k] int32 logical experts, place [NS] int16 slot -> expert -> phys [T,k] int32 slots (NEXT-3, R18)."""
+    ids = _c(ids, np.int32); place = _c(place, np.int16)
+    T, k = ids.shape
+    out = np.empty((T, k), np.int32)
+    lib().oracle_expert_map(_p(ids, C.c_int32), _p(place, C.c_int16), C.c_int(T), C.c_int(k), C.c_int(place.shape[0]),
+                            _p(out, C.c_int32))
+    return out
+
+
 # -- a4 ---------------------------------------------------------------------------------
 def update_window(A_win, Cstep, A_pub, step: int, window_len: int) -> bool:
     """in place on int64 arrays; returns True when the window was published."""

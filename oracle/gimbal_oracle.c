@@ -576,6 +576,29 @@ int oracle_greedy_place(const int16_t *prev /*[L,NS]*/, const double *A /*[L,S,E
     return ok;
 }
 
+/* ------------------------------------------------------------------------------------ */
+/* NEXT-3  Expert mapping, logical -> physical ("fuse source counting with expert mapping",
+ *     PAPER.md:276, 368; R18): under placement `place` (slot -> expert) the slots
+ *     hosting expert e, in ascending order, are s_0 < ... < s_{r-1}; the choice (t, j) with
+ *     ids[t,j] = e goes to slot s_{t mod r} (t = token index in the step).  r = 1 in the paper.
+ *     phys[t,j] = -1 when no slot hosts e.                                                 */
+/* ------------------------------------------------------------------------------------ */
+void oracle_expert_map(const int32_t *ids /*[T,k]*/, const int16_t *place /*[NS]*/, int T, int k, int NS,
+                       int32_t *phys /*[T,k]*/)
+{
+    for (int t = 0; t < T; ++t)
+        for (int j = 0; j < k; ++j) {
+            int e = ids[(size_t)t * k + j], r = 0, pick = -1;
+            for (int s = 0; s < NS; ++s) r += (place[s] == e);
+            if (r > 0) {
+                int want = t % r, seen = 0;
+                for (int s = 0; s < NS; ++s)
+                    if (place[s] == e) { if (seen == want) { pick = s; break; } ++seen; }
+            }
+            phys[(size_t)t * k + j] = pick;
+        }
+}
+
 /* threads the OpenMP loops above will use (reported as cpu_baseline.cores by bench.py) */
 #ifdef _OPENMP
 #include <omp.h>

@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = [
     "gimbal_route_stats_workspace_bytes", "gimbal_route_stats", "gimbal_route_stats_result_bytes",
     "gimbal_route_stats_host",
     "gimbal_eval_placements_workspace_bytes", "gimbal_eval_placements", "gimbal_eval_placements_host",
-    "gimbal_eval_moves_workspace_bytes", "gimbal_eval_moves", "gimbal_greedy_place",
+    "gimbal_eval_moves_workspace_bytes", "gimbal_eval_moves", "gimbal_greedy_place", "gimbal_build_expert_map",
     "gimbal_kernel_timing", "gimbal_kernel_elapsed_ms",
 ]
 KERNEL_ROUTER, KERNEL_GATE, KERNEL_SCORE, KERNEL_MOVES, KERNEL_GREEDY = 0, 1, 2, 3, 4
@@ -39,6 +39,10 @@ class _StatsState(C.Structure):
                 ("A_step", C.c_void_p), ("A_win", C.c_void_p), ("A_pub", C.c_void_p), ("B_pub", C.c_void_p),
                 ("A_ema", C.c_void_p), ("B", C.c_void_p), ("pressure_raw", C.c_void_p), ("pressure_rel", C.c_void_p),
                 ("step_counter", C.c_void_p), ("status", C.c_void_p)]
+
+
+class _ExpertMap(C.Structure):
+    _fields_ = [("rep_off", C.c_void_p), ("rep_slots", C.c_void_p), ("phys_ids", C.c_void_p), ("NS", C.c_int32)]
 
 
 class _PlacementCfg(C.Structure):
@@ -68,7 +72,7 @@ def lib():
                   "gimbal_eval_placements_workspace_bytes", "gimbal_eval_moves_workspace_bytes"):
             getattr(L, n).restype = C.c_size_t
         for n in ("gimbal_route_stats", "gimbal_route_stats_host", "gimbal_eval_placements",
-                  "gimbal_eval_placements_host", "gimbal_eval_moves", "gimbal_greedy_place"):
+                  "gimbal_eval_placements_host", "gimbal_eval_moves", "gimbal_greedy_place", "gimbal_build_expert_map"):
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -199,17 +203,35 @@ def route_stats_workspace_bytes(cfg: RouterCfg, n_layers: int, T: int) -> int:
 def route_stats(cfg: RouterCfg, state: StatsState, *, T: int, hidden=None, w_router=None, select_bias=None,
                 src_logit_bias=None, src_offsets=None, layer0: int = 0, n_layers: int | None = None,
                 logits_mode: int = LOGITS_NONE, logits=None, topk_ids=None, topk_w=None, cur_placement=None,
-                dp_of_rank=None, G: int = 0, slots_per_rank: int = 0, workspace=None, stream=None):
-    """gimbal_route_stats (a1..a5).  All tensors are CUDA tensors owned by the caller."""
+                dp_of_rank=None, G: int = 0, slots_per_rank: int = 0, expert_map=None, phys_ids=None, workspace=None,
+                stream=None):
+    """gimbal_route_stats (a1..a5).  All tensors are CUDA tensors owned by the caller.
+    expert_map = ExpertMap (build_expert_map) + phys_ids [n_layers,T,k] int32: physical slot ids (NEXT-3)."""
     n_layers = cfg.L - layer0 if n_layers is None else n_layers
     c, s = cfg.c(), state.c()
+    m = None
+    if expert_map is not None:
+        m = _ExpertMap(expert_map.rep_off.data_ptr(), expert_map.rep_slots.data_ptr(), phys_ids.data_ptr(), expert_map.NS)
     rc = lib().gimbal_route_stats(C.byref(c), C.c_int(layer0), C.c_int(n_layers), C.c_int(T), _ptr(hidden), _ptr(w_router),
                                   _ptr(select_bias), _ptr(src_logit_bias), _ptr(src_offsets), C.c_int(logits_mode),
                                   _ptr(logits), _ptr(topk_ids), _ptr(topk_w), _ptr(cur_placement), _ptr(dp_of_rank),
-                                  C.c_int(G), C.c_int(slots_per_rank), C.byref(s), _ptr(workspace),
+                                  C.c_int(G), C.c_int(slots_per_rank), C.byref(s), C.byref(m) if m is not None else C.c_void_p(None),
+                                  _ptr(workspace),
                                   C.c_size_t(0 if workspace is None else workspace.numel() * workspace.element_size()),
                                   _stream(stream))
     _check(rc, "gimbal_route_stats")
+
+
+class ExpertMap:
+    """Device buffers of gimbal_expert_map (allocation + gimbal_build_expert_map)."""
+
+    def __init__(self, L: int, E: int, G: int, slots_per_rank: int, placement, status=None, stream=None):
+        self.NS = G * slots_per_rank
+        self.rep_off = torch.empty(L, E + 1, dtype=torch.int32, device=placement.device)
+        self.rep_slots = torch.empty(L, self.NS, dtype=torch.int16, device=placement.device)
+        rc = lib().gimbal_build_expert_map(C.c_int(L), C.c_int(E), C.c_int(G), C.c_int(slots_per_rank), _ptr(placement),
+                                           _ptr(self.rep_off), _ptr(self.rep_slots), _ptr(status), _stream(stream))
+        _check(rc, "gimbal_build_expert_map")
 
 
 def route_stats_host(cfg: RouterCfg, state: StatsState, *, T: int, hidden_host, src_offsets_host, hidden_stage,

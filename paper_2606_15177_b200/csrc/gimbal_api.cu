@@ -206,6 +206,34 @@ static int launch_score_fast(const ScoreParams& sp, bool dup, dim3 grid, size_t 
     return dup ? launch_score_fast_v<SP, G, true, false>(sp, grid, smem, stream) : launch_score_fast_v<SP, G, false, false>(sp, grid, smem, stream);
 }
 
+// inverse of a slot -> expert placement: one block per layer, thread e collects expert e's slots in
+// ascending order (deterministic)
+__global__ void __launch_bounds__(256) expert_map_kernel(int E, int NS, const int16_t* placement, int32_t* rep_off, int16_t* rep_slots,
+                                                         int32_t* status) {
+    __shared__ int cnt_s[kMaxE + 1];
+    __shared__ int16_t pl_s[kMaxG * 16];
+    const int l = blockIdx.x, tid = threadIdx.x;
+    for (int e = tid; e <= E; e += 256) cnt_s[e] = 0;
+    __syncthreads();
+    bool bad = false;
+    for (int j = tid; j < NS; j += 256) {
+        const int e = placement[(size_t)l * NS + j];
+        pl_s[j] = (int16_t)e;
+        if (e < 0 || e >= E) bad = true; else atomicAdd(&cnt_s[e + 1], 1);
+    }
+    if (bad && status) atomicOr(status, 1);
+    __syncthreads();
+    if (tid == 0)
+        for (int e = 0; e < E; ++e) cnt_s[e + 1] += cnt_s[e];          // exclusive offsets in cnt_s[0..E]
+    __syncthreads();
+    for (int e = tid; e <= E; e += 256) rep_off[(size_t)l * (E + 1) + e] = cnt_s[e];
+    for (int e = tid; e < E; e += 256) {
+        int pos = cnt_s[e];
+        for (int j = 0; j < NS; ++j)
+            if (pl_s[j] == e) rep_slots[(size_t)l * NS + pos++] = (int16_t)j;
+    }
+}
+
 }  // namespace
 
 extern "C" {
@@ -237,9 +265,11 @@ size_t gimbal_route_stats_result_bytes(const gimbal_router_cfg* cfg) {
 int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, int T, const void* hidden, const void* w_router,
                        const float* select_bias, const float* src_logit_bias, const int32_t* src_offsets, int logits_mode,
                        float* logits, int32_t* topk_ids, float* topk_w, const int16_t* cur_placement, const int32_t* dp_of_rank,
-                       int G, int slots_per_rank, gimbal_stats_state* st, void* workspace, size_t workspace_bytes,
-                       gimbal_stream_t stream_) {
+                       int G, int slots_per_rank, gimbal_stats_state* st, const gimbal_expert_map* map, void* workspace,
+                       size_t workspace_bytes, gimbal_stream_t stream_) {
     int rc = validate_router_cfg(cfg);
+    if (map && (!map->rep_off || !map->rep_slots || !map->phys_ids || map->NS < cfg->E))
+        return fail(GIMBAL_ERR_INVALID_ARG, "expert map needs rep_off, rep_slots, phys_ids and NS >= E");
     if (rc) return rc;
     if (layer0 < 0 || n_layers < 1 || layer0 + n_layers > cfg->L) return fail(GIMBAL_ERR_INVALID_ARG, "layer range [%d,%d) outside [0,%d)", layer0, layer0 + n_layers, cfg->L);
     if (T < 0) return fail(GIMBAL_ERR_INVALID_ARG, "T=%d", T);
@@ -279,6 +309,7 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
         a.cfg = cfg; a.layer0 = layer0; a.n_layers = n_layers; a.T = T; a.hidden = hidden; a.w_router = w_router;
         a.select_bias = select_bias; a.src_logit_bias = src_logit_bias; a.src_offsets = src_offsets;
         a.topk_ids = topk_ids; a.topk_w = topk_w; a.A_step = st->A_step; a.stream = stream;
+        if (map) { a.rep_off = map->rep_off; a.rep_slots = map->rep_slots; a.phys_ids = map->phys_ids; a.map_NS = map->NS; }
         a.cta_group = pick_cta_group(T);
         if (logits_mode == GIMBAL_LOGITS_IN) {
             a.logits = logits;
@@ -356,7 +387,7 @@ int gimbal_route_stats_host(const gimbal_router_cfg* cfg, int T, const void* hid
         CUDA_TRY(cudaEventRecord(ev_copied[slot], copy_stream));
         CUDA_TRY(cudaStreamWaitEvent(stream, ev_copied[slot], 0));
         rc = gimbal_route_stats(cfg, l, 1, T, dst, w_router, select_bias, src_logit_bias, src_offsets_stage, GIMBAL_LOGITS_NONE,
-                                nullptr, nullptr, nullptr, cur_placement, dp_of_rank, G, slots_per_rank, st, workspace,
+                                nullptr, nullptr, nullptr, cur_placement, dp_of_rank, G, slots_per_rank, st, nullptr, workspace,
                                 workspace_bytes, stream_);
         if (rc) return rc;
         CUDA_TRY(cudaEventRecord(ev_done[slot], stream));
@@ -540,6 +571,18 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
         best_to_index_kernel<<<(cfg->L + 255) / 256, 256, 0, stream>>>(w.best, best_per_layer, cfg->L);
         LAUNCH_CHECK("best_to_index_kernel");
     }
+    return GIMBAL_OK;
+}
+
+int gimbal_build_expert_map(int L, int E, int G, int slots_per_rank, const int16_t* placement, int32_t* rep_off, int16_t* rep_slots,
+                            int32_t* status, gimbal_stream_t stream_) {
+    if (L < 1 || E < 1 || E > kMaxE || G < 1 || G > kMaxG || slots_per_rank < 1 || slots_per_rank > 16)
+        return fail(GIMBAL_ERR_INVALID_ARG, "expert map: L >= 1, 1 <= E <= %d, 1 <= G <= %d, 1 <= slots_per_rank <= 16", kMaxE, kMaxG);
+    if (!placement || !rep_off || !rep_slots) return fail(GIMBAL_ERR_INVALID_ARG, "NULL argument");
+    int rc = require_device();
+    if (rc) return rc;
+    expert_map_kernel<<<L, 256, 0, static_cast<cudaStream_t>(stream_)>>>(E, G * slots_per_rank, placement, rep_off, rep_slots, status);
+    LAUNCH_CHECK("expert_map_kernel");
     return GIMBAL_OK;
 }
 

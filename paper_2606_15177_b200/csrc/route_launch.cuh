@@ -17,12 +17,13 @@ int launch_gemm_t(const RouteArgs& a) {
     GemmParams p{};
     p.n_layers = a.n_layers; p.layer0 = a.layer0; p.T = a.T; p.H = c->H; p.S = c->S;
     p.m_tiles = (a.T + kBlockM * kCG - 1) / (kBlockM * kCG);
-    const bool out = a.fuse_gate && (a.topk_ids || a.topk_w);
+    const bool out = a.fuse_gate && (a.topk_ids || a.topk_w || a.rep_off);
     p.stages = gemm_pick_stages<N, kCG>(c->S, out);
     if (p.stages < 2) return fail(GIMBAL_ERR_UNSUPPORTED, "router GEMM: not enough shared memory for E=%d S=%d", N, c->S);
     p.src_logit_bias = a.src_logit_bias; p.src_offsets = a.src_offsets; p.logits = a.logits;
     p.do_gate = a.fuse_gate; p.select_bias = a.select_bias; p.topk_ids = a.topk_ids; p.topk_w = a.topk_w;
     p.A_step = a.A_step; p.gp = gate_params(c);
+    p.map = ExpertMap{a.rep_off, a.rep_slots, a.phys_ids, a.map_NS};
     const size_t smem = gemm_smem_bytes<N, kCG>(c->S, p.stages, out);
     auto kern = router_gemm_kernel<N, kCG, kSig>;
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -71,10 +72,11 @@ int launch_gate_t(const RouteArgs& a) {
     p.logits = a.logits; p.select_bias = a.select_bias; p.src_offsets = a.src_offsets;
     p.topk_ids = a.topk_ids; p.topk_w = a.topk_w; p.A_step = a.A_step;
     p.layer0 = a.layer0; p.T = a.T; p.S = a.cfg->S; p.gp = gate_params(a.cfg);
-    const size_t smem = gate_smem_bytes<E, kWarps>(a.cfg->S, a.topk_ids || a.topk_w);
+    p.map = ExpertMap{a.rep_off, a.rep_slots, a.phys_ids, a.map_NS};
+    const size_t smem = gate_smem_bytes<E, kWarps>(a.cfg->S, a.topk_ids || a.topk_w || a.rep_off);
     if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "gating: E=%d S=%d needs %zu B of shared memory", E, a.cfg->S, smem);
     dim3 grid((a.T + kWarps * 32 - 1) / (kWarps * 32), a.n_layers);
-    const bool sig = a.cfg->score_fn == GIMBAL_SCORE_SIGMOID, out = a.topk_ids || a.topk_w;
+    const bool sig = a.cfg->score_fn == GIMBAL_SCORE_SIGMOID, out = a.topk_ids || a.topk_w || a.rep_off;
     ktime_begin(GIMBAL_KERNEL_GATE, a.stream);
     int rc;
     if (sig) rc = out ? launch_gate_v<E, true, true>(p, grid, smem, a.stream) : launch_gate_v<E, true, false>(p, grid, smem, a.stream);

@@ -35,6 +35,7 @@ struct GemmParams {
     float* topk_w;
     int32_t* A_step;                // [L,S,E]
     GateParams gp;
+    ExpertMap map;
 };
 
 constexpr int kGemmThreads = 256;
@@ -276,7 +277,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
                 int32_t ids[kTopK];
                 float w[kTopK];
                 const bool valid = t < p.T;
-                if (p.topk_ids || p.topk_w) {
+                if (p.topk_ids || p.topk_w || p.map.rep_off) {
                     gate_row<N, kSig, true>(p.gp, sb_s, src, valid, hist + s * N, list_s + ep_tid, 128, ids, w);
                     if (valid && p.topk_ids) {
                         int32_t* o = p.topk_ids + ((size_t)li * p.T + t) * p.gp.k;
@@ -290,6 +291,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
                         for (int j = 0; j < kTopK; ++j)
                             if (j < p.gp.k) o[j] = w[j];
                     }
+                    if (valid && p.map.rep_off) map_row<N>(p.map, layer, li, p.T, t, p.gp.k, ids);
                 } else {
                     gate_row<N, kSig, false>(p.gp, sb_s, src, valid, hist + s * N, nullptr, 0, ids, w);
                 }

@@ -507,3 +507,52 @@ def test_greedy_place_invalid_x0_and_other_weights():
         ok, ref = oracle.greedy_place(to_np(prev), to_np(A), to_np(B), to_np(D), None, 1.0, G=cfg.G, sp=cfg.slots_per_rank,
                                       weights=tuple(float(np.float32(x)) for x in wts))
         np.testing.assert_array_equal(to_np(out), ref)
+
+
+# ------------------------------------------------------------------------------------------
+# NEXT-3: logical -> physical expert mapping fused with counting (R18)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", list(SHAPES))
+@pytest.mark.parametrize("mode", ["logits_in", "fused"])
+def test_expert_mapping_parity(name, mode):
+    w = _wl(name)
+    r = w.router
+    cfg = g.RouterCfg.from_workload(r)
+    rng = np.random.default_rng(12)
+    place = gen.prev_placement(w, rng.integers(1, 1000, (r.L, r.E)), DEV)
+    status = torch.zeros(1, dtype=torch.int32, device=DEV)
+    emap = g.ExpertMap(r.L, r.E, w.G, w.slots_per_rank, place, status=status)
+    st = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+    ids = torch.full((r.L, w.T, r.k), -9, dtype=torch.int32, device=DEV)
+    phys = torch.full((r.L, w.T, r.k), -9, dtype=torch.int32, device=DEV)
+    ws = ws_tensor(g.route_stats_workspace_bytes(cfg, r.L, w.T))
+    sb = gen.select_bias(w, DEV)
+    if mode == "logits_in":
+        x, off = _synthetic_logits(w, 21)
+        g.route_stats(cfg, st, T=w.T, select_bias=sb, src_offsets=off, logits_mode=g.LOGITS_IN, logits=x, topk_ids=ids,
+                      expert_map=emap, phys_ids=phys, workspace=ws)
+    else:
+        hidden, W, slb, sb, off = _router_inputs(w)
+        g.route_stats(cfg, st, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off,
+                      topk_ids=ids, expert_map=emap, phys_ids=phys, workspace=ws)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0
+    pl = to_np(place)
+    for l in range(r.L):
+        ref = oracle.expert_map(to_np(ids[l]), pl[l])
+        np.testing.assert_array_equal(to_np(phys[l]), ref)                   # bit-exact slots
+        assert (pl[l][ref] == to_np(ids[l])).all()                           # every slot hosts the chosen expert
+        # the inverse tables themselves: slots grouped by expert, ascending inside a group
+        off_l, slots_l = to_np(emap.rep_off[l]), to_np(emap.rep_slots[l])
+        for e in range(r.E):
+            np.testing.assert_array_equal(slots_l[off_l[e]:off_l[e + 1]], np.nonzero(pl[l] == e)[0])
+    # the mapping does not disturb the counts; without topk_ids the same slots come out
+    st2 = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+    phys2 = torch.full_like(phys, -9)
+    if mode == "logits_in":
+        g.route_stats(cfg, st2, T=w.T, select_bias=sb, src_offsets=off, logits_mode=g.LOGITS_IN, logits=x, expert_map=emap,
+                      phys_ids=phys2, workspace=ws)
+    else:
+        g.route_stats(cfg, st2, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off,
+                      expert_map=emap, phys_ids=phys2, workspace=ws)
+    assert torch.equal(phys2, phys) and torch.equal(st2.A_step, st.A_step)

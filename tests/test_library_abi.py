@@ -50,17 +50,17 @@ def test_host_side_validation():
     c = cfg.c()
     st = g.binding._StatsState()
     rc = g.lib().gimbal_route_stats(C.byref(c), 0, 2, 16, None, None, None, None, None, 0, None, None, None, None, None, 0, 0,
-                                    C.byref(st), None, C.c_size_t(0), None)
+                                    C.byref(st), None, None, C.c_size_t(0), None)
     assert rc == -2 and "E=48" in g.last_error()
     cfg = g.RouterCfg(L=2, H=250, E=64, k=2, S=2)
     c = cfg.c()
     rc = g.lib().gimbal_route_stats(C.byref(c), 0, 2, 16, None, None, None, None, None, 0, None, None, None, None, None, 0, 0,
-                                    C.byref(st), None, C.c_size_t(0), None)
+                                    C.byref(st), None, None, C.c_size_t(0), None)
     assert rc == -2 and "multiple of 64" in g.last_error()
     cfg = g.RouterCfg(L=2, H=256, E=64, k=2, S=2)
     c = cfg.c()
     rc = g.lib().gimbal_route_stats(C.byref(c), 0, 3, 16, None, None, None, None, None, 0, None, None, None, None, None, 0, 0,
-                                    C.byref(st), None, C.c_size_t(0), None)
+                                    C.byref(st), None, None, C.c_size_t(0), None)
     assert rc == -1 and "layer range" in g.last_error()
     pc = g.PlacementCfg(L=1, E=16, G=3, slots_per_rank=6, S=2).c()
     rc = g.lib().gimbal_eval_placements(C.byref(pc), 1, None, None, None, None, None, C.c_float(1.0), None, None, None, None,
@@ -78,5 +78,5 @@ def test_no_cpu_fallback_without_gpu():
     st.A_step = st.A_win = st.A_pub = st.B_pub = st.B = st.step_counter = 16
     st.mode, st.window_len = 0, 1
     rc = g.lib().gimbal_route_stats(C.byref(c), 0, 1, 16, one, one, None, None, one, 0, None, None, None, None, None, 0, 0,
-                                    C.byref(st), one, C.c_size_t(1 << 20), None)
+                                    C.byref(st), None, one, C.c_size_t(1 << 20), None)
     assert rc == -2 and "CUDA" in g.last_error()

@@ -538,3 +538,30 @@ def test_greedy_against_bruteforce_optimum_on_small_instances():
         assert Jopt <= Jg * (1 + 1e-12)
         gaps.append((Jg - Jopt) / (Jrand - Jopt))
     assert np.median(gaps) < 0.5, gaps      # typical instance: well inside the optimum's half of the range
+
+
+# =========================================================================== NEXT-3 expert mapping
+def test_expert_map_hand_example_and_library_restatement():
+    # by hand (R18): expert 0 is hosted by slots 1 and 3, experts 1 and 2 by one slot each
+    place = np.array([2, 0, 1, 0], np.int16)
+    ids = np.array([[0, 2], [0, 2], [0, 1], [0, 1], [5, 1]], np.int32)          # expert 5 is hosted nowhere
+    assert oracle.expert_map(ids, place).tolist() == [[1, 0], [3, 0], [1, 2], [3, 2], [-1, 2]]
+    # numpy restatement on a random placement with replicas: slot = nonzero(place == e)[t mod r]
+    rng = np.random.default_rng(9)
+    E, NS, T, k = 24, 32, 500, 4
+    place = rng.permutation(np.concatenate([np.arange(E), rng.choice(E, NS - E, replace=False)])).astype(np.int16)
+    ids = np.stack([rng.permutation(E)[:k] for _ in range(T)]).astype(np.int32)
+    phys = oracle.expert_map(ids, place)
+    for t in range(0, T, 7):
+        for j in range(k):
+            slots = np.nonzero(place == ids[t, j])[0]
+            assert phys[t, j] == slots[t % len(slots)]
+    assert (place[phys] == ids).all()                                           # the chosen slot hosts the chosen expert
+    # without replicas the mapping is the inverse permutation
+    perm = rng.permutation(E).astype(np.int16)
+    inv = np.argsort(perm)
+    assert (oracle.expert_map(ids, perm) == inv[ids]).all()
+    # replicas share an expert's tokens evenly: over consecutive tokens the copies take turns
+    e = int(np.nonzero(np.bincount(place, minlength=E) == 2)[0][0])
+    hits = oracle.expert_map(np.full((10, 1), e, np.int32), place)[:, 0]
+    assert hits[::2].tolist() == [hits[0]] * 5 and hits[1::2].tolist() == [hits[1]] * 5 and hits[0] < hits[1]
