@@ -269,6 +269,22 @@ def run_ours(args, w):
     for _ in range(4):
         g.greedy_place(pc, A_live, B_live, D, prev, greedy_out)
         greedy_ms.append(g.kernel_elapsed_ms(g.KERNEL_GREEDY))
+    # K2 (not part of the timed step): the standalone gating + histogram kernel on given logits (LOGITS_IN), the
+    # kernel whose roofline is plain HBM: 4*E bytes read per token-layer.  Logits of `nl` layers (> L2) are
+    # written once by the fused kernel's LOGITS_OUT mode, then re-read from HBM.
+    nl = min(r.L, max(1, (768 << 20) // (w.T * r.E * 4)))
+    lg = torch.empty(nl, w.T, r.E, device=dev)
+    st2 = g.StatsState(g.RouterCfg(nl, r.H, r.E, r.k, r.S, r.score_fn, r.renorm, r.n_groups, r.topk_groups, r.group_score_topn,
+                                   r.routed_scale), w.mode, window_len=1, ema_decay=w.ema_decay, device=dev)
+    g.route_stats(st2.cfg, st2, T=w.T, hidden=hidden[:nl], w_router=W[:nl], select_bias=None if sb is None else sb[:nl],
+                  src_logit_bias=slb[:nl], src_offsets=off, logits_mode=g.LOGITS_OUT, logits=lg, workspace=ws_r)
+    gate_ms = []
+    for _ in range(4):
+        flush.zero_()
+        g.route_stats(st2.cfg, st2, T=w.T, select_bias=None if sb is None else sb[:nl], src_offsets=off, logits_mode=g.LOGITS_IN,
+                      logits=lg, workspace=ws_r)
+        gate_ms.append(g.kernel_elapsed_ms(g.KERNEL_GATE))
+    del lg
     for _ in range(max(args.warmup, 3)):
         step()
     torch.cuda.synchronize()
@@ -318,7 +334,12 @@ def run_ours(args, w):
                              note="same kernel against the HBM roofline: 2*H bytes of hidden per token-layer"))
     score_ms, moves_ms = statistics.mean(k_score), statistics.mean(k_moves)
     cand_bytes = 2.0 * r.L * w.NS * w.P
+    gate_bytes = 4.0 * r.E * w.T * nl
     extra = dict(
+        gate_hist_kernel=dict(ms=min(gate_ms[1:]), layers=nl, bound="hbm", achieved=gate_bytes / (min(gate_ms[1:]) * 1e-3) / 1e9,
+                              peak=peaks["hbm"], unit="GB/s", frac=gate_bytes / (min(gate_ms[1:]) * 1e-3) / 1e9 / peaks["hbm"],
+                              algorithmic_bytes="4*E per token-layer (logits read once; counts only)",
+                              note="a2+a3 standalone on given logits (LOGITS_IN); outside the timed step"),
         greedy_place_kernel=dict(ms=min(greedy_ms[1:]), layers=r.L, note="NEXT-1, PAPER.md:260-268; outside the timed step"),
         placements_per_s=world * w.P / (score_ms * 1e-3), moves_per_s=world * n_moves / (moves_ms * 1e-3),
         place_score_kernel=dict(ms=score_ms, bound="hbm", achieved=cand_bytes / (score_ms * 1e-3) / 1e9, peak=peaks["hbm"],

@@ -57,30 +57,28 @@ int launch_gemm_n(const RouteArgs& a) {
 
 // ---- standalone gating ---------------------------------------------------------------------
 template <int E, bool kSig, bool kOut>
-int launch_gate_v(const GateKernelParams& p, dim3 grid, size_t smem, cudaStream_t stream) {
-    constexpr int kWarps = 4;
-    auto kern = gate_hist_kernel<E, kSig, kOut, kWarps>;
+int launch_gate_v(const GateKernelParams& p, dim3 grid, int S, cudaStream_t stream) {
+    const size_t smem = gate_smem_bytes<E, kOut>(S);
+    if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "gating: E=%d S=%d needs %zu B of shared memory", E, S, smem);
+    auto kern = gate_hist_kernel<E, kSig, kOut>;
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<grid, kWarps * 32, smem, stream>>>(p);
+    kern<<<grid, gate_warps<E, kOut>() * 32, smem, stream>>>(p);
     return GIMBAL_OK;
 }
 
 template <int E>
 int launch_gate_t(const RouteArgs& a) {
-    constexpr int kWarps = 4;
     GateKernelParams p{};
     p.logits = a.logits; p.select_bias = a.select_bias; p.src_offsets = a.src_offsets;
     p.topk_ids = a.topk_ids; p.topk_w = a.topk_w; p.A_step = a.A_step;
     p.layer0 = a.layer0; p.T = a.T; p.S = a.cfg->S; p.gp = gate_params(a.cfg);
     p.map = ExpertMap{a.rep_off, a.rep_slots, a.phys_ids, a.map_NS};
-    const size_t smem = gate_smem_bytes<E, kWarps>(a.cfg->S, a.topk_ids || a.topk_w || a.rep_off);
-    if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "gating: E=%d S=%d needs %zu B of shared memory", E, a.cfg->S, smem);
-    dim3 grid((a.T + kWarps * 32 - 1) / (kWarps * 32), a.n_layers);
+    dim3 grid((a.T + kGateRowsPerBlock - 1) / kGateRowsPerBlock, a.n_layers);
     const bool sig = a.cfg->score_fn == GIMBAL_SCORE_SIGMOID, out = a.topk_ids || a.topk_w || a.rep_off;
     ktime_begin(GIMBAL_KERNEL_GATE, a.stream);
     int rc;
-    if (sig) rc = out ? launch_gate_v<E, true, true>(p, grid, smem, a.stream) : launch_gate_v<E, true, false>(p, grid, smem, a.stream);
-    else rc = out ? launch_gate_v<E, false, true>(p, grid, smem, a.stream) : launch_gate_v<E, false, false>(p, grid, smem, a.stream);
+    if (sig) rc = out ? launch_gate_v<E, true, true>(p, grid, a.cfg->S, a.stream) : launch_gate_v<E, true, false>(p, grid, a.cfg->S, a.stream);
+    else rc = out ? launch_gate_v<E, false, true>(p, grid, a.cfg->S, a.stream) : launch_gate_v<E, false, false>(p, grid, a.cfg->S, a.stream);
     if (rc) return rc;
     ktime_end(GIMBAL_KERNEL_GATE, a.stream);
     LAUNCH_CHECK("gate_hist_kernel");
