@@ -36,9 +36,9 @@ from workloads.configs import MODE_WINDOW  # noqa: E402
 
 METRIC = "routed tokens/s (stats path + placement scoring, whole hot path)"
 # dram__bytes_read + dram__bytes_write of router_gemm_kernel per token-layer at the V3 shape, from the committed
-# `ncu --set full` capture profiles/r1_ncu_k1_router_gemm.txt: (5.661685e9 + 5.92e6) B over 65536 tokens x 6 layers
+# `ncu --set full` capture profiles/r1_ncu_k1_router_gemm.txt: (5.661509e9 + 3.763712e6) B over 65536 tokens x 6 layers
 # (algorithmic: 2*H = 14336 B).  The capture covers 6 of the 58 layers; traffic per launch scales it by T*L.
-NCU_DRAM_BYTES_PER_TOKEN_LAYER_V3 = (5.661685e9 + 5.92e6) / (65536 * 6)
+NCU_DRAM_BYTES_PER_TOKEN_LAYER_V3 = (5.661509e9 + 3.763712e6) / (65536 * 6)
 
 
 def _peaks():
