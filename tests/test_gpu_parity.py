@@ -556,3 +556,62 @@ def test_expert_mapping_parity(name, mode):
         g.route_stats(cfg, st2, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off,
                       expert_map=emap, phys_ids=phys2, workspace=ws)
     assert torch.equal(phys2, phys) and torch.equal(st2.A_step, st.A_step)
+
+
+# ------------------------------------------------------------------------------------------
+# the calls are asynchronous, allocation-free and capturable in a CUDA graph (include/gimbal.h conventions)
+# ------------------------------------------------------------------------------------------
+def test_cuda_graph_capture_of_a_whole_step():
+    w = _wl("decode")
+    r = w.router
+    cfg = g.RouterCfg.from_workload(r)
+    hidden, W, slb, sb, off = _router_inputs(w)
+    dp = gen.dp_of_rank(w, DEV)
+    pc = g.PlacementCfg(L=r.L, E=r.E, G=w.G, slots_per_rank=w.slots_per_rank, S=r.S, counts_dtype=g.COUNTS_F32)
+    prev = gen.prev_placement(w, np.ones((r.L, r.E)), DEV)
+    cands = gen.candidates(w, prev, w.P, DEV)
+    D = gen.comm_cost_D(w, "binary", DEV)
+    ws = ws_tensor(g.route_stats_workspace_bytes(cfg, r.L, w.T))
+    wsp = ws_tensor(g.eval_placements_workspace_bytes(pc, w.P))
+    n = r.L * w.NS * (w.NS - 1) // 2
+
+    def make():
+        st = g.StatsState(cfg, MODE_EMA, ema_decay=0.9)
+        return st, torch.zeros(w.P, 5, device=DEV), torch.zeros(n, 5, device=DEV), torch.zeros(r.L, dtype=torch.int32, device=DEV), \
+            torch.zeros_like(prev)
+
+    def step(st, out, delta, best, greedy, stream=None):
+        g.route_stats(cfg, st, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off,
+                      cur_placement=prev, dp_of_rank=dp, G=w.G, slots_per_rank=w.slots_per_rank, workspace=ws, stream=stream)
+        g.eval_placements(pc, cands, st.A_ema, st.B, D, prev, out, workspace=wsp, stream=stream)
+        g.eval_moves(pc, prev, prev, st.A_ema, st.B, D, delta, best_per_layer=best, workspace=wsp, stream=stream)
+        g.greedy_place(pc, st.A_ema, st.B, D, prev, greedy, stream=stream)
+
+    g.kernel_timing(False)                        # event brackets must be off while capturing
+    # eager: three steps
+    ref = make()
+    for _ in range(3):
+        step(*ref)
+    torch.cuda.synchronize()
+    # captured once, replayed three times on fresh state
+    cap = make()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        step(*cap, stream=side)                   # warm-up outside the capture (function attributes, module load)
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    for t in (cap[0].A_ema, cap[0].B, cap[0].step_counter, cap[0].A_step):
+        t.zero_()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        step(*cap, stream=side)
+    for t in (cap[0].A_ema, cap[0].B, cap[0].step_counter, cap[0].A_step):
+        t.zero_()                                 # the capture itself ran nothing; start from the initial state
+    for _ in range(3):
+        graph.replay()
+    torch.cuda.synchronize()
+    assert int(cap[0].step_counter.item()) == 3 == int(ref[0].step_counter.item())
+    assert torch.equal(cap[0].A_ema, ref[0].A_ema) and torch.equal(cap[0].B, ref[0].B)
+    assert torch.equal(cap[1], ref[1]) and torch.equal(cap[3], ref[3]) and torch.equal(cap[4], ref[4])
+    assert torch.equal(torch.nan_to_num(cap[2]), torch.nan_to_num(ref[2]))
