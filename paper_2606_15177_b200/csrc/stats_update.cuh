@@ -42,15 +42,28 @@ __global__ void __launch_bounds__(kUpdateThreads) stats_update_kernel(const Upda
     __syncthreads();
 
     if (e < p.E) {
+        // sources are read eight at a time before anything is written back: the loads of a batch are in
+        // flight together instead of one global round trip per source
         if (p.mode == 0) {
             int64_t b = 0;
-            for (int s = 0; s < p.S; ++s) {
-                const size_t i = ((size_t)l * p.S + s) * p.E + e;
-                const int64_t w = (int64_t)p.A_win[i] + p.A_step[i];
-                if (w > INT32_MAX) bad_s = 1;        // window sum must fit int32
-                b += w;
-                if (publish) { p.A_pub[i] = (int32_t)w; p.A_win[i] = 0; }
-                else p.A_win[i] = (int32_t)w;
+            for (int s0 = 0; s0 < p.S; s0 += 8) {
+                int32_t win[8], stp[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const size_t i = ((size_t)l * p.S + min(s0 + j, p.S - 1)) * p.E + e;
+                    win[j] = p.A_win[i]; stp[j] = p.A_step[i];
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    if (s0 + j < p.S) {
+                        const size_t i = ((size_t)l * p.S + s0 + j) * p.E + e;
+                        const int64_t w = (int64_t)win[j] + stp[j];
+                        if (w > INT32_MAX) bad_s = 1;        // window sum must fit int32
+                        b += w;
+                        if (publish) { p.A_pub[i] = (int32_t)w; p.A_win[i] = 0; }
+                        else p.A_win[i] = (int32_t)w;
+                    }
+                }
             }
             if (b > INT32_MAX) bad_s = 1;
             reinterpret_cast<int32_t*>(p.B)[(size_t)l * p.E + e] = (int32_t)b;
@@ -58,11 +71,21 @@ __global__ void __launch_bounds__(kUpdateThreads) stats_update_kernel(const Upda
             b_s[e] = (double)b;
         } else {
             float b = 0.0f;
-            for (int s = 0; s < p.S; ++s) {
-                const size_t i = ((size_t)l * p.S + s) * p.E + e;
-                const float a = __fmaf_rn(p.ema_decay, p.A_ema[i], (float)p.A_step[i]);
-                p.A_ema[i] = a;
-                b = __fadd_rn(b, a);
+            for (int s0 = 0; s0 < p.S; s0 += 8) {
+                float ema[8]; int32_t stp[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const size_t i = ((size_t)l * p.S + min(s0 + j, p.S - 1)) * p.E + e;
+                    ema[j] = p.A_ema[i]; stp[j] = p.A_step[i];
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    if (s0 + j < p.S) {
+                        const float a = __fmaf_rn(p.ema_decay, ema[j], (float)stp[j]);
+                        p.A_ema[((size_t)l * p.S + s0 + j) * p.E + e] = a;
+                        b = __fadd_rn(b, a);
+                    }
+                }
             }
             reinterpret_cast<float*>(p.B)[(size_t)l * p.E + e] = b;
             b_s[e] = (double)b;
