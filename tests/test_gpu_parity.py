@@ -615,3 +615,61 @@ def test_cuda_graph_capture_of_a_whole_step():
     assert torch.equal(cap[0].A_ema, ref[0].A_ema) and torch.equal(cap[0].B, ref[0].B)
     assert torch.equal(cap[1], ref[1]) and torch.equal(cap[3], ref[3]) and torch.equal(cap[4], ref[4])
     assert torch.equal(torch.nan_to_num(cap[2]), torch.nan_to_num(ref[2]))
+
+
+# ------------------------------------------------------------------------------------------
+# gating variants that no BASELINE.json config exercises (E = 32, grouped softmax, ungrouped sigmoid, topn = 1, k < 8)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("E,k,score_fn,renorm,n_groups,topk_groups,topn,bias", [
+    (32, 4, 0, 0, 1, 1, 1, False),
+    (16, 1, 1, 0, 1, 1, 1, True),
+    (64, 3, 1, 1, 1, 1, 1, True),
+    (64, 8, 0, 1, 2, 1, 2, False),
+    (128, 5, 0, 0, 4, 2, 1, False),
+    (256, 3, 1, 0, 8, 3, 1, False),
+    (256, 8, 1, 1, 8, 2, 2, True),
+])
+def test_gating_variants(E, k, score_fn, renorm, n_groups, topk_groups, topn, bias):
+    from workloads.configs import RouterCfg as WRouterCfg
+    L, T, S, H = 2, 700, 3, 128
+    r = WRouterCfg(L=L, H=H, E=E, k=k, S=S, score_fn=score_fn, renorm=renorm, n_groups=n_groups, topk_groups=topk_groups,
+                   group_score_topn=topn, routed_scale=1.5)
+    cfg = g.RouterCfg.from_workload(r)
+    gen_ = torch.Generator(device=DEV); gen_.manual_seed(E * 100 + k)
+    x = torch.randn(L, T, E, generator=gen_, device=DEV) * 2.0
+    x[:, 0::5] = torch.round(x[:, 0::5] * 2) / 2                           # many exact ties
+    x[:, 3, :] = -1.0                                                       # an all-equal row
+    off = torch.tensor([0, 250, 250, T], dtype=torch.int32, device=DEV)     # one empty source
+    sb = (0.05 * torch.randn(L, E, generator=gen_, device=DEV)) if bias else None
+    ws = ws_tensor(g.route_stats_workspace_bytes(cfg, L, T))
+
+    def check(ids, wts, st, logits):
+        for l in range(L):
+            rid, rw = oracle.gate(to_np(logits[l]), r, None if sb is None else to_np(sb)[l], tier=1)
+            np.testing.assert_array_equal(to_np(ids[l]), rid)
+            np.testing.assert_allclose(to_np(wts[l]), rw, rtol=1e-5, atol=1e-30)
+            np.testing.assert_array_equal(to_np(st.A_step[l]), oracle.counts(rid, to_np(off), S, E))
+
+    # standalone kernel: with outputs (one lane per row) and without (R lanes per row) must agree with the oracle
+    st = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+    ids = torch.full((L, T, k), -9, dtype=torch.int32, device=DEV)
+    wts = torch.full((L, T, k), -9.0, device=DEV)
+    g.route_stats(cfg, st, T=T, select_bias=sb, src_offsets=off, logits_mode=g.LOGITS_IN, logits=x, topk_ids=ids, topk_w=wts, workspace=ws)
+    check(ids, wts, st, x)
+    st2 = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+    g.route_stats(cfg, st2, T=T, select_bias=sb, src_offsets=off, logits_mode=g.LOGITS_IN, logits=x, workspace=ws)
+    assert torch.equal(st2.A_step, st.A_step)
+    # fused GEMM epilogue on its own logits
+    hidden = torch.randn(L, T, H, generator=gen_, device=DEV).to(torch.bfloat16)
+    W = (0.2 * torch.randn(L, E, H, generator=gen_, device=DEV)).to(torch.bfloat16)
+    for cg in ("1", "2"):
+        os.environ["GIMBAL_CTA_GROUP"] = cg
+        st3 = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+        logits = torch.empty(L, T, E, device=DEV)
+        g.route_stats(cfg, st3, T=T, hidden=hidden, w_router=W, select_bias=sb, src_offsets=off, logits_mode=g.LOGITS_OUT, logits=logits,
+                      topk_ids=ids, topk_w=wts, workspace=ws)
+        check(ids, wts, st3, logits)
+        st4 = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+        g.route_stats(cfg, st4, T=T, hidden=hidden, w_router=W, select_bias=sb, src_offsets=off, workspace=ws)
+        assert torch.equal(st4.A_step, st3.A_step)
+    os.environ.pop("GIMBAL_CTA_GROUP")
