@@ -283,6 +283,7 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
     if (logits_mode != GIMBAL_LOGITS_NONE && logits_mode != GIMBAL_LOGITS_OUT && logits_mode != GIMBAL_LOGITS_IN)
         return fail(GIMBAL_ERR_INVALID_ARG, "logits_mode=%d", logits_mode);
     if (logits_mode != GIMBAL_LOGITS_NONE && !logits) return fail(GIMBAL_ERR_INVALID_ARG, "logits is NULL");
+    if (logits_mode != GIMBAL_LOGITS_NONE && (reinterpret_cast<uintptr_t>(logits) & 15)) return fail(GIMBAL_ERR_INVALID_ARG, "logits must be 16-byte aligned");
     if (logits_mode != GIMBAL_LOGITS_IN) {
         if (!hidden || !w_router) return fail(GIMBAL_ERR_INVALID_ARG, "hidden / w_router is NULL");
         if ((reinterpret_cast<uintptr_t>(hidden) & 15) || (reinterpret_cast<uintptr_t>(w_router) & 15))
@@ -317,7 +318,7 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
             if (rc) return rc;
         } else {
             // fused epilogue needs the block histogram next to the ring; fall back to two kernels otherwise
-            const bool can_fuse = pick_fuse() && (size_t)cfg->S * cfg->E * 4 <= 32 * 1024;
+            const bool can_fuse = pick_fuse() && (size_t)cfg->S * cfg->E * 4 <= 64 * 1024;   // every supported (S, E) fits
             if (can_fuse) {
                 a.logits = logits_mode == GIMBAL_LOGITS_OUT ? logits : nullptr;
                 a.fuse_gate = 1;

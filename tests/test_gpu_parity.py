@@ -673,3 +673,34 @@ def test_gating_variants(E, k, score_fn, renorm, n_groups, topk_groups, topn, bi
         g.route_stats(cfg, st4, T=T, hidden=hidden, w_router=W, select_bias=sb, src_offsets=off, workspace=ws)
         assert torch.equal(st4.A_step, st3.A_step)
     os.environ.pop("GIMBAL_CTA_GROUP")
+
+
+def test_route_stats_edges_empty_step_and_many_sources():
+    """T = 0 (an idle step still advances the window / EMA) and S = 64 sources with E = 256 (the largest histogram)."""
+    from workloads.configs import RouterCfg as WRouterCfg
+    r = WRouterCfg(L=2, H=128, E=256, k=8, S=64, score_fn=1, renorm=1, n_groups=8, topk_groups=4, group_score_topn=2, routed_scale=2.5)
+    cfg = g.RouterCfg.from_workload(r)
+    T = 900
+    gen_ = torch.Generator(device=DEV); gen_.manual_seed(3)
+    hidden = torch.randn(r.L, T, r.H, generator=gen_, device=DEV).to(torch.bfloat16)
+    W = (0.3 * torch.randn(r.L, r.E, r.H, generator=gen_, device=DEV)).to(torch.bfloat16)
+    cuts = np.sort(np.random.default_rng(1).integers(0, T + 1, r.S - 1))
+    off = torch.from_numpy(np.concatenate([[0], cuts, [T]]).astype(np.int32)).to(DEV)
+    ws = ws_tensor(g.route_stats_workspace_bytes(cfg, r.L, T))
+    st = g.StatsState(cfg, MODE_EMA, ema_decay=0.5)
+    logits = torch.empty(r.L, T, r.E, device=DEV)
+    ids = torch.empty(r.L, T, r.k, dtype=torch.int32, device=DEV)
+    g.route_stats(cfg, st, T=T, hidden=hidden, w_router=W, src_offsets=off, logits_mode=g.LOGITS_OUT, logits=logits, topk_ids=ids, workspace=ws)
+    st_f = g.StatsState(cfg, MODE_EMA, ema_decay=0.5)
+    g.route_stats(cfg, st_f, T=T, hidden=hidden, w_router=W, src_offsets=off, workspace=ws)     # fused, nothing written
+    for l in range(r.L):
+        rid, _ = oracle.gate(to_np(logits[l]), r, None, 1)
+        np.testing.assert_array_equal(to_np(ids[l]), rid)
+        np.testing.assert_array_equal(to_np(st.A_step[l]), oracle.counts(rid, to_np(off), r.S, r.E))
+    assert torch.equal(st_f.A_step, st.A_step) and torch.equal(st_f.A_ema, st.A_ema)
+    # an empty step: counts are zero, the EMA decays, the step counter advances
+    before = st.A_ema.clone()
+    off0 = torch.zeros(r.S + 1, dtype=torch.int32, device=DEV)
+    g.route_stats(cfg, st, T=0, hidden=hidden, w_router=W, src_offsets=off0, workspace=ws)
+    assert int(st.A_step.abs().sum().item()) == 0 and int(st.step_counter.item()) == 2
+    assert torch.equal(st.A_ema, before * 0.5)
