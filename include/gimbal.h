@@ -282,6 +282,32 @@ GIMBAL_API int gimbal_greedy_place(const gimbal_placement_cfg *cfg, const void *
                         const float *M, float M_scalar, const int16_t *prev, int16_t *out, int32_t *status,
                         gimbal_stream_t stream);
 
+/* ---------------------------------------------------------------------------------------
+ * gimbal_select_engines -- Algorithm 1, Global DP Engine Scheduling (section
+ * 4.3; readings DESIGN.md R19), batched: B independent scheduler instances, each with N DP
+ * engines and R incoming requests handled in order.  Per request: incomplete traces -> ordered
+ * dispatch Next(E); else the KV rule (max kv > high_kv and max - min kv > large_gap -> the engine
+ * with the lowest kv); else score_i = pre_rem_i + wait_i + comp_i + lambda_kv*kv_i +
+ * lambda_moe*moe_i, ordered dispatch when max - min score < close_frac * len(r), otherwise the
+ * argmin of (score, kv, i).  After each assignment comp[e*] += len(r).
+ *   trace    [B,N,4] f32   {kv in [0,1], pre_rem tokens, wait tokens, moe = relative MoE pressure
+ *                          (pressure_rel of gimbal_route_stats, mean 1)}; 16-byte aligned
+ *   complete [B] u8 | NULL  0: this instance's traces are incomplete
+ *   req_len  [B,R] f32      prefill tokens of the incoming requests
+ *   comp     [B,N] f64 inout  compensation load; the caller zeroes it when it loads a fresh trace
+ *   rr       [B] i32 inout    ordered-dispatch pointer
+ *   engine   [B,R] i32 out    selected engine per request
+ * Supported: 1 <= N <= 64.  Decisions are taken in IEEE double (bit-exact against the oracle). */
+typedef struct gimbal_sched_cfg {
+    int32_t N, R;
+    float high_kv, large_gap;       /* 0.90, 0.10 */
+    float lambda_kv, lambda_moe;    /* token-equivalent weights of P_kv, P_moe (R19) */
+    float close_frac;               /* CLOSE threshold as a fraction of the request length (R19) */
+} gimbal_sched_cfg;
+
+GIMBAL_API int gimbal_select_engines(const gimbal_sched_cfg *cfg, int B, const float *trace, const uint8_t *complete,
+                          const float *req_len, double *comp, int32_t *rr, int32_t *engine, gimbal_stream_t stream);
+
 /* Counters for bench.py: kernels launched by this library since load. */
 GIMBAL_API int64_t gimbal_launch_count(void);
 

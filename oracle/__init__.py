@@ -225,6 +225,21 @@ def greedy_place(prev, A, B, D, M=None, M_scalar=1.0, *, G, sp, weights=(1.0, 0.
     return bool(ok), out
 
 
+# -- NEXT-2: Algorithm 1 ----------------------------------------------------------------
+def select_engines(trace, complete, req_len, comp, rr, *, high_kv=0.9, large_gap=0.1, lambda_kv=0.0, lambda_moe=0.0,
+                   close_frac=0.0):
+    """One scheduler instance: trace [N,4] f32 {kv, pre_rem, wait, moe}, req_len [R] f32, comp [N] f64 (updated in
+    place), rr int -> (engine [R] int32, new rr).  PAPER.md:143-167, R19."""
+    trace = _c(trace, np.float32); req_len = _c(req_len, np.float32)
+    assert comp.dtype == np.float64 and comp.flags.c_contiguous
+    N, R = trace.shape[0], req_len.shape[0]
+    out = np.empty(R, np.int32); rrv = C.c_int32(int(rr))
+    lib().oracle_select_engines(_p(trace, C.c_float), C.c_int(int(bool(complete))), _p(req_len, C.c_float), C.c_int(N), C.c_int(R),
+                                C.c_double(high_kv), C.c_double(large_gap), C.c_double(lambda_kv), C.c_double(lambda_moe),
+                                C.c_double(close_frac), _p(comp, C.c_double), C.byref(rrv), _p(out, C.c_int32))
+    return out, int(rrv.value)
+
+
 # -- brute force ------------------------------------------------------------------------
 def bruteforce(prev, A, B, D, M=None, M_scalar=1.0, *, G, sp, weights=(1.0, 0.0025, 1.0)):
     """One layer, NS == E.  A [S,E], B [E], prev [NS] -> (count, best_J, best_place [NS])."""

@@ -599,6 +599,64 @@ void oracle_expert_map(const int32_t *ids /*[T,k]*/, const int16_t *place /*[NS]
         }
 }
 
+/* ------------------------------------------------------------------------------------ */
+/* NEXT-2  Algorithm 1, Global DP Engine Scheduling (section 4.3), for one
+ *     scheduler instance and a sequence of R incoming requests, in the algorithm's order.
+ *     The extracted listing lost some step numbers; the steps are
+ *     unambiguous.  Undefined pieces take the readings of DESIGN.md R19:
+ *       HighKV(kv)  = kv > high_kv          (90 %)
+ *       LargeGap(d) = d  > large_gap        (10 %)
+ *       P_kv(kv)    = lambda_kv  * kv       token-equivalent penalties, linear;
+ *       P_moe(moe)  = lambda_moe * moe      moe is the relative MoE pressure (mean 1)
+ *       CLOSE(D, r) = D < close_frac * len(r)
+ *       Next(E)     = engine rr, then rr <- (rr + 1) mod N (ordered dispatch)
+ *       compensation: after a request is assigned, comp[e*] += len(r), "a
+ *       temporary pressure estimate" that lasts until the caller loads a fresh trace.
+ *     trace[n] = {kv, pre_rem, wait, moe}.  score = (((pre_rem + wait) + comp) + lambda_kv*kv)
+ *     + lambda_moe*moe in IEEE double, one rounding per operation; argmin over the
+ *     lexicographic key (score, kv, i).  argmin / argmax of kv: lowest index.  */
+/* ------------------------------------------------------------------------------------ */
+void oracle_select_engines(const float *trace /*[N,4]*/, int complete, const float *req_len /*[R]*/, int N, int R,
+                           double high_kv, double large_gap, double lambda_kv, double lambda_moe, double close_frac,
+                           double *comp /*[N] inout*/, int32_t *rr /*[1] inout*/, int32_t *engine /*[R]*/)
+{
+    for (int q = 0; q < R; ++q) {
+        double len = (double)req_len[q];
+        int pick = -1;
+        if (!complete) {                                   /* line 1-2: traces incomplete -> ordered dispatch */
+            pick = *rr; *rr = (*rr + 1) % N;
+        } else {
+            int imin = 0, imax = 0;                        /* line 6 */
+            for (int i = 1; i < N; ++i) {
+                if (trace[i * 4] < trace[imin * 4]) imin = i;
+                if (trace[i * 4] > trace[imax * 4]) imax = i;
+            }
+            double kvmax = (double)trace[imax * 4], kvmin = (double)trace[imin * 4];
+            if (kvmax > high_kv && (kvmax - kvmin) > large_gap) {      /* line 7-8 */
+                pick = imin;
+            } else {
+                double smin = 0.0, smax = 0.0; int best = 0; double bs = 0.0, bkv = 0.0;
+                for (int i = 0; i < N; ++i) {              /* line 10-12 */
+                    double kv = (double)trace[i * 4], pre = (double)trace[i * 4 + 1], wait = (double)trace[i * 4 + 2],
+                           moe = (double)trace[i * 4 + 3];
+                    double sc = (((pre + wait) + comp[i]) + (lambda_kv * kv)) + (lambda_moe * moe);
+                    if (i == 0 || sc < smin) smin = sc;
+                    if (i == 0 || sc > smax) smax = sc;
+                    if (i == 0 || sc < bs || (sc == bs && kv < bkv)) { best = i; bs = sc; bkv = kv; }
+                }
+                double delta = smax - smin;                /* line 13 */
+                if (delta < close_frac * len) {            /* line 14-15 */
+                    pick = *rr; *rr = (*rr + 1) % N;
+                } else {
+                    pick = best;                           /* line 17 */
+                }
+            }
+        }
+        engine[q] = pick;
+        comp[pick] += len;                                 /* compensation */
+    }
+}
+
 /* threads the OpenMP loops above will use (reported as cpu_baseline.cores by bench.py) */
 #ifdef _OPENMP
 #include <omp.h>

@@ -20,6 +20,7 @@ EXPORTED_SYMBOLS = [
     "gimbal_route_stats_host",
     "gimbal_eval_placements_workspace_bytes", "gimbal_eval_placements", "gimbal_eval_placements_host",
     "gimbal_eval_moves_workspace_bytes", "gimbal_eval_moves", "gimbal_greedy_place", "gimbal_build_expert_map",
+    "gimbal_select_engines",
     "gimbal_kernel_timing", "gimbal_kernel_elapsed_ms",
 ]
 KERNEL_ROUTER, KERNEL_GATE, KERNEL_SCORE, KERNEL_MOVES, KERNEL_GREEDY = 0, 1, 2, 3, 4
@@ -72,7 +73,7 @@ def lib():
                   "gimbal_eval_placements_workspace_bytes", "gimbal_eval_moves_workspace_bytes"):
             getattr(L, n).restype = C.c_size_t
         for n in ("gimbal_route_stats", "gimbal_route_stats_host", "gimbal_eval_placements",
-                  "gimbal_eval_placements_host", "gimbal_eval_moves", "gimbal_greedy_place", "gimbal_build_expert_map"):
+                  "gimbal_eval_placements_host", "gimbal_eval_moves", "gimbal_greedy_place", "gimbal_build_expert_map", "gimbal_select_engines"):
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -303,3 +304,20 @@ def greedy_place(cfg: PlacementCfg, A, B, D, prev, out, *, M=None, M_scalar: flo
     rc = lib().gimbal_greedy_place(C.byref(c), _ptr(A), _ptr(B), _ptr(D), _ptr(M), C.c_float(M_scalar), _ptr(prev), _ptr(out),
                                    _ptr(status), _stream(stream))
     _check(rc, "gimbal_greedy_place")
+
+
+class _SchedCfg(C.Structure):
+    _fields_ = [("N", C.c_int32), ("R", C.c_int32)] + [(n, C.c_float) for n in ("high_kv", "large_gap", "lambda_kv", "lambda_moe",
+                                                                               "close_frac")]
+
+
+def select_engines(trace, req_len, comp, rr, engine, *, complete=None, high_kv=0.9, large_gap=0.1, lambda_kv=0.0, lambda_moe=0.0,
+                   close_frac=0.0, stream=None):
+    """gimbal_select_engines (NEXT-2, Algorithm 1): trace [B,N,4] f32, req_len [B,R] f32, comp [B,N] f64 inout, rr [B] i32
+    inout, engine [B,R] i32 out."""
+    B, N = trace.shape[0], trace.shape[1]
+    R = req_len.shape[1]
+    c = _SchedCfg(N, R, high_kv, large_gap, lambda_kv, lambda_moe, close_frac)
+    rc = lib().gimbal_select_engines(C.byref(c), C.c_int(B), _ptr(trace), _ptr(complete), _ptr(req_len), _ptr(comp), _ptr(rr),
+                                     _ptr(engine), _stream(stream))
+    _check(rc, "gimbal_select_engines")

@@ -12,6 +12,7 @@
 #include "host_common.h"
 #include "greedy.cuh"
 #include "placement.cuh"
+#include "sched.cuh"
 #include "stats_update.cuh"
 
 using namespace gimbal;
@@ -608,6 +609,25 @@ int gimbal_greedy_place(const gimbal_placement_cfg* cfg, const void* A, const vo
     greedy_place_kernel<<<cfg->L, kGreedyThreads, smem, stream>>>(gp);
     ktime_end(GIMBAL_KERNEL_GREEDY, stream);
     LAUNCH_CHECK("greedy_place_kernel");
+    return GIMBAL_OK;
+}
+
+int gimbal_select_engines(const gimbal_sched_cfg* cfg, int B, const float* trace, const uint8_t* complete, const float* req_len,
+                          double* comp, int32_t* rr, int32_t* engine, gimbal_stream_t stream_) {
+    if (!cfg) return fail(GIMBAL_ERR_INVALID_ARG, "cfg is NULL");
+    if (cfg->N < 1 || cfg->N > 64 || cfg->R < 0 || B < 0) return fail(GIMBAL_ERR_INVALID_ARG, "need 1 <= N <= 64, R >= 0, B >= 0");
+    if (B > 0 && (!trace || !comp || !rr || (cfg->R > 0 && (!req_len || !engine)))) return fail(GIMBAL_ERR_INVALID_ARG, "NULL argument");
+    if (reinterpret_cast<uintptr_t>(trace) & 15) return fail(GIMBAL_ERR_INVALID_ARG, "trace must be 16-byte aligned");
+    int rc = require_device();
+    if (rc) return rc;
+    if (B == 0) return GIMBAL_OK;
+    SchedParams sp{};
+    sp.B = B; sp.N = cfg->N; sp.R = cfg->R;
+    sp.high_kv = cfg->high_kv; sp.large_gap = cfg->large_gap; sp.lambda_kv = cfg->lambda_kv; sp.lambda_moe = cfg->lambda_moe;
+    sp.close_frac = cfg->close_frac;
+    sp.trace = trace; sp.complete = complete; sp.req_len = req_len; sp.comp = comp; sp.rr = rr; sp.engine = engine;
+    select_engines_kernel<<<(B + kSchedWarps - 1) / kSchedWarps, kSchedWarps * 32, 0, static_cast<cudaStream_t>(stream_)>>>(sp);
+    LAUNCH_CHECK("select_engines_kernel");
     return GIMBAL_OK;
 }
 

@@ -704,3 +704,66 @@ def test_route_stats_edges_empty_step_and_many_sources():
     g.route_stats(cfg, st, T=0, hidden=hidden, w_router=W, src_offsets=off0, workspace=ws)
     assert int(st.A_step.abs().sum().item()) == 0 and int(st.step_counter.item()) == 2
     assert torch.equal(st.A_ema, before * 0.5)
+
+
+# ------------------------------------------------------------------------------------------
+# NEXT-2: Algorithm 1, Global DP Engine Scheduling (R19) -- integer output, bit-exact
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,R,params", [
+    (2, 40, dict()),
+    (8, 64, dict(lambda_kv=200.0, lambda_moe=150.0, close_frac=0.25)),
+    (16, 50, dict(lambda_kv=50.0, lambda_moe=500.0, close_frac=0.05)),
+    (33, 30, dict(lambda_moe=80.0)),
+    (64, 70, dict(lambda_kv=10.0, lambda_moe=10.0, close_frac=1.0)),
+])
+def test_select_engines_parity(N, R, params):
+    rng = np.random.default_rng(N * 7 + R)
+    B = 1500
+    tr = np.stack([rng.uniform(0.05, 0.99, (B, N)), rng.integers(0, 4000, (B, N)), rng.integers(0, 2000, (B, N)),
+                   rng.uniform(0.3, 2.0, (B, N))], -1).astype(np.float32)
+    tr[::5, :, 0] = rng.uniform(0.05, 0.85, (len(tr[::5]), N))            # instances where the KV rule cannot fire
+    tr[1::7, :, 1:3] = 100.0                                              # equal pressure: ties / CLOSE decide
+    lens = np.ceil(rng.lognormal(6.0, 1.0, (B, R))).astype(np.float32)
+    complete = (rng.random(B) > 0.1).astype(np.uint8)
+    rr0 = rng.integers(0, N, B).astype(np.int32)
+    comp0 = rng.integers(0, 500, (B, N)).astype(np.float64)
+    t = lambda a: torch.from_numpy(a).to(DEV)
+    comp, rr, eng = t(comp0.copy()), t(rr0.copy()), torch.full((B, R), -3, dtype=torch.int32, device=DEV)
+    g.select_engines(t(tr), t(lens), comp, rr, eng, complete=t(complete), **params)
+    torch.cuda.synchronize()
+    p32 = {k: float(np.float32(v)) for k, v in params.items()}            # the C struct carries fp32 parameters
+    p32.setdefault("high_kv", float(np.float32(0.9))); p32.setdefault("large_gap", float(np.float32(0.1)))
+    ge, gc, gr = to_np(eng), to_np(comp), to_np(rr)
+    for b in range(0, B, 3):
+        c = comp0[b].copy()
+        e, r_after = oracle.select_engines(tr[b], complete[b], lens[b], c, rr0[b], **p32)
+        np.testing.assert_array_equal(ge[b], e)
+        np.testing.assert_array_equal(gc[b], c)
+        assert gr[b] == r_after
+    assert ((ge >= 0) & (ge < N)).all()
+    np.testing.assert_allclose(gc.sum(1), comp0.sum(1) + lens.astype(np.float64).sum(1), rtol=1e-12)   # every request is assigned once
+
+
+def test_select_engines_consumes_route_stats_pressure():
+    """the loop the paper closes: pressure_rel of the stats path is the moe column of the trace"""
+    w = _wl("qwen3")
+    r = w.router
+    cfg = g.RouterCfg.from_workload(r)
+    x, off = _synthetic_logits(w, 31)
+    place = gen.prev_placement(w, np.random.default_rng(2).integers(1, 1000, (r.L, r.E)), DEV)
+    dp = gen.dp_of_rank(w, DEV)
+    st = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+    ws = ws_tensor(g.route_stats_workspace_bytes(cfg, r.L, w.T))
+    g.route_stats(cfg, st, T=w.T, src_offsets=off, logits_mode=g.LOGITS_IN, logits=x, cur_placement=place, dp_of_rank=dp, G=w.G,
+                  slots_per_rank=w.slots_per_rank, workspace=ws)
+    N, R = r.S, 32
+    tr = torch.zeros(1, N, 4, device=DEV)
+    tr[0, :, 0] = 0.5; tr[0, :, 1] = 1000.0; tr[0, :, 3] = st.pressure_rel
+    lens = torch.full((1, R), 10.0, device=DEV)
+    comp = torch.zeros(1, N, dtype=torch.float64, device=DEV); rr = torch.zeros(1, dtype=torch.int32, device=DEV)
+    eng = torch.empty(1, R, dtype=torch.int32, device=DEV)
+    g.select_engines(tr, lens, comp, rr, eng, lambda_moe=1000.0)
+    c = np.zeros(N)
+    e, _ = oracle.select_engines(to_np(tr)[0], 1, to_np(lens)[0], c, 0, lambda_moe=1000.0)
+    np.testing.assert_array_equal(to_np(eng)[0], e)
+    assert int(to_np(eng)[0, 0]) == int(np.argmin(to_np(st.pressure_rel)))       # the engine with the least MoE pressure goes first

@@ -565,3 +565,57 @@ def test_expert_map_hand_example_and_library_restatement():
     e = int(np.nonzero(np.bincount(place, minlength=E) == 2)[0][0])
     hits = oracle.expert_map(np.full((10, 1), e, np.int32), place)[:, 0]
     assert hits[::2].tolist() == [hits[0]] * 5 and hits[1::2].tolist() == [hits[1]] * 5 and hits[0] < hits[1]
+
+
+# =========================================================================== NEXT-2 Algorithm 1
+def test_alg1_worked_examples():
+    gold = json.load(open(os.path.join(GOLD, "alg1_worked_examples.json")))
+    for c in gold["cases"]:
+        tr = np.array(c["trace"], np.float32)
+        comp = np.zeros(tr.shape[0])
+        eng, rr = oracle.select_engines(tr, c["complete"], np.array(c["req_len"], np.float32), comp, c["rr"], **c["params"])
+        assert eng.tolist() == c["engine"], c["name"]
+        assert comp.tolist() == c["comp"] and rr == c["rr_after"], c["name"]
+
+
+def test_alg1_is_least_loaded_list_scheduling_without_penalties():
+    """lambda = 0, CLOSE off, no KV pressure: each request goes to the engine with the least pending tokens (trace +
+    compensation) -- textbook greedy list scheduling, restated with a heap; ties fall to (kv, index)."""
+    import heapq
+    rng = np.random.default_rng(4)
+    N, R = 7, 200
+    tr = np.zeros((N, 4), np.float32)
+    tr[:, 0] = rng.permutation(N) * 0.05 + 0.1                 # distinct kv < 0.9
+    tr[:, 1] = rng.integers(0, 500, N); tr[:, 2] = rng.integers(0, 500, N); tr[:, 3] = 1.0
+    lens = rng.integers(1, 400, R).astype(np.float32)
+    comp = np.zeros(N)
+    eng, _ = oracle.select_engines(tr, 1, lens, comp, 0)
+    heap = [(float(tr[i, 1] + tr[i, 2]), float(tr[i, 0]), i) for i in range(N)]
+    heapq.heapify(heap)
+    for q in range(R):
+        load, kv, i = heapq.heappop(heap)
+        assert eng[q] == i
+        heapq.heappush(heap, (load + float(lens[q]), kv, i))
+    np.testing.assert_array_equal(comp, np.bincount(eng, weights=lens.astype(np.float64), minlength=N))
+
+
+def test_alg1_invariants():
+    rng = np.random.default_rng(10)
+    N, R = 5, 64
+    tr = np.stack([rng.uniform(0.1, 0.8, N), rng.integers(0, 300, N), rng.integers(0, 300, N), rng.uniform(0.5, 1.5, N)], 1).astype(np.float32)
+    lens = rng.integers(1, 200, R).astype(np.float32)
+    # CLOSE with a huge threshold = pure ordered dispatch, and so are incomplete traces
+    for kw, complete in ((dict(close_frac=1e9), 1), (dict(), 0)):
+        comp = np.zeros(N)
+        eng, rr = oracle.select_engines(tr, complete, lens, comp, 3, **kw)
+        assert eng.tolist() == [(3 + q) % N for q in range(R)] and rr == (3 + R) % N
+    # a prohibitive MoE penalty on one engine keeps it idle until the others have caught up
+    tr2 = tr.copy(); tr2[:, 3] = 1.0; tr2[2, 3] = 3.0
+    comp = np.zeros(N)
+    eng, _ = oracle.select_engines(tr2, 1, lens[:8], comp, 0, lambda_moe=1e6)
+    assert 2 not in eng
+    # the KV rule sends everything to the emptiest cache
+    tr3 = tr.copy(); tr3[4, 0] = 0.99
+    comp = np.zeros(N)
+    eng, _ = oracle.select_engines(tr3, 1, lens, comp, 0)
+    assert (eng == int(np.argmin(tr3[:, 0]))).all()
