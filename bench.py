@@ -38,6 +38,11 @@ METRIC = "routed tokens/s (stats path + placement scoring, whole hot path)"
 # dram__bytes_read + dram__bytes_write of router_gemm_kernel per token-layer at the V3 shape, from the committed
 # `ncu --set full` capture profiles/r1_ncu_k1_router_gemm.txt: (5.661509e9 + 3.763712e6) B over 65536 tokens x 6 layers
 # (algorithmic: 2*H = 14336 B).  The capture covers 6 of the 58 layers; traffic per launch scales it by T*L.
+# smsp__inst_executed.sum of place_score_fast_kernel<9,32,1,0> per (candidate, layer) at the V3 shape, from
+# profiles/r1_ncu_k4_k5_placement.txt (46,644,992 warp instructions for 4096 x 58 units): the kernel is issue-bound, so
+# its ALU roofline (148 SMs x 4 schedulers x 1 warp instruction per clock at the maximum SM clock)
+# is reported next to the HBM one.
+NCU_WARP_INSTR_PER_UNIT_K4_V3 = 46644992 / (4096 * 58)
 NCU_DRAM_BYTES_PER_TOKEN_LAYER_V3 = (5.661509e9 + 3.763712e6) / (65536 * 6)
 
 
@@ -344,7 +349,12 @@ def run_ours(args, w):
         placements_per_s=world * w.P / (score_ms * 1e-3), moves_per_s=world * n_moves / (moves_ms * 1e-3),
         place_score_kernel=dict(ms=score_ms, bound="hbm", achieved=cand_bytes / (score_ms * 1e-3) / 1e9, peak=peaks["hbm"],
                                 unit="GB/s", frac=cand_bytes / (score_ms * 1e-3) / 1e9 / peaks["hbm"],
-                                algorithmic_bytes="2*L*NS per candidate"),
+                                algorithmic_bytes="2*L*NS per candidate",
+                                alu=(dict(achieved=NCU_WARP_INSTR_PER_UNIT_K4_V3 * w.P * r.L / (score_ms * 1e-3) / 1e9,
+                                          peak=148 * 4 * 1.965, unit="G warp-instructions/s",
+                                          frac=NCU_WARP_INSTR_PER_UNIT_K4_V3 * w.P * r.L / (score_ms * 1e-3) / 1e9 / (148 * 4 * 1.965),
+                                          note="issue-bound kernel: instructions per unit from the committed ncu capture; peak at "
+                                               "the maximum SM clock (1965 MHz)") if w.name == "v3" else None)),
         move_delta_kernel=dict(ms=moves_ms, bound="hbm", achieved=20.0 * n_moves / (moves_ms * 1e-3) / 1e9, peak=peaks["hbm"],
                                unit="GB/s", frac=20.0 * n_moves / (moves_ms * 1e-3) / 1e9 / peaks["hbm"],
                                algorithmic_bytes="20 B written per move (implicit neighbourhood)"))

@@ -308,6 +308,18 @@ typedef struct gimbal_sched_cfg {
 GIMBAL_API int gimbal_select_engines(const gimbal_sched_cfg *cfg, int B, const float *trace, const uint8_t *complete,
                           const float *req_len, double *comp, int32_t *rr, int32_t *engine, gimbal_stream_t stream);
 
+/* ---------------------------------------------------------------------------------------
+ * gimbal_order_queues -- Algorithm 2, Request Scheduler with SJF and Aging (PAPER.md:179-200,
+ * section 4.4; R20), batched over B waiting queues.  A request that has waited
+ * now - arrival >= theta_age (5 s in the paper) is high priority; the others are
+ * ordered by prefill length.  Total order: aged first, oldest first; then shortest prefill,
+ * equal lengths oldest first; then the position in the input queue.
+ *   arrival [B,Q] f32 seconds, prefill [B,Q] i32 tokens, qlen [B] i32 (requests in each queue, <= Q)
+ *   order   [B,Q] i32 out: order[b,i] = input position of the i-th request to run; -1 past qlen[b]
+ * Supported: Q <= 2048.                                                                     */
+GIMBAL_API int gimbal_order_queues(int B, int Q, const float *arrival, const int32_t *prefill, const int32_t *qlen,
+                        float now, float theta_age, int32_t *order, gimbal_stream_t stream);
+
 /* Counters for bench.py: kernels launched by this library since load. */
 GIMBAL_API int64_t gimbal_launch_count(void);
 

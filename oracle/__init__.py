@@ -240,6 +240,15 @@ def select_engines(trace, complete, req_len, comp, rr, *, high_kv=0.9, large_gap
     return out, int(rrv.value)
 
 
+def order_queue(arrival, prefill, now: float, theta_age: float = 5.0):
+    """Algorithm 2 (R20): arrival [n] f32 seconds, prefill [n] i32 tokens -> order [n] i32."""
+    arrival = _c(arrival, np.float32); prefill = _c(prefill, np.int32)
+    out = np.empty(arrival.shape[0], np.int32)
+    lib().oracle_order_queue(_p(arrival, C.c_float), _p(prefill, C.c_int32), C.c_int(arrival.shape[0]), C.c_float(now),
+                             C.c_float(theta_age), _p(out, C.c_int32))
+    return out
+
+
 # -- brute force ------------------------------------------------------------------------
 def bruteforce(prev, A, B, D, M=None, M_scalar=1.0, *, G, sp, weights=(1.0, 0.0025, 1.0)):
     """One layer, NS == E.  A [S,E], B [E], prev [NS] -> (count, best_J, best_place [NS])."""

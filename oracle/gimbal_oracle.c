@@ -657,6 +657,35 @@ void oracle_select_engines(const float *trace /*[N,4]*/, int complete, const flo
     }
 }
 
+/* ------------------------------------------------------------------------------------ */
+/* Algorithm 2, Request Scheduler with SJF and Aging (section 4.4; the
+ *     extracted listing is scrambled, R20): for every request r of the waiting queue,
+ *     waiting time w_r = now - arrival_r; if w_r >= theta_age the request gets high priority,
+ *     otherwise its priority is its prefill length; the queue is sorted by priority ascending.
+ *     Reading R20 for what the paper leaves open: aged requests come first, oldest first; the
+ *     others by prefill length (shortest first), equal lengths oldest first; a last tie goes to
+ *     the position in the input queue.  order[i] = input position of the i-th request to run.   */
+/* ------------------------------------------------------------------------------------ */
+static int alg2_before(const float *arrival, const int32_t *prefill, float now, float theta, int a, int b)
+{
+    int aged_a = (now - arrival[a]) >= theta, aged_b = (now - arrival[b]) >= theta;
+    if (aged_a != aged_b) return aged_a;                        /* high priority first */
+    if (!aged_a && prefill[a] != prefill[b]) return prefill[a] < prefill[b];
+    if (arrival[a] != arrival[b]) return arrival[a] < arrival[b];
+    return a < b;
+}
+
+void oracle_order_queue(const float *arrival /*[n]*/, const int32_t *prefill /*[n]*/, int n, float now, float theta_age,
+                        int32_t *order /*[n]*/)
+{
+    for (int i = 0; i < n; ++i) order[i] = i;
+    for (int i = 1; i < n; ++i) {                               /* insertion sort under the total order */
+        int x = order[i], j = i - 1;
+        while (j >= 0 && alg2_before(arrival, prefill, now, theta_age, x, order[j])) { order[j + 1] = order[j]; --j; }
+        order[j + 1] = x;
+    }
+}
+
 /* threads the OpenMP loops above will use (reported as cpu_baseline.cores by bench.py) */
 #ifdef _OPENMP
 #include <omp.h>

@@ -20,7 +20,7 @@ EXPORTED_SYMBOLS = [
     "gimbal_route_stats_host",
     "gimbal_eval_placements_workspace_bytes", "gimbal_eval_placements", "gimbal_eval_placements_host",
     "gimbal_eval_moves_workspace_bytes", "gimbal_eval_moves", "gimbal_greedy_place", "gimbal_build_expert_map",
-    "gimbal_select_engines",
+    "gimbal_select_engines", "gimbal_order_queues",
     "gimbal_kernel_timing", "gimbal_kernel_elapsed_ms",
 ]
 KERNEL_ROUTER, KERNEL_GATE, KERNEL_SCORE, KERNEL_MOVES, KERNEL_GREEDY = 0, 1, 2, 3, 4
@@ -73,7 +73,7 @@ def lib():
                   "gimbal_eval_placements_workspace_bytes", "gimbal_eval_moves_workspace_bytes"):
             getattr(L, n).restype = C.c_size_t
         for n in ("gimbal_route_stats", "gimbal_route_stats_host", "gimbal_eval_placements",
-                  "gimbal_eval_placements_host", "gimbal_eval_moves", "gimbal_greedy_place", "gimbal_build_expert_map", "gimbal_select_engines"):
+                  "gimbal_eval_placements_host", "gimbal_eval_moves", "gimbal_greedy_place", "gimbal_build_expert_map", "gimbal_select_engines", "gimbal_order_queues"):
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -321,3 +321,11 @@ def select_engines(trace, req_len, comp, rr, engine, *, complete=None, high_kv=0
     rc = lib().gimbal_select_engines(C.byref(c), C.c_int(B), _ptr(trace), _ptr(complete), _ptr(req_len), _ptr(comp), _ptr(rr),
                                      _ptr(engine), _stream(stream))
     _check(rc, "gimbal_select_engines")
+
+
+def order_queues(arrival, prefill, qlen, now: float, order, *, theta_age: float = 5.0, stream=None):
+    """gimbal_order_queues (Algorithm 2): arrival [B,Q] f32, prefill [B,Q] i32, qlen [B] i32 -> order [B,Q] i32."""
+    B, Q = arrival.shape
+    rc = lib().gimbal_order_queues(C.c_int(B), C.c_int(Q), _ptr(arrival), _ptr(prefill), _ptr(qlen), C.c_float(now),
+                                   C.c_float(theta_age), _ptr(order), _stream(stream))
+    _check(rc, "gimbal_order_queues")

@@ -631,4 +631,17 @@ int gimbal_select_engines(const gimbal_sched_cfg* cfg, int B, const float* trace
     return GIMBAL_OK;
 }
 
+int gimbal_order_queues(int B, int Q, const float* arrival, const int32_t* prefill, const int32_t* qlen, float now, float theta_age,
+                        int32_t* order, gimbal_stream_t stream_) {
+    if (B < 0 || Q < 1 || Q > kQueueMax) return fail(GIMBAL_ERR_INVALID_ARG, "need B >= 0 and 1 <= Q <= %d", kQueueMax);
+    if (B > 0 && (!arrival || !prefill || !qlen || !order)) return fail(GIMBAL_ERR_INVALID_ARG, "NULL argument");
+    int rc = require_device();
+    if (rc) return rc;
+    if (B == 0) return GIMBAL_OK;
+    QueueParams qp{B, Q, now, theta_age, arrival, prefill, qlen, order};
+    order_queues_kernel<<<B, kQueueThreads, 0, static_cast<cudaStream_t>(stream_)>>>(qp);
+    LAUNCH_CHECK("order_queues_kernel");
+    return GIMBAL_OK;
+}
+
 }  // extern "C"

@@ -114,4 +114,53 @@ __global__ void __launch_bounds__(kSchedWarps * 32) select_engines_kernel(const 
     if (lane == 0) p.rr[b] = rr;
 }
 
+// ------------------------------------------------------------------------------------------
+// Algorithm 2, SJF with aging (R20), batched over B waiting queues: one block per queue,
+// position of request j = number of requests that come before it in the total order (aged first and oldest
+// first, then shortest prefill, then oldest, then input position) -- a counting rank, deterministic, no sort.
+// The waiting time uses the same fp32 subtraction as the oracle.
+// ------------------------------------------------------------------------------------------
+struct QueueParams {
+    int B, Q;                      // queues, capacity of a queue (row pitch)
+    float now, theta_age;
+    const float* arrival;          // [B,Q]
+    const int32_t* prefill;        // [B,Q]
+    const int32_t* qlen;           // [B]
+    int32_t* order;                // [B,Q]; entries past qlen are -1
+};
+
+constexpr int kQueueThreads = 256;
+constexpr int kQueueMax = 2048;
+
+__global__ void __launch_bounds__(kQueueThreads) order_queues_kernel(const QueueParams p) {
+    __shared__ float arr_s[kQueueMax];
+    __shared__ int32_t pre_s[kQueueMax];
+    const int b = blockIdx.x;
+    const int n = min(max(p.qlen[b], 0), p.Q);
+    for (int j = threadIdx.x; j < n; j += kQueueThreads) {
+        arr_s[j] = p.arrival[(size_t)b * p.Q + j];
+        pre_s[j] = p.prefill[(size_t)b * p.Q + j];
+    }
+    for (int j = n + threadIdx.x; j < p.Q; j += kQueueThreads) p.order[(size_t)b * p.Q + j] = -1;
+    __syncthreads();
+    for (int j = threadIdx.x; j < n; j += kQueueThreads) {
+        const float aj = arr_s[j];
+        const int pj = pre_s[j];
+        const bool aged_j = __fsub_rn(p.now, aj) >= p.theta_age;
+        int pos = 0;
+        for (int i = 0; i < n; ++i) {
+            const float ai = arr_s[i];
+            const int pi = pre_s[i];
+            const bool aged_i = __fsub_rn(p.now, ai) >= p.theta_age;
+            bool before;
+            if (aged_i != aged_j) before = aged_i;
+            else if (!aged_i && pi != pj) before = pi < pj;
+            else if (ai != aj) before = ai < aj;
+            else before = i < j;
+            pos += before;
+        }
+        p.order[(size_t)b * p.Q + pos] = j;
+    }
+}
+
 }  // namespace gimbal

@@ -767,3 +767,26 @@ def test_select_engines_consumes_route_stats_pressure():
     e, _ = oracle.select_engines(to_np(tr)[0], 1, to_np(lens)[0], c, 0, lambda_moe=1000.0)
     np.testing.assert_array_equal(to_np(eng)[0], e)
     assert int(to_np(eng)[0, 0]) == int(np.argmin(to_np(st.pressure_rel)))       # the engine with the least MoE pressure goes first
+
+
+# ------------------------------------------------------------------------------------------
+# Algorithm 2, SJF with aging (R20) -- a permutation, bit-exact
+# ------------------------------------------------------------------------------------------
+def test_order_queues_parity():
+    rng = np.random.default_rng(17)
+    B, Q = 300, 700
+    arrival = rng.uniform(0, 20, (B, Q)).round(1).astype(np.float32)
+    prefill = np.ceil(rng.lognormal(5.0, 1.2, (B, Q))).astype(np.int32)
+    prefill[:, ::9] = 64                                                  # equal lengths
+    qlen = rng.integers(0, Q + 1, B).astype(np.int32)
+    qlen[:3] = [0, 1, Q]
+    now, theta = 20.0, 5.0
+    t = lambda a: torch.from_numpy(a).to(DEV)
+    order = torch.full((B, Q), -5, dtype=torch.int32, device=DEV)
+    g.order_queues(t(arrival), t(prefill), t(qlen), now, order, theta_age=theta)
+    torch.cuda.synchronize()
+    go = to_np(order)
+    for b in range(B):
+        n = int(qlen[b])
+        np.testing.assert_array_equal(go[b, :n], oracle.order_queue(arrival[b, :n], prefill[b, :n], now, theta))
+        assert (go[b, n:] == -1).all()

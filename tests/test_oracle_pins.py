@@ -619,3 +619,24 @@ def test_alg1_invariants():
     comp = np.zeros(N)
     eng, _ = oracle.select_engines(tr3, 1, lens, comp, 0)
     assert (eng == int(np.argmin(tr3[:, 0]))).all()
+
+
+# =========================================================================== Algorithm 2 (SJF + aging)
+def test_alg2_worked_examples_and_library_sort():
+    gold = json.load(open(os.path.join(GOLD, "alg2_worked_examples.json")))
+    for c in gold["cases"]:
+        got = oracle.order_queue(np.array(c["arrival"], np.float32), np.array(c["prefill"], np.int32), c["now"], c["theta_age"])
+        assert got.tolist() == c["order"], c["name"]
+    # numpy.lexsort restatement of the total order on a random queue
+    rng = np.random.default_rng(13)
+    n = 400
+    arrival = rng.uniform(0, 12, n).round(1).astype(np.float32)          # rounded: many equal arrival times
+    prefill = rng.integers(1, 40, n).astype(np.int32)                    # many equal lengths
+    now, theta = 12.0, 5.0
+    aged = (np.float32(now) - arrival) >= np.float32(theta)
+    key2 = np.where(aged, 0, prefill)                                    # aged requests ignore the length
+    ref = np.lexsort((np.arange(n), arrival, key2, ~aged))
+    np.testing.assert_array_equal(oracle.order_queue(arrival, prefill, now, theta), ref)
+    # no aging (theta = inf) is plain SJF; everybody aged (theta = 0) is FIFO
+    np.testing.assert_array_equal(oracle.order_queue(arrival, prefill, now, np.inf), np.lexsort((np.arange(n), arrival, prefill)))
+    np.testing.assert_array_equal(oracle.order_queue(arrival, prefill, now, 0.0), np.lexsort((np.arange(n), arrival)))
