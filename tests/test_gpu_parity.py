@@ -790,3 +790,42 @@ def test_order_queues_parity():
         n = int(qlen[b])
         np.testing.assert_array_equal(go[b, :n], oracle.order_queue(arrival[b, :n], prefill[b, :n], now, theta))
         assert (go[b, n:] == -1).all()
+
+
+# ------------------------------------------------------------------------------------------
+# NEXT-4: calibration sweep of (beta, gamma) against the exhaustive reference (analogue of Fig. 6)
+# ------------------------------------------------------------------------------------------
+def test_calibration_sweep_against_oracle():
+    import math
+    from paper_2606_15177_b200 import calibrate
+    rng = np.random.default_rng(21)
+    n, S, E, G, sp = 6, 2, 8, 4, 2
+    A = rng.integers(0, 400, (n, S, E))
+    A[:, 0, :E // 2] += 300; A[:, 1, E // 2:] += 300                    # source-dependent skew
+    B = A.sum(1)
+    D = (np.arange(G)[None, :] * S // G != np.arange(S)[:, None]).astype(np.float32)
+    prev = np.stack([rng.permutation(E) for _ in range(n)]).astype(np.int16)
+    betas, gammas = [0.0, 0.0025, 0.05], [0.0, 1.0, 100.0]
+    res = calibrate.calibration_sweep(A, B, D, prev, G, sp, betas, gammas, device=DEV)
+    assert calibrate.all_placements(E, G, sp).shape[0] == math.factorial(E) // math.factorial(sp) ** G == 2520
+    Af, Bf = A.astype(np.float64), B.astype(np.float64)
+    for i in range(n):      # the reference is a minimiser of the printed objective (weights 1,1,1): same J as the oracle's brute force
+        cnt, Jopt, _ = oracle.bruteforce(prev[i], Af[i], Bf[i], D, None, 1.0, G=G, sp=sp, weights=(1.0, 1.0, 1.0))
+        Jref = oracle.objective(res["ref"][i][None], prev[i][None], Af[i][None], Bf[i][None], D, None, 1.0, G=G, sp=sp, weights=(1.0, 1.0, 1.0))
+        assert cnt == 2520 and abs(Jref[0] - Jopt) <= 1e-5 * Jopt
+        np.testing.assert_allclose(res["ref_comm"][i], Jref[2], rtol=1e-5)
+    # agreement / communication gap recomputed with the oracle's greedy and objective
+    for bi, beta in enumerate(betas):
+        for gi, gamma in enumerate(gammas):
+            wts = tuple(float(np.float32(x)) for x in (1.0, beta, gamma))
+            ok, placed = oracle.greedy_place(prev, Af, Bf, D, None, 1.0, G=G, sp=sp, weights=wts)
+            assert ok
+            same = [float((calibrate.rank_of(placed[i], sp) == calibrate.rank_of(res["ref"][i], sp)).mean()) for i in range(n)]
+            comm = [oracle.objective(placed[i][None], prev[i][None], Af[i][None], Bf[i][None], D, None, 1.0, G=G, sp=sp)[2] for i in range(n)]
+            assert abs(res["agree"][bi, gi] - np.mean(same)) < 1e-12
+            np.testing.assert_allclose(res["comm_gap"][bi, gi], np.mean(np.array(comm) / res["ref_comm"] - 1.0), rtol=1e-4, atol=1e-6)
+    # a prohibitive migration weight freezes the placement at x0: the heuristic then agrees with the reference exactly as much as x0 does
+    x0_agree = np.mean([(calibrate.rank_of(prev[i], sp) == calibrate.rank_of(res["ref"][i], sp)).mean() for i in range(n)])
+    frozen = calibrate.calibration_sweep(A, B, D, prev, G, sp, [0.0025], [1e9], device=DEV)
+    assert abs(frozen["agree"][0, 0] - x0_agree) < 1e-12
+    assert res["best"][0] in betas and res["best"][1] in gammas
