@@ -829,3 +829,33 @@ def test_calibration_sweep_against_oracle():
     frozen = calibrate.calibration_sweep(A, B, D, prev, G, sp, [0.0025], [1e9], device=DEV)
     assert abs(frozen["agree"][0, 0] - x0_agree) < 1e-12
     assert res["best"][0] in betas and res["best"][1] in gammas
+
+
+@pytest.mark.parametrize("H,T,E", [(64, 1, 16), (64, 129, 64), (192, 257, 128), (320, 511, 256), (7168, 130, 256)])
+def test_router_gemm_odd_shapes(H, T, E):
+    """one k-block, a single token, tiles with ragged tails, both CTA-group modes: logits against the fp64 oracle, counts
+    against the oracle on the GPU's logits"""
+    from workloads.configs import RouterCfg as WRouterCfg
+    L, S, k = 3, 2, min(4, E)
+    r = WRouterCfg(L=L, H=H, E=E, k=k, S=S)
+    cfg = g.RouterCfg.from_workload(r)
+    gen_ = torch.Generator(device=DEV); gen_.manual_seed(H + T + E)
+    hidden = torch.randn(L, T, H, generator=gen_, device=DEV).to(torch.bfloat16)
+    W = (0.1 * torch.randn(L, E, H, generator=gen_, device=DEV)).to(torch.bfloat16)
+    off = torch.tensor([0, T // 3, T], dtype=torch.int32, device=DEV)
+    ws = ws_tensor(g.route_stats_workspace_bytes(cfg, L, T))
+    hb, wb, offn = bf16_bits(hidden), bf16_bits(W), to_np(off)
+    for cgm in ("1", "2"):
+        os.environ["GIMBAL_CTA_GROUP"] = cgm
+        st = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+        logits = torch.full((L, T, E), 9.0, device=DEV)
+        g.route_stats(cfg, st, T=T, hidden=hidden, w_router=W, src_offsets=off, logits_mode=g.LOGITS_OUT, logits=logits, workspace=ws)
+        st2 = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+        g.route_stats(cfg, st2, T=T, hidden=hidden, w_router=W, src_offsets=off, workspace=ws)
+        for l in range(L):
+            l64, _ = oracle.router_logits(hb[l], wb[l], None, offn)
+            assert _logit_err(to_np(logits[l]), l64) < 2e-4
+            rid, _ = oracle.gate(to_np(logits[l]), r, None, 1)
+            np.testing.assert_array_equal(to_np(st.A_step[l]), oracle.counts(rid, offn, S, E))
+        assert torch.equal(st2.A_step, st.A_step)
+    os.environ.pop("GIMBAL_CTA_GROUP")
