@@ -553,9 +553,10 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
         }
         const size_t smem = move_all_smem_bytes((int)NS, cfg->G, ap.has_M);
         if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "move neighbourhood: NS=%lld G=%d needs %zu B of shared memory", NS, cfg->G, smem);
-        CUDA_TRY(cudaFuncSetAttribute(move_all_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        auto kern = ap.has_M ? move_all_kernel<true> : move_all_kernel<false>;
+        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         ktime_begin(GIMBAL_KERNEL_MOVES, stream);
-        move_all_kernel<<<dim3(bpl, cfg->L), kMoveAllThreads, smem, stream>>>(ap);
+        kern<<<dim3(bpl, cfg->L), kMoveAllThreads, smem, stream>>>(ap);
         ktime_end(GIMBAL_KERNEL_MOVES, stream);
         LAUNCH_CHECK("move_all_kernel");
     } else if (n_moves > 0) {

@@ -731,13 +731,14 @@ struct MoveAllParams {
 // pair {a, NS-2-a} -- NS-1 moves whatever a is.  Inside a row the lanes walk b: everything that
 // depends on a (expert, rank, load, its table row) is warp-uniform, and the results of 32
 // consecutive b are contiguous in `delta`.
+template <bool kHasM>
 __global__ void __launch_bounds__(kMoveAllThreads) move_all_kernel(const MoveAllParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int NS = p.G * p.sp, GP = place_gp(p.G), PITCH = p.G + 1;
     const int l = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     float* Cs = reinterpret_cast<float*>(smem_raw);
     float* Ms = Cs + (size_t)NS * PITCH;
-    size_t off = sizeof(float) * (size_t)NS * PITCH * (p.has_M ? 2 : 1);
+    size_t off = sizeof(float) * (size_t)NS * PITCH * (kHasM ? 2 : 1);
     off = (off + 15) & ~size_t(15);
     double* ws = reinterpret_cast<double*>(smem_raw + off); off += sizeof(double) * NS;
     unsigned long long* cms = reinterpret_cast<unsigned long long*>(smem_raw + off); off += sizeof(unsigned long long) * NS;
@@ -762,7 +763,7 @@ __global__ void __launch_bounds__(kMoveAllThreads) move_all_kernel(const MoveAll
             const float4 v = src[i];
             float* d = Cs + j * PITCH + g;
             d[0] = v.x; d[1] = v.y; d[2] = v.z; d[3] = v.w;
-            if (p.has_M) {
+            if constexpr (kHasM) {
                 const float4 m = srcm[i];
                 float* dm = Ms + j * PITCH + g;
                 dm[0] = m.x; dm[1] = m.y; dm[2] = m.z; dm[3] = m.w;
@@ -787,7 +788,7 @@ __global__ void __launch_bounds__(kMoveAllThreads) move_all_kernel(const MoveAll
             const double w1 = ws[a], L1 = Lgs[g1];
             const unsigned long long cm1 = cms[a];
             const float t11 = Cs[a * PITCH + g1];
-            const float m11 = p.has_M ? Ms[a * PITCH + g1] : p.M_scalar;
+            const float m11 = kHasM ? Ms[a * PITCH + g1] : p.M_scalar;
             const int row0 = a * NS - a * (a + 1) / 2 - a - 1;           // pair index of (a, b) = row0 + b
             for (int bb = a + 1; bb < NS; bb += 32) {
                 const int b = bb + lane;
@@ -805,8 +806,8 @@ __global__ void __launch_bounds__(kMoveAllThreads) move_all_kernel(const MoveAll
                             const double dl = ws[b] - w1;                                 // moved onto g1
                             dload = (float)(2.0 * dl * (L1 - L2) + 2.0 * dl * dl);        // the mean cancels
                             dcomm = (fabsf(t12) - fabsf(t11)) + (fabsf(t21) - fabsf(t22));
-                            const float m12 = p.has_M ? Ms[a * PITCH + g2] : p.M_scalar;
-                            const float m21 = p.has_M ? Ms[b * PITCH + g1] : p.M_scalar, m22 = p.has_M ? Ms[b * PITCH + g2] : p.M_scalar;
+                            const float m12 = kHasM ? Ms[a * PITCH + g2] : p.M_scalar;
+                            const float m21 = kHasM ? Ms[b * PITCH + g1] : p.M_scalar, m22 = kHasM ? Ms[b * PITCH + g2] : p.M_scalar;
                             // leaving a cell x0 has: +M, leaving a cell x0 lacks: -M; entering: the opposite
                             dmig = (__float_as_int(t11) < 0 ? m11 : -m11) + (__float_as_int(t12) < 0 ? -m12 : m12) +
                                    (__float_as_int(t22) < 0 ? m22 : -m22) + (__float_as_int(t21) < 0 ? -m21 : m21);
