@@ -859,3 +859,23 @@ def test_router_gemm_odd_shapes(H, T, E):
             np.testing.assert_array_equal(to_np(st.A_step[l]), oracle.counts(rid, offn, S, E))
         assert torch.equal(st2.A_step, st.A_step)
     os.environ.pop("GIMBAL_CTA_GROUP")
+
+
+def test_repeated_launches_are_deterministic():
+    """the persistent tcgen05 kernel, its mbarrier pipeline and the histogram flushes give the same integers on every
+    launch (a lost arrival or a race would show up as a differing count or a hang)"""
+    w = scaled(get_workload("v3"), L=3, T=4100)
+    r = w.router
+    cfg = g.RouterCfg.from_workload(r)
+    hidden, W, slb, sb, off = _router_inputs(w)
+    ws = ws_tensor(g.route_stats_workspace_bytes(cfg, r.L, w.T))
+    st = g.StatsState(cfg, MODE_WINDOW, window_len=1000)
+    first = None
+    for it in range(40):
+        g.route_stats(cfg, st, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off, workspace=ws)
+        if first is None:
+            first = st.A_step.clone()
+        else:
+            assert torch.equal(st.A_step, first)
+    torch.cuda.synchronize()
+    assert torch.equal(st.A_win, first * 40) and int(st.step_counter.item()) == 40
