@@ -320,6 +320,23 @@ GIMBAL_API int gimbal_select_engines(const gimbal_sched_cfg *cfg, int B, const f
 GIMBAL_API int gimbal_order_queues(int B, int Q, const float *arrival, const int32_t *prefill, const int32_t *qlen,
                         float now, float theta_age, int32_t *order, gimbal_stream_t stream);
 
+/* ---------------------------------------------------------------------------------------
+ * gimbal_refine_placement -- swap-based local search on top of gimbal_eval_moves (SURVEY.md
+ * section 8f, NEXT-1; not in the paper, R21): `iters` rounds; in each round every layer
+ * applies its best single slot exchange of the whole neighbourhood when
+ *     dJ < -1e-4 * (alpha*|dC_comm| + beta*|dC_load| + gamma*|dC_mig|)
+ * (a margin above fp32 rounding, so that the search cannot cycle on noise).  Asynchronous, no host
+ * round trip between rounds.
+ *   cur     [L,NS] i16 inout   placement being refined (must stay valid: x0's expert copies)
+ *   delta   [L*NS*(NS-1)/2, 5] f32  scratch = the deltas of the last round (as gimbal_eval_moves)
+ *   best    [L] i32            scratch = best move of each layer in the last round
+ *   applied [L] i32 out | NULL number of exchanges applied per layer (zeroed by the call)
+ * Other arguments as in gimbal_eval_moves (same workspace size).                            */
+GIMBAL_API int gimbal_refine_placement(const gimbal_placement_cfg *cfg, int16_t *cur, const int16_t *prev, int iters,
+                            const void *A, const void *B, const float *D, const float *M, float M_scalar,
+                            float *delta, int32_t *best, int32_t *applied,
+                            void *workspace, size_t workspace_bytes, gimbal_stream_t stream);
+
 /* Counters for bench.py: kernels launched by this library since load. */
 GIMBAL_API int64_t gimbal_launch_count(void);
 

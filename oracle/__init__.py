@@ -249,6 +249,18 @@ def order_queue(arrival, prefill, now: float, theta_age: float = 5.0):
     return out
 
 
+def refine(cur, prev, A, B, D, M=None, M_scalar=1.0, *, G, sp, weights=(1.0, 0.0025, 1.0), iters=1):
+    """Swap-based local search by full re-evaluation (R21) -> (refined placement [L,NS], applied [L])."""
+    A, B, D, M = _obj_args(A, B, D, M)
+    cur = np.array(cur, dtype=np.int16, order="C", copy=True); prev = _c(prev, np.int16)
+    L, S, E = A.shape
+    applied = np.zeros(L, np.int32)
+    lib().oracle_refine(_p(cur, C.c_int16), _p(prev, C.c_int16), _p(A, C.c_double), _p(B, C.c_double), _p(D, C.c_double),
+                        _p(M, C.c_double), C.c_double(M_scalar), C.c_int(L), C.c_int(S), C.c_int(E), C.c_int(G), C.c_int(sp),
+                        C.c_double(weights[0]), C.c_double(weights[1]), C.c_double(weights[2]), C.c_int(iters), _p(applied, C.c_int32))
+    return cur, applied
+
+
 # -- brute force ------------------------------------------------------------------------
 def bruteforce(prev, A, B, D, M=None, M_scalar=1.0, *, G, sp, weights=(1.0, 0.0025, 1.0)):
     """One layer, NS == E.  A [S,E], B [E], prev [NS] -> (count, best_J, best_place [NS])."""

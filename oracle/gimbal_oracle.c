@@ -686,6 +686,46 @@ void oracle_order_queue(const float *arrival /*[n]*/, const int32_t *prefill /*[
     }
 }
 
+/* ------------------------------------------------------------------------------------ */
+/* Swap-based refinement of a placement (the local search SURVEY.md section 8f attaches to
+ *     NEXT-1; not in the paper, R21): `iters` rounds; in each round and each layer
+ *     the best single slot exchange (lowest dJ by FULL re-evaluation, canonical order a < b,
+ *     first on ties, invalid moves skipped) is applied when
+ *         dJ < -1e-4 * (alpha*|dC_comm| + beta*|dC_load| + gamma*|dC_mig|)
+ *     (a margin above rounding so that the fp32 kernel and this fp64 text cannot cycle on
+ *     noise).  cur is updated in place; applied[l] counts the exchanges of layer l.          */
+/* ------------------------------------------------------------------------------------ */
+void oracle_refine(int16_t *cur /*[L,NS] inout*/, const int16_t *prev, const double *A, const double *B, const double *D,
+                   const double *M, double M_scalar, int L, int S, int E, int G, int sp,
+                   double alpha, double beta, double gamma, int iters, int32_t *applied /*[L]*/)
+{
+    const int NS = G * sp;
+    const int64_t npairs = (int64_t)NS * (NS - 1) / 2;
+    int32_t *mv = (int32_t *)malloc(sizeof(int32_t) * 3 * (size_t)npairs);
+    double *dl = (double *)malloc(sizeof(double) * 5 * (size_t)npairs);
+    for (int l = 0; l < L; ++l) applied[l] = 0;
+    for (int it = 0; it < iters; ++it)
+        for (int l = 0; l < L; ++l) {
+            int64_t q = 0;
+            for (int a = 0; a < NS; ++a)
+                for (int b = a + 1; b < NS; ++b) { mv[q * 3] = l; mv[q * 3 + 1] = a; mv[q * 3 + 2] = b; ++q; }
+            oracle_move_deltas(cur, prev, mv, npairs, A, B, D, M, M_scalar, L, S, E, G, sp, alpha, beta, gamma, dl);
+            int64_t best = -1;
+            for (int64_t i = 0; i < npairs; ++i) {
+                if (dl[i * 5] != dl[i * 5]) continue;
+                if (best < 0 || dl[i * 5] < dl[best * 5]) best = i;
+            }
+            if (best < 0) continue;
+            double thr = 1e-4 * (alpha * fabs(dl[best * 5 + 2]) + beta * fabs(dl[best * 5 + 1]) + gamma * fabs(dl[best * 5 + 3]));
+            if (dl[best * 5] < -thr) {
+                int a = mv[best * 3 + 1], b = mv[best * 3 + 2];
+                int16_t t = cur[(size_t)l * NS + a]; cur[(size_t)l * NS + a] = cur[(size_t)l * NS + b]; cur[(size_t)l * NS + b] = t;
+                applied[l]++;
+            }
+        }
+    free(mv); free(dl);
+}
+
 /* threads the OpenMP loops above will use (reported as cpu_baseline.cores by bench.py) */
 #ifdef _OPENMP
 #include <omp.h>

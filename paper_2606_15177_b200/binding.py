@@ -20,7 +20,7 @@ EXPORTED_SYMBOLS = [
     "gimbal_route_stats_host",
     "gimbal_eval_placements_workspace_bytes", "gimbal_eval_placements", "gimbal_eval_placements_host",
     "gimbal_eval_moves_workspace_bytes", "gimbal_eval_moves", "gimbal_greedy_place", "gimbal_build_expert_map",
-    "gimbal_select_engines", "gimbal_order_queues",
+    "gimbal_select_engines", "gimbal_order_queues", "gimbal_refine_placement",
     "gimbal_kernel_timing", "gimbal_kernel_elapsed_ms",
 ]
 KERNEL_ROUTER, KERNEL_GATE, KERNEL_SCORE, KERNEL_MOVES, KERNEL_GREEDY = 0, 1, 2, 3, 4
@@ -73,7 +73,7 @@ def lib():
                   "gimbal_eval_placements_workspace_bytes", "gimbal_eval_moves_workspace_bytes"):
             getattr(L, n).restype = C.c_size_t
         for n in ("gimbal_route_stats", "gimbal_route_stats_host", "gimbal_eval_placements",
-                  "gimbal_eval_placements_host", "gimbal_eval_moves", "gimbal_greedy_place", "gimbal_build_expert_map", "gimbal_select_engines", "gimbal_order_queues"):
+                  "gimbal_eval_placements_host", "gimbal_eval_moves", "gimbal_greedy_place", "gimbal_build_expert_map", "gimbal_select_engines", "gimbal_order_queues", "gimbal_refine_placement"):
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -329,3 +329,13 @@ def order_queues(arrival, prefill, qlen, now: float, order, *, theta_age: float 
     rc = lib().gimbal_order_queues(C.c_int(B), C.c_int(Q), _ptr(arrival), _ptr(prefill), _ptr(qlen), C.c_float(now),
                                    C.c_float(theta_age), _ptr(order), _stream(stream))
     _check(rc, "gimbal_order_queues")
+
+
+def refine_placement(cfg: PlacementCfg, cur, prev, A, B, D, delta, best, *, iters: int = 1, M=None, M_scalar: float = 1.0, applied=None,
+                     workspace=None, stream=None):
+    """gimbal_refine_placement: `iters` rounds of "apply each layer's best slot exchange"; cur [L,NS] is updated in place."""
+    c = cfg.c()
+    rc = lib().gimbal_refine_placement(C.byref(c), _ptr(cur), _ptr(prev), C.c_int(iters), _ptr(A), _ptr(B), _ptr(D), _ptr(M),
+                                       C.c_float(M_scalar), _ptr(delta), _ptr(best), _ptr(applied), _ptr(workspace),
+                                       C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream))
+    _check(rc, "gimbal_refine_placement")

@@ -577,6 +577,29 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
     return GIMBAL_OK;
 }
 
+int gimbal_refine_placement(const gimbal_placement_cfg* cfg, int16_t* cur, const int16_t* prev, int iters, const void* A, const void* B,
+                            const float* D, const float* M, float M_scalar, float* delta, int32_t* best, int32_t* applied,
+                            void* workspace, size_t workspace_bytes, gimbal_stream_t stream_) {
+    int rc = validate_place_cfg(cfg);
+    if (rc) return rc;
+    if (iters < 0 || !best || !delta) return fail(GIMBAL_ERR_INVALID_ARG, "iters < 0 or NULL scratch");
+    const long long NS = (long long)cfg->G * cfg->slots_per_rank;
+    const long long n = (long long)cfg->L * NS * (NS - 1) / 2;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    if (applied) {
+        rc = require_device();
+        if (rc) return rc;
+        CUDA_TRY(cudaMemsetAsync(applied, 0, sizeof(int32_t) * cfg->L, stream));
+    }
+    for (int it = 0; it < iters; ++it) {
+        rc = gimbal_eval_moves(cfg, cur, prev, n, nullptr, A, B, D, M, M_scalar, delta, best, workspace, workspace_bytes, stream_);
+        if (rc) return rc;
+        apply_best_moves_kernel<<<(cfg->L + 127) / 128, 128, 0, stream>>>(cfg->L, (int)NS, cfg->alpha, cfg->beta, cfg->gamma, best, delta, cur, applied);
+        LAUNCH_CHECK("apply_best_moves_kernel");
+    }
+    return GIMBAL_OK;
+}
+
 int gimbal_build_expert_map(int L, int E, int G, int slots_per_rank, const int16_t* placement, int32_t* rep_off, int16_t* rep_slots,
                             int32_t* status, gimbal_stream_t stream_) {
     if (L < 1 || E < 1 || E > kMaxE || G < 1 || G > kMaxG || slots_per_rank < 1 || slots_per_rank > 16)

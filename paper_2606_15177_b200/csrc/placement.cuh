@@ -852,4 +852,24 @@ __global__ void __launch_bounds__(kMoveAllThreads) move_all_kernel(const MoveAll
     }
 }
 
+// refinement step (gimbal_refine_placement): one thread per layer applies that layer's best exchange when its dJ is
+// below minus the rounding margin; the move index is decoded back to the slot pair (a < b, a outer)
+__global__ void apply_best_moves_kernel(int L, int NS, float alpha, float beta, float gamma, const int32_t* best, const float* delta,
+                                        int16_t* cur, int32_t* applied) {
+    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= L) return;
+    const int bi = best[l];
+    if (bi < 0) return;
+    const float* d = delta + (size_t)bi * 5;
+    const float thr = 1e-4f * (alpha * fabsf(d[2]) + beta * fabsf(d[1]) + gamma * fabsf(d[3]));
+    if (!(d[0] < -thr)) return;
+    const int npairs = NS * (NS - 1) / 2;
+    int r = bi - l * npairs, a = 0;
+    while (r >= NS - 1 - a) { r -= NS - 1 - a; ++a; }
+    const int b = a + 1 + r;
+    int16_t* row = cur + (size_t)l * NS;
+    const int16_t t = row[a]; row[a] = row[b]; row[b] = t;
+    if (applied) applied[l] += 1;
+}
+
 }  // namespace gimbal

@@ -879,3 +879,42 @@ def test_repeated_launches_are_deterministic():
             assert torch.equal(st.A_step, first)
     torch.cuda.synchronize()
     assert torch.equal(st.A_win, first * 40) and int(st.step_counter.item()) == 40
+
+
+# ------------------------------------------------------------------------------------------
+# swap-based refinement on top of a7 (R21)
+# ------------------------------------------------------------------------------------------
+def test_refine_placement_bit_exact_on_integer_instances_and_monotone_elsewhere():
+    # (1) integer counts, binary D, M = 1, weights (1,1,1): every delta is an integer that fp32 holds exactly, so the
+    # kernel and the fp64 oracle take the same decisions -> identical placements
+    rng = np.random.default_rng(41)
+    L, S, E, G, sp = 3, 2, 16, 4, 4
+    A = rng.integers(0, 60, (L, S, E)); B = A.sum(1)
+    D = (np.arange(G)[None, :] * S // G != np.arange(S)[:, None]).astype(np.float32)
+    prev = np.stack([rng.permutation(E) for _ in range(L)]).astype(np.int16)
+    cfg = g.PlacementCfg(L=L, E=E, G=G, slots_per_rank=sp, S=S, alpha=1.0, beta=1.0, gamma=1.0)
+    t = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(device=DEV, dtype=dt)
+    A_t, B_t, D_t, prev_t = t(A, torch.int32), t(B, torch.int32), t(D, torch.float32), t(prev, torch.int16)
+    n = L * (E * (E - 1) // 2)
+    delta = torch.empty(n, 5, device=DEV); best = torch.empty(L, dtype=torch.int32, device=DEV)
+    applied = torch.full((L,), -1, dtype=torch.int32, device=DEV)
+    ws = ws_tensor(g.eval_moves_workspace_bytes(cfg))
+    cur = prev_t.clone()
+    g.refine_placement(cfg, cur, prev_t, A_t, B_t, D_t, delta, best, iters=12, applied=applied, workspace=ws)
+    ref, ref_applied = oracle.refine(prev, prev, A, B, D, None, 1.0, G=G, sp=sp, weights=(1.0, 1.0, 1.0), iters=12)
+    np.testing.assert_array_equal(to_np(cur), ref)
+    np.testing.assert_array_equal(to_np(applied), ref_applied)
+    assert ref_applied.sum() > 0
+    # (2) a V3-shaped instance with fp32 counts and an M table: the objective (oracle) never increases from round to round
+    w, cfg, A, B, D, M, prev = _placement_instance("v3", 6, "f32", True, True)
+    cur = gen.candidates(w, prev, 4, DEV)[3].contiguous()
+    n = cfg.L * cfg.NS * (cfg.NS - 1) // 2
+    delta = torch.empty(n, 5, device=DEV); best = torch.empty(cfg.L, dtype=torch.int32, device=DEV)
+    ws = ws_tensor(g.eval_moves_workspace_bytes(cfg))
+    kw = _oracle_kw(cfg)
+    J = [oracle.objective(to_np(cur), to_np(prev), to_np(A), to_np(B), to_np(D), to_np(M), 0.75, **kw)[0]]
+    for it in range(4):
+        g.refine_placement(cfg, cur, prev, A, B, D, delta, best, iters=1, M=M, M_scalar=0.75, workspace=ws)
+        J.append(oracle.objective(to_np(cur), to_np(prev), to_np(A), to_np(B), to_np(D), to_np(M), 0.75, **kw)[0])
+        assert not np.isnan(J[-1]) and J[-1] <= J[-2] * (1 + 1e-9)
+    assert J[-1] < J[0]
