@@ -221,8 +221,11 @@ GIMBAL_API int gimbal_route_stats_host(const gimbal_router_cfg *cfg, int T,
  *   M [L,E,G] f32 | NULL      migration cost; NULL: M_scalar everywhere
  *   prev [L,NS] i16           x0, the placement before rebalancing (must be valid)
  *   out [P,5] f32             {J, C_load, C_comm, C_mig, maxload}; an invalid candidate
- *                             (id out of range, expert missing, expert twice on a rank)
- *                             gets five NaNs
+ *                             (id out of range, expert missing, expert twice on a rank,
+ *                             other expert copies than x0) gets five NaNs.  Range and
+ *                             same-rank duplicates are checked exactly; "same expert copies
+ *                             as x0" is a 32-bit multiset checksum per layer (a corrupted
+ *                             row passes with probability 2^-32)
  *   argmin [1] i32 | NULL     lowest index among the candidates of minimal J (NaNs skipped;
  *                             -1 if none is valid)
  * Supported: E <= 256, G <= 64, slots_per_rank <= 16, S <= 64.                            */
