@@ -416,8 +416,10 @@ def run_e2e(g, w, cfg, pc, st, hidden, off, cands, W, sb, slb, cur, dp, D, prev,
     best_host = torch.zeros(r.L, dtype=torch.int32, pin_memory=True)
     torch.cuda.synchronize()
 
+    ctx = g.HostCtx()
+
     def step():
-        g.route_stats_host(cfg, st, T=w.T, hidden_host=hidden_host, src_offsets_host=off_host, hidden_stage=stage,
+        g.route_stats_host(ctx, cfg, st, T=w.T, hidden_host=hidden_host, src_offsets_host=off_host, hidden_stage=stage,
                            src_offsets_stage=off_stage, w_router=W, select_bias=sb, src_logit_bias=slb, cur_placement=cur,
                            dp_of_rank=dp, G=w.G, slots_per_rank=w.slots_per_rank, result_host=result_host, workspace=ws_r)
         A_live = st.A_step if w.mode == MODE_WINDOW else st.A_ema

@@ -117,12 +117,28 @@ typedef struct gimbal_stats_state {
  * x[l,e,g] in {0,1} = rank g hosts expert e.  With redundant slots (NS > E,
  * DESIGN.md R12) an expert may be hosted by r >= 1 ranks and its tokens split evenly over
  * them.  A valid placement hosts every expert at least once and never twice on one rank.
- * counts_dtype says whether A and B hold int32 or float.                                  */
+ * counts_dtype says whether A and B hold int32 or float.
+ *   encoding  of the `candidates` of gimbal_eval_placements:
+ *             SLOT_TO_EXPERT_I16  [P,L,NS] int16, as above (any supported shape);
+ *             EXPERT_TO_RANK_U8   [P,L,E] uint8, byte e = the rank hosting expert e; only without
+ *                                 replicas (NS == E) and E in {16,32,64,128,256}.  Half the bytes.
+ *   flags     GIMBAL_PLACE_TRUSTED: the caller guarantees that every candidate is valid and hosts
+ *             as many copies of each expert as x0 (true of anything made from x0 by slot exchanges,
+ *             e.g. the output of gimbal_refine_placement or a rebalancer's own proposals); the
+ *             validation pass is skipped.  A candidate that breaks the promise gets finite but
+ *             meaningless numbers -- never a fault (ids are masked to the tables).
+ * Supported: E <= 256 and even, G a power of two <= 64, slots_per_rank <= 16, S <= 64.       */
+#define GIMBAL_ENC_SLOT_TO_EXPERT_I16 0
+#define GIMBAL_ENC_EXPERT_TO_RANK_U8 1
+#define GIMBAL_PLACE_TRUSTED 1
+
 typedef struct gimbal_placement_cfg {
     int32_t L, E, G, slots_per_rank, S;
     float alpha, beta, gamma; /* J = alpha*C_comm + beta*C_load + gamma*C_mig; paper's
                                  calibrated (1.0, 0.0025, 1.0); R6 */
     int32_t counts_dtype;
+    int32_t encoding;
+    int32_t flags;
 } gimbal_placement_cfg;
 
 /* Expert mapping (NEXT-3; "fuse source counting with expert mapping"): the
@@ -188,16 +204,24 @@ GIMBAL_API int gimbal_route_stats(const gimbal_router_cfg *cfg, int layer0, int 
 GIMBAL_API int gimbal_build_expert_map(int L, int E, int G, int slots_per_rank, const int16_t *placement,
                             int32_t *rep_off, int16_t *rep_slots, int32_t *status, gimbal_stream_t stream);
 
+/* Context of the *_host entry points that overlap copies with kernels: a private copy stream and
+ * its events on the device that is current at creation.  One context serves one host thread at a
+ * time; create one per thread / device.  Creation allocates (the only entry point that does);
+ * destroy waits for the copy stream.                                                          */
+typedef struct gimbal_host_ctx gimbal_host_ctx;
+GIMBAL_API int gimbal_host_ctx_create(gimbal_host_ctx **ctx);
+GIMBAL_API int gimbal_host_ctx_destroy(gimbal_host_ctx *ctx);
+
 /* Same step with the per-step inputs in HOST memory: hidden_host [n_layers,T,H] bf16 and
  * src_offsets_host [S+1] are copied to the device staging buffers the caller provides
- * (hidden_stage: at least 2 layers of [T,H] bf16; copies overlap the kernels layer by layer),
- * and after the step A_step, B and both pressure vectors are copied back to
+ * (hidden_stage: at least 2 layers of [T,H] bf16; the copy of layer i+1 runs on ctx's stream while
+ * layer i computes), and after the step A_step, B and both pressure vectors are copied back to
  * result_host (layout: A_step i32 [L,S,E] | B [L,E] | pressure_raw [S] | pressure_rel [S]),
  * gimbal_route_stats_result_bytes() bytes.  logits_mode is NONE.  Weights, biases, the
  * placement and the state stay device-resident (they persist across steps).  Synchronises
- * `stream` before returning.                                                              */
+ * `stream` before returning.  INVALID_ARG if ctx is NULL or belongs to another device.        */
 GIMBAL_API size_t gimbal_route_stats_result_bytes(const gimbal_router_cfg *cfg);
-GIMBAL_API int gimbal_route_stats_host(const gimbal_router_cfg *cfg, int T,
+GIMBAL_API int gimbal_route_stats_host(gimbal_host_ctx *ctx, const gimbal_router_cfg *cfg, int T,
                             const void *hidden_host, const int32_t *src_offsets_host,
                             void *hidden_stage, size_t hidden_stage_bytes, int32_t *src_offsets_stage,
                             const void *w_router, const float *select_bias, const float *src_logit_bias,
@@ -213,33 +237,38 @@ GIMBAL_API int gimbal_route_stats_host(const gimbal_router_cfg *cfg, int T,
  *   C_mig    = sum_l sum_e sum_g M[l,e,g] |x[l,e,g] - x0[l,e,g]|
  *   J        = alpha*C_comm + beta*C_load + gamma*C_mig
  *   maxload  = sum_l max_g L[l,g]                                           (R7)
+ * r[l,e] is the CANDIDATE's replica count (R12): a candidate may replicate other experts
+ * than x0 does.
  * Arguments
- *   candidates [P,L,NS] i16   slot -> expert
- *   A [L,S,E], B [L,E]        i32 or f32 (cfg->counts_dtype); B is an input of its own
+ *   candidates [P,L,NS] i16   slot -> expert (or [P,L,E] u8 expert -> rank, cfg->encoding); 16-byte aligned
+ *   A [L,S,E], B [L,E]        i32 or f32 (cfg->counts_dtype), >= 0; B is an input of its own
  *                             because the paper collects it on another window (R9)
  *   D [S,G] f32 (>= 0)        source -> rank communication cost
- *   M [L,E,G] f32 | NULL      migration cost; NULL: M_scalar everywhere
- *   prev [L,NS] i16           x0, the placement before rebalancing (must be valid)
- *   out [P,5] f32             {J, C_load, C_comm, C_mig, maxload}; an invalid candidate
- *                             (id out of range, expert missing, expert twice on a rank,
- *                             other expert copies than x0) gets five NaNs.  Range and
- *                             same-rank duplicates are checked exactly; "same expert copies
- *                             as x0" is a 32-bit multiset checksum per layer (a corrupted
- *                             row passes with probability 2^-32)
+ *   M [L,E,G] f32 (>= 0) | NULL   migration cost; NULL: M_scalar everywhere
+ *   prev [L,NS] i16           x0, the placement before rebalancing (must be valid; an invalid x0
+ *                             turns every output into NaN)
+ *   out [P,5] f32             {J, C_load, C_comm, C_mig, maxload}; an invalid candidate (id or rank
+ *                             out of range, an expert hosted nowhere, an expert twice on a rank, a
+ *                             rank over capacity) gets five NaNs.  Validity is decided exactly: a
+ *                             warp builds the candidate's x[e,g] bit matrix in shared memory and
+ *                             reads every condition off it (skipped with GIMBAL_PLACE_TRUSTED).
+ *                             C_mig adds up the entering and the leaving cells directly, so it is
+ *                             exactly 0 for a candidate equal to x0.
  *   argmin [1] i32 | NULL     lowest index among the candidates of minimal J (NaNs skipped;
  *                             -1 if none is valid)
- * Supported: E <= 256, G <= 64, slots_per_rank <= 16, S <= 64.                            */
+ * EXPERT_TO_RANK_U8 sums a rank's load with shared-memory float atomics: with f32 counts the last
+ * bits of C_load depend on the order of the additions (integer counts below 2^24 are exact).    */
 GIMBAL_API size_t gimbal_eval_placements_workspace_bytes(const gimbal_placement_cfg *cfg, int P);
 
-GIMBAL_API int gimbal_eval_placements(const gimbal_placement_cfg *cfg, int P, const int16_t *candidates,
+GIMBAL_API int gimbal_eval_placements(const gimbal_placement_cfg *cfg, int P, const void *candidates,
                            const void *A, const void *B, const float *D, const float *M, float M_scalar,
                            const int16_t *prev, float *out, int32_t *argmin,
                            void *workspace, size_t workspace_bytes, gimbal_stream_t stream);
 
-/* Candidates and results in HOST memory (cand_stage: device buffer of P*L*NS int16;
+/* Candidates and results in HOST memory (cand_stage: device buffer of the candidates' size;
  * out_stage: device [P,5] f32).  Synchronises `stream` before returning.                  */
-GIMBAL_API int gimbal_eval_placements_host(const gimbal_placement_cfg *cfg, int P, const int16_t *candidates_host,
-                                int16_t *cand_stage, float *out_stage,
+GIMBAL_API int gimbal_eval_placements_host(const gimbal_placement_cfg *cfg, int P, const void *candidates_host,
+                                void *cand_stage, float *out_stage,
                                 const void *A, const void *B, const float *D, const float *M, float M_scalar,
                                 const int16_t *prev, float *out_host, int32_t *argmin_host,
                                 void *workspace, size_t workspace_bytes, gimbal_stream_t stream);
@@ -256,7 +285,10 @@ GIMBAL_API int gimbal_eval_placements_host(const gimbal_placement_cfg *cfg, int 
  *                            L*NS*(NS-1)/2
  *   best_per_layer [L] i32 | NULL  index (into the n moves) of the lowest dJ of each layer,
  *                            lowest index on ties, -1 if the layer has no valid move
- * Other arguments as in gimbal_eval_placements; `cur` and `prev` must be valid.            */
+ * Other arguments as in gimbal_eval_placements; `cur` and `prev` must be valid and host the same
+ * number of copies of every expert (an exchange keeps them), else every delta is NaN.  The whole
+ * neighbourhood runs in a kernel that stages the layer's per-slot rows in shared memory when they
+ * fit (every BASELINE.json shape does), otherwise -- like an explicit list -- one thread per move.  */
 GIMBAL_API size_t gimbal_eval_moves_workspace_bytes(const gimbal_placement_cfg *cfg);
 
 GIMBAL_API int gimbal_eval_moves(const gimbal_placement_cfg *cfg, const int16_t *cur, const int16_t *prev,
@@ -264,6 +296,18 @@ GIMBAL_API int gimbal_eval_moves(const gimbal_placement_cfg *cfg, const int16_t 
                       const void *A, const void *B, const float *D, const float *M, float M_scalar,
                       float *delta, int32_t *best_per_layer,
                       void *workspace, size_t workspace_bytes, gimbal_stream_t stream);
+
+/* The per-call inputs in HOST memory: cur_host / prev_host [L,NS] and the optional move list
+ * moves_host [n,3] are copied to their *_stage device buffers; best_host [L] (optional) and, when
+ * delta_host is not NULL, delta [n,5] are copied back (delta_stage [n,5] always receives the
+ * deltas on the device: a whole neighbourhood is 20 bytes per move, so a caller that only wants
+ * the best move per layer leaves delta_host NULL).  Synchronises `stream` before returning.     */
+GIMBAL_API int gimbal_eval_moves_host(const gimbal_placement_cfg *cfg, const int16_t *cur_host, const int16_t *prev_host,
+                           int16_t *cur_stage, int16_t *prev_stage, int64_t n_moves, const int32_t *moves_host,
+                           int32_t *moves_stage, const void *A, const void *B, const float *D, const float *M,
+                           float M_scalar, float *delta_stage, float *delta_host /* | NULL */,
+                           int32_t *best_stage, int32_t *best_host /* | NULL */,
+                           void *workspace, size_t workspace_bytes, gimbal_stream_t stream);
 
 /* ---------------------------------------------------------------------------------------
  * gimbal_greedy_place -- the online greedy placement heuristic (section
@@ -340,6 +384,24 @@ GIMBAL_API int gimbal_refine_placement(const gimbal_placement_cfg *cfg, int16_t 
                             float *delta, int32_t *best, int32_t *applied,
                             void *workspace, size_t workspace_bytes, gimbal_stream_t stream);
 
+/* Process-wide switches for tests and A/B measurements (not for concurrent use; production keeps
+ * the defaults).  They replace environment variables: nothing in the library reads the environment.
+ *   GIMBAL_OPT_CTA_GROUP         0 (default: cta_group::2 when T > 128), 1 or 2: router GEMM pairing
+ *   GIMBAL_OPT_FUSE_GATE         1 (default): gating + histogram in the GEMM epilogue; 0: GEMM writes
+ *                                logits, the standalone gating kernel reads them (needs LOGITS_OUT)
+ *   GIMBAL_OPT_SCORE_GENERIC     0 (default); 1: the shape-generic scoring kernel even where a
+ *                                specialised one exists
+ *   GIMBAL_OPT_CHECK_SCORES_ALL  0 (default); 1: place_check_kernel scores every valid candidate with
+ *                                the candidate's own replica counts (the path otherwise taken only by
+ *                                candidates whose replica counts differ from x0's)                  */
+#define GIMBAL_OPT_CTA_GROUP 0
+#define GIMBAL_OPT_FUSE_GATE 1
+#define GIMBAL_OPT_SCORE_GENERIC 2
+#define GIMBAL_OPT_CHECK_SCORES_ALL 3
+#define GIMBAL_OPT_COUNT_ 4
+GIMBAL_API int gimbal_set_option(int option, int value);
+GIMBAL_API int gimbal_get_option(int option, int *value);
+
 /* Counters for bench.py: kernels launched by this library since load. */
 GIMBAL_API int64_t gimbal_launch_count(void);
 
@@ -352,6 +414,7 @@ GIMBAL_API int64_t gimbal_launch_count(void);
 #define GIMBAL_KERNEL_SCORE 2  /* placement scoring                          a6    */
 #define GIMBAL_KERNEL_MOVES 3  /* move deltas                                a7    */
 #define GIMBAL_KERNEL_GREEDY 4 /* greedy placement heuristic                 NEXT-1 */
+#define GIMBAL_KERNEL_CHECK 5  /* exact candidate validation                 a6    */
 GIMBAL_API int gimbal_kernel_timing(int enable);
 GIMBAL_API int gimbal_kernel_elapsed_ms(int which, float *ms);
 

@@ -620,6 +620,7 @@ void oracle_select_engines(const float *trace /*[N,4]*/, int complete, const flo
                            double high_kv, double large_gap, double lambda_kv, double lambda_moe, double close_frac,
                            double *comp /*[N] inout*/, int32_t *rr /*[1] inout*/, int32_t *engine /*[R]*/)
 {
+    *rr = ((*rr % N) + N) % N;                              /* Next(E) counts modulo N (R19) */
     for (int q = 0; q < R; ++q) {
         double len = (double)req_len[q];
         int pick = -1;
@@ -671,7 +672,7 @@ static int alg2_before(const float *arrival, const int32_t *prefill, float now, 
     int aged_a = (now - arrival[a]) >= theta, aged_b = (now - arrival[b]) >= theta;
     if (aged_a != aged_b) return aged_a;                        /* high priority first */
     if (!aged_a && prefill[a] != prefill[b]) return prefill[a] < prefill[b];
-    if (arrival[a] != arrival[b]) return arrival[a] < arrival[b];
+    if (arrival[a] < arrival[b] || arrival[b] < arrival[a]) return arrival[a] < arrival[b];   /* a NaN arrival ties (R20) */
     return a < b;
 }
 

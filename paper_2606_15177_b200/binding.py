@@ -17,13 +17,17 @@ COUNTS_I32, COUNTS_F32 = 0, 1
 EXPORTED_SYMBOLS = [
     "gimbal_version", "gimbal_last_error", "gimbal_launch_count",
     "gimbal_route_stats_workspace_bytes", "gimbal_route_stats", "gimbal_route_stats_result_bytes",
-    "gimbal_route_stats_host",
+    "gimbal_route_stats_host", "gimbal_host_ctx_create", "gimbal_host_ctx_destroy", "gimbal_eval_moves_host",
+    "gimbal_set_option", "gimbal_get_option",
     "gimbal_eval_placements_workspace_bytes", "gimbal_eval_placements", "gimbal_eval_placements_host",
     "gimbal_eval_moves_workspace_bytes", "gimbal_eval_moves", "gimbal_greedy_place", "gimbal_build_expert_map",
     "gimbal_select_engines", "gimbal_order_queues", "gimbal_refine_placement",
     "gimbal_kernel_timing", "gimbal_kernel_elapsed_ms",
 ]
-KERNEL_ROUTER, KERNEL_GATE, KERNEL_SCORE, KERNEL_MOVES, KERNEL_GREEDY = 0, 1, 2, 3, 4
+KERNEL_ROUTER, KERNEL_GATE, KERNEL_SCORE, KERNEL_MOVES, KERNEL_GREEDY, KERNEL_CHECK = 0, 1, 2, 3, 4, 5
+ENC_SLOT_TO_EXPERT_I16, ENC_EXPERT_TO_RANK_U8 = 0, 1
+PLACE_TRUSTED = 1
+OPT_CTA_GROUP, OPT_FUSE_GATE, OPT_SCORE_GENERIC, OPT_CHECK_SCORES_ALL = 0, 1, 2, 3
 
 
 class GimbalError(RuntimeError):
@@ -48,7 +52,8 @@ class _ExpertMap(C.Structure):
 
 class _PlacementCfg(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("L", "E", "G", "slots_per_rank", "S")] + \
-               [(n, C.c_float) for n in ("alpha", "beta", "gamma")] + [("counts_dtype", C.c_int32)]
+               [(n, C.c_float) for n in ("alpha", "beta", "gamma")] + [("counts_dtype", C.c_int32), ("encoding", C.c_int32),
+                                                                       ("flags", C.c_int32)]
 
 
 def lib_path() -> str:
@@ -73,7 +78,9 @@ def lib():
                   "gimbal_eval_placements_workspace_bytes", "gimbal_eval_moves_workspace_bytes"):
             getattr(L, n).restype = C.c_size_t
         for n in ("gimbal_route_stats", "gimbal_route_stats_host", "gimbal_eval_placements",
-                  "gimbal_eval_placements_host", "gimbal_eval_moves", "gimbal_greedy_place", "gimbal_build_expert_map", "gimbal_select_engines", "gimbal_order_queues", "gimbal_refine_placement"):
+                  "gimbal_eval_placements_host", "gimbal_eval_moves", "gimbal_eval_moves_host", "gimbal_greedy_place",
+                  "gimbal_build_expert_map", "gimbal_select_engines", "gimbal_order_queues", "gimbal_refine_placement",
+                  "gimbal_host_ctx_create", "gimbal_host_ctx_destroy", "gimbal_set_option", "gimbal_get_option"):
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -156,6 +163,8 @@ class PlacementCfg:
     beta: float = 0.0025
     gamma: float = 1.0
     counts_dtype: int = COUNTS_I32
+    encoding: int = ENC_SLOT_TO_EXPERT_I16
+    flags: int = 0
 
     @property
     def NS(self):
@@ -163,7 +172,7 @@ class PlacementCfg:
 
     def c(self):
         return _PlacementCfg(self.L, self.E, self.G, self.slots_per_rank, self.S, self.alpha, self.beta, self.gamma,
-                             self.counts_dtype)
+                             self.counts_dtype, self.encoding, self.flags)
 
 
 class StatsState:
@@ -235,17 +244,36 @@ class ExpertMap:
         _check(rc, "gimbal_build_expert_map")
 
 
-def route_stats_host(cfg: RouterCfg, state: StatsState, *, T: int, hidden_host, src_offsets_host, hidden_stage,
+class HostCtx:
+    """gimbal_host_ctx: the copy stream + events of the *_host entry points (one per host thread and device)."""
+
+    def __init__(self):
+        self.handle = C.c_void_p(None)
+        _check(lib().gimbal_host_ctx_create(C.byref(self.handle)), "gimbal_host_ctx_create")
+
+    def close(self):
+        if self.handle:
+            lib().gimbal_host_ctx_destroy(self.handle)
+            self.handle = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def route_stats_host(ctx: HostCtx, cfg: RouterCfg, state: StatsState, *, T: int, hidden_host, src_offsets_host, hidden_stage,
                      src_offsets_stage, w_router, select_bias=None, src_logit_bias=None, cur_placement=None,
                      dp_of_rank=None, G: int = 0, slots_per_rank: int = 0, result_host=None, workspace=None, stream=None):
     """gimbal_route_stats_host: hidden / src_offsets in (pinned) host memory, results back to host."""
     c, s = cfg.c(), state.c()
-    rc = lib().gimbal_route_stats_host(C.byref(c), C.c_int(T), _ptr(hidden_host), _ptr(src_offsets_host), _ptr(hidden_stage),
-                                       C.c_size_t(hidden_stage.numel() * hidden_stage.element_size()), _ptr(src_offsets_stage),
-                                       _ptr(w_router), _ptr(select_bias), _ptr(src_logit_bias), _ptr(cur_placement),
-                                       _ptr(dp_of_rank), C.c_int(G), C.c_int(slots_per_rank), C.byref(s), _ptr(result_host),
-                                       _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()),
-                                       _stream(stream))
+    rc = lib().gimbal_route_stats_host(ctx.handle, C.byref(c), C.c_int(T), _ptr(hidden_host), _ptr(src_offsets_host),
+                                       _ptr(hidden_stage), C.c_size_t(hidden_stage.numel() * hidden_stage.element_size()),
+                                       _ptr(src_offsets_stage), _ptr(w_router), _ptr(select_bias), _ptr(src_logit_bias),
+                                       _ptr(cur_placement), _ptr(dp_of_rank), C.c_int(G), C.c_int(slots_per_rank), C.byref(s),
+                                       _ptr(result_host), _ptr(workspace),
+                                       C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream))
     _check(rc, "gimbal_route_stats_host")
 
 
@@ -296,6 +324,30 @@ def eval_moves(cfg: PlacementCfg, cur, prev, A, B, D, delta, *, moves=None, n_mo
                                  _ptr(D), _ptr(M), C.c_float(M_scalar), _ptr(delta), _ptr(best_per_layer), _ptr(workspace),
                                  C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream))
     _check(rc, "gimbal_eval_moves")
+
+
+def eval_moves_host(cfg: PlacementCfg, cur_host, prev_host, cur_stage, prev_stage, A, B, D, delta_stage, *, moves_host=None,
+                    moves_stage=None, n_moves: int | None = None, M=None, M_scalar: float = 1.0, delta_host=None, best_stage=None,
+                    best_host=None, workspace=None, stream=None):
+    """gimbal_eval_moves_host: cur / prev / moves in host memory; best_host and (optionally) delta_host copied back."""
+    c = cfg.c()
+    if n_moves is None:
+        n_moves = moves_host.shape[0] if moves_host is not None else cfg.L * cfg.NS * (cfg.NS - 1) // 2
+    rc = lib().gimbal_eval_moves_host(C.byref(c), _ptr(cur_host), _ptr(prev_host), _ptr(cur_stage), _ptr(prev_stage),
+                                      C.c_int64(n_moves), _ptr(moves_host), _ptr(moves_stage), _ptr(A), _ptr(B), _ptr(D), _ptr(M),
+                                      C.c_float(M_scalar), _ptr(delta_stage), _ptr(delta_host), _ptr(best_stage), _ptr(best_host),
+                                      _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream))
+    _check(rc, "gimbal_eval_moves_host")
+
+
+def set_option(option: int, value: int) -> None:
+    _check(lib().gimbal_set_option(C.c_int(option), C.c_int(value)), "gimbal_set_option")
+
+
+def get_option(option: int) -> int:
+    v = C.c_int(0)
+    _check(lib().gimbal_get_option(C.c_int(option), C.byref(v)), "gimbal_get_option")
+    return int(v.value)
 
 
 def greedy_place(cfg: PlacementCfg, A, B, D, prev, out, *, M=None, M_scalar: float = 1.0, status=None, stream=None):

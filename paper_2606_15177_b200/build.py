@@ -17,7 +17,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libgimbal.so")
 SOURCES = ["gimbal_api.cu", "host_common.cu", "route_e16.cu", "route_e32.cu", "route_e64.cu", "route_e128.cu",
            "route_e256.cu"]
-HEADERS = ["ptx.cuh", "gating.cuh", "router_gemm.cuh", "stats_update.cuh", "placement.cuh", "greedy.cuh", "sched.cuh", "host_common.h",
+HEADERS = ["ptx.cuh", "gating.cuh", "router_gemm.cuh", "stats_update.cuh", "placement.cuh", "placement_e2r.cuh", "greedy.cuh", "sched.cuh", "host_common.h",
            "route_launch.cuh", os.path.join("..", "..", "include", "gimbal.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -5,13 +5,16 @@
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
 
+#include <atomic>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <new>
 
 #include "host_common.h"
 #include "greedy.cuh"
 #include "placement.cuh"
+#include "placement_e2r.cuh"
 #include "sched.cuh"
 #include "stats_update.cuh"
 
@@ -25,6 +28,8 @@ void copy_last_error(char* buf, size_t n);
 }
 
 namespace {
+
+constexpr int kHostCtxSlots = 64;
 
 // ---- workspace carving ---------------------------------------------------------------------
 struct Carver {
@@ -98,18 +103,16 @@ size_t route_ws_carve(const gimbal_router_cfg* c, void* ws, RouteWs* out) {
     return cv.off + 256;
 }
 
-// force 1-CTA or 2-CTA pairs from the environment (debug / A-B measurement); default 2
+// process-wide switches set through gimbal_set_option (tests and A/B measurements); defaults = production
+std::atomic<int> g_opt[GIMBAL_OPT_COUNT_] = {{0}, {1}, {0}, {0}};
+
 int pick_cta_group(int T) {
-    const char* e = getenv("GIMBAL_CTA_GROUP");     // read per call: tests flip it
-    const int forced = e ? atoi(e) : 0;
+    const int forced = g_opt[GIMBAL_OPT_CTA_GROUP].load(std::memory_order_relaxed);
     if (forced == 1 || forced == 2) return forced;
     return T > 128 ? 2 : 1;
 }
 
-int pick_fuse() {
-    const char* e = getenv("GIMBAL_FUSE_GATE");
-    return e ? atoi(e) : 1;
-}
+int pick_fuse() { return g_opt[GIMBAL_OPT_FUSE_GATE].load(std::memory_order_relaxed); }
 
 // ------------------------------------------------------------------------------------------
 static int validate_place_cfg(const gimbal_placement_cfg* c) {
@@ -137,11 +140,14 @@ static size_t place_ws_carve(const gimbal_placement_cfg* c, int P, void* ws, Pla
     PlaceWs w{};
     const int GP = place_gp(c->G);
     const size_t LE = (size_t)c->L * c->E;
+    const size_t NSl = (size_t)c->L * c->G * c->slots_per_rank;
     w.t.wc = cv.take<float2>(LE * GP);
     w.t.m = cv.take<float>(LE * GP);
+    w.t.mu = cv.take<uint32_t>(LE * GP);
+    w.t.mx0 = cv.take<float>(NSl);
+    w.t.c_raw = cv.take<float>(LE * c->G);
+    w.t.b_raw = cv.take<double>(LE);
     w.t.w_e = cv.take<double>(LE);
-    w.t.hsum = cv.take<uint32_t>(c->L);
-    w.t.base_mig = cv.take<float>(c->L);
     w.t.sumB = cv.take<double>(c->L);
     w.t.r = cv.take<int32_t>(LE);
     w.t.pmask = cv.take<uint64_t>(LE);
@@ -153,7 +159,6 @@ static size_t place_ws_carve(const gimbal_placement_cfg* c, int P, void* ws, Pla
     w.mp.top_g = cv.take<int32_t>((size_t)c->L * 4);
     w.mp.cmask = cv.take<uint64_t>(LE);
     w.mp.bad = cv.take<int32_t>(64);
-    const size_t NSl = (size_t)c->L * c->G * c->slots_per_rank;
     w.mp.slotC = cv.take<float>(NSl * c->G);
     w.mp.slotM = cv.take<float>(NSl * c->G);
     w.mp.slot_w = cv.take<double>(NSl);
@@ -174,9 +179,20 @@ static int launch_tables(const gimbal_placement_cfg* c, const void* A, const voi
     return GIMBAL_OK;
 }
 
-template <int SP, bool kDup, bool kHasM>
+template <bool kHasM>
+static int launch_score_generic(const ScoreParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
+    auto kern = place_score_generic_kernel<kHasM>;
+    CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ktime_begin(GIMBAL_KERNEL_SCORE, stream);
+    kern<<<grid, kScoreThreads, smem, stream>>>(sp);
+    ktime_end(GIMBAL_KERNEL_SCORE, stream);
+    LAUNCH_CHECK("place_score_generic_kernel");
+    return GIMBAL_OK;
+}
+
+template <int SP, int G, bool kHasM>
 static int launch_score_v(const ScoreParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
-    auto kern = place_score_kernel<SP, kDup, kHasM>;
+    auto kern = place_score_kernel<SP, G, kHasM>;
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ktime_begin(GIMBAL_KERNEL_SCORE, stream);
     kern<<<grid, kScoreThreads, smem, stream>>>(sp);
@@ -185,26 +201,42 @@ static int launch_score_v(const ScoreParams& sp, dim3 grid, size_t smem, cudaStr
     return GIMBAL_OK;
 }
 
-static int launch_score_generic(const ScoreParams& sp, bool dup, dim3 grid, size_t smem, cudaStream_t stream) {
-    if (sp.has_M) return dup ? launch_score_v<0, true, true>(sp, grid, smem, stream) : launch_score_v<0, false, true>(sp, grid, smem, stream);
-    return dup ? launch_score_v<0, true, false>(sp, grid, smem, stream) : launch_score_v<0, false, false>(sp, grid, smem, stream);
+template <int SP, int G>
+static int launch_score(const ScoreParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
+    return sp.has_M ? launch_score_v<SP, G, true>(sp, grid, smem, stream) : launch_score_v<SP, G, false>(sp, grid, smem, stream);
 }
 
-template <int SP, int G, bool kDup, bool kHasM>
-static int launch_score_fast_v(const ScoreParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
-    auto kern = place_score_fast_kernel<SP, G, kDup, kHasM>;
+template <int E>
+static int launch_e2r_e(const E2RParams& ep, bool has_M, dim3 grid, size_t smem, cudaStream_t stream) {
+    auto kern = has_M ? place_score_e2r_kernel<E, true> : place_score_e2r_kernel<E, false>;
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ktime_begin(GIMBAL_KERNEL_SCORE, stream);
-    kern<<<grid, kScoreThreads, smem, stream>>>(sp);
+    kern<<<grid, kE2RWarps * 32, smem, stream>>>(ep);
     ktime_end(GIMBAL_KERNEL_SCORE, stream);
-    LAUNCH_CHECK("place_score_fast_kernel");
+    LAUNCH_CHECK("place_score_e2r_kernel");
     return GIMBAL_OK;
 }
 
-template <int SP, int G>
-static int launch_score_fast(const ScoreParams& sp, bool dup, dim3 grid, size_t smem, cudaStream_t stream) {
-    if (sp.has_M) return dup ? launch_score_fast_v<SP, G, true, true>(sp, grid, smem, stream) : launch_score_fast_v<SP, G, false, true>(sp, grid, smem, stream);
-    return dup ? launch_score_fast_v<SP, G, true, false>(sp, grid, smem, stream) : launch_score_fast_v<SP, G, false, false>(sp, grid, smem, stream);
+static int launch_e2r(const gimbal_placement_cfg* c, int P, const uint8_t* cand, const float* M, float M_scalar, const PlaceTables& t,
+                      float4* partial, size_t smem, int sms, cudaStream_t stream) {
+    E2RParams ep{};
+    ep.P = P; ep.L = c->L; ep.G = c->G; ep.sp = c->slots_per_rank; ep.check = !(c->flags & GIMBAL_PLACE_TRUSTED);
+    ep.M_scalar = M_scalar; ep.cand = cand; ep.M = M; ep.t = t; ep.partial = partial;
+    const int per_sm = (int)((kSmemLimit - 1024) / (smem + 1024)) < 1 ? 1 : (int)((kSmemLimit - 1024) / (smem + 1024));
+    int nchunk = (per_sm > 4 ? 4 : per_sm) * sms / c->L;
+    const int maxc = (P + kE2RWarps - 1) / kE2RWarps;
+    if (nchunk > maxc) nchunk = maxc;
+    if (nchunk < 1) nchunk = 1;
+    ep.chunk = (P + nchunk - 1) / nchunk;
+    dim3 grid((P + ep.chunk - 1) / ep.chunk, c->L);
+    switch (c->E) {
+        case 16: return launch_e2r_e<16>(ep, M != nullptr, grid, smem, stream);
+        case 32: return launch_e2r_e<32>(ep, M != nullptr, grid, smem, stream);
+        case 64: return launch_e2r_e<64>(ep, M != nullptr, grid, smem, stream);
+        case 128: return launch_e2r_e<128>(ep, M != nullptr, grid, smem, stream);
+        case 256: return launch_e2r_e<256>(ep, M != nullptr, grid, smem, stream);
+    }
+    return fail(GIMBAL_ERR_UNSUPPORTED, "EXPERT_TO_RANK_U8 needs E in {16,32,64,128,256}, got %d", c->E);
 }
 
 // inverse of a slot -> expert placement: one block per layer, thread e collects expert e's slots in
@@ -248,6 +280,20 @@ void gimbal_last_error(char* buf, size_t n) {
 
 int64_t gimbal_launch_count(void) { return gimbal::launches(); }
 
+int gimbal_set_option(int option, int value) {
+    if (option < 0 || option >= GIMBAL_OPT_COUNT_) return fail(GIMBAL_ERR_INVALID_ARG, "option %d", option);
+    if (option == GIMBAL_OPT_CTA_GROUP && (value < 0 || value > 2)) return fail(GIMBAL_ERR_INVALID_ARG, "GIMBAL_OPT_CTA_GROUP takes 0 (auto), 1 or 2");
+    if (option != GIMBAL_OPT_CTA_GROUP && value != 0 && value != 1) return fail(GIMBAL_ERR_INVALID_ARG, "option %d takes 0 or 1", option);
+    g_opt[option].store(value, std::memory_order_relaxed);
+    return GIMBAL_OK;
+}
+
+int gimbal_get_option(int option, int* value) {
+    if (option < 0 || option >= GIMBAL_OPT_COUNT_ || !value) return fail(GIMBAL_ERR_INVALID_ARG, "option %d", option);
+    *value = g_opt[option].load(std::memory_order_relaxed);
+    return GIMBAL_OK;
+}
+
 int gimbal_kernel_timing(int enable) { return gimbal::ktime_enable(enable); }
 
 int gimbal_kernel_elapsed_ms(int which, float* ms) { return gimbal::ktime_elapsed(which, ms); }
@@ -269,9 +315,9 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
                        int G, int slots_per_rank, gimbal_stats_state* st, const gimbal_expert_map* map, void* workspace,
                        size_t workspace_bytes, gimbal_stream_t stream_) {
     int rc = validate_router_cfg(cfg);
+    if (rc) return rc;
     if (map && (!map->rep_off || !map->rep_slots || !map->phys_ids || map->NS < cfg->E))
         return fail(GIMBAL_ERR_INVALID_ARG, "expert map needs rep_off, rep_slots, phys_ids and NS >= E");
-    if (rc) return rc;
     if (layer0 < 0 || n_layers < 1 || layer0 + n_layers > cfg->L) return fail(GIMBAL_ERR_INVALID_ARG, "layer range [%d,%d) outside [0,%d)", layer0, layer0 + n_layers, cfg->L);
     if (T < 0) return fail(GIMBAL_ERR_INVALID_ARG, "T=%d", T);
     if (!src_offsets) return fail(GIMBAL_ERR_INVALID_ARG, "src_offsets is NULL");
@@ -289,6 +335,8 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
         if (!hidden || !w_router) return fail(GIMBAL_ERR_INVALID_ARG, "hidden / w_router is NULL");
         if ((reinterpret_cast<uintptr_t>(hidden) & 15) || (reinterpret_cast<uintptr_t>(w_router) & 15))
             return fail(GIMBAL_ERR_INVALID_ARG, "hidden / w_router must be 16-byte aligned");
+        // the fused epilogue reads a token's bias row with 16-byte loads
+        if (src_logit_bias && (reinterpret_cast<uintptr_t>(src_logit_bias) & 15)) return fail(GIMBAL_ERR_INVALID_ARG, "src_logit_bias must be 16-byte aligned");
     }
     if ((cur_placement != nullptr) != (dp_of_rank != nullptr)) return fail(GIMBAL_ERR_INVALID_ARG, "cur_placement and dp_of_rank go together");
     if (cur_placement) {
@@ -349,13 +397,50 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
     return GIMBAL_OK;
 }
 
-int gimbal_route_stats_host(const gimbal_router_cfg* cfg, int T, const void* hidden_host, const int32_t* src_offsets_host,
-                            void* hidden_stage, size_t hidden_stage_bytes, int32_t* src_offsets_stage, const void* w_router,
-                            const float* select_bias, const float* src_logit_bias, const int16_t* cur_placement,
-                            const int32_t* dp_of_rank, int G, int slots_per_rank, gimbal_stats_state* st, void* result_host,
-                            void* workspace, size_t workspace_bytes, gimbal_stream_t stream_) {
+struct gimbal_host_ctx {
+    int device;
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_start;
+    cudaEvent_t ev_copied[kHostCtxSlots], ev_done[kHostCtxSlots];
+};
+
+int gimbal_host_ctx_create(gimbal_host_ctx** out) {
+    if (!out) return fail(GIMBAL_ERR_INVALID_ARG, "ctx out pointer is NULL");
+    *out = nullptr;
+    int rc = require_device();
+    if (rc) return rc;
+    gimbal_host_ctx* c = new (std::nothrow) gimbal_host_ctx();
+    if (!c) return fail(GIMBAL_ERR_CUDA, "out of host memory");
+    CUDA_TRY(cudaGetDevice(&c->device));
+    CUDA_TRY(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    CUDA_TRY(cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));
+    for (int i = 0; i < kHostCtxSlots; ++i) {
+        CUDA_TRY(cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming));
+        CUDA_TRY(cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming));
+    }
+    *out = c;
+    return GIMBAL_OK;
+}
+
+int gimbal_host_ctx_destroy(gimbal_host_ctx* c) {
+    if (!c) return GIMBAL_OK;
+    cudaStreamSynchronize(c->copy_stream);
+    for (int i = 0; i < kHostCtxSlots; ++i) { cudaEventDestroy(c->ev_copied[i]); cudaEventDestroy(c->ev_done[i]); }
+    cudaEventDestroy(c->ev_start);
+    cudaStreamDestroy(c->copy_stream);
+    delete c;
+    return GIMBAL_OK;
+}
+
+int gimbal_route_stats_host(gimbal_host_ctx* ctx, const gimbal_router_cfg* cfg, int T, const void* hidden_host,
+                            const int32_t* src_offsets_host, void* hidden_stage, size_t hidden_stage_bytes,
+                            int32_t* src_offsets_stage, const void* w_router, const float* select_bias, const float* src_logit_bias,
+                            const int16_t* cur_placement, const int32_t* dp_of_rank, int G, int slots_per_rank,
+                            gimbal_stats_state* st, void* result_host, void* workspace, size_t workspace_bytes,
+                            gimbal_stream_t stream_) {
     int rc = validate_router_cfg(cfg);
     if (rc) return rc;
+    if (!ctx) return fail(GIMBAL_ERR_INVALID_ARG, "host ctx is NULL (gimbal_host_ctx_create)");
     if (!hidden_host || !src_offsets_host || !hidden_stage || !src_offsets_stage || !result_host || !st)
         return fail(GIMBAL_ERR_INVALID_ARG, "NULL host / staging pointer");
     const size_t layer_bytes = (size_t)T * cfg->H * 2;
@@ -364,35 +449,29 @@ int gimbal_route_stats_host(const gimbal_router_cfg* cfg, int T, const void* hid
     if (slots < 2) return fail(GIMBAL_ERR_WORKSPACE, "hidden_stage must hold at least 2 layers (%zu bytes)", 2 * layer_bytes);
     rc = require_device();
     if (rc) return rc;
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != ctx->device) return fail(GIMBAL_ERR_INVALID_ARG, "host ctx belongs to device %d, current device is %d", ctx->device, dev);
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-    // a second stream carries the copies so that layer i+1 streams in while layer i computes
-    static cudaStream_t copy_stream = nullptr;
-    static cudaEvent_t ev_copied[64], ev_done[64];
-    if (!copy_stream) {
-        CUDA_TRY(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
-        for (int i = 0; i < 64; ++i) {
-            CUDA_TRY(cudaEventCreateWithFlags(&ev_copied[i], cudaEventDisableTiming));
-            CUDA_TRY(cudaEventCreateWithFlags(&ev_done[i], cudaEventDisableTiming));
-        }
-    }
-    const size_t nslot = slots > 64 ? 64 : slots;
+    // the context's second stream carries the copies so that layer i+1 streams in while layer i computes
+    cudaStream_t copy_stream = ctx->copy_stream;
+    const size_t nslot = slots > (size_t)kHostCtxSlots ? (size_t)kHostCtxSlots : slots;
     CUDA_TRY(cudaMemcpyAsync(src_offsets_stage, src_offsets_host, sizeof(int32_t) * (cfg->S + 1), cudaMemcpyHostToDevice, stream));
-    cudaEvent_t ev_start = ev_done[0];
-    CUDA_TRY(cudaEventRecord(ev_start, stream));
-    CUDA_TRY(cudaStreamWaitEvent(copy_stream, ev_start, 0));
+    CUDA_TRY(cudaEventRecord(ctx->ev_start, stream));
+    CUDA_TRY(cudaStreamWaitEvent(copy_stream, ctx->ev_start, 0));
     for (int l = 0; l < cfg->L; ++l) {
         const size_t slot = (size_t)l % nslot;
         unsigned char* dst = static_cast<unsigned char*>(hidden_stage) + slot * layer_bytes;
-        if ((size_t)l >= nslot) CUDA_TRY(cudaStreamWaitEvent(copy_stream, ev_done[slot], 0));   // slot's previous layer consumed
+        if ((size_t)l >= nslot) CUDA_TRY(cudaStreamWaitEvent(copy_stream, ctx->ev_done[slot], 0));   // slot's previous layer consumed
         CUDA_TRY(cudaMemcpyAsync(dst, static_cast<const unsigned char*>(hidden_host) + (size_t)l * layer_bytes, layer_bytes,
                                  cudaMemcpyHostToDevice, copy_stream));
-        CUDA_TRY(cudaEventRecord(ev_copied[slot], copy_stream));
-        CUDA_TRY(cudaStreamWaitEvent(stream, ev_copied[slot], 0));
+        CUDA_TRY(cudaEventRecord(ctx->ev_copied[slot], copy_stream));
+        CUDA_TRY(cudaStreamWaitEvent(stream, ctx->ev_copied[slot], 0));
         rc = gimbal_route_stats(cfg, l, 1, T, dst, w_router, select_bias, src_logit_bias, src_offsets_stage, GIMBAL_LOGITS_NONE,
                                 nullptr, nullptr, nullptr, cur_placement, dp_of_rank, G, slots_per_rank, st, nullptr, workspace,
                                 workspace_bytes, stream_);
         if (rc) return rc;
-        CUDA_TRY(cudaEventRecord(ev_done[slot], stream));
+        CUDA_TRY(cudaEventRecord(ctx->ev_done[slot], stream));
     }
     unsigned char* out = static_cast<unsigned char*>(result_host);
     const size_t nA = sizeof(int32_t) * (size_t)cfg->L * cfg->S * cfg->E, nB = 4 * (size_t)cfg->L * cfg->E, nP = sizeof(float) * cfg->S;
@@ -416,7 +495,7 @@ size_t gimbal_eval_moves_workspace_bytes(const gimbal_placement_cfg* cfg) {
     return place_ws_carve(cfg, 0, nullptr, nullptr);
 }
 
-int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const int16_t* candidates, const void* A, const void* B,
+int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const void* candidates, const void* A, const void* B,
                            const float* D, const float* M, float M_scalar, const int16_t* prev, float* out, int32_t* argmin,
                            void* workspace, size_t workspace_bytes, gimbal_stream_t stream_) {
     int rc = validate_place_cfg(cfg);
@@ -424,12 +503,17 @@ int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const int16_t
     if (P < 0) return fail(GIMBAL_ERR_INVALID_ARG, "P=%d", P);
     if (!A || !B || !D || !prev || (P > 0 && (!candidates || !out))) return fail(GIMBAL_ERR_INVALID_ARG, "NULL argument");
     if (reinterpret_cast<uintptr_t>(candidates) & 15) return fail(GIMBAL_ERR_INVALID_ARG, "candidates must be 16-byte aligned");
+    const int NS = cfg->G * cfg->slots_per_rank;
+    const bool e2r = cfg->encoding == GIMBAL_ENC_EXPERT_TO_RANK_U8;
+    if (e2r && NS != cfg->E) return fail(GIMBAL_ERR_INVALID_ARG, "EXPERT_TO_RANK_U8 needs G*slots_per_rank == E (no replicas)");
+    if (e2r && cfg->E % 4 != 0) return fail(GIMBAL_ERR_UNSUPPORTED, "EXPERT_TO_RANK_U8 needs E %% 4 == 0");
     PlaceWs w;
     const size_t need = place_ws_carve(cfg, P, workspace, &w);
     if (!workspace || workspace_bytes < need) return fail(GIMBAL_ERR_WORKSPACE, "workspace %zu < %zu bytes", workspace_bytes, need);
     const int GP = place_gp(cfg->G);
-    const size_t smem = (size_t)cfg->E * GP * (M ? 12 : 8);
+    const size_t smem = e2r ? e2r_smem_bytes(cfg->E, cfg->G, M != nullptr) : (size_t)cfg->E * GP * (M ? 12 : 8);
     if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "E=%d G=%d with an M table needs %zu B of shared memory", cfg->E, cfg->G, smem);
+    const size_t smem_chk = place_check_smem_bytes(cfg->E, cfg->G);
     rc = require_device();
     if (rc) return rc;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
@@ -440,33 +524,55 @@ int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const int16_t
     if (P > 0) {
         rc = launch_tables(cfg, A, B, D, M, M_scalar, prev, w, stream);
         if (rc) return rc;
-        ScoreParams sp{};
-        sp.P = P; sp.L = cfg->L; sp.E = cfg->E; sp.G = cfg->G; sp.sp = cfg->slots_per_rank; sp.M_scalar = M_scalar; sp.has_M = M != nullptr;
-        sp.cand = candidates; sp.t = w.t; sp.partial = w.partial;
-        // one wave: two resident blocks per SM (one when the table needs more than half the shared memory)
         const int sms = device_info().sms;
-        const int per_sm = 2 * smem + 2048 <= kSmemLimit ? 2 : 1;
-        int nchunk = per_sm * sms / cfg->L;
-        const int units_per_pass = (kScoreThreads / 32) * (cfg->G < 32 ? 32 / cfg->G : 1);
-        int max_chunks = (P + units_per_pass - 1) / units_per_pass;
-        if (nchunk > max_chunks) nchunk = max_chunks;
-        if (nchunk < 1) nchunk = 1;
-        sp.chunk = (P + nchunk - 1) / nchunk;
-        dim3 grid((P + sp.chunk - 1) / sp.chunk, cfg->L);
-        const bool dup = cfg->G * cfg->slots_per_rank > cfg->E;
-        // the five configuration shapes have specialised kernels (E must be a power of two there)
-        const bool pow2E = (cfg->E & (cfg->E - 1)) == 0;
-        const char* force = getenv("GIMBAL_SCORE_GENERIC");     // tests: run the generic kernel on a specialised shape
-        const int key = (pow2E && !(force && atoi(force))) ? cfg->slots_per_rank * 100 + cfg->G : 0;
-        switch (key) {
-            case 932: rc = launch_score_fast<9, 32>(sp, dup, grid, smem, stream); break;
-            case 816: rc = launch_score_fast<8, 16>(sp, dup, grid, smem, stream); break;
-            case 808: rc = launch_score_fast<8, 8>(sp, dup, grid, smem, stream); break;
-            case 464: rc = launch_score_fast<4, 64>(sp, dup, grid, smem, stream); break;
-            case 404: rc = launch_score_fast<4, 4>(sp, dup, grid, smem, stream); break;
-            default: rc = launch_score_generic(sp, dup, grid, smem, stream); break;
+        if (e2r) {
+            rc = launch_e2r(cfg, P, static_cast<const uint8_t*>(candidates), M, M_scalar, w.t, w.partial, smem, sms, stream);
+            if (rc) return rc;
+        } else {
+            ScoreParams sp{};
+            sp.P = P; sp.L = cfg->L; sp.E = cfg->E; sp.G = cfg->G; sp.sp = cfg->slots_per_rank; sp.M_scalar = M_scalar; sp.has_M = M != nullptr;
+            sp.cand = static_cast<const int16_t*>(candidates); sp.t = w.t; sp.partial = w.partial;
+            // one wave: two resident blocks per SM (one when the table needs more than half the shared memory)
+            const bool pow2E = (cfg->E & (cfg->E - 1)) == 0;
+            const int key = (pow2E && !g_opt[GIMBAL_OPT_SCORE_GENERIC].load(std::memory_order_relaxed)) ? cfg->slots_per_rank * 100 + cfg->G : 0;
+            const bool fast = key == 932 || key == 816 || key == 808 || key == 464 || key == 404;
+            const int per_sm = (fast && 2 * smem + 2048 <= kSmemLimit) ? 2 : 1;
+            int nchunk = per_sm * sms / cfg->L;
+            const int units_per_pass = (kScoreThreads / 32) * (cfg->G < 32 ? 32 / cfg->G : 1);
+            int max_chunks = (P + units_per_pass - 1) / units_per_pass;
+            if (nchunk > max_chunks) nchunk = max_chunks;
+            if (nchunk < 1) nchunk = 1;
+            sp.chunk = (P + nchunk - 1) / nchunk;
+            dim3 grid((P + sp.chunk - 1) / sp.chunk, cfg->L);
+            // the five configuration shapes have specialised kernels (E must be a power of two there)
+            switch (key) {
+                case 932: rc = launch_score<9, 32>(sp, grid, smem, stream); break;
+                case 816: rc = launch_score<8, 16>(sp, grid, smem, stream); break;
+                case 808: rc = launch_score<8, 8>(sp, grid, smem, stream); break;
+                case 464: rc = launch_score<4, 64>(sp, grid, smem, stream); break;
+                case 404: rc = launch_score<4, 4>(sp, grid, smem, stream); break;
+                default: rc = sp.has_M ? launch_score_generic<true>(sp, grid, smem, stream) : launch_score_generic<false>(sp, grid, smem, stream); break;
+            }
+            if (rc) return rc;
+            if (!(cfg->flags & GIMBAL_PLACE_TRUSTED)) {
+                // exact validation; overwrites the partials of invalid candidates (NaN) and of valid ones whose replica
+                // counts differ from x0's (scored with their own r)
+                CheckParams cp{};
+                cp.P = P; cp.L = cfg->L; cp.E = cfg->E; cp.G = cfg->G; cp.sp = cfg->slots_per_rank;
+                cp.sp_magic = ((1 << 20) + cfg->slots_per_rank - 1) / cfg->slots_per_rank;
+                cp.force_general = g_opt[GIMBAL_OPT_CHECK_SCORES_ALL].load(std::memory_order_relaxed);
+                cp.M_scalar = M_scalar; cp.cand = sp.cand; cp.prev = prev; cp.M = M; cp.t = w.t; cp.partial = w.partial;
+                int nck = 8 * sms / cfg->L;
+                const int maxck = (P + kCheckWarps - 1) / kCheckWarps;
+                if (nck > maxck) nck = maxck;
+                if (nck < 1) nck = 1;
+                cp.chunk = (P + nck - 1) / nck;
+                ktime_begin(GIMBAL_KERNEL_CHECK, stream);
+                place_check_kernel<<<dim3((P + cp.chunk - 1) / cp.chunk, cfg->L), kCheckWarps * 32, smem_chk, stream>>>(cp);
+                ktime_end(GIMBAL_KERNEL_CHECK, stream);
+                LAUNCH_CHECK("place_check_kernel");
+            }
         }
-        if (rc) return rc;
         FinalizeParams fp{};
         fp.P = P; fp.L = cfg->L; fp.G = cfg->G; fp.alpha = cfg->alpha; fp.beta = cfg->beta; fp.gamma = cfg->gamma;
         fp.partial = w.partial; fp.bad_prev = w.t.bad; fp.out = out; fp.best = argmin ? w.best : nullptr;
@@ -480,20 +586,22 @@ int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const int16_t
     return GIMBAL_OK;
 }
 
-int gimbal_eval_placements_host(const gimbal_placement_cfg* cfg, int P, const int16_t* candidates_host, int16_t* cand_stage,
+int gimbal_eval_placements_host(const gimbal_placement_cfg* cfg, int P, const void* candidates_host, void* cand_stage,
                                 float* out_stage, const void* A, const void* B, const float* D, const float* M, float M_scalar,
                                 const int16_t* prev, float* out_host, int32_t* argmin_host, void* workspace, size_t workspace_bytes,
                                 gimbal_stream_t stream_) {
     int rc = validate_place_cfg(cfg);
     if (rc) return rc;
+    if (P < 0) return fail(GIMBAL_ERR_INVALID_ARG, "P=%d", P);
     if (!candidates_host || !cand_stage || !out_stage || !out_host) return fail(GIMBAL_ERR_INVALID_ARG, "NULL host / staging pointer");
+    PlaceWs w;
+    const size_t need = place_ws_carve(cfg, P, workspace, &w);
+    if (!workspace || workspace_bytes < need) return fail(GIMBAL_ERR_WORKSPACE, "workspace %zu < %zu bytes", workspace_bytes, need);
     rc = require_device();
     if (rc) return rc;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-    const size_t nb = sizeof(int16_t) * (size_t)P * cfg->L * cfg->G * cfg->slots_per_rank;
-    CUDA_TRY(cudaMemcpyAsync(cand_stage, candidates_host, nb, cudaMemcpyHostToDevice, stream));
-    PlaceWs w;
-    place_ws_carve(cfg, P, workspace, &w);
+    const size_t row = cfg->encoding == GIMBAL_ENC_EXPERT_TO_RANK_U8 ? (size_t)cfg->E : sizeof(int16_t) * (size_t)cfg->G * cfg->slots_per_rank;
+    CUDA_TRY(cudaMemcpyAsync(cand_stage, candidates_host, row * (size_t)P * cfg->L, cudaMemcpyHostToDevice, stream));
     int32_t* argmin_dev = argmin_host ? reinterpret_cast<int32_t*>(w.mp.bad + 32) : nullptr;
     rc = gimbal_eval_placements(cfg, P, cand_stage, A, B, D, M, M_scalar, prev, out_stage, argmin_dev, workspace, workspace_bytes, stream_);
     if (rc) return rc;
@@ -517,6 +625,8 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
     PlaceWs w;
     const size_t need = place_ws_carve(cfg, 0, workspace, &w);
     if (!workspace || workspace_bytes < need) return fail(GIMBAL_ERR_WORKSPACE, "workspace %zu < %zu bytes", workspace_bytes, need);
+    // the whole-neighbourhood kernel stages the layer's per-slot rows in shared memory; larger shapes take the per-move kernel
+    const bool use_all = n_moves > 0 && !moves && cfg->G >= 4 && move_all_smem_bytes((int)NS, cfg->G, M != nullptr) <= kSmemLimit;
     rc = require_device();
     if (rc) return rc;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
@@ -531,7 +641,7 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
         fill_u64_kernel<<<(cfg->L + 255) / 256, 256, 0, stream>>>(w.best, ~0ull, cfg->L);
         LAUNCH_CHECK("fill_u64_kernel");
     }
-    if (n_moves > 0 && !moves && cfg->G >= 4) {
+    if (use_all) {
         // implicit neighbourhood: blocks of ~2048 pair indices of one layer, tables staged in shared memory
         MoveAllParams ap{};
         ap.L = cfg->L; ap.E = cfg->E; ap.G = cfg->G; ap.sp = cfg->slots_per_rank; ap.has_M = M != nullptr;
@@ -552,7 +662,6 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
             LAUNCH_CHECK("move_slots_kernel");
         }
         const size_t smem = move_all_smem_bytes((int)NS, cfg->G, ap.has_M);
-        if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "move neighbourhood: NS=%lld G=%d needs %zu B of shared memory", NS, cfg->G, smem);
         auto kern = ap.has_M ? move_all_kernel<true> : move_all_kernel<false>;
         CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         ktime_begin(GIMBAL_KERNEL_MOVES, stream);
@@ -574,6 +683,32 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
         best_to_index_kernel<<<(cfg->L + 255) / 256, 256, 0, stream>>>(w.best, best_per_layer, cfg->L);
         LAUNCH_CHECK("best_to_index_kernel");
     }
+    return GIMBAL_OK;
+}
+
+int gimbal_eval_moves_host(const gimbal_placement_cfg* cfg, const int16_t* cur_host, const int16_t* prev_host, int16_t* cur_stage,
+                           int16_t* prev_stage, int64_t n_moves, const int32_t* moves_host, int32_t* moves_stage, const void* A,
+                           const void* B, const float* D, const float* M, float M_scalar, float* delta_stage, float* delta_host,
+                           int32_t* best_stage, int32_t* best_host, void* workspace, size_t workspace_bytes, gimbal_stream_t stream_) {
+    int rc = validate_place_cfg(cfg);
+    if (rc) return rc;
+    if (n_moves < 0) return fail(GIMBAL_ERR_INVALID_ARG, "n_moves < 0");
+    if (!cur_host || !prev_host || !cur_stage || !prev_stage || (n_moves > 0 && !delta_stage) || (moves_host && !moves_stage) ||
+        (best_host && !best_stage))
+        return fail(GIMBAL_ERR_INVALID_ARG, "NULL host / staging pointer");
+    rc = require_device();
+    if (rc) return rc;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const size_t nb = sizeof(int16_t) * (size_t)cfg->L * cfg->G * cfg->slots_per_rank;
+    CUDA_TRY(cudaMemcpyAsync(cur_stage, cur_host, nb, cudaMemcpyHostToDevice, stream));
+    CUDA_TRY(cudaMemcpyAsync(prev_stage, prev_host, nb, cudaMemcpyHostToDevice, stream));
+    if (moves_host && n_moves > 0) CUDA_TRY(cudaMemcpyAsync(moves_stage, moves_host, sizeof(int32_t) * 3 * (size_t)n_moves, cudaMemcpyHostToDevice, stream));
+    rc = gimbal_eval_moves(cfg, cur_stage, prev_stage, n_moves, moves_host ? moves_stage : nullptr, A, B, D, M, M_scalar, delta_stage,
+                           best_host ? best_stage : nullptr, workspace, workspace_bytes, stream_);
+    if (rc) return rc;
+    if (delta_host && n_moves > 0) CUDA_TRY(cudaMemcpyAsync(delta_host, delta_stage, sizeof(float) * 5 * (size_t)n_moves, cudaMemcpyDeviceToHost, stream));
+    if (best_host) CUDA_TRY(cudaMemcpyAsync(best_host, best_stage, sizeof(int32_t) * cfg->L, cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaStreamSynchronize(stream));
     return GIMBAL_OK;
 }
 

@@ -23,11 +23,12 @@ int fail(int code, const char* fmt, ...) {
 void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 
 static bool g_ktime_on = false;
-static cudaEvent_t g_kev[5][2];
-static bool g_kev_made = false, g_kev_rec[5] = {false, false, false, false, false};
+constexpr int kTimedKernels = 8;
+static cudaEvent_t g_kev[kTimedKernels][2];
+static bool g_kev_made = false, g_kev_rec[kTimedKernels] = {};
 int ktime_enable(int on) {
     if (on && !g_kev_made) {
-        for (int i = 0; i < 5; ++i)
+        for (int i = 0; i < kTimedKernels; ++i)
             for (int j = 0; j < 2; ++j)
                 if (cudaEventCreate(&g_kev[i][j]) != cudaSuccess) return fail(GIMBAL_ERR_CUDA, "cudaEventCreate failed");
         g_kev_made = true;
@@ -38,7 +39,7 @@ int ktime_enable(int on) {
 void ktime_begin(int which, cudaStream_t s) { if (g_ktime_on) cudaEventRecord(g_kev[which][0], s); }
 void ktime_end(int which, cudaStream_t s) { if (g_ktime_on) { cudaEventRecord(g_kev[which][1], s); g_kev_rec[which] = true; } }
 int ktime_elapsed(int which, float* ms) {
-    if (which < 0 || which > 4 || !ms) return fail(GIMBAL_ERR_INVALID_ARG, "kernel id %d", which);
+    if (which < 0 || which >= kTimedKernels || !ms) return fail(GIMBAL_ERR_INVALID_ARG, "kernel id %d", which);
     if (!g_kev_made || !g_kev_rec[which]) return fail(GIMBAL_ERR_INVALID_ARG, "kernel %d was not timed", which);
     if (cudaEventSynchronize(g_kev[which][1]) != cudaSuccess) return fail(GIMBAL_ERR_CUDA, "cudaEventSynchronize failed");
     if (cudaEventElapsedTime(ms, g_kev[which][0], g_kev[which][1]) != cudaSuccess) return fail(GIMBAL_ERR_CUDA, "cudaEventElapsedTime failed");

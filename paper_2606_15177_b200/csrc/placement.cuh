@@ -1,22 +1,30 @@
 // a6 + a7: batched placement objective and single-move deltas (section 5.2).
 //
-// The objective is linear in the slots of a candidate except for C_load, so every (layer)
-// gets a small table indexed [expert][rank] that holds what one slot contributes:
+// The objective is linear in the slots of a candidate except for C_load, so every layer gets a
+// small table indexed [expert][rank] that holds what one slot contributes:
 //     w  = B[l,e] / r[l,e]                                   (rank load share,   PAPER.md:236)
 //     c  = sum_s A[l,s,e] D[s,g] / r[l,e]                    (communication,     PAPER.md:244)
 //     m  = M[l,e,g]                                          (migration,         PAPER.md:248)
 // with the sign bit of c carrying "x0 already hosts e on g" (c >= 0 because A, D >= 0).
-// C_mig = sum |x - x0| M = (M over the candidate's cells that x0 lacks) + (M over x0's cells -
-// M over the cells both have) for binary x; exact for a scalar M, and with an M table the
-// rounding is relative to sum of M over x0's cells.  r[l,e] is taken from x0: candidates place the
-// same expert copies as x0 (R12); a candidate with another multiset of experts,
-// an id out of range or an expert twice on one rank gets NaN.
 //
-// Scoring kernel: one block per (candidate chunk, layer); the layer's table sits in shared
-// memory laid out [E][32] so that lane g only ever touches bank g (conflict-free gathers);
-// lane <-> rank, so a rank's load is a lane-local sum and only the per-candidate reductions
-// use shuffles.  Per-(candidate, layer) partials go to the workspace and a small finalize
-// kernel reduces them over layers in fixed order.
+// Three kernels share the work (K4):
+//   place_score_kernel   the throughput kernel.  It assumes what place_check_kernel proves: the
+//                        candidate is valid and hosts as many copies of every expert as x0 (so the
+//                        tables' r = r0 is the candidate's r).  One block per (candidate chunk,
+//                        layer); the layer's table sits in shared memory laid out [E][32] so that
+//                        lane g only ever touches bank g (conflict-free gathers); lane <-> rank, so
+//                        a rank's load is a lane-local sum and only the per-candidate reductions
+//                        use shuffles.  Five instructions per slot with a scalar M.
+//   place_check_kernel   exact validation (R12): a warp builds the candidate's binary
+//                        x[e,g] as per-expert rank masks in shared memory (one atomicOr per slot:
+//                        the returned word tells "twice on one rank", its popcount is r[l,e]).
+//                        Invalid -> NaN; valid with other replica counts than x0 -> scored right here
+//                        with the candidate's own r (the plain definition, from global memory);
+//                        valid with x0's counts -> left to place_score_kernel.
+//   place_finalize_kernel reduces the per-(candidate, layer) partials over layers in fixed order.
+// C_mig = sum M |x - x0| is accumulated directly from the cells that enter (candidate slot on a cell
+// x0 lacks) and the cells that leave (x0 slot whose cell the candidate lacks): no subtraction of
+// nearly equal sums, so a candidate equal to x0 gives exactly 0.
 #pragma once
 #include <cuda_runtime.h>
 #include <math_constants.h>
@@ -28,11 +36,14 @@ constexpr int kMaxE = 256;
 constexpr int kMaxG = 64;
 
 struct PlaceTables {
-    float2* wc;        // [L][E][GP]  {w, c with sign bit = member of x0}
-    float* m;          // [L][E][GP]  M[l,e,g] (only when an M table is given)
+    float2* wc;        // [L][GP/32][E][32]  {w, c with sign bit = member of x0}
+    float* m;          // [L][GP/32][E][32]  M[l,e,g]                                   (M table only)
+    uint32_t* mu;      // [L][GP/32][E][32]  scoring word: float bits of M where x0 lacks the cell, else
+                       //                    0x80000000 | 1 << (position of e among x0's slots of rank g)   (M table only)
+    float* mx0;        // [L][NS]     M of x0's own cell of every slot                  (M table only)
+    float* c_raw;      // [L][E][G]   sum_s A D, not divided by r   (place_check_kernel's own scoring)
+    double* b_raw;     // [L][E]      B as double                   (same)
     double* w_e;       // [L][E]      w in double (move deltas subtract nearly equal loads)
-    uint32_t* hsum;    // [L]         multiset hash of x0's slot contents
-    float* base_mig;   // [L]         sum over x0's cells of M
     double* sumB;      // [L]         sum_e B[l,e]
     int32_t* r;        // [L][E]      replica count in x0
     uint64_t* pmask;   // [L][E]      bit g set: x0 hosts e on rank g
@@ -40,12 +51,8 @@ struct PlaceTables {
 };
 
 __host__ __device__ inline int place_gp(int G) { return G < 32 ? 32 : G; }
-
-// multiset checksum term of one slot: two integer multiply-adds in the scoring loop; injective on [0, 256)
-__device__ __forceinline__ uint32_t slot_hash(uint32_t e) {
-    const uint32_t t = e * 0x9E3779B1u + 0x7F4A7C15u;
-    return t * t;
-}
+// cell (expert e, table column gp) of a layer's [GP/32][E][32] table; column gp serves rank gp % G
+__host__ __device__ inline size_t tab_idx(int E, int e, int gp) { return ((size_t)(gp >> 5) * E + e) * 32 + (gp & 31); }
 
 struct TableParams {
     int L, E, G, sp, S, counts_f32;
@@ -70,50 +77,54 @@ __device__ __forceinline__ double block_sum_256(double v, double* red) {
 constexpr int kTableSplit = 4;      // blocks per layer (the [E][G'] cells are split between them)
 
 // grid (L, kTableSplit), 256 threads.  Every block rebuilds the layer's replica counts / rank
-// masks of x0 (cheap); block y = 0 also writes the per-layer scalars.
+// masks of x0 (cheap); block y = 0 also writes the per-layer scalars and the per-slot entries.
 __global__ void __launch_bounds__(256) place_tables_kernel(const TableParams p) {
     __shared__ int r_s[kMaxE];
     __shared__ unsigned long long pm_s[kMaxE];
     __shared__ float D_s[64 * 64];
     __shared__ double red_s[256];
     __shared__ int bad_s;
-    __shared__ unsigned int hs_s;
     const int l = blockIdx.x, tid = threadIdx.x;
     const int NS = p.G * p.sp, GP = place_gp(p.G);
     const int16_t* pv = p.prev + (size_t)l * NS;
-    if (tid == 0) { bad_s = 0; hs_s = 0; }
+    if (tid == 0) bad_s = 0;
     for (int e = tid; e < p.E; e += 256) { r_s[e] = 0; pm_s[e] = 0ull; }
     for (int i = tid; i < p.S * p.G; i += 256) D_s[i] = p.D[i];
     __syncthreads();
-    double bm = 0.0;
     for (int j = tid; j < NS; j += 256) {
         const int e = pv[j], g = j / p.sp;
         if (e < 0 || e >= p.E) { bad_s = 1; continue; }
         atomicAdd(&r_s[e], 1);
         const unsigned long long old = atomicOr(&pm_s[e], 1ull << g);
         if ((old >> g) & 1ull) bad_s = 1;                         // twice on one rank
-        atomicAdd(&hs_s, slot_hash((uint32_t)e));
-        bm += p.M ? (double)p.M[((size_t)l * p.E + e) * p.G + g] : (double)p.M_scalar;
     }
     __syncthreads();
+    const size_t tab = (size_t)l * (GP / 32) * p.E * 32;
     if (blockIdx.y == 0) {
-        const double bm_tot = block_sum_256(bm, red_s);
         double sb = 0.0;
         for (int e = tid; e < p.E; e += 256) {
             if (r_s[e] < 1) bad_s = 1;
             const double b = p.counts_f32 ? (double)reinterpret_cast<const float*>(p.B)[(size_t)l * p.E + e]
                                           : (double)reinterpret_cast<const int32_t*>(p.B)[(size_t)l * p.E + e];
             sb += b;
+            p.t.b_raw[(size_t)l * p.E + e] = b;
             p.t.w_e[(size_t)l * p.E + e] = b / (double)max(r_s[e], 1);
             p.t.r[(size_t)l * p.E + e] = r_s[e];
             p.t.pmask[(size_t)l * p.E + e] = pm_s[e];
         }
         const double sb_tot = block_sum_256(sb, red_s);
         if (tid == 0) {
-            p.t.hsum[l] = hs_s;
-            p.t.base_mig[l] = (float)bm_tot;
             p.t.sumB[l] = sb_tot;
             if (bad_s) atomicOr(p.t.bad, 1);
+        }
+        if (p.M) {
+            // x0's own cells: the scoring word names the slot's position inside its rank, mx0 holds its M
+            for (int j = tid; j < NS; j += 256) {
+                const int e = pv[j], g = j / p.sp;
+                if (e < 0 || e >= p.E) { p.t.mx0[(size_t)l * NS + j] = 0.0f; continue; }
+                p.t.mx0[(size_t)l * NS + j] = p.M[((size_t)l * p.E + e) * p.G + g];
+                for (int gp = g; gp < GP; gp += p.G) p.t.mu[tab + tab_idx(p.E, e, gp)] = 0x80000000u | (1u << (j - g * p.sp));
+            }
         }
     }
     // table entries; column gp of the table serves rank gp % G (replicated when G < 32)
@@ -127,6 +138,7 @@ __global__ void __launch_bounds__(256) place_tables_kernel(const TableParams p) 
                                          : (float)reinterpret_cast<const int32_t*>(p.A)[((size_t)l * p.S + s) * p.E + e];
             c = __fmaf_rn(a, D_s[s * p.G + g], c);
         }
+        if (gp < p.G) p.t.c_raw[((size_t)l * p.E + e) * p.G + g] = fabsf(c);
         const int re = max(r_s[e], 1);
         const float inv = 1.0f / (float)re;
         c = fabsf(c * inv);
@@ -134,8 +146,13 @@ __global__ void __launch_bounds__(256) place_tables_kernel(const TableParams p) 
         const double b = p.counts_f32 ? (double)reinterpret_cast<const float*>(p.B)[(size_t)l * p.E + e]
                                       : (double)reinterpret_cast<const int32_t*>(p.B)[(size_t)l * p.E + e];
         const float w = (float)(b / (double)re);
-        p.t.wc[((size_t)l * p.E + e) * GP + gp] = make_float2(w, member ? -c : c);   // -0.0f keeps the flag when c == 0
-        if (p.M) p.t.m[((size_t)l * p.E + e) * GP + gp] = p.M[((size_t)l * p.E + e) * p.G + g];
+        const size_t at = tab + tab_idx(p.E, e, gp);
+        p.t.wc[at] = make_float2(w, member ? -c : c);   // -0.0f keeps the flag when c == 0
+        if (p.M) {
+            const float mm = p.M[((size_t)l * p.E + e) * p.G + g];
+            p.t.m[at] = mm;
+            if (!member) p.t.mu[at] = __float_as_uint(fabsf(mm));
+        }
     }
 }
 
@@ -151,187 +168,49 @@ struct ScoreParams {
 
 constexpr int kScoreThreads = 512;
 
-// The slots of one rank as 16-bit ids packed two per word, SP = slots per rank (0: runtime sp,
-// scalar loads).  `row` points at the first slot of the candidate's layer row, g is the rank.
-template <int SP>
-struct RankSlots {
-    static constexpr int NW = SP == 0 ? 8 : (SP + 1) / 2;   // words fetched
-    uint32_t w[NW];
-    __device__ __forceinline__ void load(const int16_t* row, int g, int sp) {
-        if constexpr (SP == 8) {
-            const uint4 q = __ldcs(reinterpret_cast<const uint4*>(row + g * 8));
-            w[0] = q.x; w[1] = q.y; w[2] = q.z; w[3] = q.w;
-        } else if constexpr (SP == 4) {
-            const uint2 q = __ldcs(reinterpret_cast<const uint2*>(row + g * 4));
-            w[0] = q.x; w[1] = q.y;
-        } else if constexpr (SP == 0) {
+// reduce (sq, comm) over the SEG lanes of a unit with a transposed butterfly (the first step folds
+// both values into one register); returns comm's total, leaves sq's total in `sq` on the unit's lanes
+// with bit SEG/2 clear
+template <int SEG>
+__device__ __forceinline__ float reduce_pair(float& sq, float comm, int lane, int sub) {
+    if constexpr (SEG > 1) {
+        constexpr int h = SEG >> 1;
+        const bool up = (lane & h) != 0;
+        float v = (up ? comm : sq) + __shfl_xor_sync(0xffffffffu, up ? sq : comm, h);
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const uint32_t lo = 2 * j < sp ? (uint16_t)__ldcs(row + g * sp + 2 * j) : 0xffffu;
-                const uint32_t hi = 2 * j + 1 < sp ? (uint16_t)__ldcs(row + g * sp + 2 * j + 1) : 0xffffu;
-                w[j] = lo | (hi << 16);
-            }
-        } else {
-            // odd SP: the rank's slots start on a word boundary for even g and in the middle of a
-            // word for odd g; fetch the NW aligned words that cover them (rows are 4-byte aligned
-            // because NS * 2 is)
-            const uint32_t* base = reinterpret_cast<const uint32_t*>(row) + ((g * SP) >> 1);
-#pragma unroll
-            for (int j = 0; j < NW; ++j) w[j] = __ldcs(base + j);
-        }
-    }
-    // id of slot j of the rank (g only matters for odd SP)
-    __device__ __forceinline__ uint32_t id(int j, int g) const {
-        if constexpr (SP == 0 || SP % 2 == 0) {
-            return (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu);
-        } else {
-            // odd g: slot j sits at half-word j + 1 of the fetched words
-            const uint32_t even = (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu);
-            const uint32_t odd = ((j + 1) & 1) ? (w[(j + 1) >> 1] >> 16) : (w[(j + 1) >> 1] & 0xffffu);
-            return (g & 1) ? odd : even;
-        }
-    }
-};
-
-// SP: compile-time slots per rank (0 = generic, runtime p.sp <= 16); kDup: NS > E, so a rank can
-// hold the same expert twice and the per-rank duplicate check is needed; kHasM: M table.
-template <int SP, bool kDup, bool kHasM>
-__global__ void __launch_bounds__(kScoreThreads, SP == 0 ? 1 : 2) place_score_kernel(const ScoreParams p) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int GP = place_gp(p.G);
-    float2* wc_s = reinterpret_cast<float2*>(smem_raw);                       // [E][GP]
-    float* m_s = reinterpret_cast<float*>(smem_raw + sizeof(float2) * (size_t)p.E * GP);   // [E][GP] (kHasM)
-    const int l = blockIdx.y;
-    const int NS = p.G * p.sp;
-    const int sp = SP > 0 ? SP : p.sp;
-    {
-        const uint4* src = reinterpret_cast<const uint4*>(p.t.wc + (size_t)l * p.E * GP);
-        uint4* dst = reinterpret_cast<uint4*>(wc_s);
-        for (int i = threadIdx.x; i < p.E * GP / 2; i += kScoreThreads) dst[i] = src[i];
-        if constexpr (kHasM) {
-            const uint4* ms = reinterpret_cast<const uint4*>(p.t.m + (size_t)l * p.E * GP);
-            uint4* md = reinterpret_cast<uint4*>(m_s);
-            for (int i = threadIdx.x; i < p.E * GP / 4; i += kScoreThreads) md[i] = ms[i];
-        }
-    }
-    __syncthreads();
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int seg = p.G < 32 ? p.G : 32;                // lanes of one (candidate, layer) unit
-    const int upw = 32 / seg;                           // units per warp
-    const int rpl = p.G > 32 ? p.G / 32 : 1;            // ranks per lane
-    const int sub = lane / seg;
-    const int g0 = lane % seg;
-    const uint32_t seg_mask = seg == 32 ? 0xffffffffu : (((1u << seg) - 1u) << (sub * seg));
-    const double Gd = (double)p.G;
-    const double sumB = p.t.sumB[l];
-    const uint32_t want_hash = p.t.hsum[l];
-    const float base_mig = p.t.base_mig[l];
-    const uint32_t emax = (uint32_t)p.E - 1u;
-    const int col = p.G < 32 ? lane : g0;               // table column of this lane (rank g0 + 32*rr -> col + 32*rr)
-
-    const int p_begin = blockIdx.x * p.chunk, p_end = min(p.P, p_begin + p.chunk);
-    const int stride = (kScoreThreads / 32) * upw;
-    RankSlots<SP> cur, nxt;
-    int pc = p_begin + warp * upw;
-    if (pc + sub < p_end && rpl == 1) cur.load(p.cand + ((size_t)(pc + sub) * p.L + l) * NS, g0, sp);
-    for (; pc < p_end; pc += stride) {
-        const int cand = pc + sub;
-        const bool active = cand < p_end;
-        if (rpl == 1 && cand + stride < p_end) nxt.load(p.cand + ((size_t)(cand + stride) * p.L + l) * NS, g0, sp);
-        float sq = 0.0f, comm = 0.0f, mig_in = 0.0f, mig_kept = 0.0f, mx = 0.0f;
-        uint32_t hs = 0, orall = 0, kept = 0;
-        bool dup = false;
-        if (active) {
-            for (int rr = 0; rr < rpl; ++rr) {
-                const int g = g0 + rr * 32;
-                if (rpl > 1) cur.load(p.cand + ((size_t)cand * p.L + l) * NS, g, sp);
-                uint32_t e[SP == 0 ? 16 : SP];
-                float lg = 0.0f;
-#pragma unroll
-                for (int j = 0; j < (SP == 0 ? 16 : SP); ++j) {
-                    if (SP != 0 || j < sp) {
-                        const uint32_t raw = cur.id(j, g);
-                        orall |= raw > emax ? 1u : 0u;
-                        const uint32_t x = min(raw, emax);
-                        e[j] = x;
-                        hs += slot_hash(x);
-                        const int idx = x * GP + col + rr * 32;
-                        const float2 wc = wc_s[idx];
-                        lg += wc.x;
-                        comm += fabsf(wc.y);
-                        const uint32_t member = __float_as_uint(wc.y) >> 31;
-                        kept += member;
-                        if constexpr (kHasM) {
-                            const float mm = m_s[idx];
-                            if (member) mig_kept += mm; else mig_in += mm;     // retained / entering cell of x0
-                        }
-                    } else e[j] = 0xffff0000u + j;
-                }
-                if constexpr (kDup) {
-#pragma unroll
-                    for (int a = 0; a < (SP == 0 ? 16 : SP); ++a)
-#pragma unroll
-                        for (int b = a + 1; b < (SP == 0 ? 16 : SP); ++b) dup |= (e[a] == e[b]);
-                }
-                const float d = (float)((double)lg * Gd - sumB);  // G*L_g - sum_g L_g, exact difference for integer counts
-                sq = __fmaf_rn(d, d, sq);
-                mx = fmaxf(mx, lg);
-            }
-        }
-        // reduce over the `seg` lanes of this unit: integers with redux, the two float sums with a
-        // transposed butterfly (first step folds both values into one register)
-        hs = __reduce_add_sync(seg_mask, hs);
-        kept = __reduce_add_sync(seg_mask, kept);
-        const uint32_t bad = __reduce_or_sync(seg_mask, orall | (dup ? 1u : 0u));
-        const float mxa = __uint_as_float(__reduce_max_sync(seg_mask, __float_as_uint(mx)));   // loads are >= 0
-        float commt = comm;
-        if (seg > 1) {
-            const int h = seg >> 1;
-            const bool up = (lane & h) != 0;
-            float v = (up ? comm : sq) + __shfl_xor_sync(0xffffffffu, up ? sq : comm, h);
-            for (int o = h >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-            commt = __shfl_sync(0xffffffffu, v, sub * seg + h);
-            sq = v;                                                                  // valid on unit lanes with bit h clear
-        }
-        if constexpr (kHasM) {
-            for (int o = seg >> 1; o > 0; o >>= 1) {
-                mig_in += __shfl_xor_sync(0xffffffffu, mig_in, o);
-                mig_kept += __shfl_xor_sync(0xffffffffu, mig_kept, o);
-            }
-        }
-        if (active && g0 == 0) {
-            // C_mig = entering cells + (x0's cells - retained cells); exact for a scalar M
-            const float mig = kHasM ? mig_in + (base_mig - mig_kept) : p.M_scalar * (float)(2 * (NS - (int)kept));
-            float4 out = make_float4(sq, commt, mig, mxa);
-            if (bad || hs != want_hash) out.x = CUDART_NAN_F;
-            p.partial[(size_t)cand * p.L + l] = out;
-        }
-        if (rpl == 1) cur = nxt;
+        for (int o = h >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        const float commt = __shfl_sync(0xffffffffu, v, sub * SEG + h);
+        sq = v;
+        return commt;
+    } else {
+        return comm;
     }
 }
 
-// Specialised scoring kernel for compile-time (slots per rank, ranks) and a power-of-two E:
-// ids are fetched as aligned 32-bit words (two per word), the range check is one OR per word,
-// the cross-lane reductions are fully unrolled.  Same results, bit for bit, as the generic kernel.
-template <int SP, int G, bool kDup, bool kHasM>
-__global__ void __launch_bounds__(kScoreThreads, 2) place_score_fast_kernel(const ScoreParams p) {
-    constexpr int GP = G < 32 ? 32 : G;
-    constexpr int SEG = G < 32 ? G : 32, UPW = 32 / SEG, RPL = G > 32 ? G / 32 : 1;
+// Throughput kernel for compile-time (slots per rank, ranks) and a power-of-two E <= 256.  Slot ids
+// arrive as aligned 32-bit words (two per word; ranks with an odd slot count are realigned with a
+// funnel shift); one PRMT turns an id into the byte offset of its table cell ((id & 255) << 8 | lane * 8),
+// one 8-byte shared load fetches {w, c}, two adds and one shift-add (x0 membership) finish the slot.
+// Ids are masked to the table, so a row that place_check_kernel would reject cannot fault here.
+template <int SP, int G, bool kHasM>
+__global__ void __launch_bounds__(kScoreThreads, 2) place_score_kernel(const ScoreParams p) {
+    constexpr int H = G > 32 ? G / 32 : 1;              // table halves == ranks per lane
+    constexpr int SEG = G < 32 ? G : 32, UPW = 32 / SEG;
     constexpr int NS = G * SP;
     constexpr int NW = (SP + 1) / 2;                    // words holding one rank's ids
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2* wc_s = reinterpret_cast<float2*>(smem_raw);                       // [E][GP]
-    float* m_s = reinterpret_cast<float*>(smem_raw + sizeof(float2) * (size_t)p.E * GP);   // [E][GP] (kHasM)
+    const int E = p.E;
+    const unsigned char* wc_b = smem_raw;                               // [H][E][32] float2
+    const unsigned char* mu_b = smem_raw + (size_t)H * E * 256;         // [H][E][32] u32 (kHasM)
     const int l = blockIdx.y;
     {
-        const uint4* src = reinterpret_cast<const uint4*>(p.t.wc + (size_t)l * p.E * GP);
-        uint4* dst = reinterpret_cast<uint4*>(wc_s);
-        for (int i = threadIdx.x; i < p.E * GP / 2; i += kScoreThreads) dst[i] = src[i];
+        const uint4* src = reinterpret_cast<const uint4*>(p.t.wc + (size_t)l * H * E * 32);
+        uint4* dst = reinterpret_cast<uint4*>(smem_raw);
+        for (int i = threadIdx.x; i < H * E * 16; i += kScoreThreads) dst[i] = src[i];
         if constexpr (kHasM) {
-            const uint4* ms = reinterpret_cast<const uint4*>(p.t.m + (size_t)l * p.E * GP);
-            uint4* md = reinterpret_cast<uint4*>(m_s);
-            for (int i = threadIdx.x; i < p.E * GP / 4; i += kScoreThreads) md[i] = ms[i];
+            const uint4* ms = reinterpret_cast<const uint4*>(p.t.mu + (size_t)l * H * E * 32);
+            uint4* md = reinterpret_cast<uint4*>(smem_raw + (size_t)H * E * 256);
+            for (int i = threadIdx.x; i < H * E * 8; i += kScoreThreads) md[i] = ms[i];
         }
     }
     __syncthreads();
@@ -341,21 +220,26 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_fast_kernel(cons
     const uint32_t seg_mask = SEG == 32 ? 0xffffffffu : (((1u << SEG) - 1u) << (sub * SEG));
     const double Gd = (double)G;
     const double sumB = p.t.sumB[l];
-    const uint32_t want_hash = p.t.hsum[l];
-    const float base_mig = p.t.base_mig[l];
-    const uint32_t emask = (uint32_t)p.E - 1u;
-    const uint32_t okbits = emask | (emask << 16);
-    const int col = G < 32 ? lane : g0;                 // table column of rank g0 (+32 for the lane's second rank)
+    const uint32_t emask = (uint32_t)E - 1u;
+    const uint32_t emask2 = emask | (emask << 16);
+    const uint32_t lane8 = (uint32_t)lane * 8u;         // table column of this lane's rank (replicated columns when G < 32)
+    float mx0[kHasM ? H : 1][kHasM ? SP : 1];           // M of x0's own cells on this lane's rank(s)
+    if constexpr (kHasM) {
+#pragma unroll
+        for (int rr = 0; rr < H; ++rr)
+#pragma unroll
+            for (int j = 0; j < SP; ++j) mx0[rr][j] = p.t.mx0[(size_t)l * NS + (g0 + rr * 32) * SP + j];
+    }
 
     const int p_begin = blockIdx.x * p.chunk, p_end = min(p.P, p_begin + p.chunk);
     constexpr int kStride = (kScoreThreads / 32) * UPW;
     const size_t step_words = (size_t)kStride * p.L * NS / 2;
     int cand = p_begin + warp * UPW + sub;
     const uint32_t* rowp = reinterpret_cast<const uint32_t*>(p.cand + ((size_t)cand * p.L + l) * NS);
-    uint32_t cur[RPL][NW], nxt[RPL][NW];
-    auto fetch = [&](const uint32_t* row, uint32_t (&w)[RPL][NW]) {
+    uint32_t cur[H][NW], nxt[H][NW];
+    auto fetch = [&](const uint32_t* row, uint32_t (&w)[H][NW]) {
 #pragma unroll
-        for (int rr = 0; rr < RPL; ++rr) {
+        for (int rr = 0; rr < H; ++rr) {
             const int g = g0 + rr * 32;
             if constexpr (SP % 8 == 0) {
 #pragma unroll
@@ -380,12 +264,11 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_fast_kernel(cons
         const bool active = cand < p_end;
         rowp += step_words;
         if (cand + kStride < p_end) fetch(rowp, nxt);
-        float sq = 0.0f, comm = 0.0f, mig_in = 0.0f, mig_kept = 0.0f, mx = 0.0f;
-        uint32_t hs = 0, orall = 0, kept = 0;
-        bool dup = false;
+        float sq = 0.0f, comm = 0.0f, mig = 0.0f, mx = 0.0f;
+        uint32_t kept = 0;
         if (active) {
 #pragma unroll
-            for (int rr = 0; rr < RPL; ++rr) {
+            for (int rr = 0; rr < H; ++rr) {
                 uint32_t w[NW];
 #pragma unroll
                 for (int j = 0; j < NW; ++j) w[j] = cur[rr][j];
@@ -394,73 +277,220 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_fast_kernel(cons
                     const uint32_t sh = ((g0 + rr * 32) & 1) * 16;
 #pragma unroll
                     for (int j = 0; j + 1 < NW; ++j) w[j] = __funnelshift_r(w[j], w[j + 1], sh);
-                    w[NW - 1] = (w[NW - 1] >> sh) & 0xffffu;
+                    w[NW - 1] = w[NW - 1] >> sh;
                 }
-                uint32_t e[SP];
-                float lg = 0.0f;
 #pragma unroll
-                for (int j = 0; j < NW; ++j) orall |= w[j];
+                for (int j = 0; j < NW; ++j) w[j] &= emask2;        // keeps every id inside the staged table
+                float lg = 0.0f;
+                uint32_t kbits = 0;
 #pragma unroll
                 for (int j = 0; j < SP; ++j) {
-                    const uint32_t x = ((j & 1) ? (w[j >> 1] >> 16) : w[j >> 1]) & emask;
-                    e[j] = x;
-                    hs += slot_hash(x);
-                    const int idx = x * GP + col + rr * 32;
-                    const float2 wc = wc_s[idx];
+                    const uint32_t off = __byte_perm(w[j >> 1], lane8, (j & 1) ? 0x5524 : 0x5504);   // id << 8 | lane * 8
+                    const float2 wc = *reinterpret_cast<const float2*>(wc_b + rr * E * 256 + off);
                     lg += wc.x;
                     comm += fabsf(wc.y);
-                    const uint32_t member = __float_as_uint(wc.y) >> 31;
-                    kept += member;
                     if constexpr (kHasM) {
-                        const float mm = m_s[idx];
-                        if (member) mig_kept += mm; else mig_in += mm;     // retained / entering cell of x0
+                        const uint32_t u = *reinterpret_cast<const uint32_t*>(mu_b + rr * E * 128 + (off >> 1));
+                        mig += fmaxf(__uint_as_float(u), 0.0f);                         // entering cell: + M
+                        kbits |= (uint32_t)((int32_t)u >> 31) & u;                      // retained cell: which of x0's slots
+                    } else {
+                        kept += __float_as_uint(wc.y) >> 31;
                     }
                 }
-                if constexpr (kDup) {
+                if constexpr (kHasM) {
 #pragma unroll
-                    for (int a = 0; a < SP; ++a)
-#pragma unroll
-                        for (int b = a + 1; b < SP; ++b) dup |= (e[a] == e[b]);
+                    for (int j = 0; j < SP; ++j) mig += ((kbits >> j) & 1u) ? 0.0f : mx0[rr][j];   // leaving cells, x0's slot order
                 }
                 const float d = (float)((double)lg * Gd - sumB);  // G*L_g - sum_g L_g, exact difference for integer counts
                 sq = __fmaf_rn(d, d, sq);
                 mx = fmaxf(mx, lg);
             }
         }
-        const uint32_t flags = ((orall & ~okbits) ? 1u : 0u) | (dup ? 1u : 0u);
-        hs = __reduce_add_sync(seg_mask, hs);
-        kept = __reduce_add_sync(seg_mask, kept);
-        const uint32_t bad = __reduce_or_sync(seg_mask, flags);
         const float mxa = __uint_as_float(__reduce_max_sync(seg_mask, __float_as_uint(mx)));   // loads are >= 0
-        float commt = comm;
-        if constexpr (SEG > 1) {
-            constexpr int h = SEG >> 1;
-            const bool up = (lane & h) != 0;
-            float v = (up ? comm : sq) + __shfl_xor_sync(0xffffffffu, up ? sq : comm, h);
-#pragma unroll
-            for (int o = h >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-            commt = __shfl_sync(0xffffffffu, v, sub * SEG + h);
-            sq = v;                                                                  // valid on unit lanes with bit h clear
-        }
+        const float commt = reduce_pair<SEG>(sq, comm, lane, sub);
         if constexpr (kHasM) {
 #pragma unroll
-            for (int o = SEG >> 1; o > 0; o >>= 1) {
-                mig_in += __shfl_xor_sync(0xffffffffu, mig_in, o);
-                mig_kept += __shfl_xor_sync(0xffffffffu, mig_kept, o);
-            }
+            for (int o = SEG >> 1; o > 0; o >>= 1) mig += __shfl_xor_sync(0xffffffffu, mig, o);
+        } else {
+            kept = __reduce_add_sync(seg_mask, kept);
+            mig = p.M_scalar * (float)(2 * (NS - (int)kept));       // entering + leaving cells, M each: exact
         }
-        if (active && g0 == 0) {
-            const float mig = kHasM ? mig_in + (base_mig - mig_kept) : p.M_scalar * (float)(2 * (NS - (int)kept));
-            float4 out = make_float4(sq, commt, mig, mxa);
-            if (bad || hs != want_hash) out.x = CUDART_NAN_F;
-            p.partial[(size_t)cand * p.L + l] = out;
-        }
+        if (active && g0 == 0) p.partial[(size_t)cand * p.L + l] = make_float4(sq, commt, mig, mxa);
 #pragma unroll
-        for (int rr = 0; rr < RPL; ++rr)
+        for (int rr = 0; rr < H; ++rr)
 #pragma unroll
             for (int j = 0; j < NW; ++j) cur[rr][j] = nxt[rr][j];
     }
 }
+
+// Same contract for any supported shape (runtime slots per rank <= 16, G a power of two <= 64, any E <= 256):
+// scalar loads, ids clamped to the table.
+template <bool kHasM>
+__global__ void __launch_bounds__(kScoreThreads, 1) place_score_generic_kernel(const ScoreParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int GP = place_gp(p.G), H = GP / 32, E = p.E, sp = p.sp, NS = p.G * p.sp;
+    const float2* wc_s = reinterpret_cast<const float2*>(smem_raw);                       // [H][E][32]
+    const uint32_t* mu_s = reinterpret_cast<const uint32_t*>(smem_raw + (size_t)H * E * 256);
+    const int l = blockIdx.y;
+    {
+        const uint4* src = reinterpret_cast<const uint4*>(p.t.wc + (size_t)l * H * E * 32);
+        uint4* dst = reinterpret_cast<uint4*>(smem_raw);
+        for (int i = threadIdx.x; i < H * E * 16; i += kScoreThreads) dst[i] = src[i];
+        if constexpr (kHasM) {
+            const uint4* ms = reinterpret_cast<const uint4*>(p.t.mu + (size_t)l * H * E * 32);
+            uint4* md = reinterpret_cast<uint4*>(smem_raw + (size_t)H * E * 256);
+            for (int i = threadIdx.x; i < H * E * 8; i += kScoreThreads) md[i] = ms[i];
+        }
+    }
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int seg = p.G < 32 ? p.G : 32, upw = 32 / seg;
+    const int sub = lane / seg, g0 = lane % seg;
+    const double Gd = (double)p.G, sumB = p.t.sumB[l];
+    const uint32_t emax = (uint32_t)E - 1u;
+    const int p_begin = blockIdx.x * p.chunk, p_end = min(p.P, p_begin + p.chunk);
+    const int stride = (kScoreThreads / 32) * upw;
+    for (int pc = p_begin + warp * upw; pc < p_end; pc += stride) {
+        const int cand = pc + sub;
+        const bool active = cand < p_end;
+        float sq = 0.0f, comm = 0.0f, mig = 0.0f, mx = 0.0f;
+        int kept = 0;
+        if (active) {
+            const int16_t* row = p.cand + ((size_t)cand * p.L + l) * NS;
+            for (int rr = 0; rr < H; ++rr) {
+                const int g = g0 + rr * 32;
+                float lg = 0.0f;
+                uint32_t kbits = 0;
+                for (int j = 0; j < sp; ++j) {
+                    const uint32_t x = min((uint32_t)(uint16_t)__ldcs(row + g * sp + j), emax);
+                    const int idx = (rr * E + (int)x) * 32 + lane;
+                    const float2 wc = wc_s[idx];
+                    lg += wc.x;
+                    comm += fabsf(wc.y);
+                    if constexpr (kHasM) {
+                        const uint32_t u = mu_s[idx];
+                        mig += fmaxf(__uint_as_float(u), 0.0f);
+                        kbits |= (uint32_t)((int32_t)u >> 31) & u;
+                    } else {
+                        kept += (int)(__float_as_uint(wc.y) >> 31);
+                    }
+                }
+                if constexpr (kHasM) {
+                    for (int j = 0; j < sp; ++j) mig += ((kbits >> j) & 1u) ? 0.0f : p.t.mx0[(size_t)l * NS + g * sp + j];
+                }
+                const float d = (float)((double)lg * Gd - sumB);
+                sq = __fmaf_rn(d, d, sq);
+                mx = fmaxf(mx, lg);
+            }
+        }
+        // butterflies over the seg lanes of the unit (xor offsets below seg stay inside it)
+        for (int o = seg >> 1; o > 0; o >>= 1) {
+            sq += __shfl_xor_sync(0xffffffffu, sq, o);
+            comm += __shfl_xor_sync(0xffffffffu, comm, o);
+            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+            if constexpr (kHasM) mig += __shfl_xor_sync(0xffffffffu, mig, o);
+            else kept += __shfl_xor_sync(0xffffffffu, kept, o);
+        }
+        if constexpr (!kHasM) mig = p.M_scalar * (float)(2 * (NS - kept));
+        if (active && g0 == 0) p.partial[(size_t)cand * p.L + l] = make_float4(sq, comm, mig, mx);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Exact validation, and the plain definition for candidates whose replica counts differ from x0's.
+// ------------------------------------------------------------------------------------------
+struct CheckParams {
+    int P, L, E, G, sp, chunk;
+    int sp_magic;                       // ceil(2^20 / sp): slot -> rank without a division
+    int force_general;                  // tests: score every valid candidate here
+    float M_scalar;
+    const int16_t* cand;                // [P,L,NS]
+    const int16_t* prev;                // [L,NS]
+    const float* M;                     // caller's [L,E,G] | nullptr
+    PlaceTables t;
+    float4* partial;
+};
+
+constexpr int kCheckWarps = 8;
+
+// grid (chunks, L), kCheckWarps warps; a warp takes one (candidate, layer) at a time.
+__global__ void __launch_bounds__(kCheckWarps * 32) place_check_kernel(const CheckParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int E = p.E, NS = p.G * p.sp, H = p.G > 32 ? 2 : 1;
+    uint32_t* mk_all = reinterpret_cast<uint32_t*>(smem_raw);                     // [warps][H][E] rank masks
+    uint8_t* r0_s = reinterpret_cast<uint8_t*>(mk_all + kCheckWarps * H * E);     // [E] replica counts of x0
+    const int l = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int e = threadIdx.x; e < E; e += kCheckWarps * 32) r0_s[e] = (uint8_t)min(p.t.r[(size_t)l * E + e], 255);
+    __syncthreads();
+    uint32_t* mk = mk_all + warp * H * E;
+    const int p_begin = blockIdx.x * p.chunk, p_end = min(p.P, p_begin + p.chunk);
+    const double Gd = (double)p.G, sumB = p.t.sumB[l];
+    for (int c = p_begin + warp; c < p_end; c += kCheckWarps) {
+        const int16_t* row = p.cand + ((size_t)c * p.L + l) * NS;
+        for (int i = lane; i < H * E; i += 32) mk[i] = 0u;
+        __syncwarp();
+        bool bad = false;
+        const uint32_t* roww = reinterpret_cast<const uint32_t*>(row);
+        for (int i = lane; i < NS / 2; i += 32) {
+            const uint32_t wv = roww[i];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const uint32_t e = (wv >> (16 * h)) & 0xffffu;
+                const int g = ((2 * i + h) * p.sp_magic) >> 20;
+                if (e >= (uint32_t)E) bad = true;
+                else {
+                    const uint32_t bit = 1u << (g & 31);
+                    if (atomicOr(&mk[(g >> 5) * E + e], bit) & bit) bad = true;      // twice on one rank
+                }
+            }
+        }
+        __syncwarp();
+        bool diff = false;
+        for (int e = lane; e < E; e += 32) {
+            const int r = __popc(mk[e]) + (H == 2 ? __popc(mk[E + e]) : 0);
+            if (r == 0) bad = true;                                                   // expert hosted nowhere
+            else if (r != (int)r0_s[e]) diff = true;
+        }
+        bad = __any_sync(0xffffffffu, bad);
+        diff = __any_sync(0xffffffffu, diff);
+        if (bad) {
+            if (lane == 0) p.partial[(size_t)c * p.L + l] = make_float4(CUDART_NAN_F, CUDART_NAN_F, CUDART_NAN_F, CUDART_NAN_F);
+        } else if (diff || p.force_general) {
+            // the plain definition with the candidate's own r (R12); lane <-> rank
+            float sq = 0.0f, comm = 0.0f, mig = 0.0f, mx = 0.0f;
+            const int16_t* pv = p.prev + (size_t)l * NS;
+            for (int rr = 0; rr < H; ++rr) {
+                const int g = lane + rr * 32;
+                if (g >= p.G) break;
+                double lgd = 0.0;
+                for (int j = 0; j < p.sp; ++j) {
+                    const int e = row[g * p.sp + j];
+                    const int r = __popc(mk[e]) + (H == 2 ? __popc(mk[E + e]) : 0);
+                    lgd += p.t.b_raw[(size_t)l * E + e] / (double)r;
+                    comm += p.t.c_raw[((size_t)l * E + e) * p.G + g] / (float)r;
+                    if (!((p.t.pmask[(size_t)l * E + e] >> g) & 1ull))                 // cell enters
+                        mig += p.M ? p.M[((size_t)l * E + e) * p.G + g] : p.M_scalar;
+                    const int e0 = pv[g * p.sp + j];
+                    if (!((mk[(g >> 5) * E + e0] >> (g & 31)) & 1u))                   // x0's cell leaves
+                        mig += p.M ? p.M[((size_t)l * E + e0) * p.G + g] : p.M_scalar;
+                }
+                const float d = (float)(lgd * Gd - sumB);
+                sq = __fmaf_rn(d, d, sq);
+                mx = fmaxf(mx, (float)lgd);
+            }
+            for (int o = 16; o > 0; o >>= 1) {
+                sq += __shfl_xor_sync(0xffffffffu, sq, o);
+                comm += __shfl_xor_sync(0xffffffffu, comm, o);
+                mig += __shfl_xor_sync(0xffffffffu, mig, o);
+                mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+            }
+            if (lane == 0) p.partial[(size_t)c * p.L + l] = make_float4(sq, comm, mig, mx);
+        }
+        __syncwarp();
+    }
+}
+
+inline size_t place_check_smem_bytes(int E, int G) { return sizeof(uint32_t) * (size_t)kCheckWarps * (G > 32 ? 2 : 1) * E + (size_t)((E + 15) & ~15); }
 
 struct FinalizeParams {
     int P, L, G;
@@ -631,7 +661,8 @@ __global__ void __launch_bounds__(256) move_delta_kernel(const MoveParams p) {
             if (((cm1 >> g2) & 1ull) || ((cm2 >> g1) & 1ull)) nan = true;      // second copy on a rank
             else {
                 const float2* wc = p.t.wc + (size_t)l * p.E * GP;
-                const float2 t11 = wc[e1 * GP + g1], t12 = wc[e1 * GP + g2], t21 = wc[e2 * GP + g1], t22 = wc[e2 * GP + g2];
+                const size_t i11 = tab_idx(p.E, e1, g1), i12 = tab_idx(p.E, e1, g2), i21 = tab_idx(p.E, e2, g1), i22 = tab_idx(p.E, e2, g2);
+                const float2 t11 = wc[i11], t12 = wc[i12], t21 = wc[i21], t22 = wc[i22];
                 // loads in double: L1 - L2 and w2 - w1 subtract nearly equal numbers that can exceed 2^24
                 const double w1 = p.t.w_e[(size_t)l * p.E + e1], w2 = p.t.w_e[(size_t)l * p.E + e2];
                 const double L1 = p.mp.Lg[(size_t)l * p.G + g1], L2 = p.mp.Lg[(size_t)l * p.G + g2];
@@ -639,8 +670,8 @@ __global__ void __launch_bounds__(256) move_delta_kernel(const MoveParams p) {
                 dload = (float)(2.0 * dl * (L1 - L2) + 2.0 * dl * dl);        // the mean cancels
                 dcomm = (fabsf(t12.y) - fabsf(t11.y)) + (fabsf(t21.y) - fabsf(t22.y));
                 const float* mt = p.t.m + (size_t)l * p.E * GP;
-                const float m11 = p.has_M ? mt[e1 * GP + g1] : p.M_scalar, m12 = p.has_M ? mt[e1 * GP + g2] : p.M_scalar;
-                const float m21 = p.has_M ? mt[e2 * GP + g1] : p.M_scalar, m22 = p.has_M ? mt[e2 * GP + g2] : p.M_scalar;
+                const float m11 = p.has_M ? mt[i11] : p.M_scalar, m12 = p.has_M ? mt[i12] : p.M_scalar;
+                const float m21 = p.has_M ? mt[i21] : p.M_scalar, m22 = p.has_M ? mt[i22] : p.M_scalar;
                 // leaving a cell x0 has: +M, leaving a cell x0 lacks: -M; entering: the opposite
                 dmig = (__float_as_int(t11.y) < 0 ? m11 : -m11) + (__float_as_int(t12.y) < 0 ? -m12 : m12) +
                        (__float_as_int(t22.y) < 0 ? m22 : -m22) + (__float_as_int(t21.y) < 0 ? -m21 : m21);
@@ -705,7 +736,7 @@ __global__ void __launch_bounds__(256) move_slots_kernel(const MoveSlotsParams p
     const int j = i >> p.lgG, g = i & (p.G - 1);
     int e = p.cur[(size_t)l * NS + j];
     if (e < 0 || e >= p.E) e = 0;                                      // flagged by move_prep_kernel
-    const size_t src = ((size_t)l * p.E + e) * GP + g, dst = ((size_t)l * NS + j) * p.G + g;
+    const size_t src = (size_t)l * p.E * GP + tab_idx(p.E, e, g), dst = ((size_t)l * NS + j) * p.G + g;
     p.mp.slotC[dst] = p.t.wc[src].y;
     if (p.has_M) p.mp.slotM[dst] = p.t.m[src];
     if (g == 0) {

@@ -58,6 +58,7 @@ __global__ void __launch_bounds__(kSchedWarps * 32) select_engines_kernel(const 
     }
     const bool complete = p.complete ? p.complete[b] != 0 : true;
     int rr = p.rr[b];
+    rr = ((rr % p.N) + p.N) % p.N;                                       // the pointer counts modulo N (R19)
     // KV rule (lines 6-9): argmin / argmax of kv, lowest index on ties; the same for every request of the call
     SchedKey kmin{CUDART_INF, 0.0, INT32_MAX}, kmax{CUDART_INF, 0.0, INT32_MAX};
 #pragma unroll
@@ -155,7 +156,7 @@ __global__ void __launch_bounds__(kQueueThreads) order_queues_kernel(const Queue
             bool before;
             if (aged_i != aged_j) before = aged_i;
             else if (!aged_i && pi != pj) before = pi < pj;
-            else if (ai != aj) before = ai < aj;
+            else if (ai < aj || aj < ai) before = ai < aj;                   // a NaN arrival ties with every arrival (R20)
             else before = i < j;
             pos += before;
         }

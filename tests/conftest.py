@@ -25,3 +25,16 @@ def pytest_collection_modifyitems(config, items):
     for it in items:
         if "gpu" in it.keywords:
             it.add_marker(skip)
+
+
+@pytest.fixture(autouse=True)
+def _default_library_options():
+    """the library's process-wide test switches (gimbal_set_option) are back at their defaults after every test"""
+    yield
+    try:
+        import paper_2606_15177_b200 as g
+        if os.path.exists(g.lib_path()):
+            for opt, val in ((g.OPT_CTA_GROUP, 0), (g.OPT_FUSE_GATE, 1), (g.OPT_SCORE_GENERIC, 0), (g.OPT_CHECK_SCORES_ALL, 0)):
+                g.set_option(opt, val)
+    except Exception:
+        pass

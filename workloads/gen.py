@@ -258,6 +258,38 @@ def candidates(w: Workload, prev: torch.Tensor, P: int | None = None, device="cp
     return out
 
 
+def candidates_redrawn(w: Workload, prev: torch.Tensor, P: int | None = None, device="cpu") -> torch.Tensor:
+    """[P,L,NS] int16 like `candidates`, but every (candidate, layer) draws its own NS - E redundant copies
+    (uniformly, with repetition: an expert may get 3 or more ranks), so the replica counts differ from x0's --
+    what a rebalancer searches over when it decides WHICH hot experts to replicate (EPLB-style).
+    p=0 stays x0.  Without redundant slots (NS == E) this is a random permutation."""
+    P = w.P if P is None else P
+    L, NS = prev.shape
+    E = w.router.E
+    prev = prev.to(device)
+    gen = _tgen(device, seed_for(w.cfg_id, TAG_CAND, 1))
+    base = torch.arange(E, device=device, dtype=torch.int16).repeat(P * L, 1)
+    if NS > E:
+        extra = torch.randint(0, E, (P * L, NS - E), generator=gen, device=device).to(torch.int16)
+        base = torch.cat([base, extra], dim=1)
+    perm = torch.rand(base.shape, generator=gen, device=device).argsort(-1)
+    rows = _repair(torch.gather(base, 1, perm), w.G, w.slots_per_rank, gen)
+    out = rows.view(P, L, NS).contiguous()
+    out[0] = prev
+    return out
+
+
+def to_expert_rank_u8(cands: torch.Tensor, sp: int) -> torch.Tensor:
+    """slot -> expert rows [..., NS] (no replicas, NS == E) -> expert -> rank bytes [..., E] (the EXPERT_TO_RANK_U8
+    candidate encoding of include/gimbal.h).  Pure re-indexing."""
+    NS = cands.shape[-1]
+    flat = cands.reshape(-1, NS).long()
+    rank = (torch.arange(NS, device=cands.device) // sp).to(torch.uint8).expand_as(flat)
+    out = torch.empty_like(flat, dtype=torch.uint8)
+    out.scatter_(1, flat, rank)
+    return out.view(*cands.shape[:-1], NS).contiguous()
+
+
 def explicit_moves(w: Workload, n: int, device="cpu") -> torch.Tensor:
     """[n,3] int32 (layer, slot_a, slot_b), slot_a != slot_b."""
     gen = _tgen(device, seed_for(w.cfg_id, TAG_MOVES))
