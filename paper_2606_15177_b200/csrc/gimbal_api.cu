@@ -131,6 +131,7 @@ static int validate_place_cfg(const gimbal_placement_cfg* c) {
 struct PlaceWs {
     PlaceTables t;
     float4* partial;                // [P,L]
+    uint8_t* status;                // [P,L] place_check_kernel's verdicts
     unsigned long long* best;       // [max(L,1)]
     MovePrep mp;
 };
@@ -153,6 +154,7 @@ static size_t place_ws_carve(const gimbal_placement_cfg* c, int P, void* ws, Pla
     w.t.pmask = cv.take<uint64_t>(LE);
     w.t.bad = cv.take<int32_t>(64);
     w.partial = cv.take<float4>((size_t)P * c->L);
+    w.status = cv.take<uint8_t>((size_t)P * c->L);
     w.best = cv.take<unsigned long long>(c->L + 1);
     w.mp.Lg = cv.take<double>((size_t)c->L * c->G);
     w.mp.top = cv.take<double>((size_t)c->L * 4);
@@ -190,9 +192,9 @@ static int launch_score_generic(const ScoreParams& sp, dim3 grid, size_t smem, c
     return GIMBAL_OK;
 }
 
-template <int SP, int G, bool kHasM>
+template <int SP, int G, int E, bool kHasM>
 static int launch_score_v(const ScoreParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
-    auto kern = place_score_kernel<SP, G, kHasM>;
+    auto kern = place_score_kernel<SP, G, E, kHasM>;
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ktime_begin(GIMBAL_KERNEL_SCORE, stream);
     kern<<<grid, kScoreThreads, smem, stream>>>(sp);
@@ -201,9 +203,9 @@ static int launch_score_v(const ScoreParams& sp, dim3 grid, size_t smem, cudaStr
     return GIMBAL_OK;
 }
 
-template <int SP, int G>
+template <int SP, int G, int E>
 static int launch_score(const ScoreParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
-    return sp.has_M ? launch_score_v<SP, G, true>(sp, grid, smem, stream) : launch_score_v<SP, G, false>(sp, grid, smem, stream);
+    return sp.has_M ? launch_score_v<SP, G, E, true>(sp, grid, smem, stream) : launch_score_v<SP, G, E, false>(sp, grid, smem, stream);
 }
 
 template <int E>
@@ -513,7 +515,7 @@ int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const void* c
     const int GP = place_gp(cfg->G);
     const size_t smem = e2r ? e2r_smem_bytes(cfg->E, cfg->G, M != nullptr) : (size_t)cfg->E * GP * (M ? 12 : 8);
     if (smem > kSmemLimit) return fail(GIMBAL_ERR_UNSUPPORTED, "E=%d G=%d with an M table needs %zu B of shared memory", cfg->E, cfg->G, smem);
-    const size_t smem_chk = place_check_smem_bytes(cfg->E, cfg->G);
+    const size_t smem_chk = place_check_smem_bytes(cfg->G);
     rc = require_device();
     if (rc) return rc;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
@@ -533,9 +535,10 @@ int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const void* c
             sp.P = P; sp.L = cfg->L; sp.E = cfg->E; sp.G = cfg->G; sp.sp = cfg->slots_per_rank; sp.M_scalar = M_scalar; sp.has_M = M != nullptr;
             sp.cand = static_cast<const int16_t*>(candidates); sp.t = w.t; sp.partial = w.partial;
             // one wave: two resident blocks per SM (one when the table needs more than half the shared memory)
-            const bool pow2E = (cfg->E & (cfg->E - 1)) == 0;
-            const int key = (pow2E && !g_opt[GIMBAL_OPT_SCORE_GENERIC].load(std::memory_order_relaxed)) ? cfg->slots_per_rank * 100 + cfg->G : 0;
-            const bool fast = key == 932 || key == 816 || key == 808 || key == 464 || key == 404;
+            // the five configuration shapes (slots per rank, ranks, experts) have specialised kernels
+            const long key = g_opt[GIMBAL_OPT_SCORE_GENERIC].load(std::memory_order_relaxed)
+                                 ? 0 : (long)cfg->slots_per_rank * 1000000 + cfg->G * 1000 + cfg->E;
+            const bool fast = key == 9032256 || key == 8016128 || key == 8008064 || key == 4064256 || key == 4004016;
             const int per_sm = (fast && 2 * smem + 2048 <= kSmemLimit) ? 2 : 1;
             int nchunk = per_sm * sms / cfg->L;
             const int units_per_pass = (kScoreThreads / 32) * (cfg->G < 32 ? 32 / cfg->G : 1);
@@ -544,13 +547,12 @@ int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const void* c
             if (nchunk < 1) nchunk = 1;
             sp.chunk = (P + nchunk - 1) / nchunk;
             dim3 grid((P + sp.chunk - 1) / sp.chunk, cfg->L);
-            // the five configuration shapes have specialised kernels (E must be a power of two there)
             switch (key) {
-                case 932: rc = launch_score<9, 32>(sp, grid, smem, stream); break;
-                case 816: rc = launch_score<8, 16>(sp, grid, smem, stream); break;
-                case 808: rc = launch_score<8, 8>(sp, grid, smem, stream); break;
-                case 464: rc = launch_score<4, 64>(sp, grid, smem, stream); break;
-                case 404: rc = launch_score<4, 4>(sp, grid, smem, stream); break;
+                case 9032256: rc = launch_score<9, 32, 256>(sp, grid, smem, stream); break;
+                case 8016128: rc = launch_score<8, 16, 128>(sp, grid, smem, stream); break;
+                case 8008064: rc = launch_score<8, 8, 64>(sp, grid, smem, stream); break;
+                case 4064256: rc = launch_score<4, 64, 256>(sp, grid, smem, stream); break;
+                case 4004016: rc = launch_score<4, 4, 16>(sp, grid, smem, stream); break;
                 default: rc = sp.has_M ? launch_score_generic<true>(sp, grid, smem, stream) : launch_score_generic<false>(sp, grid, smem, stream); break;
             }
             if (rc) return rc;
@@ -559,18 +561,30 @@ int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const void* c
                 // counts differ from x0's (scored with their own r)
                 CheckParams cp{};
                 cp.P = P; cp.L = cfg->L; cp.E = cfg->E; cp.G = cfg->G; cp.sp = cfg->slots_per_rank;
-                cp.sp_magic = ((1 << 20) + cfg->slots_per_rank - 1) / cfg->slots_per_rank;
                 cp.force_general = g_opt[GIMBAL_OPT_CHECK_SCORES_ALL].load(std::memory_order_relaxed);
-                cp.M_scalar = M_scalar; cp.cand = sp.cand; cp.prev = prev; cp.M = M; cp.t = w.t; cp.partial = w.partial;
+                cp.M_scalar = M_scalar; cp.cand = sp.cand; cp.prev = prev; cp.M = M; cp.t = w.t; cp.partial = w.partial; cp.status = w.status;
                 int nck = 8 * sms / cfg->L;
                 const int maxck = (P + kCheckWarps - 1) / kCheckWarps;
                 if (nck > maxck) nck = maxck;
                 if (nck < 1) nck = 1;
                 cp.chunk = (P + nck - 1) / nck;
                 ktime_begin(GIMBAL_KERNEL_CHECK, stream);
-                place_check_kernel<<<dim3((P + cp.chunk - 1) / cp.chunk, cfg->L), kCheckWarps * 32, smem_chk, stream>>>(cp);
+                const dim3 cgrid((P + cp.chunk - 1) / cp.chunk, cfg->L);
+                const int key = cfg->slots_per_rank * 10 + (cfg->G > 32 ? 2 : 1);
+                switch (key) {
+                    case 41: place_check_kernel<4, 1><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp); break;
+                    case 42: place_check_kernel<4, 2><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp); break;
+                    case 81: place_check_kernel<8, 1><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp); break;
+                    case 91: place_check_kernel<9, 1><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp); break;
+                    default:
+                        if (cfg->G > 32) place_check_kernel<0, 2><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp);
+                        else place_check_kernel<0, 1><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp);
+                        break;
+                }
                 ktime_end(GIMBAL_KERNEL_CHECK, stream);
                 LAUNCH_CHECK("place_check_kernel");
+                place_own_r_kernel<<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp);
+                LAUNCH_CHECK("place_own_r_kernel");
             }
         }
         FinalizeParams fp{};

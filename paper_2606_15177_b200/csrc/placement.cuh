@@ -187,56 +187,39 @@ __device__ __forceinline__ float reduce_pair(float& sq, float comm, int lane, in
     }
 }
 
-// Throughput kernel for compile-time (slots per rank, ranks) and a power-of-two E <= 256.  Slot ids
+// Throughput kernel for the five configuration shapes: compile-time (slots per rank, ranks, experts).  Slot ids
 // arrive as aligned 32-bit words (two per word; ranks with an odd slot count are realigned with a
-// funnel shift); one PRMT turns an id into the byte offset of its table cell ((id & 255) << 8 | lane * 8),
+// funnel shift); one PRMT turns an id into the byte offset of its table cell (id << 8 | lane * 8),
 // one 8-byte shared load fetches {w, c}, two adds and one shift-add (x0 membership) finish the slot.
 // Ids are masked to the table, so a row that place_check_kernel would reject cannot fault here.
-template <int SP, int G, bool kHasM>
+// A warp pass takes two candidates per unit: their instruction streams interleave and one transposed
+// butterfly reduces both; the rows of the next pass are prefetched into the other half of a register
+// ping-pong.  G*L_g - sum_e B is one fp32 FMA against the high part of sum_e B plus one subtraction of
+// the low part: exact whenever the difference is representable (integer counts), R11.
+constexpr int kScoreU = 2;
+
+template <int SP, int G, int E, bool kHasM>
 __global__ void __launch_bounds__(kScoreThreads, 2) place_score_kernel(const ScoreParams p) {
+    constexpr int kU = kScoreU;
     constexpr int H = G > 32 ? G / 32 : 1;              // table halves == ranks per lane
     constexpr int SEG = G < 32 ? G : 32, UPW = 32 / SEG;
     constexpr int NS = G * SP;
     constexpr int NW = (SP + 1) / 2;                    // words holding one rank's ids
+    static_assert(SEG >= 4, "the joint reduction needs four lanes per unit");
+    static_assert((E & (E - 1)) == 0 && E <= 256, "E");
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int E = p.E;
     const unsigned char* wc_b = smem_raw;                               // [H][E][32] float2
     const unsigned char* mu_b = smem_raw + (size_t)H * E * 256;         // [H][E][32] u32 (kHasM)
     const int l = blockIdx.y;
-    {
-        const uint4* src = reinterpret_cast<const uint4*>(p.t.wc + (size_t)l * H * E * 32);
-        uint4* dst = reinterpret_cast<uint4*>(smem_raw);
-        for (int i = threadIdx.x; i < H * E * 16; i += kScoreThreads) dst[i] = src[i];
-        if constexpr (kHasM) {
-            const uint4* ms = reinterpret_cast<const uint4*>(p.t.mu + (size_t)l * H * E * 32);
-            uint4* md = reinterpret_cast<uint4*>(smem_raw + (size_t)H * E * 256);
-            for (int i = threadIdx.x; i < H * E * 8; i += kScoreThreads) md[i] = ms[i];
-        }
-    }
-    __syncthreads();
-
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int sub = lane / SEG, g0 = lane % SEG;
-    const uint32_t seg_mask = SEG == 32 ? 0xffffffffu : (((1u << SEG) - 1u) << (sub * SEG));
-    const double Gd = (double)G;
-    const double sumB = p.t.sumB[l];
-    const uint32_t emask = (uint32_t)E - 1u;
-    const uint32_t emask2 = emask | (emask << 16);
-    const uint32_t lane8 = (uint32_t)lane * 8u;         // table column of this lane's rank (replicated columns when G < 32)
-    float mx0[kHasM ? H : 1][kHasM ? SP : 1];           // M of x0's own cells on this lane's rank(s)
-    if constexpr (kHasM) {
-#pragma unroll
-        for (int rr = 0; rr < H; ++rr)
-#pragma unroll
-            for (int j = 0; j < SP; ++j) mx0[rr][j] = p.t.mx0[(size_t)l * NS + (g0 + rr * 32) * SP + j];
-    }
 
     const int p_begin = blockIdx.x * p.chunk, p_end = min(p.P, p_begin + p.chunk);
-    constexpr int kStride = (kScoreThreads / 32) * UPW;
-    const size_t step_words = (size_t)kStride * p.L * NS / 2;
-    int cand = p_begin + warp * UPW + sub;
+    constexpr int kStride = (kScoreThreads / 32) * UPW;                 // candidates between two units of a warp pass
+    const size_t stride_words = (size_t)kStride * p.L * NS / 2;
+    int cand = p_begin + warp * UPW + sub;                              // unit 0 of this lane; unit u is cand + u * kStride
     const uint32_t* rowp = reinterpret_cast<const uint32_t*>(p.cand + ((size_t)cand * p.L + l) * NS);
-    uint32_t cur[H][NW], nxt[H][NW];
+    uint32_t bufA[kU][H][NW], bufB[kU][H][NW];
     auto fetch = [&](const uint32_t* row, uint32_t (&w)[H][NW]) {
 #pragma unroll
         for (int rr = 0; rr < H; ++rr) {
@@ -259,19 +242,63 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_kernel(const Sco
             }
         }
     };
-    if (cand < p_end) fetch(rowp, cur);
-    for (int pc = p_begin + warp * UPW; pc < p_end; pc += kStride, cand += kStride) {
-        const bool active = cand < p_end;
-        rowp += step_words;
-        if (cand + kStride < p_end) fetch(rowp, nxt);
-        float sq = 0.0f, comm = 0.0f, mig = 0.0f, mx = 0.0f;
-        uint32_t kept = 0;
-        if (active) {
+    // the first rows are on their way while the table is staged
+#pragma unroll
+    for (int u = 0; u < kU; ++u)
+        if (cand + u * kStride < p_end) fetch(rowp + u * stride_words, bufA[u]);
+    {
+        // all of a thread's table loads are in flight before the first store (the whole wave stages at once)
+        constexpr int N4 = H * E * 16, kIt = (N4 + kScoreThreads - 1) / kScoreThreads;
+        const uint4* src = reinterpret_cast<const uint4*>(p.t.wc + (size_t)l * H * E * 32);
+        uint4* dst = reinterpret_cast<uint4*>(smem_raw);
+        uint4 tmp[kIt];
+#pragma unroll
+        for (int k = 0; k < kIt; ++k)
+            if ((int)threadIdx.x + k * kScoreThreads < N4) tmp[k] = __ldg(src + threadIdx.x + k * kScoreThreads);
+#pragma unroll
+        for (int k = 0; k < kIt; ++k)
+            if ((int)threadIdx.x + k * kScoreThreads < N4) dst[threadIdx.x + k * kScoreThreads] = tmp[k];
+        if constexpr (kHasM) {
+            const uint4* ms = reinterpret_cast<const uint4*>(p.t.mu + (size_t)l * H * E * 32);
+            uint4* md = reinterpret_cast<uint4*>(smem_raw + (size_t)H * E * 256);
+            for (int i = threadIdx.x; i < H * E * 8; i += kScoreThreads) md[i] = ms[i];
+        }
+    }
+    const uint32_t seg_mask = SEG == 32 ? 0xffffffffu : (((1u << SEG) - 1u) << (sub * SEG));
+    const double sumB = p.t.sumB[l];
+    const float sumB_hi = (float)sumB, sumB_lo = (float)(sumB - (double)sumB_hi);
+    constexpr uint32_t emask2 = (uint32_t)(E - 1) | ((uint32_t)(E - 1) << 16);
+    const uint32_t lane8 = (uint32_t)lane * 8u;         // table column of this lane's rank (replicated columns when G < 32)
+    const float M_scalar = p.M_scalar;
+    float4* const partial = p.partial;
+    const int L = p.L;
+    float mx0[kHasM ? H : 1][kHasM ? SP : 1];           // M of x0's own cells on this lane's rank(s)
+    if constexpr (kHasM) {
+#pragma unroll
+        for (int rr = 0; rr < H; ++rr)
+#pragma unroll
+            for (int j = 0; j < SP; ++j) mx0[rr][j] = p.t.mx0[(size_t)l * NS + (g0 + rr * 32) * SP + j];
+    }
+    __syncthreads();
+
+    // one warp pass: prefetch the next pass into `nxt`, score the two candidates in `cur`, reduce, store
+    auto pass = [&](uint32_t (&cur)[kU][H][NW], uint32_t (&nxt)[kU][H][NW]) {
+        rowp += kU * stride_words;
+#pragma unroll
+        for (int u = 0; u < kU; ++u)
+            if (cand + (kU + u) * kStride < p_end) fetch(rowp + u * stride_words, nxt[u]);
+        float sq[kU], comm[kU], mig[kU], mx[kU];
+        uint32_t kept[kU];
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            // no activity test here: a unit past the end scores whatever its registers hold (ids are masked) and is not stored
+            sq[u] = comm[u] = mig[u] = mx[u] = 0.0f;
+            kept[u] = 0;
 #pragma unroll
             for (int rr = 0; rr < H; ++rr) {
                 uint32_t w[NW];
 #pragma unroll
-                for (int j = 0; j < NW; ++j) w[j] = cur[rr][j];
+                for (int j = 0; j < NW; ++j) w[j] = cur[u][rr][j];
                 if constexpr (SP % 2 == 1) {
                     // odd ranks start in the upper half of their first word: realign
                     const uint32_t sh = ((g0 + rr * 32) & 1) * 16;
@@ -279,47 +306,72 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_kernel(const Sco
                     for (int j = 0; j + 1 < NW; ++j) w[j] = __funnelshift_r(w[j], w[j + 1], sh);
                     w[NW - 1] = w[NW - 1] >> sh;
                 }
+                if constexpr (E < 256) {                // E == 256: the PRMT below only takes the low byte of an id
 #pragma unroll
-                for (int j = 0; j < NW; ++j) w[j] &= emask2;        // keeps every id inside the staged table
-                float lg = 0.0f;
+                    for (int j = 0; j < NW; ++j) w[j] &= emask2;
+                }
+                float lg2[2] = {0.0f, 0.0f}, cm2[2] = {0.0f, 0.0f};  // two chains each: half the dependent adds
+                uint32_t kp2[2] = {0u, 0u};
                 uint32_t kbits = 0;
 #pragma unroll
                 for (int j = 0; j < SP; ++j) {
                     const uint32_t off = __byte_perm(w[j >> 1], lane8, (j & 1) ? 0x5524 : 0x5504);   // id << 8 | lane * 8
                     const float2 wc = *reinterpret_cast<const float2*>(wc_b + rr * E * 256 + off);
-                    lg += wc.x;
-                    comm += fabsf(wc.y);
+                    lg2[j & 1] += wc.x;
+                    cm2[j & 1] += fabsf(wc.y);
                     if constexpr (kHasM) {
-                        const uint32_t u = *reinterpret_cast<const uint32_t*>(mu_b + rr * E * 128 + (off >> 1));
-                        mig += fmaxf(__uint_as_float(u), 0.0f);                         // entering cell: + M
-                        kbits |= (uint32_t)((int32_t)u >> 31) & u;                      // retained cell: which of x0's slots
+                        const uint32_t uw = *reinterpret_cast<const uint32_t*>(mu_b + rr * E * 128 + (off >> 1));
+                        mig[u] += fmaxf(__uint_as_float(uw), 0.0f);                     // entering cell: + M
+                        kbits |= (uint32_t)((int32_t)uw >> 31) & uw;                    // retained cell: which of x0's slots
                     } else {
-                        kept += __float_as_uint(wc.y) >> 31;
+                        kp2[j & 1] += __float_as_uint(wc.y) >> 31;
                     }
                 }
+                const float lg = lg2[0] + lg2[1];
+                comm[u] += cm2[0] + cm2[1];
+                kept[u] += kp2[0] + kp2[1];
                 if constexpr (kHasM) {
 #pragma unroll
-                    for (int j = 0; j < SP; ++j) mig += ((kbits >> j) & 1u) ? 0.0f : mx0[rr][j];   // leaving cells, x0's slot order
+                    for (int j = 0; j < SP; ++j) mig[u] += ((kbits >> j) & 1u) ? 0.0f : mx0[rr][j];   // leaving cells, x0's slot order
                 }
-                const float d = (float)((double)lg * Gd - sumB);  // G*L_g - sum_g L_g, exact difference for integer counts
-                sq = __fmaf_rn(d, d, sq);
-                mx = fmaxf(mx, lg);
+                const float d = __fsub_rn(__fmaf_rn(lg, (float)G, -sumB_hi), sumB_lo);   // G*L_g - sum_g L_g
+                sq[u] = __fmaf_rn(d, d, sq[u]);
+                mx[u] = fmaxf(mx[u], lg);
             }
         }
-        const float mxa = __uint_as_float(__reduce_max_sync(seg_mask, __float_as_uint(mx)));   // loads are >= 0
-        const float commt = reduce_pair<SEG>(sq, comm, lane, sub);
+        // one transposed butterfly for both candidates of the unit: after the first step the lanes with bit h clear
+        // work for candidate 0 and the others for candidate 1, after the second the lanes with bit h2 clear hold sq, the
+        // others comm
+        constexpr int h = SEG >> 1, h2 = SEG >> 2;
+        const bool up = (lane & h) != 0, up2 = (lane & h2) != 0;
+        float ka = (up ? sq[1] : sq[0]) + __shfl_xor_sync(0xffffffffu, up ? sq[0] : sq[1], h);
+        float kb = (up ? comm[1] : comm[0]) + __shfl_xor_sync(0xffffffffu, up ? comm[0] : comm[1], h);
+        float v = (up2 ? kb : ka) + __shfl_xor_sync(0xffffffffu, up2 ? ka : kb, h2);
+#pragma unroll
+        for (int o = h2 >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        const float commt = __shfl_xor_sync(0xffffffffu, v, h2);            // lanes with bit h2 clear: v = sq, commt = comm
+        const float mxa0 = __uint_as_float(__reduce_max_sync(seg_mask, __float_as_uint(mx[0])));   // loads are >= 0
+        const float mxa1 = __uint_as_float(__reduce_max_sync(seg_mask, __float_as_uint(mx[1])));
+        float migt;
         if constexpr (kHasM) {
+            float m = (up ? mig[1] : mig[0]) + __shfl_xor_sync(0xffffffffu, up ? mig[0] : mig[1], h);
 #pragma unroll
-            for (int o = SEG >> 1; o > 0; o >>= 1) mig += __shfl_xor_sync(0xffffffffu, mig, o);
+            for (int o = h >> 1; o > 0; o >>= 1) m += __shfl_xor_sync(0xffffffffu, m, o);
+            migt = m;
         } else {
-            kept = __reduce_add_sync(seg_mask, kept);
-            mig = p.M_scalar * (float)(2 * (NS - (int)kept));       // entering + leaving cells, M each: exact
+            const uint32_t k2 = __reduce_add_sync(seg_mask, kept[0] | (kept[1] << 16));       // each total <= NS < 2^16
+            const int k = up ? (int)(k2 >> 16) : (int)(k2 & 0xffffu);
+            migt = M_scalar * (float)(2 * (NS - k));                                          // entering + leaving cells, M each: exact
         }
-        if (active && g0 == 0) p.partial[(size_t)cand * p.L + l] = make_float4(sq, commt, mig, mxa);
-#pragma unroll
-        for (int rr = 0; rr < H; ++rr)
-#pragma unroll
-            for (int j = 0; j < NW; ++j) cur[rr][j] = nxt[rr][j];
+        // lane g0 == 0 writes candidate 0, lane g0 == h candidate 1
+        const int mine = cand + (up ? kStride : 0);
+        if ((g0 & (h - 1)) == 0 && mine < p_end) partial[(size_t)mine * L + l] = make_float4(v, commt, migt, up ? mxa1 : mxa0);
+        cand += kU * kStride;
+    };
+    for (int pc = p_begin + warp * UPW; pc < p_end; pc += 2 * kU * kStride) {
+        pass(bufA, bufB);
+        if (pc + kU * kStride >= p_end) break;
+        pass(bufB, bufA);
     }
 }
 
@@ -401,7 +453,6 @@ __global__ void __launch_bounds__(kScoreThreads, 1) place_score_generic_kernel(c
 // ------------------------------------------------------------------------------------------
 struct CheckParams {
     int P, L, E, G, sp, chunk;
-    int sp_magic;                       // ceil(2^20 / sp): slot -> rank without a division
     int force_general;                  // tests: score every valid candidate here
     float M_scalar;
     const int16_t* cand;                // [P,L,NS]
@@ -409,88 +460,179 @@ struct CheckParams {
     const float* M;                     // caller's [L,E,G] | nullptr
     PlaceTables t;
     float4* partial;
+    uint8_t* status;                    // [P,L] 0: valid, same copies as x0   1: invalid   2: valid, other replica counts
 };
 
 constexpr int kCheckWarps = 8;
+constexpr int kCheckE = 256;            // rank-mask rows per half (E <= 256, ids are masked to 8 bits)
 
-// grid (chunks, L), kCheckWarps warps; a warp takes one (candidate, layer) at a time.
+inline size_t place_check_smem_bytes(int G) { return sizeof(uint32_t) * (size_t)kCheckWarps * (G > 32 ? 2 : 1) * kCheckE + 2 * kCheckE; }
+
+// the candidate's own score (PAPER.md:236-248 with r from the candidate, R12); lane <-> rank, global tables.
+// mk: the warp's rank masks [H][256] of this candidate.
+__device__ __forceinline__ void place_score_own_r(const CheckParams& p, int l, int c, const int16_t* row, const uint32_t* mk, int lane) {
+    const int E = p.E, NS = p.G * p.sp, H = p.G > 32 ? 2 : 1;
+    const double Gd = (double)p.G, sumB = p.t.sumB[l];
+    float sq = 0.0f, comm = 0.0f, mig = 0.0f, mx = 0.0f;
+    const int16_t* pv = p.prev + (size_t)l * NS;
+    for (int rr = 0; rr < H; ++rr) {
+        const int g = lane + rr * 32;
+        if (g >= p.G) break;
+        double lgd = 0.0;
+        for (int j = 0; j < p.sp; ++j) {
+            const int e = row[g * p.sp + j];
+            const int r = __popc(mk[e]) + (H == 2 ? __popc(mk[kCheckE + e]) : 0);
+            lgd += p.t.b_raw[(size_t)l * E + e] / (double)r;
+            comm += p.t.c_raw[((size_t)l * E + e) * p.G + g] / (float)r;
+            if (!((p.t.pmask[(size_t)l * E + e] >> g) & 1ull))                 // cell enters
+                mig += p.M ? p.M[((size_t)l * E + e) * p.G + g] : p.M_scalar;
+            const int e0 = pv[g * p.sp + j];
+            if (!((mk[(g >> 5) * kCheckE + e0] >> (g & 31)) & 1u))             // x0's cell leaves
+                mig += p.M ? p.M[((size_t)l * E + e0) * p.G + g] : p.M_scalar;
+        }
+        const float d = (float)(lgd * Gd - sumB);
+        sq = __fmaf_rn(d, d, sq);
+        mx = fmaxf(mx, (float)lgd);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        sq += __shfl_xor_sync(0xffffffffu, sq, o);
+        comm += __shfl_xor_sync(0xffffffffu, comm, o);
+        mig += __shfl_xor_sync(0xffffffffu, mig, o);
+        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    }
+    if (lane == 0) p.partial[(size_t)c * p.L + l] = make_float4(sq, comm, mig, mx);
+}
+
+// grid (chunks, L), kCheckWarps warps; a warp takes one (candidate, layer) at a time, lane <-> rank (two ranks per
+// lane when G = 64).  SP: compile-time slots per rank (0: runtime, up to 16).
+//   scatter   every slot ORs its rank's bit into the candidate's x[e, .] row: mk[e] |= 1 << g.  The word that comes
+//             back tells whether the bit was already there ("twice on one rank"); ids are masked to 8 bits, the range
+//             check is one OR over the packed words (plus a compare per slot when E is not a power of two).
+//   readback  lane i owns experts 4i..4i+3 and 128+4i..: two 16-byte loads return its eight rank masks, two 16-byte
+//             stores clear them for the next candidate; their popcounts, packed four to a word, are compared with x0's
+//             replica counts in one XOR each.  All equal <=> same copies as x0 (place_score_kernel's premise).
+template <int SP, int H>
 __global__ void __launch_bounds__(kCheckWarps * 32) place_check_kernel(const CheckParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int E = p.E, NS = p.G * p.sp, H = p.G > 32 ? 2 : 1;
-    uint32_t* mk_all = reinterpret_cast<uint32_t*>(smem_raw);                     // [warps][H][E] rank masks
-    uint8_t* r0_s = reinterpret_cast<uint8_t*>(mk_all + kCheckWarps * H * E);     // [E] replica counts of x0
+    const int E = p.E, sp = SP > 0 ? SP : p.sp, NS = p.G * sp;
+    uint32_t* mk_all = reinterpret_cast<uint32_t*>(smem_raw);                                 // [warps][H][256] rank masks
+    uint8_t* r0_s = reinterpret_cast<uint8_t*>(mk_all + kCheckWarps * H * kCheckE);           // [256] replica counts of x0 (0 past E)
     const int l = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int e = threadIdx.x; e < E; e += kCheckWarps * 32) r0_s[e] = (uint8_t)min(p.t.r[(size_t)l * E + e], 255);
+    for (int e = threadIdx.x; e < kCheckE; e += kCheckWarps * 32) r0_s[e] = e < E ? (uint8_t)min(p.t.r[(size_t)l * E + e], 255) : 0;
+    for (int i = threadIdx.x; i < kCheckWarps * H * kCheckE; i += kCheckWarps * 32) mk_all[i] = 0u;
     __syncthreads();
-    uint32_t* mk = mk_all + warp * H * E;
+    uint32_t* mk = mk_all + warp * H * kCheckE;
+    const uint32_t r0a = reinterpret_cast<const uint32_t*>(r0_s)[lane], r0b = reinterpret_cast<const uint32_t*>(r0_s)[32 + lane];
+    const bool pow2E = (E & (E - 1)) == 0;
+    const uint32_t id_ok = pow2E ? (uint32_t)(E - 1) : 0xffu;                                  // bits a valid id may use
+    const uint32_t bit = 1u << lane;
+    constexpr int MAXSP = SP > 0 ? SP : 16, NWL = MAXSP / 2 + 1;                              // words that can hold a rank's ids
     const int p_begin = blockIdx.x * p.chunk, p_end = min(p.P, p_begin + p.chunk);
-    const double Gd = (double)p.G, sumB = p.t.sumB[l];
+    // this lane's ranks: where their ids start in a row (word, half-word shift) and how many words they span
+    int w0[H], nw[H];
+    uint32_t sh[H];
+#pragma unroll
+    for (int rr = 0; rr < H; ++rr) {
+        const int hw0 = (lane + rr * 32) * sp;
+        w0[rr] = hw0 >> 1; sh[rr] = (hw0 & 1) * 16; nw[rr] = (lane + rr * 32 < p.G) ? (sp + (hw0 & 1) + 1) >> 1 : 0;
+    }
+    uint32_t Wn[H][NWL];                                                                       // the next candidate's words
+    auto fetch = [&](int c) {
+        const uint32_t* roww = reinterpret_cast<const uint32_t*>(p.cand + ((size_t)c * p.L + l) * NS);
+#pragma unroll
+        for (int rr = 0; rr < H; ++rr)
+#pragma unroll
+            for (int k = 0; k < NWL; ++k) Wn[rr][k] = k < nw[rr] ? __ldcs(roww + w0[rr] + k) : 0u;
+    };
+    if (p_begin + warp < p_end) fetch(p_begin + warp);
     for (int c = p_begin + warp; c < p_end; c += kCheckWarps) {
         const int16_t* row = p.cand + ((size_t)c * p.L + l) * NS;
-        for (int i = lane; i < H * E; i += 32) mk[i] = 0u;
-        __syncwarp();
-        bool bad = false;
-        const uint32_t* roww = reinterpret_cast<const uint32_t*>(row);
-        for (int i = lane; i < NS / 2; i += 32) {
-            const uint32_t wv = roww[i];
+        uint32_t W[H][NWL + 1];
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const uint32_t e = (wv >> (16 * h)) & 0xffffu;
-                const int g = ((2 * i + h) * p.sp_magic) >> 20;
-                if (e >= (uint32_t)E) bad = true;
-                else {
-                    const uint32_t bit = 1u << (g & 31);
-                    if (atomicOr(&mk[(g >> 5) * E + e], bit) & bit) bad = true;      // twice on one rank
+        for (int rr = 0; rr < H; ++rr) {
+#pragma unroll
+            for (int k = 0; k < NWL; ++k) W[rr][k] = Wn[rr][k];
+            W[rr][NWL] = 0u;
+        }
+        if (c + kCheckWarps < p_end) fetch(c + kCheckWarps);                                   // in flight during this candidate
+        uint32_t viol = 0, range = 0;
+        bool oob = false;
+#pragma unroll
+        for (int rr = 0; rr < H; ++rr) {
+            if (nw[rr] > 0) {
+#pragma unroll
+                for (int k = 0; k < NWL; ++k) W[rr][k] = __funnelshift_r(W[rr][k], W[rr][k + 1], sh[rr]);   // slot j of the rank = halfword j
+                uint32_t* mkr = mk + rr * kCheckE;
+#pragma unroll
+                for (int j = 0; j < MAXSP; ++j) {
+                    if (SP > 0 || j < sp) {
+                        const uint32_t wj = W[rr][j >> 1];
+                        const uint32_t raw = (j & 1) ? (wj >> 16) : (wj & 0xffffu);
+                        range |= raw;
+                        if (!pow2E) oob |= raw >= (uint32_t)E;
+                        viol |= atomicOr(mkr + (raw & 255u), bit);
+                    }
                 }
             }
         }
         __syncwarp();
-        bool diff = false;
-        for (int e = lane; e < E; e += 32) {
-            const int r = __popc(mk[e]) + (H == 2 ? __popc(mk[E + e]) : 0);
-            if (r == 0) bad = true;                                                   // expert hosted nowhere
-            else if (r != (int)r0_s[e]) diff = true;
+        // readback + clear
+        uint32_t diff = 0, zero = 0;
+#pragma unroll
+        for (int rr = 0; rr < H; ++rr) {
+            {
+                uint4* q = reinterpret_cast<uint4*>(mk + rr * kCheckE);
+                const uint4 a = q[lane], b = q[32 + lane];
+                q[lane] = make_uint4(0u, 0u, 0u, 0u);
+                q[32 + lane] = make_uint4(0u, 0u, 0u, 0u);
+                const uint32_t ca = __popc(a.x) | (__popc(a.y) << 8) | (__popc(a.z) << 16) | (__popc(a.w) << 24);
+                const uint32_t cb = __popc(b.x) | (__popc(b.y) << 8) | (__popc(b.z) << 16) | (__popc(b.w) << 24);
+                if (rr == 0) { diff = ca; zero = cb; } else { diff += ca; zero += cb; }        // packed counts (each <= 64)
+            }
         }
-        bad = __any_sync(0xffffffffu, bad);
-        diff = __any_sync(0xffffffffu, diff);
-        if (bad) {
-            if (lane == 0) p.partial[(size_t)c * p.L + l] = make_float4(CUDART_NAN_F, CUDART_NAN_F, CUDART_NAN_F, CUDART_NAN_F);
-        } else if (diff || p.force_general) {
-            // the plain definition with the candidate's own r (R12); lane <-> rank
-            float sq = 0.0f, comm = 0.0f, mig = 0.0f, mx = 0.0f;
-            const int16_t* pv = p.prev + (size_t)l * NS;
-            for (int rr = 0; rr < H; ++rr) {
-                const int g = lane + rr * 32;
-                if (g >= p.G) break;
-                double lgd = 0.0;
-                for (int j = 0; j < p.sp; ++j) {
-                    const int e = row[g * p.sp + j];
-                    const int r = __popc(mk[e]) + (H == 2 ? __popc(mk[E + e]) : 0);
-                    lgd += p.t.b_raw[(size_t)l * E + e] / (double)r;
-                    comm += p.t.c_raw[((size_t)l * E + e) * p.G + g] / (float)r;
-                    if (!((p.t.pmask[(size_t)l * E + e] >> g) & 1ull))                 // cell enters
-                        mig += p.M ? p.M[((size_t)l * E + e) * p.G + g] : p.M_scalar;
-                    const int e0 = pv[g * p.sp + j];
-                    if (!((mk[(g >> 5) * E + e0] >> (g & 31)) & 1u))                   // x0's cell leaves
-                        mig += p.M ? p.M[((size_t)l * E + e0) * p.G + g] : p.M_scalar;
-                }
-                const float d = (float)(lgd * Gd - sumB);
-                sq = __fmaf_rn(d, d, sq);
-                mx = fmaxf(mx, (float)lgd);
-            }
-            for (int o = 16; o > 0; o >>= 1) {
-                sq += __shfl_xor_sync(0xffffffffu, sq, o);
-                comm += __shfl_xor_sync(0xffffffffu, comm, o);
-                mig += __shfl_xor_sync(0xffffffffu, mig, o);
-                mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-            }
-            if (lane == 0) p.partial[(size_t)c * p.L + l] = make_float4(sq, comm, mig, mx);
+        const uint32_t cnta = diff, cntb = zero;
+        const bool same = (cnta == r0a) && (cntb == r0b);
+        // an expert of [0,E) hosted nowhere: a zero byte where x0's count is not zero (x0 valid: r0 >= 1 below E)
+        const uint32_t za = ~(((cnta & 0x7f7f7f7fu) + 0x7f7f7f7fu) | cnta) & 0x80808080u, zb = ~(((cntb & 0x7f7f7f7fu) + 0x7f7f7f7fu) | cntb) & 0x80808080u;
+        const uint32_t na = ~(((r0a & 0x7f7f7f7fu) + 0x7f7f7f7fu) | r0a) & 0x80808080u, nb = ~(((r0b & 0x7f7f7f7fu) + 0x7f7f7f7fu) | r0b) & 0x80808080u;
+        const bool missing = ((za & ~na) | (zb & ~nb)) != 0;
+        const bool bad_lane = ((viol & bit) != 0) || ((range & ~id_ok) != 0) || oob || missing;
+        const bool bad = __any_sync(0xffffffffu, bad_lane);
+        const bool all_same = __all_sync(0xffffffffu, same);
+        if (lane == 0) {
+            if (bad) p.partial[(size_t)c * p.L + l] = make_float4(CUDART_NAN_F, CUDART_NAN_F, CUDART_NAN_F, CUDART_NAN_F);
+            p.status[(size_t)c * p.L + l] = bad ? 1 : ((!all_same || p.force_general) ? 2 : 0);
         }
         __syncwarp();
     }
 }
 
-inline size_t place_check_smem_bytes(int E, int G) { return sizeof(uint32_t) * (size_t)kCheckWarps * (G > 32 ? 2 : 1) * E + (size_t)((E + 15) & ~15); }
+// The candidates place_check_kernel marked "valid, other replica counts than x0" (status 2): rebuild the rank masks and
+// score with the candidate's own r.  Same grid as the check; warps skip everything else.
+__global__ void __launch_bounds__(kCheckWarps * 32) place_own_r_kernel(const CheckParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int NS = p.G * p.sp, H = p.G > 32 ? 2 : 1;
+    uint32_t* mk_all = reinterpret_cast<uint32_t*>(smem_raw);
+    const int l = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    uint32_t* mk = mk_all + warp * H * kCheckE;
+    for (int i = lane; i < H * kCheckE; i += 32) mk[i] = 0u;
+    __syncwarp();
+    const int p_begin = blockIdx.x * p.chunk, p_end = min(p.P, p_begin + p.chunk);
+    for (int c = p_begin + warp; c < p_end; c += kCheckWarps) {
+        if (p.status[(size_t)c * p.L + l] != 2) continue;
+        const int16_t* row = p.cand + ((size_t)c * p.L + l) * NS;
+        for (int rr = 0; rr < H; ++rr) {
+            const int g = lane + rr * 32;
+            if (g < p.G)
+                for (int j = 0; j < p.sp; ++j) atomicOr(mk + rr * kCheckE + (uint16_t)row[g * p.sp + j], 1u << lane);
+        }
+        __syncwarp();
+        place_score_own_r(p, l, c, row, mk, lane);
+        __syncwarp();
+        for (int i = lane; i < H * kCheckE; i += 32) mk[i] = 0u;
+        __syncwarp();
+    }
+}
 
 struct FinalizeParams {
     int P, L, G;
