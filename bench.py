@@ -3,13 +3,15 @@
 
 A "step" is one pass of the whole hot path over one batch of synthetic input:
   gimbal_route_stats     a1-a5  router GEMM + gating + [L,S,E] histogram + window/EMA + load/pressure
-  gimbal_eval_placements a6     P candidate placements scored against the live profile
+  gimbal_eval_placements a6     P candidate placements validated and scored against the live profile
   gimbal_eval_moves      a7     the whole single-move neighbourhood of the current placement
 `value` = routed tokens/s = T / (device time of one step), inputs resident in HBM.
-`e2e`   = the same metric through the *_host C-ABI calls: hidden states, source offsets and the
-          candidates start in pinned HOST memory each step and the results are read back.
+`e2e`   = the same metric through the *_host C-ABI calls: hidden states, source offsets, the candidates and
+          the placements start in pinned HOST memory each step and the results are read back.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload v3] [--impl reference]
+    python bench.py --workload decode --episode     # BASELINE.json config 5 as it is stated: 2000 consecutive
+                                                    # steps from CUDA graphs, a re-score every 100 steps
 
 N > 1 (under torch.distributed.run): the path has no cross-GPU exchange (north_star: EP ranks
 and DP engines are logical partitions on one GPU), so every rank runs an independent replica
@@ -35,15 +37,27 @@ from workloads import gen, get_workload, scaled  # noqa: E402
 from workloads.configs import MODE_WINDOW  # noqa: E402
 
 METRIC = "routed tokens/s (stats path + placement scoring, whole hot path)"
-# dram__bytes_read + dram__bytes_write of router_gemm_kernel per token-layer at the V3 shape, from the committed
-# `ncu --set full` capture profiles/r1_ncu_k1_router_gemm.txt: (5.661509e9 + 3.763712e6) B over 65536 tokens x 6 layers
-# (algorithmic: 2*H = 14336 B).  The capture covers 6 of the 58 layers; traffic per launch scales it by T*L.
-# smsp__inst_executed.sum of place_score_fast_kernel<9,32,1,0> per (candidate, layer) at the V3 shape, from
-# profiles/r1_ncu_k4_k5_placement.txt (46,644,992 warp instructions for 4096 x 58 units): the kernel is issue-bound, so
-# its ALU roofline (148 SMs x 4 schedulers x 1 warp instruction per clock at the maximum SM clock)
-# is reported next to the HBM one.
-NCU_WARP_INSTR_PER_UNIT_K4_V3 = 46644992 / (4096 * 58)
-NCU_DRAM_BYTES_PER_TOKEN_LAYER_V3 = (5.661509e9 + 3.763712e6) / (65536 * 6)
+PROFILES = os.path.join(ROOT, "profiles")
+
+
+def _profile_metrics(name: str) -> dict:
+    """metric -> value of a committed ncu summary (profiles/<name>.csv: `metric,value,unit` rows written from the
+    `ncu --set full` capture named in profiles/<name>.md).  Empty when the file is missing."""
+    path = os.path.join(PROFILES, name + ".csv")
+    out = {}
+    if os.path.exists(path):
+        for line in open(path):
+            f = line.strip().split(",")
+            if len(f) >= 2 and not line.startswith("#"):
+                try:
+                    out[f[0]] = float(f[1])
+                except ValueError:
+                    pass
+    return out
+
+
+K1_PROFILE = "r2_ncu_k1_router_gemm"       # V3 shape, `--layers 6`: counters are per launch of 6 layers x 65536 tokens
+K4_PROFILE = "r2_ncu_k4_place_score"       # V3 shape, P = 4096, 58 layers
 
 
 def _peaks():
@@ -107,9 +121,9 @@ class ClockSampler:
 # --------------------------------------------------------------------------------------------
 # oracle timing (cpu_baseline / --impl reference)
 # --------------------------------------------------------------------------------------------
-def oracle_step_time(w, sample_tokens, sample_layers, sample_P, sample_moves, place_layers=None):
+def oracle_step_time(w, sample_tokens, sample_layers, sample_P, sample_moves, place_layers=None, single_thread=True):
     """Times the CPU oracle, as it stands, on a bounded sample of the workload and extrapolates
-    to one full step.  Returns (seconds per full step, description, threads)."""
+    to one full step.  Returns (seconds per full step, description, threads, rates)."""
     import oracle
     r = w.router
     ws = scaled(w, L=sample_layers, T=sample_tokens)
@@ -146,12 +160,34 @@ def oracle_step_time(w, sample_tokens, sample_layers, sample_P, sample_moves, pl
     moves_per_s = sample_moves / t_mv
     n_moves = r.L * w.NS * (w.NS - 1) // 2
     step_s = w.T * r.L / tok_layers_per_s + w.P * r.L / cand_layers_per_s + n_moves / moves_per_s
+    rates = dict(token_layers_per_s=tok_layers_per_s, candidate_layers_per_s=cand_layers_per_s, moves_per_s=moves_per_s)
+    threads = oracle.num_threads()
+    if single_thread and threads > 1:
+        # the same code on ONE thread, on a sixteenth of the sample
+        oracle.set_num_threads(1)
+        try:
+            nt, nl = max(64, sample_tokens // 16), min(sample_layers, 2)
+            t0 = time.perf_counter()
+            oracle.route_stats_layers(np.ascontiguousarray(hb[:nl, :nt]), wb[:nl], r, np.minimum(off, nt).astype(np.int32), slb[:nl],
+                                      None if sb is None else sb.numpy()[:nl], tier=1)
+            t1 = time.perf_counter() - t0
+            nP = max(4, sample_P // 16)
+            t0 = time.perf_counter()
+            oracle.objective_batch(cands[:nP], prev.numpy(), A_full, B_full, D, None, 1.0, G=w.G, sp=w.slots_per_rank)
+            t2 = time.perf_counter() - t0
+            nM = max(32, sample_moves // 16)
+            t0 = time.perf_counter()
+            oracle.move_deltas(prev.numpy(), prev.numpy(), moves[:nM], A_full, B_full, D, None, 1.0, G=w.G, sp=w.slots_per_rank)
+            t3 = time.perf_counter() - t0
+            rates["single_thread"] = dict(token_layers_per_s=nt * nl / t1, candidate_layers_per_s=nP * place_layers / t2,
+                                          moves_per_s=nM / t3)
+        finally:
+            oracle.set_num_threads(threads)
     desc = (f"oracle as it stands: a1-a5 on {sample_tokens} tokens x {sample_layers} layers ({t_stats:.1f}s, "
             f"{tok_layers_per_s:.0f} token-layers/s), a6 on {sample_P} candidates x {place_layers} layers ({t_obj:.1f}s, "
             f"{cand_layers_per_s:.0f} candidate-layers/s), a7 on {sample_moves} moves ({t_mv:.1f}s, {moves_per_s:.0f} moves/s); "
             f"extrapolated to one full step (T={w.T}, L={r.L}, P={w.P}, {n_moves} moves)")
-    return step_s, desc, oracle.num_threads(), dict(token_layers_per_s=tok_layers_per_s, candidate_layers_per_s=cand_layers_per_s,
-                                                     moves_per_s=moves_per_s)
+    return step_s, desc, threads, rates
 
 
 SAMPLES = {   # workload -> (tokens, layers, candidates, moves, placement layers) of the oracle sample (~10-30 s of CPU work)
@@ -165,6 +201,32 @@ def _sample(w, scale: float = 1.0):
     tok, lay, P, mv, pl = SAMPLES[w.name]
     tok, P, mv = max(256, int(tok * scale)), max(16, int(P * scale)), max(120, int(mv * scale))
     return min(tok, w.T), min(lay, w.router.L), min(P, w.P), mv, min(pl, w.router.L)
+
+
+def flip_rate(g, w, cfg, hidden, W, sb, slb, off, ws_r, n_tokens=16384, layers=(0,)):
+    """End-to-end top-k flip rate (north_star: "reported"): the fused GPU path's ids (bf16 inputs, fp32 accumulation in
+    TMEM) against the oracle run end to end from the same bytes (fp64 GEMM -> fp32 logits -> gating) on a row subset.
+    A flip = a token whose selected SET differs.  Returns dict(rate, token_layers)."""
+    import oracle
+    r = w.router
+    n = min(n_tokens, w.T)
+    flips = tot = 0
+    offn = np.minimum(off.cpu().numpy(), n).astype(np.int32)
+    off_n = torch.from_numpy(offn).to(hidden.device)
+    for l in layers:
+        st = g.StatsState(cfg, MODE_WINDOW, window_len=1, device=hidden.device)
+        ids = torch.empty(1, n, r.k, dtype=torch.int32, device=hidden.device)
+        g.route_stats(cfg, st, T=n, hidden=hidden[l:l + 1, :n].contiguous(), w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off_n,
+                      layer0=l, n_layers=1, topk_ids=ids, workspace=ws_r)
+        torch.cuda.synchronize()
+        hb = hidden[l, :n].cpu().contiguous().view(torch.int16).numpy().view(np.uint16)
+        wb = W[l].cpu().contiguous().view(torch.int16).numpy().view(np.uint16)
+        _, l32 = oracle.router_logits(hb, wb, slb[l].cpu().numpy(), offn)
+        eid, _ = oracle.gate(l32, r, None if sb is None else sb[l].cpu().numpy(), 1)
+        flips += int((np.sort(eid, 1) != np.sort(ids[0].cpu().numpy(), 1)).any(1).sum())
+        tot += n
+    return dict(rate=flips / tot, flipped=flips, token_layers=tot,
+                note="tokens whose top-k set differs between the fused GPU path and the oracle run end to end (fp64 GEMM) on the same bytes")
 
 
 # --------------------------------------------------------------------------------------------
@@ -191,7 +253,7 @@ def run_reference(args, w):
     times, desc, threads = [], "", 1
     scale = min(1.0, 8.0 / (args.warmup + args.steps))         # a full sample is ~15 s; keep the whole run near 2 minutes
     for i in range(args.warmup + args.steps):
-        s, desc, threads, _ = oracle_step_time(w, *_sample(w, scale))
+        s, desc, threads, _ = oracle_step_time(w, *_sample(w, scale), single_thread=False)
         if i >= args.warmup:
             times.append(s)
     step_s = sum(times) / len(times)
@@ -199,7 +261,9 @@ def run_reference(args, w):
     cb = dict(value=value, unit="routed tokens/s", cores=threads, kind="oracle", sample=desc)
     line = dict(impl="reference", metric=METRIC, value=value, unit="routed tokens/s", n_gpus=args.gpus, steps=args.steps,
                 warmup=args.warmup, ms_per_step=step_s * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
-                data="synthetic", config=_config(w, args), cpu_baseline=cb,
+                data="synthetic", config=_config(w, args), cpu_baseline=cb, extrapolated=True,
+                extrapolated_note="every step times the oracle on a bounded sample of the workload (cpu_baseline.sample) and "
+                                  "ms_per_step is that time scaled to one full step: K real steps would not end within minutes",
                 e2e=dict(value=value, unit="routed tokens/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0))
     print(json.dumps(line))
 
@@ -211,8 +275,35 @@ def _config(w, args):
                 parallelism="replicas only (no cross-GPU exchange on this path)",
                 l2="hidden states of one step (>> L2) stream through L2 between the placement kernels; an explicit 256 MiB flush runs "
                    "between timed steps, outside the timed events",
+                placements="default call: every candidate is validated exactly (place_check_kernel) and scored (place_score_kernel)",
                 outputs="A_step/B/pressure (a3-a5), out[P,5]+argmin (a6), delta[n,5]+best_per_layer (a7); top-k ids and weights "
                         + ("written" if getattr(args, "with_ids", False) else "not written"))
+
+
+def _setup(args, w, g, dev, rank):
+    """inputs resident in HBM + one un-timed stats step that gives the profile the placement side starts from"""
+    r = w.router
+    cfg = g.RouterCfg.from_workload(r)
+    x = dict(cfg=cfg)
+    x["hidden"] = gen.hidden_all(w, rank, dev)                      # [L,T,H] bf16, distinct per layer (and per rank)
+    x["W"] = gen.w_router(w, dev)
+    x["slb"] = gen.src_logit_bias(w, 0, dev)
+    x["sb"] = gen.select_bias(w, dev)
+    x["off"] = gen.src_offsets(w, 0, w.T, dev)
+    x["dp"] = gen.dp_of_rank(w, dev)
+    x["D"] = gen.comm_cost_D(w, "binary", dev)
+    x["st"] = g.StatsState(cfg, w.mode, window_len=max(w.window_len, 1), ema_decay=w.ema_decay, device=dev)
+    x["ws_r"] = torch.empty(g.route_stats_workspace_bytes(cfg, r.L, w.T), dtype=torch.uint8, device=dev)
+    x["pc"] = g.PlacementCfg(L=r.L, E=r.E, G=w.G, slots_per_rank=w.slots_per_rank, S=r.S,
+                             counts_dtype=g.COUNTS_I32 if w.mode == MODE_WINDOW else g.COUNTS_F32)
+    g.route_stats(cfg, x["st"], T=w.T, hidden=x["hidden"], w_router=x["W"], select_bias=x["sb"], src_logit_bias=x["slb"],
+                  src_offsets=x["off"], workspace=x["ws_r"])
+    torch.cuda.synchronize()
+    x["prev"] = gen.prev_placement(w, x["st"].B.cpu().numpy(), dev)
+    x["cands"] = gen.candidates(w, x["prev"], w.P, dev)
+    x["cur"] = x["cands"][min(2, w.P - 1)].contiguous()
+    x["ws_p"] = torch.empty(g.eval_placements_workspace_bytes(x["pc"], w.P), dtype=torch.uint8, device=dev)
+    return x
 
 
 def run_ours(args, w):
@@ -231,33 +322,16 @@ def run_ours(args, w):
         raise SystemExit("libgimbal.so missing: run __graft_entry__.build() -- there is no CPU fallback")
     peaks = _peaks()
     r = w.router
-    cfg = g.RouterCfg.from_workload(r)
     torch.manual_seed(1234 + rank)
-
-    # ---- inputs, resident in HBM -------------------------------------------------------------
-    hidden = gen.hidden_all(w, rank, dev)                      # [L,T,H] bf16, distinct per layer (and per rank)
-    W = gen.w_router(w, dev)
-    slb = gen.src_logit_bias(w, 0, dev)
-    sb = gen.select_bias(w, dev)
-    off = gen.src_offsets(w, 0, w.T, dev)
-    dp = gen.dp_of_rank(w, dev)
-    D = gen.comm_cost_D(w, "binary", dev)
-    st = g.StatsState(cfg, w.mode, window_len=max(w.window_len, 1), ema_decay=w.ema_decay, device=dev)
-    ws_r = torch.empty(g.route_stats_workspace_bytes(cfg, r.L, w.T), dtype=torch.uint8, device=dev)
-    pc = g.PlacementCfg(L=r.L, E=r.E, G=w.G, slots_per_rank=w.slots_per_rank, S=r.S,
-                        counts_dtype=g.COUNTS_I32 if w.mode == MODE_WINDOW else g.COUNTS_F32)
-    # one un-timed stats step gives the profile the placement side starts from
-    g.route_stats(cfg, st, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off, workspace=ws_r)
-    torch.cuda.synchronize()
-    prev = gen.prev_placement(w, st.B.cpu().numpy(), dev)
-    cands = gen.candidates(w, prev, w.P, dev)
-    cur = cands[min(2, w.P - 1)].contiguous()
+    x = _setup(args, w, g, dev, rank)
+    cfg, pc, st = x["cfg"], x["pc"], x["st"]
+    hidden, W, slb, sb, off, dp, D, prev, cands, cur, ws_r, ws_p = (x[k] for k in ("hidden", "W", "slb", "sb", "off", "dp", "D", "prev",
+                                                                                  "cands", "cur", "ws_r", "ws_p"))
     n_moves = r.L * w.NS * (w.NS - 1) // 2
     out = torch.empty(w.P, 5, device=dev)
     argmin = torch.zeros(1, dtype=torch.int32, device=dev)
     delta = torch.empty(n_moves, 5, device=dev)
     best = torch.zeros(r.L, dtype=torch.int32, device=dev)
-    ws_p = torch.empty(g.eval_placements_workspace_bytes(pc, w.P), dtype=torch.uint8, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     # profile the placement side reads: this step's counts (window mode) or the EMA state
     A_live, B_live = (st.A_step if w.mode == MODE_WINDOW else st.A_ema), st.B
@@ -279,6 +353,13 @@ def run_ours(args, w):
     for _ in range(4):
         g.greedy_place(pc, A_live, B_live, D, prev, greedy_out)
         greedy_ms.append(g.kernel_elapsed_ms(g.KERNEL_GREEDY))
+    # a6 with GIMBAL_PLACE_TRUSTED (not part of the timed step): the scoring kernel alone, after an L2 flush
+    pc_t = g.PlacementCfg(**{**pc.__dict__, "flags": g.PLACE_TRUSTED})
+    trusted_ms = []
+    for _ in range(4):
+        flush.zero_()
+        g.eval_placements(pc_t, cands, A_live, B_live, D, prev, out, workspace=ws_p)
+        trusted_ms.append(g.kernel_elapsed_ms(g.KERNEL_SCORE))
     # K2 (not part of the timed step): the standalone gating + histogram kernel on given logits (LOGITS_IN), the
     # kernel whose roofline is plain HBM: 4*E bytes read per token-layer.  Logits of `nl` layers (> L2) are
     # written once by the fused kernel's LOGITS_OUT mode, then re-read from HBM.
@@ -306,7 +387,7 @@ def run_ours(args, w):
     torch.cuda.synchronize()
     sampler.start()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    k_router, k_score, k_moves = [], [], []
+    k_router, k_score, k_check, k_moves = [], [], [], []
     launches0 = g.launch_count()
     for s0, s1 in ev:
         flush.zero_()
@@ -315,6 +396,7 @@ def run_ours(args, w):
         s1.record()
         k_router.append(g.kernel_elapsed_ms(g.KERNEL_ROUTER))
         k_score.append(g.kernel_elapsed_ms(g.KERNEL_SCORE))
+        k_check.append(g.kernel_elapsed_ms(g.KERNEL_CHECK))
         k_moves.append(g.kernel_elapsed_ms(g.KERNEL_MOVES))
     torch.cuda.synchronize()
     launches = g.launch_count() - launches0
@@ -330,11 +412,17 @@ def run_ours(args, w):
     # ---- roofline of the dominant kernel (router GEMM with fused gating + histogram) -------------------
     gemm_ms = statistics.mean(k_router)
     flops = 2.0 * w.T * r.H * r.E * r.L                       # 2*H*E flop per token-layer
-    bytes_hidden = 2.0 * w.T * r.H * r.L                      # 2*H bytes per token-layer, read exactly once
+    bytes_hidden = 2.0 * w.T * r.H * r.L                      # 2*H bytes of hidden per token-layer, read exactly once
     tf = flops / (gemm_ms * 1e-3) / 1e12
+    k1p = _profile_metrics(K1_PROFILE)
+    traffic = None
+    if w.name == "v3" and "dram__bytes_read.sum" in k1p:
+        # the committed capture covers `profile_layers` of the 58 layers; one launch of the bench covers all of them
+        per_tl = (k1p["dram__bytes_read.sum"] + k1p.get("dram__bytes_write.sum", 0.0)) / (65536 * k1p.get("profile_layers", 6))
+        traffic = per_tl * w.T * r.L
     roofline = dict(bound="tensor", achieved=tf, peak=peaks["tf_sustained"], unit="TFLOP/s", frac=tf / peaks["tf_sustained"],
-                    traffic=(NCU_DRAM_BYTES_PER_TOKEN_LAYER_V3 * w.T * r.L if w.name == "v3" else None),
-                    traffic_unit="bytes per launch (ncu dram read+write per token-layer x T x L, profiles/r1_ncu_k1_router_gemm.txt)",
+                    traffic=traffic,
+                    traffic_unit=f"bytes per launch: (dram__bytes_read.sum + dram__bytes_write.sum) per token-layer of profiles/{K1_PROFILE}.csv x T x L",
                     algorithmic_bytes=bytes_hidden, algorithmic_flops=flops,
                     kernel="router_gemm_kernel (a1 + fused a2/a3)", ms=gemm_ms, share_of_step=gemm_ms / ms_per_step,
                     peak_source=peaks["source"] + ", sustained bf16 (kernel timed inside a long step)",
@@ -342,24 +430,39 @@ def run_ours(args, w):
                     hbm=dict(achieved=bytes_hidden / (gemm_ms * 1e-3) / 1e9, peak=peaks["hbm"], unit="GB/s",
                              frac=bytes_hidden / (gemm_ms * 1e-3) / 1e9 / peaks["hbm"],
                              note="same kernel against the HBM roofline: 2*H bytes of hidden per token-layer"))
-    score_ms, moves_ms = statistics.mean(k_score), statistics.mean(k_moves)
+    score_ms, check_ms, moves_ms = statistics.mean(k_score), statistics.mean(k_check), statistics.mean(k_moves)
     cand_bytes = 2.0 * r.L * w.NS * w.P
     gate_bytes = 4.0 * r.E * w.T * nl
+    k4p = _profile_metrics(K4_PROFILE)
+    sm_max_ghz = (clocks.get("sm_max_mhz") or 1965.0) / 1e3
+    smem_peak = 148 * 128 * sm_max_ghz                        # GB/s: 128 B per clock per SM of shared-memory / L1 data pipe
+    smem = None
+    if "l1tex__data_pipe_lsu_wavefronts.sum" in k4p and w.name == "v3":
+        wave_bytes = k4p["l1tex__data_pipe_lsu_wavefronts.sum"] * 128.0 * (w.P * r.L / k4p.get("units", w.P * r.L))
+        smem = dict(achieved=wave_bytes / (score_ms * 1e-3) / 1e9, peak=smem_peak, unit="GB/s", frac=wave_bytes / (score_ms * 1e-3) / 1e9 / smem_peak,
+                    note=f"the kernel's real bound (DESIGN.md section 6): L1 data-pipe wavefronts x 128 B from profiles/{K4_PROFILE}.csv "
+                         "against 148 SMs x 128 B/clk at the maximum SM clock")
+    t_ms = min(trusted_ms[1:])
     extra = dict(
         gate_hist_kernel=dict(ms=min(gate_ms[1:]), layers=nl, bound="hbm", achieved=gate_bytes / (min(gate_ms[1:]) * 1e-3) / 1e9,
                               peak=peaks["hbm"], unit="GB/s", frac=gate_bytes / (min(gate_ms[1:]) * 1e-3) / 1e9 / peaks["hbm"],
                               algorithmic_bytes="4*E per token-layer (logits read once; counts only)",
                               note="a2+a3 standalone on given logits (LOGITS_IN); outside the timed step"),
         greedy_place_kernel=dict(ms=min(greedy_ms[1:]), layers=r.L, note="NEXT-1, PAPER.md:260-268; outside the timed step"),
-        placements_per_s=world * w.P / (score_ms * 1e-3), moves_per_s=world * n_moves / (moves_ms * 1e-3),
+        placements_per_s=world * w.P / ((score_ms + check_ms) * 1e-3),
+        placements_per_s_note="default call inside the timed step: exact validation + scoring (place_check_kernel + place_score_kernel)",
+        placements_per_s_trusted=world * w.P / (t_ms * 1e-3),
+        moves_per_s=world * n_moves / (moves_ms * 1e-3),
         place_score_kernel=dict(ms=score_ms, bound="hbm", achieved=cand_bytes / (score_ms * 1e-3) / 1e9, peak=peaks["hbm"],
                                 unit="GB/s", frac=cand_bytes / (score_ms * 1e-3) / 1e9 / peaks["hbm"],
                                 algorithmic_bytes="2*L*NS per candidate",
-                                alu=(dict(achieved=NCU_WARP_INSTR_PER_UNIT_K4_V3 * w.P * r.L / (score_ms * 1e-3) / 1e9,
-                                          peak=148 * 4 * 1.965, unit="G warp-instructions/s",
-                                          frac=NCU_WARP_INSTR_PER_UNIT_K4_V3 * w.P * r.L / (score_ms * 1e-3) / 1e9 / (148 * 4 * 1.965),
-                                          note="issue-bound kernel: instructions per unit from the committed ncu capture; peak at "
-                                               "the maximum SM clock (1965 MHz)") if w.name == "v3" else None)),
+                                alone=dict(ms=t_ms, achieved=cand_bytes / (t_ms * 1e-3) / 1e9, frac=cand_bytes / (t_ms * 1e-3) / 1e9 / peaks["hbm"],
+                                           note="GIMBAL_PLACE_TRUSTED call outside the timed step, after an L2 flush (clocks not held "
+                                                "down by the router GEMM)"),
+                                smem=smem),
+        place_check_kernel=dict(ms=check_ms, bound="hbm", achieved=cand_bytes / (check_ms * 1e-3) / 1e9, peak=peaks["hbm"], unit="GB/s",
+                                frac=cand_bytes / (check_ms * 1e-3) / 1e9 / peaks["hbm"],
+                                note="exact validation (bit matrix in shared memory, one atomicOr per slot); reads the candidates a second time"),
         move_delta_kernel=dict(ms=moves_ms, bound="hbm", achieved=20.0 * n_moves / (moves_ms * 1e-3) / 1e9, peak=peaks["hbm"],
                                unit="GB/s", frac=20.0 * n_moves / (moves_ms * 1e-3) / 1e9 / peaks["hbm"],
                                algorithmic_bytes="20 B written per move (implicit neighbourhood)"))
@@ -376,7 +479,7 @@ def run_ours(args, w):
                    error="pinned host copies of the hidden states of all ranks do not fit host RAM")
     else:
         try:
-            e2e = run_e2e(g, w, cfg, pc, st, hidden, off, cands, W, sb, slb, cur, dp, D, prev, out, delta, best, ws_r, ws_p, args, dev)
+            e2e = run_e2e(g, w, cfg, pc, st, hidden, off, cands, W, sb, slb, cur, dp, D, prev, delta, ws_r, ws_p, args, dev)
         except Exception as ex:  # report, never fake
             e2e = dict(value=None, unit="routed tokens/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0, error=str(ex)[:300])
     if dist and fits:
@@ -384,20 +487,21 @@ def run_ours(args, w):
         e2e["value"] = replica_value(w.T, world, e2e["ms_per_step"])
 
     if rank == 0:
-        cpu = None
+        cpu = flips = None
         if world == 1 and not args.no_cpu_baseline:
             s, desc, threads, rates = oracle_step_time(w, *_sample(w))
             cpu = dict(value=w.T / s, unit="routed tokens/s", cores=threads, kind="oracle", sample=desc, **rates)
+            flips = flip_rate(g, w, cfg, hidden, W, sb, slb, off, ws_r, layers=(0, r.L - 1) if r.L > 1 else (0,))
         line = dict(metric=METRIC, value=value, unit="routed tokens/s", n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
                     ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16",
                     data="synthetic", config=_config(w, args), clocks=clocks, e2e=e2e, gpu_launches=int(launches),
-                    roofline=roofline, cpu_baseline=cpu, token_layers_per_s=value * r.L, **extra)
+                    roofline=roofline, cpu_baseline=cpu, topk_flip_rate=flips, token_layers_per_s=value * r.L, **extra)
         print(json.dumps(line))
     if dist:
         td.destroy_process_group()
 
 
-def run_e2e(g, w, cfg, pc, st, hidden, off, cands, W, sb, slb, cur, dp, D, prev, out, delta, best, ws_r, ws_p, args, dev):
+def run_e2e(g, w, cfg, pc, st, hidden, off, cands, W, sb, slb, cur, dp, D, prev, delta, ws_r, ws_p, args, dev):
     r = w.router
     layer_bytes = w.T * r.H * 2
     hidden_host = torch.empty(hidden.shape, dtype=hidden.dtype, pin_memory=True)
@@ -405,32 +509,34 @@ def run_e2e(g, w, cfg, pc, st, hidden, off, cands, W, sb, slb, cur, dp, D, prev,
     off_host = off.cpu().pin_memory()
     cands_host = torch.empty(cands.shape, dtype=cands.dtype, pin_memory=True)
     cands_host.copy_(cands)
+    cur_host, prev_host = cur.cpu().pin_memory(), prev.cpu().pin_memory()
     n_stage = 3
     stage = torch.empty(n_stage * layer_bytes, dtype=torch.uint8, device=dev)
     off_stage = torch.empty_like(off)
     cand_stage = torch.empty_like(cands)
+    out_stage = torch.empty(w.P, 5, device=dev)
+    cur_stage, prev_stage = torch.empty_like(cur), torch.empty_like(prev)
+    best_stage = torch.zeros(r.L, dtype=torch.int32, device=dev)
     res_bytes = g.route_stats_result_bytes(cfg)
     result_host = torch.empty(res_bytes, dtype=torch.uint8, pin_memory=True)
     out_host = torch.empty(w.P, 5, dtype=torch.float32, pin_memory=True)
     argmin_host = torch.zeros(1, dtype=torch.int32, pin_memory=True)
     best_host = torch.zeros(r.L, dtype=torch.int32, pin_memory=True)
-    torch.cuda.synchronize()
-
     ctx = g.HostCtx()
+    torch.cuda.synchronize()
 
     def step():
         g.route_stats_host(ctx, cfg, st, T=w.T, hidden_host=hidden_host, src_offsets_host=off_host, hidden_stage=stage,
                            src_offsets_stage=off_stage, w_router=W, select_bias=sb, src_logit_bias=slb, cur_placement=cur,
                            dp_of_rank=dp, G=w.G, slots_per_rank=w.slots_per_rank, result_host=result_host, workspace=ws_r)
         A_live = st.A_step if w.mode == MODE_WINDOW else st.A_ema
-        g.eval_placements_host(pc, cands_host, cand_stage, out, A_live, st.B, D, prev, out_host, argmin_host=argmin_host,
+        g.eval_placements_host(pc, cands_host, cand_stage, out_stage, A_live, st.B, D, prev, out_host, argmin_host=argmin_host,
                                workspace=ws_p)
-        g.eval_moves(pc, cur, prev, A_live, st.B, D, delta, best_per_layer=best, workspace=ws_p)
-        best_host.copy_(best, non_blocking=True)
-        torch.cuda.synchronize()
+        g.eval_moves_host(pc, cur_host, prev_host, cur_stage, prev_stage, A_live, st.B, D, delta, best_stage=best_stage,
+                          best_host=best_host, workspace=ws_p)
 
-    step()                                                     # warm-up (stream / event creation, page touching)
-    n = max(1, min(args.steps, 3))
+    step()                                                     # warm-up (page touching)
+    n = max(1, args.steps)
     t0 = time.perf_counter()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
@@ -440,31 +546,175 @@ def run_e2e(g, w, cfg, pc, st, hidden, off, cands, W, sb, slb, cur, dp, D, prev,
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / n
     wall_ms = (time.perf_counter() - t0) * 1e3 / n
-    h2d = hidden_host.numel() * 2 + off_host.numel() * 4 + cands_host.numel() * 2
+    ctx.close()
+    h2d = hidden_host.numel() * 2 + off_host.numel() * 4 + cands_host.numel() * 2 + cur_host.numel() * 2 + prev_host.numel() * 2
     d2h = res_bytes + out_host.numel() * 4 + 4 + best_host.numel() * 4
     return dict(value=w.T / (ms * 1e-3), unit="routed tokens/s", h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                 ms_per_step=ms, wall_ms_per_step=wall_ms, steps=n,
-                note="gimbal_route_stats_host + gimbal_eval_placements_host + gimbal_eval_moves; pinned host buffers; "
-                     "H2D of hidden overlaps the kernels layer by layer; bounded by the host link")
+                note="gimbal_route_stats_host + gimbal_eval_placements_host + gimbal_eval_moves_host; pinned host buffers; H2D of "
+                     "hidden overlaps the kernels layer by layer; the 20-byte-per-move delta array of the whole neighbourhood "
+                     f"({delta.numel() * 4} B) stays on the device (delta_host = NULL), best_per_layer is read back; bounded by the host link")
+
+
+# --------------------------------------------------------------------------------------------
+# decode-streaming episode (BASELINE.json config 5): consecutive steps replayed from CUDA graphs
+# --------------------------------------------------------------------------------------------
+def run_episode(args, w):
+    """K = --steps consecutive decode steps (default 2000): every step runs gimbal_route_stats (EMA update each step) on its
+    own hidden states -- a ring of `--ring` step buffers, far larger than L2 --, every `rescore_every`-th step also re-scores
+    the P candidates.  One CUDA graph holds `rescore_every` steps and is replayed K / rescore_every times; device time of the
+    replays by CUDA events.  `value` = T * K / time."""
+    import paper_2606_15177_b200 as g
+    assert int(os.environ.get("WORLD_SIZE", "1")) == 1, "the episode mode is a single-GPU measurement"
+    torch.cuda.set_device(0)
+    dev = "cuda:0"
+    peaks = _peaks()
+    r = w.router
+    cfg = g.RouterCfg.from_workload(r)
+    per = max(1, w.rescore_every)
+    K = args.steps if args.steps_given else w.steps
+    K = max(per, (K // per) * per)
+    ring = args.ring
+    hidden = torch.empty(ring, r.L, w.T, r.H, dtype=torch.bfloat16, device=dev)
+    for s in range(ring):
+        hidden[s] = gen.hidden_all(w, s, dev)
+    W = gen.w_router(w, dev); slb = gen.src_logit_bias(w, 0, dev); sb = gen.select_bias(w, dev)
+    off = gen.src_offsets(w, 0, w.T, dev); dp = gen.dp_of_rank(w, dev); D = gen.comm_cost_D(w, "binary", dev)
+    st = g.StatsState(cfg, w.mode, window_len=max(w.window_len, 1), ema_decay=w.ema_decay, device=dev)
+    ws_r = torch.empty(g.route_stats_workspace_bytes(cfg, r.L, w.T), dtype=torch.uint8, device=dev)
+    pc = g.PlacementCfg(L=r.L, E=r.E, G=w.G, slots_per_rank=w.slots_per_rank, S=r.S, counts_dtype=g.COUNTS_F32)
+    g.route_stats(cfg, st, T=w.T, hidden=hidden[0], w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off, workspace=ws_r)
+    torch.cuda.synchronize()
+    prev = gen.prev_placement(w, st.B.cpu().numpy(), dev)
+    cands = gen.candidates(w, prev, w.P, dev)
+    ws_p = torch.empty(g.eval_placements_workspace_bytes(pc, w.P), dtype=torch.uint8, device=dev)
+    out = torch.empty(w.P, 5, device=dev); argmin = torch.zeros(1, dtype=torch.int32, device=dev)
+
+    def one(i, stream=None):
+        g.route_stats(cfg, st, T=w.T, hidden=hidden[i % ring], w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off,
+                      cur_placement=prev, dp_of_rank=dp, G=w.G, slots_per_rank=w.slots_per_rank, workspace=ws_r, stream=stream)
+
+    def rescore(stream=None):
+        g.eval_placements(pc, cands, st.A_ema, st.B, D, prev, out, argmin=argmin, workspace=ws_p, stream=stream)
+
+    # per-kernel times of one eager step (events around the kernels; never while capturing)
+    g.kernel_timing(True)
+    k1, ksc, kck = [], [], []
+    for i in range(8):
+        one(i); k1.append(g.kernel_elapsed_ms(g.KERNEL_ROUTER))
+    for _ in range(3):
+        rescore(); ksc.append(g.kernel_elapsed_ms(g.KERNEL_SCORE)); kck.append(g.kernel_elapsed_ms(g.KERNEL_CHECK))
+    g.kernel_timing(False)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    launches0 = g.launch_count()
+    with torch.cuda.graph(graph, stream=side):
+        for i in range(per):
+            one(i, side)
+        rescore(side)
+    launches_per_graph = g.launch_count() - launches0
+    for _ in range(max(args.warmup, 3)):
+        graph.replay()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(K // per):
+        graph.replay()
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    ms_per_step = ms / K
+    value = w.T * K / (ms * 1e-3)
+    k1_ms = statistics.median(k1[2:])
+    step_bytes = 2.0 * r.L * (w.T * r.H + r.E * r.H)            # hidden + W_router of every layer, each read once per step
+    roofline = dict(bound="hbm", achieved=step_bytes / (k1_ms * 1e-3) / 1e9, peak=peaks["hbm"], unit="GB/s",
+                    frac=step_bytes / (k1_ms * 1e-3) / 1e9 / peaks["hbm"], traffic=None,
+                    kernel="router_gemm_kernel (a1 + fused a2/a3), one 256-token tile per layer", ms=k1_ms,
+                    algorithmic_bytes=step_bytes, share_of_step=k1_ms / ms_per_step,
+                    note="decode regime: one tile per CTA pair, the GEMM is bound by streaming hidden and W_router once")
+    bound_lo, bound_hi = 3.6e6, 3.9e6                           # SURVEY.md section 8d: unfused / fused traffic at HBM peak, before launch overhead
+    cand_bytes = 2.0 * r.L * w.NS * w.P
+    # e2e: the same episode with the step's hidden states coming from pinned host memory
+    n_e2e = min(K, 2 * per)
+    hidden_host = torch.empty(hidden[0].shape, dtype=hidden.dtype, pin_memory=True); hidden_host.copy_(hidden[0])
+    off_host = off.cpu().pin_memory(); cands_host = torch.empty(cands.shape, dtype=cands.dtype, pin_memory=True); cands_host.copy_(cands)
+    stage = torch.empty(3 * w.T * r.H * 2, dtype=torch.uint8, device=dev); off_stage = torch.empty_like(off)
+    cand_stage = torch.empty_like(cands); out_stage = torch.empty(w.P, 5, device=dev)
+    result_host = torch.empty(g.route_stats_result_bytes(cfg), dtype=torch.uint8, pin_memory=True)
+    out_host = torch.empty(w.P, 5, pin_memory=True); am_host = torch.zeros(1, dtype=torch.int32, pin_memory=True)
+    ctx = g.HostCtx()
+
+    def host_step(i):
+        g.route_stats_host(ctx, cfg, st, T=w.T, hidden_host=hidden_host, src_offsets_host=off_host, hidden_stage=stage,
+                           src_offsets_stage=off_stage, w_router=W, select_bias=sb, src_logit_bias=slb, cur_placement=prev, dp_of_rank=dp,
+                           G=w.G, slots_per_rank=w.slots_per_rank, result_host=result_host, workspace=ws_r)
+        if (i + 1) % per == 0:
+            g.eval_placements_host(pc, cands_host, cand_stage, out_stage, st.A_ema, st.B, D, prev, out_host, argmin_host=am_host, workspace=ws_p)
+
+    host_step(0)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for i in range(n_e2e):
+        host_step(i)
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / n_e2e
+    ctx.close()
+    h2d = hidden_host.numel() * 2 + off_host.numel() * 4 + cands_host.numel() * 2 / per
+    d2h = result_host.numel() + (out_host.numel() * 4 + 4) / per
+    line = dict(metric="routed tokens/s (decode-streaming episode: stats path every step, placement re-score every "
+                       f"{per} steps)", value=value, unit="routed tokens/s", n_gpus=1, steps=K, warmup=max(args.warmup, 3) * per,
+                ms_per_step=ms_per_step, steps_per_s=1e3 / ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="bf16", data="synthetic",
+                config=dict(workload=f"decode episode: L={r.L} H={r.H} E={r.E} top-{r.k} S={r.S} T={w.T}/step x {K} consecutive steps, EMA "
+                                     f"{w.ema_decay} every step; G={w.G}x{w.slots_per_rank} slots, P={w.P} candidates re-scored every {per} steps",
+                            launch=f"one CUDA graph of {per} steps + 1 re-score ({launches_per_graph} kernels), replayed {K // per} times",
+                            l2=f"ring of {ring} steps of hidden states ({hidden.numel() * 2 / 1e9:.1f} GB) + 213 MB of router weights cycle "
+                               "through the 126 MB L2: every step's inputs come from HBM",
+                            parallelism="single GPU"),
+                clocks=clocks, gpu_launches=int(launches_per_graph * (K // per)),
+                e2e=dict(value=w.T / (e2e_ms * 1e-3), unit="routed tokens/s", ms_per_step=e2e_ms, steps=n_e2e,
+                         h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
+                         note="gimbal_route_stats_host every step (+ gimbal_eval_placements_host every re-score), wall clock"),
+                roofline=roofline, cpu_baseline=None,
+                bound_tokens_per_s=dict(lo=bound_lo, hi=bound_hi, frac_of_lo=value / bound_lo,
+                                        note="SURVEY.md section 8d: 3.6 M (unfused) - 3.9 M (fused) tokens/s at HBM peak, before launch overhead"),
+                rescore=dict(score_ms=statistics.median(ksc), check_ms=statistics.median(kck),
+                             place_score_frac_hbm=cand_bytes / (statistics.median(ksc) * 1e-3) / 1e9 / peaks["hbm"],
+                             amortised_ms_per_step=(statistics.median(ksc) + statistics.median(kck)) / per))
+    print(json.dumps(line))
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="v3", choices=["tiny", "v2lite", "qwen3", "v3", "decode"])
+    ap.add_argument("--episode", action="store_true", help="decode workload: the 2000-step episode from CUDA graphs (BASELINE.json config 5)")
+    ap.add_argument("--ring", type=int, default=32, help="--episode: step buffers of hidden states that the steps cycle through")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--with-ids", action="store_true", help="also write top-k ids and weights (a2 outputs) inside the timed step")
     ap.add_argument("--layers", type=int, default=0, help="profiling only: run the first N MoE layers (named in config.workload)")
     args = ap.parse_args()
+    args.steps_given = args.steps is not None
+    if args.steps is None:
+        args.steps = 20
     w = get_workload(args.workload)
     if args.layers > 0:
         w = scaled(w, L=args.layers)
     if args.impl == "reference":
         run_reference(args, w)
+    elif args.episode:
+        if w.rescore_every <= 0:
+            raise SystemExit("--episode is defined for the decode workload (BASELINE.json config 5)")
+        run_episode(args, w)
     else:
         run_ours(args, w)
 

@@ -59,6 +59,11 @@ def num_threads() -> int:
     return int(lib().oracle_num_threads())
 
 
+def set_num_threads(n: int) -> None:
+    """threads of the OpenMP loops (bench.py's single-thread rate); results do not depend on it"""
+    lib().oracle_set_num_threads(C.c_int(int(n)))
+
+
 def _p(a, ct):
     return a.ctypes.data_as(C.POINTER(ct)) if a is not None else None
 

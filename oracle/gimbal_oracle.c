@@ -731,6 +731,9 @@ void oracle_refine(int16_t *cur /*[L,NS] inout*/, const int16_t *prev, const dou
 #ifdef _OPENMP
 #include <omp.h>
 int oracle_num_threads(void) { return omp_get_max_threads(); }
+/* bench.py times the same code on one thread as well; no arithmetic depends on it */
+void oracle_set_num_threads(int n) { if (n > 0) omp_set_num_threads(n); }
 #else
 int oracle_num_threads(void) { return 1; }
+void oracle_set_num_threads(int n) { (void)n; }
 #endif

@@ -164,6 +164,7 @@ static size_t place_ws_carve(const gimbal_placement_cfg* c, int P, void* ws, Pla
     w.mp.slotC = cv.take<float>(NSl * c->G);
     w.mp.slotM = cv.take<float>(NSl * c->G);
     w.mp.slot_w = cv.take<double>(NSl);
+    w.mp.slot_u = cv.take<double>(NSl);
     w.mp.slot_cm = cv.take<uint64_t>(NSl);
     w.mp.slot_eg = cv.take<int2>(NSl);
     if (out) *out = w;
@@ -664,10 +665,18 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
         int lg = 0;
         while ((1 << lg) < cfg->G) ++lg;
         ap.lgG = lg;
-        // a warp task = the row pair {a, NS-2-a} (NS-1 moves); 16 tasks (~4600 moves at NS = 288) per block
+        // a warp task = the row pair {a, NS-2-a} (NS-1 moves).  One balanced wave: as many blocks per layer as give every SM
+        // its three resident blocks' worth (each block stages the layer's rows once), at least one task per warp
         const int n_tasks = (int)(NS / 2);
-        ap.tasks_per_block = 2 * (kMoveAllThreads / 32);
-        const int bpl = (n_tasks + ap.tasks_per_block - 1) / ap.tasks_per_block;
+        const size_t smem_all = move_all_smem_bytes((int)NS, cfg->G, M != nullptr);
+        int per_sm = (int)((kSmemLimit - 1024) / (smem_all + 1024));
+        per_sm = per_sm > 4 ? 4 : (per_sm < 1 ? 1 : per_sm);
+        int bpl = per_sm * device_info().sms / cfg->L;
+        const int max_bpl = (n_tasks + kMoveAllThreads / 32 - 1) / (kMoveAllThreads / 32);
+        if (bpl > max_bpl) bpl = max_bpl;
+        if (bpl < 1) bpl = 1;
+        ap.tasks_per_block = (n_tasks + bpl - 1) / bpl;
+        bpl = (n_tasks + ap.tasks_per_block - 1) / ap.tasks_per_block;
         {
             MoveSlotsParams sl{};
             sl.L = cfg->L; sl.E = cfg->E; sl.G = cfg->G; sl.sp = cfg->slots_per_rank; sl.lgG = lg; sl.has_M = ap.has_M;
@@ -675,7 +684,7 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
             move_slots_kernel<<<dim3((unsigned)((NS * cfg->G + 255) / 256), cfg->L), 256, 0, stream>>>(sl);
             LAUNCH_CHECK("move_slots_kernel");
         }
-        const size_t smem = move_all_smem_bytes((int)NS, cfg->G, ap.has_M);
+        const size_t smem = smem_all;
         auto kern = ap.has_M ? move_all_kernel<true> : move_all_kernel<false>;
         CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         ktime_begin(GIMBAL_KERNEL_MOVES, stream);

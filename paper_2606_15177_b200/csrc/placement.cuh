@@ -702,6 +702,7 @@ struct MovePrep {
     float* slotC;       // [L][NS][G]  c (sign = x0 hosts it) of the slot's expert on every rank
     float* slotM;       // [L][NS][G]  M of the slot's expert on every rank (M table only)
     double* slot_w;     // [L][NS]     load share of the slot's expert
+    double* slot_u;     // [L][NS]     load of the slot's rank minus that share
     uint64_t* slot_cm;  // [L][NS]     ranks hosting the slot's expert in cur
     int2* slot_eg;      // [L][NS]     {expert, rank} of the slot
 };
@@ -847,17 +848,23 @@ __global__ void __launch_bounds__(256) move_delta_kernel(const MoveParams p) {
 }
 
 // The whole neighbourhood of `cur` in canonical order (l, a < b): one block per (layer, range of
-// pair indices).  The layer's per-slot rows -- communication cost of the slot's expert on every
-// rank (sign = x0 hosts it there), its load share, the ranks hosting it -- are staged in shared
-// memory (pitch G+1: lanes walk b, so rows fall in distinct banks); a warp's 32 results are
-// staged too and leave as five fully coalesced 128-byte stores.
+// row pairs).  The layer's per-slot rows -- communication cost of the slot's expert on every rank (sign =
+// x0 hosts it there), its load share w, U = L[rank] - w, the ranks hosting it -- are staged in shared
+// memory (pitch G+1: lanes walk b, so rows fall in distinct banks); a warp's 32 results are staged too
+// and leave as five fully coalesced 128-byte stores.
+//   dC_load = 2 (w2 - w1) (U1 - U2)                 (= 2 d (L1 - L2) + 2 d^2 with d = w2 - w1; double)
+//   dC_comm = (c[e1,g2] - c[e1,g1]) + (c[e2,g1] - c[e2,g2])
+//   dC_mig  = 2 M (n11 + n22 - n12 - n21), n = "x0 hosts the cell" (scalar M; with a table the four M's with those signs)
+//   dmaxload from the layer's three largest rank loads, in fp32 (compared relative to the largest load)
+// Same rank or same expert: zeros.  A second copy of an expert on a rank: NaN.  No data-dependent branch.
 constexpr int kMoveAllThreads = 256;
 
 __host__ __device__ inline size_t move_all_smem_bytes(int NS, int G, int has_M) {
     size_t b = sizeof(float) * (size_t)NS * (G + 1) * (has_M ? 2 : 1);   // Cs (+ Ms)
     b = (b + 15) & ~size_t(15);
-    b += sizeof(double) * NS + sizeof(unsigned long long) * NS + sizeof(int2) * NS;   // w, cmask, (e, g)
-    b += sizeof(double) * 64;                                                       // Lg
+    b += (sizeof(double) * 2 + sizeof(unsigned long long) + sizeof(uint32_t)) * (size_t)NS;   // w, U, cmask, (e | g << 16)
+    b = (b + 15) & ~size_t(15);
+    b += sizeof(float) * 64;                                                        // rank loads (fp32)
     b += sizeof(float) * (kMoveAllThreads / 32) * 160;                              // output staging
     b += sizeof(unsigned long long) * (kMoveAllThreads / 32);                       // block argmin
     return b;
@@ -882,7 +889,9 @@ __global__ void __launch_bounds__(256) move_slots_kernel(const MoveSlotsParams p
     p.mp.slotC[dst] = p.t.wc[src].y;
     if (p.has_M) p.mp.slotM[dst] = p.t.m[src];
     if (g == 0) {
-        p.mp.slot_w[(size_t)l * NS + j] = p.t.w_e[(size_t)l * p.E + e];
+        const double w = p.t.w_e[(size_t)l * p.E + e];
+        p.mp.slot_w[(size_t)l * NS + j] = w;
+        p.mp.slot_u[(size_t)l * NS + j] = p.mp.Lg[(size_t)l * p.G + j / p.sp] - w;
         p.mp.slot_cm[(size_t)l * NS + j] = p.mp.cmask[(size_t)l * p.E + e];
         p.mp.slot_eg[(size_t)l * NS + j] = make_int2(e, j / p.sp);
     }
@@ -905,29 +914,33 @@ struct MoveAllParams {
 // depends on a (expert, rank, load, its table row) is warp-uniform, and the results of 32
 // consecutive b are contiguous in `delta`.
 template <bool kHasM>
-__global__ void __launch_bounds__(kMoveAllThreads) move_all_kernel(const MoveAllParams p) {
+__global__ void __launch_bounds__(kMoveAllThreads, 4) move_all_kernel(const MoveAllParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int NS = p.G * p.sp, GP = place_gp(p.G), PITCH = p.G + 1;
+    const int NS = p.G * p.sp, PITCH = p.G + 1;
     const int l = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     float* Cs = reinterpret_cast<float*>(smem_raw);
     float* Ms = Cs + (size_t)NS * PITCH;
     size_t off = sizeof(float) * (size_t)NS * PITCH * (kHasM ? 2 : 1);
     off = (off + 15) & ~size_t(15);
     double* ws = reinterpret_cast<double*>(smem_raw + off); off += sizeof(double) * NS;
+    double* us = reinterpret_cast<double*>(smem_raw + off); off += sizeof(double) * NS;
     unsigned long long* cms = reinterpret_cast<unsigned long long*>(smem_raw + off); off += sizeof(unsigned long long) * NS;
-    int2* eg = reinterpret_cast<int2*>(smem_raw + off); off += sizeof(int2) * NS;
-    double* Lgs = reinterpret_cast<double*>(smem_raw + off); off += sizeof(double) * 64;
+    uint32_t* eg = reinterpret_cast<uint32_t*>(smem_raw + off); off += sizeof(uint32_t) * NS;
+    off = (off + 15) & ~size_t(15);
+    float* Lf = reinterpret_cast<float*>(smem_raw + off); off += sizeof(float) * 64;
     float* stage = reinterpret_cast<float*>(smem_raw + off) + warp * 160; off += sizeof(float) * (kMoveAllThreads / 32) * 160;
     unsigned long long* bests = reinterpret_cast<unsigned long long*>(smem_raw + off);
 
     const int npairs = NS * (NS - 1) / 2;
     const bool poisoned = (*p.mp.bad != 0) || (*p.t.bad != 0);
     for (int j = tid; j < NS; j += kMoveAllThreads) {
-        eg[j] = p.mp.slot_eg[(size_t)l * NS + j];
+        const int2 s = p.mp.slot_eg[(size_t)l * NS + j];
+        eg[j] = (uint32_t)s.x | ((uint32_t)s.y << 16);
         ws[j] = p.mp.slot_w[(size_t)l * NS + j];
+        us[j] = p.mp.slot_u[(size_t)l * NS + j];
         cms[j] = p.mp.slot_cm[(size_t)l * NS + j];
     }
-    if (tid < p.G) Lgs[tid] = p.mp.Lg[(size_t)l * p.G + tid];
+    if (tid < p.G) Lf[tid] = (float)p.mp.Lg[(size_t)l * p.G + tid];
     {   // coalesced 16-byte reads of the [NS][G] rows, written at pitch G+1
         const float4* src = reinterpret_cast<const float4*>(p.mp.slotC + (size_t)l * NS * p.G);
         const float4* srcm = reinterpret_cast<const float4*>(p.mp.slotM + (size_t)l * NS * p.G);
@@ -944,11 +957,13 @@ __global__ void __launch_bounds__(kMoveAllThreads) move_all_kernel(const MoveAll
         }
     }
     __syncthreads();
-    double top[3]; int top_g[3];
+    // the three largest rank loads of the layer (fp32) and their ranks
+    float top[3]; int top_g[3];
 #pragma unroll
-    for (int q = 0; q < 3; ++q) { top[q] = p.mp.top[l * 4 + q]; top_g[q] = p.mp.top_g[l * 4 + q]; }
+    for (int q = 0; q < 3; ++q) { top[q] = (float)p.mp.top[l * 4 + q]; top_g[q] = p.mp.top_g[l * 4 + q]; }
+    const float alpha = p.alpha, beta = p.beta, gamma = p.gamma, M2 = 2.0f * p.M_scalar;
+    const float ov_nan = poisoned ? CUDART_NAN_F : 0.0f;
 
-    // tasks: t in [0, ceil((NS-1)/2)) -> rows t and NS-2-t (the middle row of an even count once)
     const int n_tasks = NS / 2;                                         // NS-1 rows: (NS-1+1)/2 pairs
     const int t_begin = blockIdx.x * p.tasks_per_block, t_end = min(n_tasks, t_begin + p.tasks_per_block);
     unsigned long long best = ~0ull;
@@ -956,48 +971,56 @@ __global__ void __launch_bounds__(kMoveAllThreads) move_all_kernel(const MoveAll
         for (int half = 0; half < 2; ++half) {
             const int a = half == 0 ? task : NS - 2 - task;
             if (half == 1 && a <= task) break;                          // middle row already done
-            const int2 s1 = eg[a];
-            const int e1 = s1.x, g1 = s1.y;
-            const double w1 = ws[a], L1 = Lgs[g1];
+            const uint32_t s1 = eg[a];
+            const int e1 = (int)(s1 & 0xffffu), g1 = (int)(s1 >> 16);
+            const double w1 = ws[a], U1 = us[a];
             const unsigned long long cm1 = cms[a];
-            const float t11 = Cs[a * PITCH + g1];
-            const float m11 = kHasM ? Ms[a * PITCH + g1] : p.M_scalar;
+            const float* Ca = Cs + a * PITCH;
+            const float t11 = Ca[g1];
+            const uint32_t n11 = __float_as_uint(t11) >> 31;
+            const float L1f = Lf[g1], w1f = (float)w1;
+            // largest load among the ranks other than g1 (and than g2, decided per lane)
+            const float r0v = top_g[0] != g1 ? top[0] : top[1];
+            const int r0g = top_g[0] != g1 ? top_g[0] : top_g[1];
+            const float r1v = (top_g[0] != g1 && top_g[1] != g1) ? top[1] : top[2];
             const int row0 = a * NS - a * (a + 1) / 2 - a - 1;           // pair index of (a, b) = row0 + b
             for (int bb = a + 1; bb < NS; bb += 32) {
-                const int b = bb + lane;
-                float dJ = 0.0f, dload = 0.0f, dcomm = 0.0f, dmig = 0.0f, dmax = 0.0f;
-                bool nan = poisoned;
-                if (b < NS && !nan) {
-                    const int2 s2 = eg[b];
-                    const int e2 = s2.x, g2 = s2.y;
-                    if (g1 != g2 && e1 != e2) {
-                        if (((cm1 >> g2) & 1ull) || ((cms[b] >> g1) & 1ull)) nan = true;      // second copy on a rank
-                        else {
-                            const float t12 = Cs[a * PITCH + g2], t21 = Cs[b * PITCH + g1], t22 = Cs[b * PITCH + g2];
-                            // loads in double: L1 - L2 and w2 - w1 subtract nearly equal numbers that can exceed 2^24
-                            const double L2 = Lgs[g2];
-                            const double dl = ws[b] - w1;                                 // moved onto g1
-                            dload = (float)(2.0 * dl * (L1 - L2) + 2.0 * dl * dl);        // the mean cancels
-                            dcomm = (fabsf(t12) - fabsf(t11)) + (fabsf(t21) - fabsf(t22));
-                            const float m12 = kHasM ? Ms[a * PITCH + g2] : p.M_scalar;
-                            const float m21 = kHasM ? Ms[b * PITCH + g1] : p.M_scalar, m22 = kHasM ? Ms[b * PITCH + g2] : p.M_scalar;
-                            // leaving a cell x0 has: +M, leaving a cell x0 lacks: -M; entering: the opposite
-                            dmig = (__float_as_int(t11) < 0 ? m11 : -m11) + (__float_as_int(t12) < 0 ? -m12 : m12) +
-                                   (__float_as_int(t22) < 0 ? m22 : -m22) + (__float_as_int(t21) < 0 ? -m21 : m21);
-                            const double n1 = L1 + dl, n2 = L2 - dl;
-                            double rest = -CUDART_INF;
-#pragma unroll
-                            for (int q = 2; q >= 0; --q)
-                                if (top_g[q] >= 0 && top_g[q] != g1 && top_g[q] != g2) rest = top[q];
-                            dmax = (float)(fmax(fmax(n1, n2), rest) - top[0]);
-                            dJ = p.alpha * dcomm + p.beta * dload + p.gamma * dmig;
-                        }
-                    }
+                const int b = min(bb + lane, NS - 1);                    // lanes past the row repeat its last move (not stored)
+                const uint32_t s2 = eg[b];
+                const int e2 = (int)(s2 & 0xffffu), g2 = (int)(s2 >> 16);
+                const bool same = (g1 == g2) || (e1 == e2);
+                const bool dup = (((cm1 >> g2) | (cms[b] >> g1)) & 1ull) != 0;
+                const float* Cb = Cs + b * PITCH;
+                const float t12 = Ca[g2], t21 = Cb[g1], t22 = Cb[g2];
+                const double w2 = ws[b];
+                const double dl = w2 - w1;                                // load moved onto g1
+                float dload = (float)((dl + dl) * (U1 - us[b]));          // 2 d (L1 - L2) + 2 d^2: the mean cancels
+                float dcomm = (fabsf(t12) - fabsf(t11)) + (fabsf(t21) - fabsf(t22));
+                float dmig;
+                if constexpr (kHasM) {
+                    const float* Ma = Ms + a * PITCH; const float* Mb = Ms + b * PITCH;
+                    // leaving a cell x0 has: +M, leaving a cell x0 lacks: -M; entering: the opposite
+                    const float m11 = __uint_as_float(__float_as_uint(Ma[g1]) ^ (~__float_as_uint(t11) & 0x80000000u));
+                    const float m12 = __uint_as_float(__float_as_uint(Ma[g2]) ^ (__float_as_uint(t12) & 0x80000000u));
+                    const float m22 = __uint_as_float(__float_as_uint(Mb[g2]) ^ (~__float_as_uint(t22) & 0x80000000u));
+                    const float m21 = __uint_as_float(__float_as_uint(Mb[g1]) ^ (__float_as_uint(t21) & 0x80000000u));
+                    dmig = (m11 + m12) + (m22 + m21);
+                } else {
+                    const int k = (int)(n11 + (__float_as_uint(t22) >> 31)) - (int)((__float_as_uint(t12) >> 31) + (__float_as_uint(t21) >> 31));
+                    dmig = M2 * (float)k;
                 }
-                if (nan) dJ = dload = dcomm = dmig = dmax = CUDART_NAN_F;
-                if (b < NS && !nan && p.best) {
+                const float dlf = (float)w2 - w1f;
+                const float rest = (g2 == r0g) ? r1v : r0v;
+                float dmax = fmaxf(fmaxf(L1f + dlf, Lf[g2] - dlf), rest) - top[0];
+                float dJ = __fmaf_rn(gamma, dmig, __fmaf_rn(beta, dload, alpha * dcomm));
+                // overrides: zeros for a move inside one rank / between two copies of one expert, NaN for a second copy on a rank
+                const bool use_ov = same || dup || poisoned;
+                const float ov = (dup && !same) ? CUDART_NAN_F : ov_nan;
+                dJ = use_ov ? ov : dJ; dload = use_ov ? ov : dload; dcomm = use_ov ? ov : dcomm; dmig = use_ov ? ov : dmig; dmax = use_ov ? ov : dmax;
+                if (p.best) {
+                    const bool cnt = (bb + lane < NS) && !(dJ != dJ);
                     const unsigned long long key = ((unsigned long long)ordered_u32(dJ + 0.0f) << 32) | (unsigned long long)(uint32_t)(l * npairs + row0 + b);
-                    best = key < best ? key : best;
+                    best = (cnt && key < best) ? key : best;
                 }
                 // stage the warp's 32 x 5 results, then write them as contiguous words
                 stage[lane * 5 + 0] = dJ; stage[lane * 5 + 1] = dload; stage[lane * 5 + 2] = dcomm; stage[lane * 5 + 3] = dmig; stage[lane * 5 + 4] = dmax;
