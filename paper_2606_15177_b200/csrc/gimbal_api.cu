@@ -177,7 +177,9 @@ static int launch_tables(const gimbal_placement_cfg* c, const void* A, const voi
     TableParams tp{};
     tp.L = c->L; tp.E = c->E; tp.G = c->G; tp.sp = c->slots_per_rank; tp.S = c->S; tp.counts_f32 = c->counts_dtype == GIMBAL_COUNTS_F32;
     tp.A = A; tp.B = B; tp.D = D; tp.M = M; tp.M_scalar = M_scalar; tp.prev = prev; tp.t = w.t;
-    place_tables_kernel<<<dim3(c->L, kTableSplit), 256, 0, stream>>>(tp);
+    const size_t smem_a = sizeof(float) * (size_t)c->S * c->E;           // the layer's [S][E] counts, at most 64 KB
+    if (smem_a > 24 * 1024) CUDA_TRY(cudaFuncSetAttribute(place_tables_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
+    place_tables_kernel<<<dim3(c->L, kTableSplit), 256, smem_a, stream>>>(tp);
     LAUNCH_CHECK("place_tables_kernel");
     return GIMBAL_OK;
 }
@@ -591,7 +593,7 @@ int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const void* c
         FinalizeParams fp{};
         fp.P = P; fp.L = cfg->L; fp.G = cfg->G; fp.alpha = cfg->alpha; fp.beta = cfg->beta; fp.gamma = cfg->gamma;
         fp.partial = w.partial; fp.bad_prev = w.t.bad; fp.out = out; fp.best = argmin ? w.best : nullptr;
-        place_finalize_kernel<<<(P + 255) / 256, 256, 0, stream>>>(fp);
+        place_finalize_kernel<<<(P + 7) / 8, 256, 0, stream>>>(fp);
         LAUNCH_CHECK("place_finalize_kernel");
     }
     if (argmin) {

@@ -84,12 +84,17 @@ __global__ void __launch_bounds__(256) place_tables_kernel(const TableParams p) 
     __shared__ float D_s[64 * 64];
     __shared__ double red_s[256];
     __shared__ int bad_s;
+    extern __shared__ __align__(16) unsigned char tab_smem[];
+    float* A_s = reinterpret_cast<float*>(tab_smem);              // [S][E] this layer's counts as fp32
     const int l = blockIdx.x, tid = threadIdx.x;
     const int NS = p.G * p.sp, GP = place_gp(p.G);
     const int16_t* pv = p.prev + (size_t)l * NS;
     if (tid == 0) bad_s = 0;
     for (int e = tid; e < p.E; e += 256) { r_s[e] = 0; pm_s[e] = 0ull; }
     for (int i = tid; i < p.S * p.G; i += 256) D_s[i] = p.D[i];
+    for (int i = tid; i < p.S * p.E; i += 256)
+        A_s[i] = p.counts_f32 ? reinterpret_cast<const float*>(p.A)[(size_t)l * p.S * p.E + i]
+                              : (float)reinterpret_cast<const int32_t*>(p.A)[(size_t)l * p.S * p.E + i];
     __syncthreads();
     for (int j = tid; j < NS; j += 256) {
         const int e = pv[j], g = j / p.sp;
@@ -133,11 +138,7 @@ __global__ void __launch_bounds__(256) place_tables_kernel(const TableParams p) 
     for (int i = blockIdx.y * per + tid; i < i_end; i += 256) {
         const int e = i / GP, gp = i % GP, g = gp % p.G;
         float c = 0.0f;
-        for (int s = 0; s < p.S; ++s) {
-            const float a = p.counts_f32 ? reinterpret_cast<const float*>(p.A)[((size_t)l * p.S + s) * p.E + e]
-                                         : (float)reinterpret_cast<const int32_t*>(p.A)[((size_t)l * p.S + s) * p.E + e];
-            c = __fmaf_rn(a, D_s[s * p.G + g], c);
-        }
+        for (int s = 0; s < p.S; ++s) c = __fmaf_rn(A_s[s * p.E + e], D_s[s * p.G + g], c);
         if (gp < p.G) p.t.c_raw[((size_t)l * p.E + e) * p.G + g] = fabsf(c);
         const int re = max(r_s[e], 1);
         const float inv = 1.0f / (float)re;
@@ -460,7 +461,7 @@ struct CheckParams {
     const float* M;                     // caller's [L,E,G] | nullptr
     PlaceTables t;
     float4* partial;
-    uint8_t* status;                    // [P,L] 0: valid, same copies as x0   1: invalid   2: valid, other replica counts
+    uint8_t* status;                    // [L,P] 0: valid, same copies as x0   1: invalid   2: valid, other replica counts
 };
 
 constexpr int kCheckWarps = 8;
@@ -601,7 +602,7 @@ __global__ void __launch_bounds__(kCheckWarps * 32) place_check_kernel(const Che
         const bool all_same = __all_sync(0xffffffffu, same);
         if (lane == 0) {
             if (bad) p.partial[(size_t)c * p.L + l] = make_float4(CUDART_NAN_F, CUDART_NAN_F, CUDART_NAN_F, CUDART_NAN_F);
-            p.status[(size_t)c * p.L + l] = bad ? 1 : ((!all_same || p.force_general) ? 2 : 0);
+            p.status[(size_t)l * p.P + c] = bad ? 1 : ((!all_same || p.force_general) ? 2 : 0);
         }
         __syncwarp();
     }
@@ -618,8 +619,12 @@ __global__ void __launch_bounds__(kCheckWarps * 32) place_own_r_kernel(const Che
     for (int i = lane; i < H * kCheckE; i += 32) mk[i] = 0u;
     __syncwarp();
     const int p_begin = blockIdx.x * p.chunk, p_end = min(p.P, p_begin + p.chunk);
+    // most calls have nothing to do here: the block reads its verdicts in one go and leaves
+    int mine = 0;
+    for (int c = p_begin + threadIdx.x; c < p_end; c += kCheckWarps * 32) mine |= p.status[(size_t)l * p.P + c] == 2;
+    if (!__syncthreads_or(mine)) return;
     for (int c = p_begin + warp; c < p_end; c += kCheckWarps) {
-        if (p.status[(size_t)c * p.L + l] != 2) continue;
+        if (p.status[(size_t)l * p.P + c] != 2) continue;
         const int16_t* row = p.cand + ((size_t)c * p.L + l) * NS;
         for (int rr = 0; rr < H; ++rr) {
             const int g = lane + rr * 32;
@@ -648,34 +653,35 @@ __device__ __forceinline__ uint32_t ordered_u32(float v) {
     return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
 }
 
+// a warp per candidate: lanes take the layers in strides of 32, fixed-shape tree over the lanes (deterministic), in double
 __global__ void __launch_bounds__(256) place_finalize_kernel(const FinalizeParams p) {
-    const int c = blockIdx.x * 256 + threadIdx.x;
+    const int c = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     unsigned long long key = ~0ull;
     if (c < p.P) {
         double sq = 0.0, comm = 0.0, mig = 0.0, mx = 0.0;
         bool bad = *p.bad_prev != 0;
-        for (int l = 0; l < p.L; ++l) {
+        for (int l = lane; l < p.L; l += 32) {
             const float4 v = p.partial[(size_t)c * p.L + l];
             if (v.x != v.x) bad = true;
             sq += v.x; comm += v.y; mig += v.z; mx += v.w;
         }
+        for (int o = 16; o > 0; o >>= 1) {
+            sq += __shfl_xor_sync(0xffffffffu, sq, o);
+            comm += __shfl_xor_sync(0xffffffffu, comm, o);
+            mig += __shfl_xor_sync(0xffffffffu, mig, o);
+            mx += __shfl_xor_sync(0xffffffffu, mx, o);
+        }
+        bad = __any_sync(0xffffffffu, bad);
         const double load = sq / ((double)p.G * (double)p.G);
         float* o = p.out + (size_t)c * 5;
-        if (bad) {
-            for (int i = 0; i < 5; ++i) o[i] = CUDART_NAN_F;
-        } else {
-            const float J = (float)((double)p.alpha * comm + (double)p.beta * load + (double)p.gamma * mig);
-            o[0] = J; o[1] = (float)load; o[2] = (float)comm; o[3] = (float)mig; o[4] = (float)mx;
-            key = ((unsigned long long)ordered_u32(J + 0.0f) << 32) | (unsigned)c;
+        const float J = (float)((double)p.alpha * comm + (double)p.beta * load + (double)p.gamma * mig);
+        if (lane < 5) {
+            const float vals[5] = {J, (float)load, (float)comm, (float)mig, (float)mx};
+            o[lane] = bad ? CUDART_NAN_F : vals[lane];
         }
+        if (!bad) key = ((unsigned long long)ordered_u32(J + 0.0f) << 32) | (unsigned)c;
     }
-    if (p.best) {
-        for (int o = 16; o > 0; o >>= 1) {
-            const unsigned long long other = __shfl_xor_sync(0xffffffffu, key, o);
-            key = other < key ? other : key;
-        }
-        if ((threadIdx.x & 31) == 0 && key != ~0ull) atomicMin(p.best, key);
-    }
+    if (p.best && lane == 0 && key != ~0ull) atomicMin(p.best, key);
 }
 
 __global__ void best_to_index_kernel(const unsigned long long* best, int32_t* out, int n) {
