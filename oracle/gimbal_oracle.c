@@ -667,12 +667,18 @@ void oracle_select_engines(const float *trace /*[N,4]*/, int complete, const flo
  *     others by prefill length (shortest first), equal lengths oldest first; a last tie goes to
  *     the position in the input queue.  order[i] = input position of the i-th request to run.   */
 /* ------------------------------------------------------------------------------------ */
+static float alg2_arrival(const float *arrival, int a)
+{
+    return arrival[a] != arrival[a] ? INFINITY : arrival[a];      /* a NaN arrival is the youngest request (R20) */
+}
+
 static int alg2_before(const float *arrival, const int32_t *prefill, float now, float theta, int a, int b)
 {
-    int aged_a = (now - arrival[a]) >= theta, aged_b = (now - arrival[b]) >= theta;
+    float ta = alg2_arrival(arrival, a), tb = alg2_arrival(arrival, b);
+    int aged_a = (now - ta) >= theta, aged_b = (now - tb) >= theta;
     if (aged_a != aged_b) return aged_a;                        /* high priority first */
     if (!aged_a && prefill[a] != prefill[b]) return prefill[a] < prefill[b];
-    if (arrival[a] < arrival[b] || arrival[b] < arrival[a]) return arrival[a] < arrival[b];   /* a NaN arrival ties (R20) */
+    if (ta != tb) return ta < tb;
     return a < b;
 }
 

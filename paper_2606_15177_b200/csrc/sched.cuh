@@ -139,7 +139,8 @@ __global__ void __launch_bounds__(kQueueThreads) order_queues_kernel(const Queue
     const int b = blockIdx.x;
     const int n = min(max(p.qlen[b], 0), p.Q);
     for (int j = threadIdx.x; j < n; j += kQueueThreads) {
-        arr_s[j] = p.arrival[(size_t)b * p.Q + j];
+        const float a = p.arrival[(size_t)b * p.Q + j];
+        arr_s[j] = a != a ? CUDART_INF_F : a;                               // a NaN arrival is the youngest request (R20)
         pre_s[j] = p.prefill[(size_t)b * p.Q + j];
     }
     for (int j = n + threadIdx.x; j < p.Q; j += kQueueThreads) p.order[(size_t)b * p.Q + j] = -1;
@@ -156,7 +157,7 @@ __global__ void __launch_bounds__(kQueueThreads) order_queues_kernel(const Queue
             bool before;
             if (aged_i != aged_j) before = aged_i;
             else if (!aged_i && pi != pj) before = pi < pj;
-            else if (ai < aj || aj < ai) before = ai < aj;                   // a NaN arrival ties with every arrival (R20)
+            else if (ai != aj) before = ai < aj;
             else before = i < j;
             pos += before;
         }

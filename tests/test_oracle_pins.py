@@ -673,3 +673,36 @@ def test_refine_worked_example_and_local_optimality():
                 Jn = oracle.objective(nb, prev, A, B, D, None, 1.0, **kw)
                 assert np.isnan(Jn[0]) or Jn[0] >= J[-1] - 1e-3 * abs(J[-1])
     assert sorted(cur[0].tolist()) == sorted(prev[0].tolist())
+
+
+# ------------------------------------------------------------------------------------------
+# behaviour on inputs the paper does not cover (R19 / R20 addenda), pinned by hand
+# ------------------------------------------------------------------------------------------
+def test_alg1_round_robin_pointer_counts_modulo_n():
+    """incomplete traces -> pure ordered dispatch; a pointer left at -7 or 13 by the caller starts at 3 (mod 5)"""
+    tr = np.zeros((5, 4), np.float32)
+    lens = np.ones(7, np.float32)
+    for rr0 in (-7, 13, 3):
+        comp = np.zeros(5)
+        eng, rr = oracle.select_engines(tr, 0, lens, comp, rr0)
+        assert eng.tolist() == [3, 4, 0, 1, 2, 3, 4] and rr == 0
+        assert comp.tolist() == [1.0, 1.0, 1.0, 2.0, 2.0]
+
+
+def test_alg2_nan_arrival_is_the_youngest_request():
+    """hand-ordered queue: now = 10, theta = 5.  Aged (waited >= 5): arrivals 1.0 and 4.0, oldest first.  The others by prefill,
+    equal prefill by arrival with NaN = +inf (never aged, last of its class), last tie by position."""
+    arrival = np.array([6.0, np.nan, 1.0, 7.0, 4.0, np.nan, 6.0], np.float32)
+    prefill = np.array([3, 3, 9, 3, 9, 2, 3], np.int32)
+    #  aged: idx 2 (1.0), idx 4 (4.0).  rest: prefill 2 -> idx 5; prefill 3 -> arrivals 6.0 (idx 0), 6.0 (idx 6), 7.0 (idx 3), NaN (idx 1)
+    assert oracle.order_queue(arrival, prefill, 10.0, 5.0).tolist() == [2, 4, 5, 0, 6, 3, 1]
+    # the order is a permutation for any mix of NaNs (a strict weak order), and equals numpy's lexsort on the same keys
+    rng = np.random.default_rng(8)
+    for _ in range(20):
+        a = rng.uniform(0, 10, 30).round(0).astype(np.float32); a[rng.integers(0, 30, 5)] = np.nan
+        pf = rng.integers(1, 4, 30).astype(np.int32)
+        got = oracle.order_queue(a, pf, 10.0, 5.0)
+        t = np.where(np.isnan(a), np.inf, a)
+        aged = (np.float32(10.0) - t) >= 5.0
+        ref = np.lexsort((np.arange(30), t, np.where(aged, 0, pf), ~aged))
+        assert got.tolist() == ref.tolist()
