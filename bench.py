@@ -276,6 +276,7 @@ def _config(w, args):
                 l2="hidden states of one step (>> L2) stream through L2 between the placement kernels; an explicit 256 MiB flush runs "
                    "between timed steps, outside the timed events",
                 placements="default call: every candidate is validated exactly (place_check_kernel) and scored (place_score_kernel)",
+                options=(list(args.opt) if getattr(args, "opt", None) else "library defaults"),
                 outputs="A_step/B/pressure (a3-a5), out[P,5]+argmin (a6), delta[n,5]+best_per_layer (a7); top-k ids and weights "
                         + ("written" if getattr(args, "with_ids", False) else "not written"))
 
@@ -702,10 +703,17 @@ def main():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--with-ids", action="store_true", help="also write top-k ids and weights (a2 outputs) inside the timed step")
     ap.add_argument("--layers", type=int, default=0, help="profiling only: run the first N MoE layers (named in config.workload)")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="A/B measurement: gimbal_set_option before the run, e.g. --opt HIST_AGG=0 (named in config.options)")
     args = ap.parse_args()
     args.steps_given = args.steps is not None
     if args.steps is None:
         args.steps = 20
+    if args.opt:
+        import paper_2606_15177_b200 as g
+        for kv in args.opt:
+            name, val = kv.split("=")
+            g.set_option(getattr(g, "OPT_" + name.upper()), int(val))
     w = get_workload(args.workload)
     if args.layers > 0:
         w = scaled(w, L=args.layers)

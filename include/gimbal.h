@@ -393,12 +393,16 @@ GIMBAL_API int gimbal_refine_placement(const gimbal_placement_cfg *cfg, int16_t 
  *                                specialised one exists
  *   GIMBAL_OPT_CHECK_SCORES_ALL  0 (default); 1: place_check_kernel scores every valid candidate with
  *                                the candidate's own replica counts (the path otherwise taken only by
- *                                candidates whose replica counts differ from x0's)                  */
+ *                                candidates whose replica counts differ from x0's)
+ *   GIMBAL_OPT_HIST_AGG          1 (default): the router GEMM epilogue counts a warp's 32 tokens by columns
+ *                                (bit-matrix transpose, one shared atomic per lane and 32 experts) when they
+ *                                share one source; 0: one predicated shared atomic per selected logit        */
 #define GIMBAL_OPT_CTA_GROUP 0
 #define GIMBAL_OPT_FUSE_GATE 1
 #define GIMBAL_OPT_SCORE_GENERIC 2
 #define GIMBAL_OPT_CHECK_SCORES_ALL 3
-#define GIMBAL_OPT_COUNT_ 4
+#define GIMBAL_OPT_HIST_AGG 4
+#define GIMBAL_OPT_COUNT_ 5
 GIMBAL_API int gimbal_set_option(int option, int value);
 GIMBAL_API int gimbal_get_option(int option, int *value);
 

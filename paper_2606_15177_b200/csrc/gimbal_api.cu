@@ -104,7 +104,7 @@ size_t route_ws_carve(const gimbal_router_cfg* c, void* ws, RouteWs* out) {
 }
 
 // process-wide switches set through gimbal_set_option (tests and A/B measurements); defaults = production
-std::atomic<int> g_opt[GIMBAL_OPT_COUNT_] = {{0}, {1}, {0}, {0}};
+std::atomic<int> g_opt[GIMBAL_OPT_COUNT_] = {{0}, {1}, {0}, {0}, {1}};
 
 int pick_cta_group(int T) {
     const int forced = g_opt[GIMBAL_OPT_CTA_GROUP].load(std::memory_order_relaxed);
@@ -366,6 +366,7 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
         a.topk_ids = topk_ids; a.topk_w = topk_w; a.A_step = st->A_step; a.stream = stream;
         if (map) { a.rep_off = map->rep_off; a.rep_slots = map->rep_slots; a.phys_ids = map->phys_ids; a.map_NS = map->NS; }
         a.cta_group = pick_cta_group(T);
+        a.hist_agg = g_opt[GIMBAL_OPT_HIST_AGG].load(std::memory_order_relaxed);
         if (logits_mode == GIMBAL_LOGITS_IN) {
             a.logits = logits;
             rc = launch_gate(a);

@@ -52,6 +52,7 @@ struct RouteArgs {
     const int32_t* rep_off; const int16_t* rep_slots; int32_t* phys_ids; int map_NS;   // expert mapping | nullptr
     int fuse_gate;
     int cta_group;          // 1 or 2
+    int hist_agg;           // epilogue counts by columns (GIMBAL_OPT_HIST_AGG)
     cudaStream_t stream;
 };
 

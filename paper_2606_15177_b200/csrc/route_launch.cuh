@@ -19,6 +19,7 @@ int launch_gemm_t(const RouteArgs& a) {
     p.m_tiles = (a.T + kBlockM * kCG - 1) / (kBlockM * kCG);
     const bool out = a.fuse_gate && (a.topk_ids || a.topk_w || a.rep_off);
     p.stages = gemm_pick_stages<N, kCG>(c->S, out);
+    p.hist_agg = a.hist_agg;
     if (p.stages < 2) return fail(GIMBAL_ERR_UNSUPPORTED, "router GEMM: not enough shared memory for E=%d S=%d", N, c->S);
     p.src_logit_bias = a.src_logit_bias; p.src_offsets = a.src_offsets; p.logits = a.logits;
     p.do_gate = a.fuse_gate; p.select_bias = a.select_bias; p.topk_ids = a.topk_ids; p.topk_w = a.topk_w;

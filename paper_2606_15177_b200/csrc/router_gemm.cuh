@@ -25,6 +25,7 @@ struct GemmParams {
     int n_layers, layer0, T, H, S;
     int m_tiles;                    // ceil(T / (128*kCG))
     int stages;                     // depth of the shared-memory ring (host: gemm_pick_stages)
+    int hist_agg;                   // count a warp's tokens by columns when they share one source
     const float* src_logit_bias;    // [L,S,E] | nullptr
     const int32_t* src_offsets;     // [S+1]
     float* logits;                  // [n_layers,T,E] | nullptr
@@ -293,7 +294,9 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
                     }
                     if (valid && p.map.rep_off) map_row<N>(p.map, layer, li, p.T, t, p.gp.k, ids);
                 } else {
-                    gate_row<N, kSig, false>(p.gp, sb_s, src, valid, hist + s * N, nullptr, 0, ids, w);
+                    // rows past T follow the last row's source; a warp whose 32 rows share one source counts by columns
+                    const bool uni = p.hist_agg && __all_sync(0xffffffffu, s == __shfl_sync(0xffffffffu, s, 0));
+                    gate_row<N, kSig, false>(p.gp, sb_s, src, valid, hist + s * N, nullptr, 0, ids, w, 0, uni);
                 }
             }
             // release this accumulator stage to the MMA issuer
