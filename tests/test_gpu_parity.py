@@ -1108,3 +1108,54 @@ def test_scheduler_kernels_on_stale_pointer_and_nan_arrival():
     for b in range(3):
         np.testing.assert_array_equal(to_np(order)[b], oracle.order_queue(arrival[b], prefill[b], 20.0, 5.0))
         assert sorted(to_np(order)[b].tolist()) == list(range(Q))
+
+
+# ------------------------------------------------------------------------------------------
+# shapes outside the five configs: the shape-generic scoring kernel, place_check_kernel<0, H>, place_own_r_kernel
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L,E,G,sp,S,table_M,counts", [
+    (3, 48, 8, 7, 3, False, "i32"),       # E not a power of two, odd slot count, 8 redundant slots
+    (2, 160, 64, 3, 5, True, "f32"),      # two ranks per lane, odd slot count, 32 redundant slots, M table
+    (2, 200, 16, 16, 4, True, "i32"),     # the largest slot count, 56 redundant slots
+    (1, 30, 4, 8, 2, False, "f32"),       # G below a warp: several candidates per warp
+])
+def test_eval_placements_and_moves_on_other_shapes(L, E, G, sp, S, table_M, counts):
+    from workloads.configs import RouterCfg as WRouterCfg, Workload
+    NS = G * sp
+    w = Workload(name="other", cfg_id=9, router=WRouterCfg(L=L, H=64, E=E, k=2, S=S), T=64, G=G, slots_per_rank=sp, P=72, steps=1,
+                 mode=MODE_WINDOW, ema_decay=0.0, window_len=1, zipf_a=1.2, rho=0.5, len_mu=0.0, len_sigma=0.0)
+    rng = np.random.default_rng(E + G)
+    A = rng.integers(0, 500, (L, S, E)); B = A.sum(1) * rng.integers(20, 60, (L, E))
+    if counts == "f32":
+        A_t = torch.from_numpy((A * 0.73).astype(np.float32)).to(DEV); B_t = torch.from_numpy((B * 0.73).astype(np.float32)).to(DEV)
+    else:
+        A_t = torch.from_numpy(A.astype(np.int32)).to(DEV); B_t = torch.from_numpy(B.astype(np.int32)).to(DEV)
+    D = gen.comm_cost_D(w, "seeded", DEV)
+    M = gen.mig_cost_M(w, DEV) if table_M else None
+    prev = gen.prev_placement(w, to_np(B_t), DEV)
+    cfg = g.PlacementCfg(L=L, E=E, G=G, slots_per_rank=sp, S=S, counts_dtype=g.COUNTS_F32 if counts == "f32" else g.COUNTS_I32)
+    cands = torch.cat([gen.candidates(w, prev, 36, DEV), gen.candidates_redrawn(w, prev, 36, DEV)]).contiguous()
+    cands[5, 0, 3] = E                                        # first id past the range (E is not always a power of two)
+    c6 = cands[6, L - 1].clone(); c6[1] = c6[0]; cands[6, L - 1] = c6    # twice on rank 0
+    out = torch.empty(72, 5, device=DEV); argmin = torch.zeros(1, dtype=torch.int32, device=DEV)
+    ws = ws_tensor(g.eval_placements_workspace_bytes(cfg, 72))
+    g.eval_placements(cfg, cands, A_t, B_t, D, prev, out, M=M, M_scalar=0.6, argmin=argmin, workspace=ws)
+    ref = oracle.objective_batch(to_np(cands), to_np(prev), to_np(A_t), to_np(B_t), to_np(D), to_np(M), 0.6, **_oracle_kw(cfg))
+    assert np.isnan(ref[[5, 6]]).all() and not np.isnan(np.delete(ref, [5, 6], 0)).any()
+    o = to_np(out).astype(np.float64)
+    _check_objective(o, ref)
+    assert o[0, 3] == 0.0 and int(argmin.item()) == int(np.nanargmin(to_np(out)[:, 0]))
+    # moves: the whole neighbourhood (the staged kernel where it fits, the per-move kernel otherwise) and a list
+    cur = cands[2].contiguous()
+    n = L * NS * (NS - 1) // 2
+    delta = torch.empty(n, 5, device=DEV); best = torch.empty(L, dtype=torch.int32, device=DEV)
+    wsm = ws_tensor(g.eval_moves_workspace_bytes(cfg))
+    g.eval_moves(cfg, cur, prev, A_t, B_t, D, delta, M=M, M_scalar=0.6, best_per_layer=best, workspace=wsm)
+    allmv = oracle.all_pair_moves(L, NS)
+    pick = np.arange(n) if n <= 40000 else np.unique(np.concatenate([np.arange(400), np.arange(n - 400, n), rng.integers(0, n, 6000)]))
+    refm = oracle.move_deltas(to_np(cur), to_np(prev), allmv[pick], to_np(A_t), to_np(B_t), to_np(D), to_np(M), 0.6, **_oracle_kw(cfg))
+    d = to_np(delta).astype(np.float64)
+    _check_deltas(cfg, d[pick], refm, allmv[pick], to_np(cur), to_np(A_t), to_np(B_t), to_np(D), to_np(M), 0.6)
+    per = n // L
+    for l in range(L):
+        assert int(best[l].item()) == l * per + int(np.nanargmin(to_np(delta)[l * per:(l + 1) * per, 0]))
