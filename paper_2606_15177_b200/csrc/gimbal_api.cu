@@ -195,9 +195,9 @@ static int launch_score_generic(const ScoreParams& sp, dim3 grid, size_t smem, c
     return GIMBAL_OK;
 }
 
-template <int SP, int G, int E, bool kHasM>
+template <int SP, int G, int E, bool kHasM, bool kCheck>
 static int launch_score_v(const ScoreParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
-    auto kern = place_score_kernel<SP, G, E, kHasM>;
+    auto kern = place_score_kernel<SP, G, E, kHasM, kCheck>;
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ktime_begin(GIMBAL_KERNEL_SCORE, stream);
     kern<<<grid, kScoreThreads, smem, stream>>>(sp);
@@ -207,8 +207,9 @@ static int launch_score_v(const ScoreParams& sp, dim3 grid, size_t smem, cudaStr
 }
 
 template <int SP, int G, int E>
-static int launch_score(const ScoreParams& sp, dim3 grid, size_t smem, cudaStream_t stream) {
-    return sp.has_M ? launch_score_v<SP, G, E, true>(sp, grid, smem, stream) : launch_score_v<SP, G, E, false>(sp, grid, smem, stream);
+static int launch_score(const ScoreParams& sp, bool check, dim3 grid, size_t smem, cudaStream_t stream) {
+    if (check) return sp.has_M ? launch_score_v<SP, G, E, true, true>(sp, grid, smem, stream) : launch_score_v<SP, G, E, false, true>(sp, grid, smem, stream);
+    return sp.has_M ? launch_score_v<SP, G, E, true, false>(sp, grid, smem, stream) : launch_score_v<SP, G, E, false, false>(sp, grid, smem, stream);
 }
 
 template <int E>
@@ -537,13 +538,18 @@ int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const void* c
         } else {
             ScoreParams sp{};
             sp.P = P; sp.L = cfg->L; sp.E = cfg->E; sp.G = cfg->G; sp.sp = cfg->slots_per_rank; sp.M_scalar = M_scalar; sp.has_M = M != nullptr;
-            sp.cand = static_cast<const int16_t*>(candidates); sp.t = w.t; sp.partial = w.partial;
-            // one wave: two resident blocks per SM (one when the table needs more than half the shared memory)
-            // the five configuration shapes (slots per rank, ranks, experts) have specialised kernels
+            sp.cand = static_cast<const int16_t*>(candidates); sp.t = w.t; sp.partial = w.partial; sp.status = w.status;
+            sp.force_general = g_opt[GIMBAL_OPT_CHECK_SCORES_ALL].load(std::memory_order_relaxed);
+            const bool trusted = (cfg->flags & GIMBAL_PLACE_TRUSTED) != 0;
+            // the five configuration shapes (slots per rank, ranks, experts) have specialised kernels, which also validate
+            // in the same pass (kCheck); any other shape: the shape-generic scoring kernel, then place_check_kernel
             const long key = g_opt[GIMBAL_OPT_SCORE_GENERIC].load(std::memory_order_relaxed)
                                  ? 0 : (long)cfg->slots_per_rank * 1000000 + cfg->G * 1000 + cfg->E;
             const bool fast = key == 9032256 || key == 8016128 || key == 8008064 || key == 4064256 || key == 4004016;
-            const int per_sm = (fast && 2 * smem + 2048 <= kSmemLimit) ? 2 : 1;
+            const bool fused = fast && !trusted && smem + place_score_mask_bytes(cfg->G, cfg->E) <= kSmemLimit;   // else: separate check kernel
+            const size_t smem_k = smem + (fused ? place_score_mask_bytes(cfg->G, cfg->E) : 0);
+            // one wave: two resident blocks per SM (one when a block needs more than half the shared memory)
+            const int per_sm = (fast && 2 * smem_k + 2048 <= kSmemLimit) ? 2 : 1;
             int nchunk = per_sm * sms / cfg->L;
             const int units_per_pass = (kScoreThreads / 32) * (cfg->G < 32 ? 32 / cfg->G : 1);
             int max_chunks = (P + units_per_pass - 1) / units_per_pass;
@@ -551,42 +557,45 @@ int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const void* c
             if (nchunk < 1) nchunk = 1;
             sp.chunk = (P + nchunk - 1) / nchunk;
             dim3 grid((P + sp.chunk - 1) / sp.chunk, cfg->L);
-            switch (key) {
-                case 9032256: rc = launch_score<9, 32, 256>(sp, grid, smem, stream); break;
-                case 8016128: rc = launch_score<8, 16, 128>(sp, grid, smem, stream); break;
-                case 8008064: rc = launch_score<8, 8, 64>(sp, grid, smem, stream); break;
-                case 4064256: rc = launch_score<4, 64, 256>(sp, grid, smem, stream); break;
-                case 4004016: rc = launch_score<4, 4, 16>(sp, grid, smem, stream); break;
+            switch (fast ? key : 0) {
+                case 9032256: rc = launch_score<9, 32, 256>(sp, fused, grid, smem_k, stream); break;
+                case 8016128: rc = launch_score<8, 16, 128>(sp, fused, grid, smem_k, stream); break;
+                case 8008064: rc = launch_score<8, 8, 64>(sp, fused, grid, smem_k, stream); break;
+                case 4064256: rc = launch_score<4, 64, 256>(sp, fused, grid, smem_k, stream); break;
+                case 4004016: rc = launch_score<4, 4, 16>(sp, fused, grid, smem_k, stream); break;
                 default: rc = sp.has_M ? launch_score_generic<true>(sp, grid, smem, stream) : launch_score_generic<false>(sp, grid, smem, stream); break;
             }
             if (rc) return rc;
-            if (!(cfg->flags & GIMBAL_PLACE_TRUSTED)) {
-                // exact validation; overwrites the partials of invalid candidates (NaN) and of valid ones whose replica
-                // counts differ from x0's (scored with their own r)
+            if (!trusted) {
                 CheckParams cp{};
                 cp.P = P; cp.L = cfg->L; cp.E = cfg->E; cp.G = cfg->G; cp.sp = cfg->slots_per_rank;
-                cp.force_general = g_opt[GIMBAL_OPT_CHECK_SCORES_ALL].load(std::memory_order_relaxed);
+                cp.force_general = sp.force_general;
                 cp.M_scalar = M_scalar; cp.cand = sp.cand; cp.prev = prev; cp.M = M; cp.t = w.t; cp.partial = w.partial; cp.status = w.status;
                 int nck = 8 * sms / cfg->L;
                 const int maxck = (P + kCheckWarps - 1) / kCheckWarps;
                 if (nck > maxck) nck = maxck;
                 if (nck < 1) nck = 1;
                 cp.chunk = (P + nck - 1) / nck;
-                ktime_begin(GIMBAL_KERNEL_CHECK, stream);
                 const dim3 cgrid((P + cp.chunk - 1) / cp.chunk, cfg->L);
-                const int key = cfg->slots_per_rank * 10 + (cfg->G > 32 ? 2 : 1);
-                switch (key) {
-                    case 41: place_check_kernel<4, 1><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp); break;
-                    case 42: place_check_kernel<4, 2><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp); break;
-                    case 81: place_check_kernel<8, 1><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp); break;
-                    case 91: place_check_kernel<9, 1><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp); break;
-                    default:
-                        if (cfg->G > 32) place_check_kernel<0, 2><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp);
-                        else place_check_kernel<0, 1><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp);
-                        break;
+                if (!fused) {
+                    // exact validation; overwrites the partials of invalid candidates (NaN) and marks the valid ones whose
+                    // replica counts differ from x0's
+                    ktime_begin(GIMBAL_KERNEL_CHECK, stream);
+                    const int ckey = cfg->slots_per_rank * 10 + (cfg->G > 32 ? 2 : 1);
+                    switch (ckey) {
+                        case 41: place_check_kernel<4, 1><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp); break;
+                        case 42: place_check_kernel<4, 2><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp); break;
+                        case 81: place_check_kernel<8, 1><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp); break;
+                        case 91: place_check_kernel<9, 1><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp); break;
+                        default:
+                            if (cfg->G > 32) place_check_kernel<0, 2><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp);
+                            else place_check_kernel<0, 1><<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp);
+                            break;
+                    }
+                    ktime_end(GIMBAL_KERNEL_CHECK, stream);
+                    LAUNCH_CHECK("place_check_kernel");
                 }
-                ktime_end(GIMBAL_KERNEL_CHECK, stream);
-                LAUNCH_CHECK("place_check_kernel");
+                // candidates with their own replica counts: scored with the candidate's r
                 place_own_r_kernel<<<cgrid, kCheckWarps * 32, smem_chk, stream>>>(cp);
                 LAUNCH_CHECK("place_own_r_kernel");
             }

@@ -165,6 +165,8 @@ struct ScoreParams {
     const int16_t* cand;                // [P,L,NS]
     PlaceTables t;
     float4* partial;                    // [P,L] {sum_g d_g^2, comm, mig, maxL}; NaN in .x if invalid
+    uint8_t* status;                    // [L,P] verdicts of the fused validation (kCheck): 0 same copies as x0, 1 invalid, 2 other replica counts
+    int force_general;                  // tests: verdict 2 for every valid candidate
 };
 
 constexpr int kScoreThreads = 512;
@@ -199,7 +201,16 @@ __device__ __forceinline__ float reduce_pair(float& sq, float comm, int lane, in
 // the low part: exact whenever the difference is representable (integer counts), R11.
 constexpr int kScoreU = 2;
 
-template <int SP, int G, int E, bool kHasM>
+// kCheck (the default call on these shapes): the exact validation of place_check_kernel runs on the ids while they are in registers --
+// one atomicOr per slot into the unit's x[e, .] rank masks in shared memory, read back (and cleared) by 16-byte loads, popcounts compared
+// with x0's replica counts -- and the verdict decides what is stored: NaN (invalid), the scores (same copies as x0), or the scores plus
+// verdict 2 for place_own_r_kernel to replace (valid, other replica counts).
+inline size_t place_score_mask_bytes(int G, int E) {
+    const int upw = G < 32 ? 32 / G : 1, h = G > 32 ? G / 32 : 1;
+    return sizeof(uint32_t) * (size_t)(kScoreThreads / 32) * upw * 2 * h * E;       // [warps][units per warp][kScoreU][H][E]
+}
+
+template <int SP, int G, int E, bool kHasM, bool kCheck>
 __global__ void __launch_bounds__(kScoreThreads, 2) place_score_kernel(const ScoreParams p) {
     constexpr int kU = kScoreU;
     constexpr int H = G > 32 ? G / 32 : 1;              // table halves == ranks per lane
@@ -280,6 +291,21 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_kernel(const Sco
 #pragma unroll
             for (int j = 0; j < SP; ++j) mx0[rr][j] = p.t.mx0[(size_t)l * NS + (g0 + rr * 32) * SP + j];
     }
+    // kCheck: this unit's rank masks, one [H][E] array per candidate in flight; lane g0 reads back experts 4*(g0 + k*SEG) .. +3
+    constexpr int EPL4 = E / SEG / 4;                    // 16-byte groups of experts per lane (1 or 2)
+    static_assert(!kCheck || (E % (4 * SEG) == 0 && EPL4 >= 1 && EPL4 <= 2), "readback layout");
+    uint32_t* mk_unit = reinterpret_cast<uint32_t*>(smem_raw + (size_t)H * E * (kHasM ? 384 : 256)) + (size_t)((warp * UPW + sub) * kU) * H * E;
+    uint32_t r0p[kCheck ? EPL4 : 1];
+    if constexpr (kCheck) {
+        for (int i = threadIdx.x; i < (kScoreThreads / 32) * UPW * kU * H * E; i += kScoreThreads)
+            reinterpret_cast<uint32_t*>(smem_raw + (size_t)H * E * (kHasM ? 384 : 256))[i] = 0u;
+#pragma unroll
+        for (int k = 0; k < EPL4; ++k) {
+            const int32_t* r4 = p.t.r + (size_t)l * E + 4 * (g0 + k * SEG);
+            r0p[k] = (uint32_t)min(r4[0], 255) | ((uint32_t)min(r4[1], 255) << 8) | ((uint32_t)min(r4[2], 255) << 16) | ((uint32_t)min(r4[3], 255) << 24);
+        }
+    }
+    const uint32_t rank_bit = 1u << g0;
     __syncthreads();
 
     // one warp pass: prefetch the next pass into `nxt`, score the two candidates in `cur`, reduce, store
@@ -290,8 +316,10 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_kernel(const Sco
             if (cand + (kU + u) * kStride < p_end) fetch(rowp + u * stride_words, nxt[u]);
         float sq[kU], comm[kU], mig[kU], mx[kU];
         uint32_t kept[kU];
+        uint32_t viol[kU], range[kU];
 #pragma unroll
         for (int u = 0; u < kU; ++u) {
+            viol[u] = range[u] = 0u;
             // no activity test here: a unit past the end scores whatever its registers hold (ids are masked) and is not stored
             sq[u] = comm[u] = mig[u] = mx[u] = 0.0f;
             kept[u] = 0;
@@ -307,6 +335,10 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_kernel(const Sco
                     for (int j = 0; j + 1 < NW; ++j) w[j] = __funnelshift_r(w[j], w[j + 1], sh);
                     w[NW - 1] = w[NW - 1] >> sh;
                 }
+                if constexpr (kCheck) {
+#pragma unroll
+                    for (int j = 0; j < NW; ++j) range[u] |= w[j];      // any bit outside an id's range marks the candidate invalid
+                }
                 if constexpr (E < 256) {                // E == 256: the PRMT below only takes the low byte of an id
 #pragma unroll
                     for (int j = 0; j < NW; ++j) w[j] &= emask2;
@@ -320,6 +352,8 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_kernel(const Sco
                     const float2 wc = *reinterpret_cast<const float2*>(wc_b + rr * E * 256 + off);
                     lg2[j & 1] += wc.x;
                     cm2[j & 1] += fabsf(wc.y);
+                    if constexpr (kCheck)                   // x[e, rank] |= 1; the word that comes back says whether it was set already
+                        viol[u] |= atomicOr(reinterpret_cast<uint32_t*>(reinterpret_cast<unsigned char*>(mk_unit + (u * H + rr) * E) + ((off >> 6) & 0x3fcu)), rank_bit);
                     if constexpr (kHasM) {
                         const uint32_t uw = *reinterpret_cast<const uint32_t*>(mu_b + rr * E * 128 + (off >> 1));
                         mig[u] += fmaxf(__uint_as_float(uw), 0.0f);                     // entering cell: + M
@@ -339,6 +373,31 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_kernel(const Sco
                 sq[u] = __fmaf_rn(d, d, sq[u]);
                 mx[u] = fmaxf(mx[u], lg);
             }
+        }
+        bool bad0 = false, bad1 = false, same0 = true, same1 = true;
+        if constexpr (kCheck) {
+            __syncwarp();
+#pragma unroll
+            for (int u = 0; u < kU; ++u) {
+                bool same = true, missing = false;
+#pragma unroll
+                for (int k = 0; k < EPL4; ++k) {
+                    uint32_t cnt = 0;
+#pragma unroll
+                    for (int rr = 0; rr < H; ++rr) {
+                        uint4* q = reinterpret_cast<uint4*>(mk_unit + (u * H + rr) * E) + g0 + k * SEG;
+                        const uint4 a = *q;
+                        *q = make_uint4(0u, 0u, 0u, 0u);
+                        cnt += __popc(a.x) | (__popc(a.y) << 8) | (__popc(a.z) << 16) | (__popc(a.w) << 24);
+                    }
+                    same = same && cnt == r0p[k];
+                    missing = missing || ((~(((cnt & 0x7f7f7f7fu) + 0x7f7f7f7fu) | cnt) & 0x80808080u) != 0u);
+                }
+                const bool bad_l = ((viol[u] & rank_bit) != 0u) || ((range[u] & ~emask2) != 0u) || missing;
+                const uint32_t bb = __ballot_sync(0xffffffffu, bad_l) & seg_mask, ss = __ballot_sync(0xffffffffu, !same) & seg_mask;
+                if (u == 0) { bad0 = bb != 0u; same0 = ss == 0u; } else { bad1 = bb != 0u; same1 = ss == 0u; }
+            }
+            __syncwarp();                                   // the masks are clear before the next pass ORs into them
         }
         // one transposed butterfly for both candidates of the unit: after the first step the lanes with bit h clear
         // work for candidate 0 and the others for candidate 1, after the second the lanes with bit h2 clear hold sq, the
@@ -366,7 +425,15 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_kernel(const Sco
         }
         // lane g0 == 0 writes candidate 0, lane g0 == h candidate 1
         const int mine = cand + (up ? kStride : 0);
-        if ((g0 & (h - 1)) == 0 && mine < p_end) partial[(size_t)mine * L + l] = make_float4(v, commt, migt, up ? mxa1 : mxa0);
+        if ((g0 & (h - 1)) == 0 && mine < p_end) {
+            float4 res = make_float4(v, commt, migt, up ? mxa1 : mxa0);
+            if constexpr (kCheck) {
+                const bool bad = up ? bad1 : bad0, same = up ? same1 : same0;
+                if (bad) res = make_float4(CUDART_NAN_F, CUDART_NAN_F, CUDART_NAN_F, CUDART_NAN_F);
+                p.status[(size_t)l * p.P + mine] = bad ? 1 : ((!same || p.force_general) ? 2 : 0);
+            }
+            partial[(size_t)mine * L + l] = res;
+        }
         cand += kU * kStride;
     };
     for (int pc = p_begin + warp * UPW; pc < p_end; pc += 2 * kU * kStride) {
