@@ -57,7 +57,8 @@ def _profile_metrics(name: str) -> dict:
 
 
 K1_PROFILE = "r2_ncu_k1_router_gemm"       # V3 shape, `--layers 6`: counters are per launch of 6 layers x 65536 tokens
-K4_PROFILE = "r2_ncu_k4_place_score"       # V3 shape, P = 4096, 58 layers
+K4_PROFILE = "r2_ncu_k4_place_score"       # V3 shape, P = 4096, 58 layers, GIMBAL_PLACE_TRUSTED (scoring only)
+K4C_PROFILE = "r2_ncu_k4_place_score_checked"   # same, default call (validation fused in)
 
 
 def _peaks():
@@ -442,15 +443,20 @@ def run_ours(args, w):
     score_ms, check_ms, moves_ms = statistics.mean(k_score), statistics.mean(k_check), statistics.mean(k_moves)
     cand_bytes = 2.0 * r.L * w.NS * w.P
     gate_bytes = 4.0 * r.E * w.T * nl
-    k4p = _profile_metrics(K4_PROFILE)
     sm_max_ghz = (clocks.get("sm_max_mhz") or 1965.0) / 1e3
     smem_peak = 148 * 128 * sm_max_ghz                        # GB/s: 128 B per clock per SM of shared-memory / L1 data pipe
-    smem = None
-    if "l1tex__data_pipe_lsu_wavefronts.sum" in k4p and w.name == "v3":
-        wave_bytes = k4p["l1tex__data_pipe_lsu_wavefronts.sum"] * 128.0 * (w.P * r.L / k4p.get("units", w.P * r.L))
-        smem = dict(achieved=wave_bytes / (score_ms * 1e-3) / 1e9, peak=smem_peak, unit="GB/s", frac=wave_bytes / (score_ms * 1e-3) / 1e9 / smem_peak,
-                    note=f"the kernel's real bound (DESIGN.md section 6): L1 data-pipe wavefronts x 128 B from profiles/{K4_PROFILE}.csv "
-                         "against 148 SMs x 128 B/clk at the maximum SM clock")
+
+    def smem_obj(profile, ms):
+        """the kernel against its real bound: L1 data-pipe wavefronts x 128 B of the committed capture / its time"""
+        k = _profile_metrics(profile)
+        pct = "l1tex__data_pipe_lsu_wavefronts.sum.pct_of_peak_sustained_elapsed"
+        if pct not in k or "sm__cycles_elapsed.avg" not in k or w.name != "v3":
+            return None
+        waves = k[pct] / 100.0 * k["sm__cycles_elapsed.avg"] * 148                  # the pipe's peak is one wavefront per clock per SM
+        wave_bytes = waves * 128.0 * (w.P * r.L / k.get("units", w.P * r.L))
+        return dict(achieved=wave_bytes / (ms * 1e-3) / 1e9, peak=smem_peak, unit="GB/s", frac=wave_bytes / (ms * 1e-3) / 1e9 / smem_peak,
+                    note=f"L1 data-pipe wavefronts x 128 B from profiles/{profile}.csv against 148 SMs x 128 B/clk at the maximum SM clock")
+
     t_ms = min(trusted_ms[1:])
     extra = dict(
         gate_hist_kernel=dict(ms=min(gate_ms[1:]), layers=nl, bound="hbm", achieved=gate_bytes / (min(gate_ms[1:]) * 1e-3) / 1e9,
@@ -470,8 +476,8 @@ def run_ours(args, w):
                                       "rank masks in shared memory)" if check_ms == 0.0 else "in the step: scoring only; validation = place_check_kernel"),
                                 alone=dict(ms=t_ms, achieved=cand_bytes / (t_ms * 1e-3) / 1e9, frac=cand_bytes / (t_ms * 1e-3) / 1e9 / peaks["hbm"],
                                            note="GIMBAL_PLACE_TRUSTED call outside the timed step, after an L2 flush (clocks not held "
-                                                "down by the router GEMM)"),
-                                smem=smem),
+                                                "down by the router GEMM)", smem=smem_obj(K4_PROFILE, t_ms)),
+                                smem=smem_obj(K4C_PROFILE if check_ms == 0.0 else K4_PROFILE, score_ms)),
         place_check_kernel=(dict(ms=check_ms, bound="hbm", achieved=cand_bytes / (check_ms * 1e-3) / 1e9, peak=peaks["hbm"], unit="GB/s",
                                  frac=cand_bytes / (check_ms * 1e-3) / 1e9 / peaks["hbm"],
                                  note="exact validation (bit matrix in shared memory, one atomicOr per slot); reads the candidates a second time")
