@@ -86,6 +86,16 @@ class ClockSampler:
                                           "-i", str(self.gpu)], stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
+            return
+        # nvidia-smi needs a moment to attach: the timed region starts once the first sample is on disk
+        t0 = time.perf_counter()
+        while time.perf_counter() - t0 < 2.0:
+            try:
+                if os.path.getsize(self.path) > 0:
+                    break
+            except OSError:
+                pass
+            time.sleep(0.01)
 
     def stop(self):
         out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[])
