@@ -396,13 +396,17 @@ GIMBAL_API int gimbal_refine_placement(const gimbal_placement_cfg *cfg, int16_t 
  *                                candidates whose replica counts differ from x0's)
  *   GIMBAL_OPT_HIST_AGG          1 (default): the router GEMM epilogue counts a warp's 32 tokens by columns
  *                                (bit-matrix transpose, one shared atomic per lane and 32 experts) when they
- *                                share one source; 0: one predicated shared atomic per selected logit        */
+ *                                share one source; 0: one predicated shared atomic per selected logit
+ *   GIMBAL_OPT_SCORE_TMA         1 (default): on the 9-slots x 32-ranks x 256-experts shape with a scalar M, the
+ *                                scoring-only pass (GIMBAL_PLACE_TRUSTED) receives its candidate rows by TMA;
+ *                                0: per-lane global loads as on every other shape                              */
 #define GIMBAL_OPT_CTA_GROUP 0
 #define GIMBAL_OPT_FUSE_GATE 1
 #define GIMBAL_OPT_SCORE_GENERIC 2
 #define GIMBAL_OPT_CHECK_SCORES_ALL 3
 #define GIMBAL_OPT_HIST_AGG 4
-#define GIMBAL_OPT_COUNT_ 5
+#define GIMBAL_OPT_SCORE_TMA 5
+#define GIMBAL_OPT_COUNT_ 6
 GIMBAL_API int gimbal_set_option(int option, int value);
 GIMBAL_API int gimbal_get_option(int option, int *value);
 

@@ -104,7 +104,7 @@ size_t route_ws_carve(const gimbal_router_cfg* c, void* ws, RouteWs* out) {
 }
 
 // process-wide switches set through gimbal_set_option (tests and A/B measurements); defaults = production
-std::atomic<int> g_opt[GIMBAL_OPT_COUNT_] = {{0}, {1}, {0}, {0}, {1}};
+std::atomic<int> g_opt[GIMBAL_OPT_COUNT_] = {{0}, {1}, {0}, {0}, {1}, {1}};
 
 int pick_cta_group(int T) {
     const int forced = g_opt[GIMBAL_OPT_CTA_GROUP].load(std::memory_order_relaxed);
@@ -203,6 +203,20 @@ static int launch_score_v(const ScoreParams& sp, dim3 grid, size_t smem, cudaStr
     kern<<<grid, kScoreThreads, smem, stream>>>(sp);
     ktime_end(GIMBAL_KERNEL_SCORE, stream);
     LAUNCH_CHECK("place_score_kernel");
+    return GIMBAL_OK;
+}
+
+// the 9 x 32 x 256 shape, scalar M, scoring only: candidate rows by TMA (place_score_tma_kernel)
+static int launch_score_tma(const ScoreParams& sp, dim3 grid, cudaStream_t stream) {
+    CUtensorMap tm;
+    int rc = make_tmap_rows_i16_4d(&tm, sp.cand, 72, 4, (uint64_t)sp.L, (uint64_t)sp.P, 80, kScoreU);
+    if (rc) return rc;
+    const size_t smem = place_score_tma_smem_bytes();
+    CUDA_TRY(cudaFuncSetAttribute(place_score_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ktime_begin(GIMBAL_KERNEL_SCORE, stream);
+    place_score_tma_kernel<<<grid, kScoreThreads, smem, stream>>>(sp, tm);
+    ktime_end(GIMBAL_KERNEL_SCORE, stream);
+    LAUNCH_CHECK("place_score_tma_kernel");
     return GIMBAL_OK;
 }
 
@@ -558,7 +572,10 @@ int gimbal_eval_placements(const gimbal_placement_cfg* cfg, int P, const void* c
             sp.chunk = (P + nchunk - 1) / nchunk;
             dim3 grid((P + sp.chunk - 1) / sp.chunk, cfg->L);
             switch (fast ? key : 0) {
-                case 9032256: rc = launch_score<9, 32, 256>(sp, fused, grid, smem_k, stream); break;
+                case 9032256:
+                    if (!fused && !sp.has_M && g_opt[GIMBAL_OPT_SCORE_TMA].load(std::memory_order_relaxed)) rc = launch_score_tma(sp, grid, stream);
+                    else rc = launch_score<9, 32, 256>(sp, fused, grid, smem_k, stream);
+                    break;
                 case 8016128: rc = launch_score<8, 16, 128>(sp, fused, grid, smem_k, stream); break;
                 case 8008064: rc = launch_score<8, 8, 64>(sp, fused, grid, smem_k, stream); break;
                 case 4064256: rc = launch_score<4, 64, 256>(sp, fused, grid, smem_k, stream); break;

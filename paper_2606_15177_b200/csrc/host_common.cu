@@ -110,6 +110,23 @@ int make_tmap_bf16_3d(CUtensorMap* m, const void* ptr, uint64_t d0, uint64_t d1,
     return GIMBAL_OK;
 }
 
+// candidate rows [P][L][NS] int16 seen as [P][L][NS/piece][piece]; the box is `box0` >= piece elements wide, so every piece
+// lands at a pitch of box0 elements in shared memory with the tail zero-filled (out-of-bounds fill), `boxP` candidates per copy
+int make_tmap_rows_i16_4d(CUtensorMap* m, const void* ptr, uint32_t piece, uint32_t npieces, uint64_t L, uint64_t P, uint32_t box0,
+                          uint32_t boxP) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return fail(GIMBAL_ERR_CUDA, "cuTensorMapEncodeTiled not available");
+    cuuint64_t dims[4] = {piece, npieces, L, P};
+    cuuint64_t strides[3] = {(cuuint64_t)piece * 2, (cuuint64_t)piece * npieces * 2, (cuuint64_t)piece * npieces * 2 * L};
+    cuuint32_t box[4] = {box0, npieces, 1, boxP};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT16, 4, const_cast<void*>(ptr), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(GIMBAL_ERR_CUDA, "cuTensorMapEncodeTiled (candidate rows) failed (%d)", (int)r);
+    return GIMBAL_OK;
+}
+
 GateParams gate_params(const gimbal_router_cfg* c) {
     GateParams g;
     g.k = c->k; g.score_fn = c->score_fn; g.renorm = c->renorm; g.n_groups = c->n_groups;

@@ -42,6 +42,9 @@ constexpr size_t kSmemLimit = 227 * 1024;
 // bf16 tensor [d2][d1][d0] (d0 contiguous), box [1][box1][64], 128-byte swizzle
 int make_tmap_bf16_3d(CUtensorMap* m, const void* ptr, uint64_t d0, uint64_t d1, uint64_t d2, uint32_t box1);
 
+int make_tmap_rows_i16_4d(CUtensorMap* m, const void* ptr, uint32_t piece, uint32_t npieces, uint64_t L, uint64_t P, uint32_t box0,
+                          uint32_t boxP);
+
 struct RouteArgs {
     const gimbal_router_cfg* cfg;
     int layer0, n_layers, T;

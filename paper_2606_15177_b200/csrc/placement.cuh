@@ -30,6 +30,8 @@
 #include <math_constants.h>
 #include <stdint.h>
 
+#include "ptx.cuh"
+
 namespace gimbal {
 
 constexpr int kMaxE = 256;
@@ -440,6 +442,171 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_kernel(const Sco
         pass(bufA, bufB);
         if (pc + kU * kStride >= p_end) break;
         pass(bufB, bufA);
+    }
+}
+
+// The 9-slots-per-rank shape (32 ranks, 288 slots, 256 experts; scalar M, no fused validation) with the candidate rows
+// delivered by TMA.  A rank's 18 bytes start on an odd half-word for every other rank, so the per-lane global loads of
+// place_score_kernel touch all 18 sectors of a row in each of their five instructions (92 tag look-ups per row); here ONE
+// tiled copy per warp pass brings two rows into the warp's shared-memory ring.  The tensor map sees a row as 4 pieces of
+// 72 ids and asks for a box 80 ids wide: each piece lands at a 160-byte pitch (tail zero-filled), which spreads the 32
+// lanes' words over the 32 banks -- five conflict-free LDS.32 per lane and row.  No L1 tag traffic, no register ping-pong.
+constexpr int kTmaRowPitch = 640;                     // 4 pieces x 160 B
+constexpr int kTmaSlots = 2;                          // ring slots per warp, one pass (two rows) each
+inline size_t place_score_tma_smem_bytes() {
+    return (size_t)256 * 256 + (size_t)(kScoreThreads / 32) * kTmaSlots * kScoreU * kTmaRowPitch + (kScoreThreads / 32) * kTmaSlots * 8;
+}
+
+__device__ __forceinline__ uint32_t lds_u32_ordered(uint32_t addr) {      // ordered among the volatile asm statements (barrier wait before, refill after)
+    uint32_t v;
+    asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ float2 lds_f32x2(uint32_t addr) {               // a table cell; its address depends on words read after the barrier wait
+    float2 v;
+    asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+
+__global__ void __launch_bounds__(kScoreThreads, 2) place_score_tma_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tm) {
+    constexpr int SP = 9, G = 32, E = 256, NS = G * SP, NW = 5, kU = kScoreU, kWarps = kScoreThreads / 32;
+    constexpr uint32_t kPassBytes = kU * kTmaRowPitch;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    const int l = blockIdx.y;
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);          // warp-uniform for the compiler too
+    const int lane = threadIdx.x & 31;
+    const int p_begin = blockIdx.x * p.chunk, p_end = min(p.P, p_begin + p.chunk);
+    constexpr int kPassStride = kWarps * kU;                                         // candidates between two passes of a warp
+    const int c_first = p_begin + warp * kU;
+    const uint32_t tab_a = __shfl_sync(0xffffffffu, ptx::smem_u32(smem_raw), 0);     // [E][32] float2
+    const uint32_t ring_a = tab_a + (uint32_t)E * 256u + (uint32_t)warp * (kTmaSlots * kPassBytes);          // [slots][kU][640] of this warp
+    const uint32_t bar_a = tab_a + (uint32_t)E * 256u + (uint32_t)kWarps * (kTmaSlots * kPassBytes) + (uint32_t)warp * (kTmaSlots * 8);
+    const uint64_t pol = ptx::policy_evict_first();
+    if (ptx::elect_one()) {
+#pragma unroll
+        for (int s = 0; s < kTmaSlots; ++s) ptx::mbar_init(bar_a + 8 * s, 1);
+        ptx::fence_barrier_init();
+        ptx::fence_proxy_async();
+        // the first rows are on their way while the table is staged
+#pragma unroll
+        for (int s = 0; s < kTmaSlots; ++s) {
+            const int c = c_first + s * kPassStride;
+            if (c < p_end) {
+                ptx::mbar_arrive_expect_tx(bar_a + 8 * s, kPassBytes);
+                ptx::tma_load_4d(ring_a + s * kPassBytes, &tm, bar_a + 8 * s, 0, 0, l, c, pol);
+            }
+        }
+    }
+    {
+        constexpr int N4 = E * 16, kIt = N4 / kScoreThreads;
+        const uint4* src = reinterpret_cast<const uint4*>(p.t.wc + (size_t)l * E * 32);
+        uint4* dst = reinterpret_cast<uint4*>(smem_raw);
+        uint4 tmp[kIt];
+#pragma unroll
+        for (int k = 0; k < kIt; ++k) tmp[k] = __ldg(src + threadIdx.x + k * kScoreThreads);
+#pragma unroll
+        for (int k = 0; k < kIt; ++k) dst[threadIdx.x + k * kScoreThreads] = tmp[k];
+    }
+    const double sumB = p.t.sumB[l];
+    const float sumB_hi = (float)sumB, sumB_lo = (float)(sumB - (double)sumB_hi);
+    const uint32_t lane8 = (uint32_t)lane * 8u;
+    const float M_scalar = p.M_scalar;
+    float4* const partial = p.partial;
+    const int L = p.L;
+    // this lane's rank: piece lane / 8, then 18 bytes per rank inside the piece (word-aligned start, odd ranks begin in the upper half)
+    const uint32_t lane_off = (uint32_t)(lane >> 3) * 160u + 4u * ((9u * (uint32_t)(lane & 7)) >> 1);
+    const uint32_t sh = (uint32_t)(lane & 1) * 16u;
+    __syncthreads();
+
+    // one warp pass: two rows out of the ring, scored into slots `q`, `q + 1` of the pending results
+    float sq[2 * kU], comm[2 * kU], mx[2 * kU];
+    uint32_t kept[2 * kU];
+    uint32_t it = 0;
+    auto pass = [&](int c0, int q) {
+        const uint32_t slot = it & (kTmaSlots - 1);
+        const uint32_t bar = bar_a + 8 * slot, rows = ring_a + slot * kPassBytes;
+        ptx::mbar_wait(bar, (it / kTmaSlots) & 1u);
+        ++it;
+        uint32_t w[kU][NW];
+#pragma unroll
+        for (int u = 0; u < kU; ++u)
+#pragma unroll
+            for (int j = 0; j < NW; ++j) w[u][j] = lds_u32_ordered(rows + u * kTmaRowPitch + 4 * j + lane_off);
+        // refill the slot with the pass after next.  (The shifts below are needed anyway; as volatile statements they sit between the
+        // loads and the copy, so the copy is issued only after the last word of every row has arrived in its register.)
+        uint32_t wlast[kU];
+#pragma unroll
+        for (int u = 0; u < kU; ++u)
+            asm volatile("shf.r.wrap.b32 %0, %1, %2, %3;" : "=r"(wlast[u]) : "r"(w[u][NW - 2]), "r"(w[u][NW - 1]), "r"(sh));
+        if (c0 + kTmaSlots * kPassStride < p_end) {
+            __syncwarp();
+            if (ptx::elect_one()) {
+                ptx::mbar_arrive_expect_tx(bar, kPassBytes);
+                ptx::tma_load_4d(rows, &tm, bar, 0, 0, l, c0 + kTmaSlots * kPassStride, pol);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+#pragma unroll
+            for (int j = 0; j + 2 < NW; ++j) w[u][j] = __funnelshift_r(w[u][j], w[u][j + 1], sh);
+            w[u][NW - 2] = wlast[u];                                                                 // realigned above
+            w[u][NW - 1] = w[u][NW - 1] >> sh;
+            float lg2[2], cm2[2];
+            uint32_t kp2[2];
+#pragma unroll
+            for (int j = 0; j < SP; ++j) {
+                const uint32_t off = __byte_perm(w[u][j >> 1], lane8, (j & 1) ? 0x5524 : 0x5504);   // id << 8 | lane * 8
+                const float2 wc = lds_f32x2(tab_a + off);
+                if (j < 2) {
+                    lg2[j] = wc.x; cm2[j] = fabsf(wc.y); kp2[j] = __float_as_uint(wc.y) >> 31;
+                } else {
+                    lg2[j & 1] += wc.x;
+                    cm2[j & 1] += fabsf(wc.y);
+                    kp2[j & 1] += __float_as_uint(wc.y) >> 31;
+                }
+            }
+            const float lg = lg2[0] + lg2[1];
+            comm[q + u] = cm2[0] + cm2[1];
+            kept[q + u] = kp2[0] + kp2[1];
+            const float d = __fsub_rn(__fmaf_rn(lg, (float)G, -sumB_hi), sumB_lo);   // G*L_g - sum_g L_g
+            sq[q + u] = d * d;
+            mx[q + u] = lg;
+        }
+    };
+    // Two passes share one transposed butterfly over their four rows (eight sums): lane bits 16 and 8 pick the row, bit 4 the
+    // kind (sq / comm) -- 4 + 2 + 1 + 1 + 1 shuffles and one exchange for four rows.  Row r = (bit16, bit8) is candidate
+    // c0 + (r & 1) of pass r >> 1.
+    const bool b16 = (lane & 16) != 0, b8 = (lane & 8) != 0, b4 = (lane & 4) != 0;
+    for (int c0 = c_first; c0 < p_end; c0 += 2 * kPassStride) {
+        pass(c0, 0);
+        const bool two = c0 + kPassStride < p_end;
+        if (two) pass(c0 + kPassStride, kU);
+        else {
+#pragma unroll
+            for (int u = 0; u < kU; ++u) sq[kU + u] = comm[kU + u] = mx[kU + u] = 0.0f, kept[kU + u] = 0u;
+        }
+        float s0 = (b16 ? sq[2] : sq[0]) + __shfl_xor_sync(0xffffffffu, b16 ? sq[0] : sq[2], 16);
+        float s1 = (b16 ? sq[3] : sq[1]) + __shfl_xor_sync(0xffffffffu, b16 ? sq[1] : sq[3], 16);
+        float m0 = (b16 ? comm[2] : comm[0]) + __shfl_xor_sync(0xffffffffu, b16 ? comm[0] : comm[2], 16);
+        float m1 = (b16 ? comm[3] : comm[1]) + __shfl_xor_sync(0xffffffffu, b16 ? comm[1] : comm[3], 16);
+        const float s = (b8 ? s1 : s0) + __shfl_xor_sync(0xffffffffu, b8 ? s0 : s1, 8);
+        const float m = (b8 ? m1 : m0) + __shfl_xor_sync(0xffffffffu, b8 ? m0 : m1, 8);
+        float v = (b4 ? m : s) + __shfl_xor_sync(0xffffffffu, b4 ? s : m, 4);
+        v += __shfl_xor_sync(0xffffffffu, v, 2);
+        v += __shfl_xor_sync(0xffffffffu, v, 1);
+        const float commt = __shfl_xor_sync(0xffffffffu, v, 4);                 // lanes with bit 4 clear: v = sq, commt = comm
+        const float mxa0 = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(mx[0])));   // loads are >= 0
+        const float mxa1 = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(mx[1])));
+        const float mxa2 = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(mx[2])));
+        const float mxa3 = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(mx[3])));
+        const uint32_t k01 = __reduce_add_sync(0xffffffffu, kept[0] | (kept[1] << 16));
+        const uint32_t k23 = __reduce_add_sync(0xffffffffu, kept[2] | (kept[3] << 16));
+        const uint32_t kk = b16 ? k23 : k01;
+        const int k = b8 ? (int)(kk >> 16) : (int)(kk & 0xffffu);
+        const float migt = M_scalar * (float)(2 * (NS - k));
+        const float mxa = b16 ? (b8 ? mxa3 : mxa2) : (b8 ? mxa1 : mxa0);
+        const int mine = c0 + (b16 ? kPassStride : 0) + (b8 ? 1 : 0);
+        if ((lane & 7) == 0 && mine < p_end) partial[(size_t)mine * L + l] = make_float4(v, commt, migt, mxa);
     }
 }
 
