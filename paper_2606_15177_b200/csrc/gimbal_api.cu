@@ -143,6 +143,8 @@ static size_t place_ws_carve(const gimbal_placement_cfg* c, int P, void* ws, Pla
     const size_t LE = (size_t)c->L * c->E;
     const size_t NSl = (size_t)c->L * c->G * c->slots_per_rank;
     w.t.wc = cv.take<float2>(LE * GP);
+    w.t.c_s = cv.take<float>(LE * GP);
+    w.t.w_f = cv.take<float>(LE);
     w.t.m = cv.take<float>(LE * GP);
     w.t.mu = cv.take<uint32_t>(LE * GP);
     w.t.mx0 = cv.take<float>(NSl);

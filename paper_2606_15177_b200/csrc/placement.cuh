@@ -39,6 +39,8 @@ constexpr int kMaxG = 64;
 
 struct PlaceTables {
     float2* wc;        // [L][GP/32][E][32]  {w, c with sign bit = member of x0}
+    float* c_s;        // [L][GP/32][E][32]  the c half of wc alone, and
+    float* w_f;        // [L][E]             its w half: what place_score_tma_kernel stages (half the bytes)
     float* m;          // [L][GP/32][E][32]  M[l,e,g]                                   (M table only)
     uint32_t* mu;      // [L][GP/32][E][32]  scoring word: float bits of M where x0 lacks the cell, else
                        //                    0x80000000 | 1 << (position of e among x0's slots of rank g)   (M table only)
@@ -116,6 +118,7 @@ __global__ void __launch_bounds__(256) place_tables_kernel(const TableParams p) 
             sb += b;
             p.t.b_raw[(size_t)l * p.E + e] = b;
             p.t.w_e[(size_t)l * p.E + e] = b / (double)max(r_s[e], 1);
+            p.t.w_f[(size_t)l * p.E + e] = (float)(b / (double)max(r_s[e], 1));
             p.t.r[(size_t)l * p.E + e] = r_s[e];
             p.t.pmask[(size_t)l * p.E + e] = pm_s[e];
         }
@@ -151,6 +154,7 @@ __global__ void __launch_bounds__(256) place_tables_kernel(const TableParams p) 
         const float w = (float)(b / (double)re);
         const size_t at = tab + tab_idx(p.E, e, gp);
         p.t.wc[at] = make_float2(w, member ? -c : c);   // -0.0f keeps the flag when c == 0
+        p.t.c_s[at] = member ? -c : c;
         if (p.M) {
             const float mm = p.M[((size_t)l * p.E + e) * p.G + g];
             p.t.m[at] = mm;
@@ -169,6 +173,7 @@ struct ScoreParams {
     float4* partial;                    // [P,L] {sum_g d_g^2, comm, mig, maxL}; NaN in .x if invalid
     uint8_t* status;                    // [L,P] verdicts of the fused validation (kCheck): 0 same copies as x0, 1 invalid, 2 other replica counts
     int force_general;                  // tests: verdict 2 for every valid candidate
+    uint32_t zero;                      // 0, opaque to the compiler (place_score_tma_kernel's ordering dependency)
 };
 
 constexpr int kScoreThreads = 512;
@@ -498,14 +503,23 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_tma_kernel(const
         }
     }
     {
-        constexpr int N4 = E * 16, kIt = N4 / kScoreThreads;
-        const uint4* src = reinterpret_cast<const uint4*>(p.t.wc + (size_t)l * E * 32);
-        uint4* dst = reinterpret_cast<uint4*>(smem_raw);
-        uint4 tmp[kIt];
+        // the table {w, c}[E][32] is put together from its compact halves: c[E][32] and w[E] (half the bytes out of L2)
+        constexpr int N4 = E * 8, kIt = N4 / kScoreThreads;
+        const float4* src = reinterpret_cast<const float4*>(p.t.c_s + (size_t)l * E * 32);
+        const float* wsrc = p.t.w_f + (size_t)l * E;
+        float4* dst = reinterpret_cast<float4*>(smem_raw);
+        float4 tmp[kIt];
+        float wv[kIt];
 #pragma unroll
-        for (int k = 0; k < kIt; ++k) tmp[k] = __ldg(src + threadIdx.x + k * kScoreThreads);
+        for (int k = 0; k < kIt; ++k) {
+            tmp[k] = __ldg(src + threadIdx.x + k * kScoreThreads);
+            wv[k] = __ldg(wsrc + ((threadIdx.x + k * kScoreThreads) >> 3));
+        }
 #pragma unroll
-        for (int k = 0; k < kIt; ++k) dst[threadIdx.x + k * kScoreThreads] = tmp[k];
+        for (int k = 0; k < kIt; ++k) {
+            dst[2 * (threadIdx.x + k * kScoreThreads)] = make_float4(wv[k], tmp[k].x, wv[k], tmp[k].y);
+            dst[2 * (threadIdx.x + k * kScoreThreads) + 1] = make_float4(wv[k], tmp[k].z, wv[k], tmp[k].w);
+        }
     }
     const double sumB = p.t.sumB[l];
     const float sumB_hi = (float)sumB, sumB_lo = (float)(sumB - (double)sumB_hi);
@@ -532,24 +546,21 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_tma_kernel(const
         for (int u = 0; u < kU; ++u)
 #pragma unroll
             for (int j = 0; j < NW; ++j) w[u][j] = lds_u32_ordered(rows + u * kTmaRowPitch + 4 * j + lane_off);
-        // refill the slot with the pass after next.  (The shifts below are needed anyway; as volatile statements they sit between the
-        // loads and the copy, so the copy is issued only after the last word of every row has arrived in its register.)
-        uint32_t wlast[kU];
-#pragma unroll
-        for (int u = 0; u < kU; ++u)
-            asm volatile("shf.r.wrap.b32 %0, %1, %2, %3;" : "=r"(wlast[u]) : "r"(w[u][NW - 2]), "r"(w[u][NW - 1]), "r"(sh));
+        // refill the slot with the pass after next: the copy (async proxy) overwrites what the loads above read, and ptxas is free to
+        // issue it while they are still queued -- at kernel start, when all warps fire at once, a queued load has been seen to lose
+        // that race.  So the copy's candidate coordinate carries a true dependency on the words of every lane: an OR-reduction over
+        // the warp of (first | last word of both rows) & p.zero, which the host sets to 0 and the compiler cannot fold.
         if (c0 + kTmaSlots * kPassStride < p_end) {
-            __syncwarp();
+            const uint32_t dep = __reduce_or_sync(0xffffffffu, (w[0][0] | w[0][NW - 1] | w[kU - 1][0] | w[kU - 1][NW - 1]) & p.zero);
             if (ptx::elect_one()) {
                 ptx::mbar_arrive_expect_tx(bar, kPassBytes);
-                ptx::tma_load_4d(rows, &tm, bar, 0, 0, l, c0 + kTmaSlots * kPassStride, pol);
+                ptx::tma_load_4d(rows, &tm, bar, 0, 0, l, c0 + kTmaSlots * kPassStride + (int)dep, pol);
             }
         }
 #pragma unroll
         for (int u = 0; u < kU; ++u) {
 #pragma unroll
-            for (int j = 0; j + 2 < NW; ++j) w[u][j] = __funnelshift_r(w[u][j], w[u][j + 1], sh);
-            w[u][NW - 2] = wlast[u];                                                                 // realigned above
+            for (int j = 0; j + 1 < NW; ++j) w[u][j] = __funnelshift_r(w[u][j], w[u][j + 1], sh);
             w[u][NW - 1] = w[u][NW - 1] >> sh;
             float lg2[2], cm2[2];
             uint32_t kp2[2];

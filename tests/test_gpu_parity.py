@@ -1159,3 +1159,39 @@ def test_eval_placements_and_moves_on_other_shapes(L, E, G, sp, S, table_M, coun
     per = n // L
     for l in range(L):
         assert int(best[l].item()) == l * per + int(np.nanargmin(to_np(delta)[l * per:(l + 1) * per, 0]))
+
+
+@pytest.mark.parametrize("P,L", [(1, 2), (2, 3), (31, 2), (33, 1), (97, 4), (1000, 5), (2051, 58)])
+def test_place_score_tma_kernel_matches_the_lane_load_kernel_and_the_oracle(P, L):
+    """The 9 x 32 x 256 shape, scalar M, GIMBAL_PLACE_TRUSTED: rows delivered by TMA (place_score_tma_kernel, the default) against
+    the per-lane-load kernel (GIMBAL_OPT_SCORE_TMA = 0) bit for bit -- odd and ragged P (a copy's second candidate past the end,
+    chunks that are not a multiple of a warp pass), one block per layer up to the bench grid -- and against the oracle on a
+    sample.  Repeated right after a large memset so that every warp's first passes really wait on their barriers; the ring's
+    write-after-read ordering (K4) once failed exactly there."""
+    w = scaled(get_workload("v3"), L=L, T=256, P=P)
+    r = w.router
+    rng = np.random.default_rng(11 + P)
+    A = torch.from_numpy(rng.integers(0, 3000, (L, r.S, r.E)).astype(np.int32)).to(DEV)
+    B = (A.sum(1) * 3).to(torch.int32)
+    cfg = g.PlacementCfg(L=L, E=r.E, G=w.G, slots_per_rank=w.slots_per_rank, S=r.S, flags=g.PLACE_TRUSTED)
+    D = gen.comm_cost_D(w, "seeded", DEV)
+    prev = gen.prev_placement(w, to_np(B), DEV)
+    cands = gen.candidates(w, prev, P, DEV)
+    ws = ws_tensor(g.eval_placements_workspace_bytes(cfg, P))
+    flush = torch.empty(64 << 20, dtype=torch.uint8, device=DEV)
+    outs = {}
+    for tma in (0, 1):
+        g.set_option(g.OPT_SCORE_TMA, tma)
+        for rep in range(1 if tma == 0 else 12):
+            out = torch.full((P, 5), -3.0, device=DEV)
+            flush.zero_()
+            g.eval_placements(cfg, cands, A, B, D, prev, out, M_scalar=0.75, workspace=ws)
+            torch.cuda.synchronize()
+            if tma in outs:
+                assert torch.equal(out, outs[tma]), f"run {rep} differs from run 0"
+            outs[tma] = out
+    assert torch.equal(outs[0], outs[1])
+    pick = np.unique(np.concatenate([[0, P - 1, P // 2], rng.integers(0, P, 12)]))
+    ref = oracle.objective_batch(to_np(cands)[pick], to_np(prev), to_np(A), to_np(B), to_np(D), None, 0.75, **_oracle_kw(cfg))
+    _check_objective(to_np(outs[1]).astype(np.float64)[pick], ref)
+    assert to_np(outs[1])[0, 3] == 0.0
