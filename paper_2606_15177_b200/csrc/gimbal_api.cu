@@ -374,13 +374,16 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
 
     // a3 accumulates into A_step: zero the slice of this call
     CUDA_TRY(cudaMemsetAsync(st->A_step + (size_t)layer0 * cfg->S * cfg->E, 0, sizeof(int32_t) * (size_t)n_layers * cfg->S * cfg->E, stream));
-    if (layer0 == 0) CUDA_TRY(cudaMemsetAsync(ws.done, 0, sizeof(unsigned int), stream));
+    // stats_update_kernel's block counter starts at 0: the router kernel of this call clears it where there is one, else a memset
+    const bool gemm_clears = layer0 == 0 && T > 0 && logits_mode != GIMBAL_LOGITS_IN;
+    if (layer0 == 0 && !gemm_clears) CUDA_TRY(cudaMemsetAsync(ws.done, 0, sizeof(unsigned int), stream));
 
     if (T > 0) {
         RouteArgs a{};
         a.cfg = cfg; a.layer0 = layer0; a.n_layers = n_layers; a.T = T; a.hidden = hidden; a.w_router = w_router;
         a.select_bias = select_bias; a.src_logit_bias = src_logit_bias; a.src_offsets = src_offsets;
         a.topk_ids = topk_ids; a.topk_w = topk_w; a.A_step = st->A_step; a.stream = stream;
+        a.zero_word = gemm_clears ? ws.done : nullptr;
         if (map) { a.rep_off = map->rep_off; a.rep_slots = map->rep_slots; a.phys_ids = map->phys_ids; a.map_NS = map->NS; }
         a.cta_group = pick_cta_group(T);
         a.hist_agg = g_opt[GIMBAL_OPT_HIST_AGG].load(std::memory_order_relaxed);

@@ -52,6 +52,7 @@ struct RouteArgs {
     const float* select_bias; const float* src_logit_bias; const int32_t* src_offsets;
     float* logits; int32_t* topk_ids; float* topk_w;
     int32_t* A_step;
+    unsigned int* zero_word;   // | nullptr: workspace word the fused router kernel clears (saves a memset node per step)
     const int32_t* rep_off; const int16_t* rep_slots; int32_t* phys_ids; int map_NS;   // expert mapping | nullptr
     int fuse_gate;
     int cta_group;          // 1 or 2

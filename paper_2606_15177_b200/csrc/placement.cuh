@@ -503,23 +503,21 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_tma_kernel(const
         }
     }
     {
-        // the table {w, c}[E][32] is put together from its compact halves: c[E][32] and w[E] (half the bytes out of L2)
-        constexpr int N4 = E * 8, kIt = N4 / kScoreThreads;
-        const float4* src = reinterpret_cast<const float4*>(p.t.c_s + (size_t)l * E * 32);
+        // the table {w, c}[E][32] is put together from its compact halves: c[E][32] and w[E] (half the bytes out of L2); a thread
+        // takes two cells at a time, so a warp's 16-byte stores are contiguous (no bank conflicts)
+        constexpr int N2 = E * 16, kIt = N2 / kScoreThreads;
+        const float2* src = reinterpret_cast<const float2*>(p.t.c_s + (size_t)l * E * 32);
         const float* wsrc = p.t.w_f + (size_t)l * E;
         float4* dst = reinterpret_cast<float4*>(smem_raw);
-        float4 tmp[kIt];
+        float2 tmp[kIt];
         float wv[kIt];
 #pragma unroll
         for (int k = 0; k < kIt; ++k) {
             tmp[k] = __ldg(src + threadIdx.x + k * kScoreThreads);
-            wv[k] = __ldg(wsrc + ((threadIdx.x + k * kScoreThreads) >> 3));
+            wv[k] = __ldg(wsrc + ((threadIdx.x + k * kScoreThreads) >> 4));
         }
 #pragma unroll
-        for (int k = 0; k < kIt; ++k) {
-            dst[2 * (threadIdx.x + k * kScoreThreads)] = make_float4(wv[k], tmp[k].x, wv[k], tmp[k].y);
-            dst[2 * (threadIdx.x + k * kScoreThreads) + 1] = make_float4(wv[k], tmp[k].z, wv[k], tmp[k].w);
-        }
+        for (int k = 0; k < kIt; ++k) dst[threadIdx.x + k * kScoreThreads] = make_float4(wv[k], tmp[k].x, wv[k], tmp[k].y);
     }
     const double sumB = p.t.sumB[l];
     const float sumB_hi = (float)sumB, sumB_lo = (float)(sumB - (double)sumB_hi);

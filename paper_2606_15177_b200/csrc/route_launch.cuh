@@ -23,7 +23,7 @@ int launch_gemm_t(const RouteArgs& a) {
     if (p.stages < 2) return fail(GIMBAL_ERR_UNSUPPORTED, "router GEMM: not enough shared memory for E=%d S=%d", N, c->S);
     p.src_logit_bias = a.src_logit_bias; p.src_offsets = a.src_offsets; p.logits = a.logits;
     p.do_gate = a.fuse_gate; p.select_bias = a.select_bias; p.topk_ids = a.topk_ids; p.topk_w = a.topk_w;
-    p.A_step = a.A_step; p.gp = gate_params(c);
+    p.A_step = a.A_step; p.gp = gate_params(c); p.zero_word = a.zero_word;
     p.map = ExpertMap{a.rep_off, a.rep_slots, a.phys_ids, a.map_NS};
     const size_t smem = gemm_smem_bytes<N, kCG>(c->S, p.stages, out);
     auto kern = router_gemm_kernel<N, kCG, kSig>;

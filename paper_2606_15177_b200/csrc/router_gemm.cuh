@@ -35,6 +35,7 @@ struct GemmParams {
     int32_t* topk_ids;
     float* topk_w;
     int32_t* A_step;                // [L,S,E]
+    unsigned int* zero_word;        // | nullptr: a workspace word this launch clears (stats_update_kernel's block counter)
     GateParams gp;
     ExpertMap map;
 };
@@ -146,6 +147,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
     const int n_tiles = p.n_layers * p.m_tiles;
     const int num_kb = (p.H + kBlockK - 1) / kBlockK;
 
+    if (blockIdx.x == 0 && threadIdx.x == 32 && p.zero_word) *p.zero_word = 0u;     // consumed by the next kernel of the stream
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tmap(&tmap_a);
         ptx::prefetch_tmap(&tmap_b);
