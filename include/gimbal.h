@@ -399,14 +399,19 @@ GIMBAL_API int gimbal_refine_placement(const gimbal_placement_cfg *cfg, int16_t 
  *                                share one source; 0: one predicated shared atomic per selected logit
  *   GIMBAL_OPT_SCORE_TMA         1 (default): on the 9-slots x 32-ranks x 256-experts shape with a scalar M, the
  *                                scoring-only pass (GIMBAL_PLACE_TRUSTED) receives its candidate rows by TMA;
- *                                0: per-lane global loads as on every other shape                              */
+ *                                0: per-lane global loads as on every other shape
+ *   GIMBAL_OPT_EPI_PARTS         0 (default: auto), 1 or 2: epilogue warps per TMEM lane quadrant of the fused router kernel.
+ *                                2 (E >= 128, counts only) splits a row's experts between two warps that meet in shared
+ *                                memory; auto picks it when no CTA pair gets more than two tiles (small-batch regime, where
+ *                                the epilogue is not hidden behind the MMAs)                                       */
 #define GIMBAL_OPT_CTA_GROUP 0
 #define GIMBAL_OPT_FUSE_GATE 1
 #define GIMBAL_OPT_SCORE_GENERIC 2
 #define GIMBAL_OPT_CHECK_SCORES_ALL 3
 #define GIMBAL_OPT_HIST_AGG 4
 #define GIMBAL_OPT_SCORE_TMA 5
-#define GIMBAL_OPT_COUNT_ 6
+#define GIMBAL_OPT_EPI_PARTS 6
+#define GIMBAL_OPT_COUNT_ 7
 GIMBAL_API int gimbal_set_option(int option, int value);
 GIMBAL_API int gimbal_get_option(int option, int *value);
 

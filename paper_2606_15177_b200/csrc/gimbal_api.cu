@@ -104,7 +104,7 @@ size_t route_ws_carve(const gimbal_router_cfg* c, void* ws, RouteWs* out) {
 }
 
 // process-wide switches set through gimbal_set_option (tests and A/B measurements); defaults = production
-std::atomic<int> g_opt[GIMBAL_OPT_COUNT_] = {{0}, {1}, {0}, {0}, {1}, {1}};
+std::atomic<int> g_opt[GIMBAL_OPT_COUNT_] = {{0}, {1}, {0}, {0}, {1}, {1}, {0}};
 
 int pick_cta_group(int T) {
     const int forced = g_opt[GIMBAL_OPT_CTA_GROUP].load(std::memory_order_relaxed);
@@ -304,8 +304,9 @@ int64_t gimbal_launch_count(void) { return gimbal::launches(); }
 
 int gimbal_set_option(int option, int value) {
     if (option < 0 || option >= GIMBAL_OPT_COUNT_) return fail(GIMBAL_ERR_INVALID_ARG, "option %d", option);
-    if (option == GIMBAL_OPT_CTA_GROUP && (value < 0 || value > 2)) return fail(GIMBAL_ERR_INVALID_ARG, "GIMBAL_OPT_CTA_GROUP takes 0 (auto), 1 or 2");
-    if (option != GIMBAL_OPT_CTA_GROUP && value != 0 && value != 1) return fail(GIMBAL_ERR_INVALID_ARG, "option %d takes 0 or 1", option);
+    if ((option == GIMBAL_OPT_CTA_GROUP || option == GIMBAL_OPT_EPI_PARTS) && (value < 0 || value > 2))
+        return fail(GIMBAL_ERR_INVALID_ARG, "option %d takes 0 (auto), 1 or 2", option);
+    if (option != GIMBAL_OPT_CTA_GROUP && option != GIMBAL_OPT_EPI_PARTS && value != 0 && value != 1) return fail(GIMBAL_ERR_INVALID_ARG, "option %d takes 0 or 1", option);
     g_opt[option].store(value, std::memory_order_relaxed);
     return GIMBAL_OK;
 }
@@ -387,6 +388,14 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
         if (map) { a.rep_off = map->rep_off; a.rep_slots = map->rep_slots; a.phys_ids = map->phys_ids; a.map_NS = map->NS; }
         a.cta_group = pick_cta_group(T);
         a.hist_agg = g_opt[GIMBAL_OPT_HIST_AGG].load(std::memory_order_relaxed);
+        {
+            // epilogue parts: auto = 2 when no CTA (pair) gets more than two tiles, i.e. when the epilogue cannot hide behind the MMAs
+            const int forced = g_opt[GIMBAL_OPT_EPI_PARTS].load(std::memory_order_relaxed);
+            const int rows = 128 * a.cta_group;
+            const long tiles = (long)n_layers * ((T + rows - 1) / rows);
+            const int pairs = device_info().sms / a.cta_group;
+            a.epi_parts = forced ? forced : (tiles <= 2L * pairs ? 2 : 1);
+        }
         if (logits_mode == GIMBAL_LOGITS_IN) {
             a.logits = logits;
             rc = launch_gate(a);

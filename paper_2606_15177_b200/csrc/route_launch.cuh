@@ -6,7 +6,7 @@
 
 namespace gimbal {
 
-template <int N, int kCG, bool kSig>
+template <int N, int kCG, bool kSig, int kEP = 1>
 int launch_gemm_t(const RouteArgs& a) {
     const gimbal_router_cfg* c = a.cfg;
     CUtensorMap ta, tb;
@@ -18,15 +18,15 @@ int launch_gemm_t(const RouteArgs& a) {
     p.n_layers = a.n_layers; p.layer0 = a.layer0; p.T = a.T; p.H = c->H; p.S = c->S;
     p.m_tiles = (a.T + kBlockM * kCG - 1) / (kBlockM * kCG);
     const bool out = a.fuse_gate && (a.topk_ids || a.topk_w || a.rep_off);
-    p.stages = gemm_pick_stages<N, kCG>(c->S, out);
+    p.stages = gemm_pick_stages<N, kCG>(c->S, out, kEP);
     p.hist_agg = a.hist_agg;
     if (p.stages < 2) return fail(GIMBAL_ERR_UNSUPPORTED, "router GEMM: not enough shared memory for E=%d S=%d", N, c->S);
     p.src_logit_bias = a.src_logit_bias; p.src_offsets = a.src_offsets; p.logits = a.logits;
     p.do_gate = a.fuse_gate; p.select_bias = a.select_bias; p.topk_ids = a.topk_ids; p.topk_w = a.topk_w;
     p.A_step = a.A_step; p.gp = gate_params(c); p.zero_word = a.zero_word;
     p.map = ExpertMap{a.rep_off, a.rep_slots, a.phys_ids, a.map_NS};
-    const size_t smem = gemm_smem_bytes<N, kCG>(c->S, p.stages, out);
-    auto kern = router_gemm_kernel<N, kCG, kSig>;
+    const size_t smem = gemm_smem_bytes<N, kCG>(c->S, p.stages, out, kEP);
+    auto kern = router_gemm_kernel<N, kCG, kSig, kEP>;
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int sms = device_info().sms;
     const int n_tiles = p.n_layers * p.m_tiles;
@@ -34,7 +34,7 @@ int launch_gemm_t(const RouteArgs& a) {
     if (pairs > n_tiles) pairs = n_tiles;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(pairs * kCG);
-    cfg.blockDim = dim3(kGemmThreads);
+    cfg.blockDim = dim3(128 + 128 * kEP);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = a.stream;
     cudaLaunchAttribute attr[1];
@@ -51,6 +51,14 @@ int launch_gemm_t(const RouteArgs& a) {
 template <int N>
 int launch_gemm_n(const RouteArgs& a) {
     const bool sig = a.cfg->score_fn == GIMBAL_SCORE_SIGMOID;
+    if constexpr (N >= 128) {
+        // two epilogue warps per TMEM lane quadrant (each half of the experts) where the epilogue is exposed: counts only and at
+        // most two tiles per CTA (pair) -- the small-batch regime, one 128 / 256-token tile per layer
+        if (a.epi_parts == 2 && a.fuse_gate && !a.logits && !a.topk_ids && !a.topk_w && !a.rep_off) {
+            if (a.cta_group == 2) return sig ? launch_gemm_t<N, 2, true, 2>(a) : launch_gemm_t<N, 2, false, 2>(a);
+            return sig ? launch_gemm_t<N, 1, true, 2>(a) : launch_gemm_t<N, 1, false, 2>(a);
+        }
+    }
     if (a.cta_group == 2) return sig ? launch_gemm_t<N, 2, true>(a) : launch_gemm_t<N, 2, false>(a);
     return sig ? launch_gemm_t<N, 1, true>(a) : launch_gemm_t<N, 1, false>(a);
 }

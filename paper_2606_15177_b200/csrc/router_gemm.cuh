@@ -52,27 +52,28 @@ constexpr int kGemmMaxStages = 12;
 
 // bytes after the ring: [aux][select_bias N f32][src_offsets S+1 (padded)][hist S*N i32][selection list, when
 // ids / weights are written: kListWords x 128 epilogue threads]
+// ... [exchange buffers of the epilogue parts, ep > 1: 4 quadrants x [ep][8][32] words]
 template <int N>
-constexpr size_t gemm_tail_bytes(int S, bool out) {
+constexpr size_t gemm_tail_bytes(int S, bool out, int ep = 1) {
     return kGemmAuxBytes + sizeof(float) * N + sizeof(int32_t) * (size_t)((S + 1 + 3) & ~3) + sizeof(int32_t) * (size_t)S * N +
-           (out ? sizeof(int32_t) * (size_t)kListWords * 128 : 0);
+           (out ? sizeof(int32_t) * (size_t)kListWords * 128 : 0) + (ep > 1 ? sizeof(int32_t) * 4 * (size_t)ep * 8 * 32 : 0);
 }
 template <int N, int kCG>
-inline int gemm_pick_stages(int S, bool out) {
-    const long avail = (long)kGemmSmemLimit - 1024 - (long)gemm_tail_bytes<N>(S, out);
+inline int gemm_pick_stages(int S, bool out, int ep = 1) {
+    const long avail = (long)kGemmSmemLimit - 1024 - (long)gemm_tail_bytes<N>(S, out, ep);
     long s = avail / gemm_stage_bytes<N, kCG>();
     if (s > kGemmMaxStages) s = kGemmMaxStages;
     return (int)s;
 }
 template <int N, int kCG>
-inline size_t gemm_smem_bytes(int S, int stages, bool out) {
-    return 1024 + (size_t)stages * gemm_stage_bytes<N, kCG>() + gemm_tail_bytes<N>(S, out);
+inline size_t gemm_smem_bytes(int S, int stages, bool out, int ep = 1) {
+    return 1024 + (size_t)stages * gemm_stage_bytes<N, kCG>() + gemm_tail_bytes<N>(S, out, ep);
 }
 
 template <int N>
 struct TmemRowSrc {
-    uint32_t taddr;                 // lane base | column base of this accumulator stage
-    const float* bias;              // src_logit_bias row for this token (global) | nullptr
+    uint32_t taddr;                 // lane base | column base of this accumulator stage (+ the first chunk of this epilogue part)
+    const float* bias;              // src_logit_bias row for this token (global), from this part's first expert | nullptr
     static constexpr int CH = N < 32 ? N : 32;
     __device__ __forceinline__ void load_raw(int c, uint32_t (&r)[CH]) {
         if constexpr (CH == 32) ptx::tmem_ld_32x32b_x32(taddr + c * 32, r);
@@ -111,8 +112,8 @@ struct TmemRowSrc {
     }
 };
 
-template <int N, int kCG, bool kSig>
-__global__ void __launch_bounds__(kGemmThreads, 1)
+template <int N, int kCG, bool kSig, int kEP = 1>
+__global__ void __launch_bounds__(128 + 128 * kEP, 1)
 router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b, const GemmParams p) {
     const int kStages = p.stages;
     constexpr int kABytes = kBlockM * kBlockK * 2;
@@ -139,6 +140,9 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
     int32_t* off_s = reinterpret_cast<int32_t*>(sb_s + N);
     int32_t* hist = off_s + ((p.S + 1 + 3) & ~3);
     int32_t* list_s = hist + p.S * N;                    // [kListWords][128] (only when ids / weights are written)
+    int32_t* xbuf_s = list_s;                            // kEP > 1 (counts only, no list): [4 quadrants][kEP][8][32] exchange words
+    constexpr int kThreads = 128 + 128 * kEP, kEpiThreads = 128 * kEP;
+    static_assert(kEP == 1 || (N / 32) % kEP == 0, "epilogue parts split the 32-expert chunks of a row");
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t cta_rank = (kCG == 2) ? ptx::cluster_ctarank() : 0u;
@@ -159,7 +163,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
         }
         for (int a = 0; a < 2; ++a) {
             ptx::mbar_init(tfull_bar + 8 * a, 1);
-            ptx::mbar_init(tempty_bar + 8 * a, 4 * kCG);   // one arrive per epilogue warp per CTA
+            ptx::mbar_init(tempty_bar + 8 * a, 4 * kEP * kCG);   // one arrive per epilogue warp per CTA
         }
         ptx::fence_barrier_init();
     }
@@ -167,7 +171,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
         ptx::tmem_alloc<kCG>(tmem_slot, kTmemCols);
         ptx::tmem_relinquish<kCG>();
     }
-    for (int i = threadIdx.x; i <= p.S; i += kGemmThreads) off_s[i] = p.src_offsets[i];
+    for (int i = threadIdx.x; i <= p.S; i += kThreads) off_s[i] = p.src_offsets[i];
     ptx::tc_fence_before();
     if constexpr (kCG == 2) ptx::cluster_sync(); else __syncthreads();
     ptx::tc_fence_after();
@@ -229,8 +233,10 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
         }
     } else if (warp >= 4) {
         // ================= epilogue: TMEM -> registers -> logits / gating =================
-        const int q = warp - 4;                       // TMEM lane quadrant (== warp % 4)
+        const int q = (warp - 4) & 3;                 // TMEM lane quadrant (== warp % 4)
+        const int part = (warp - 4) >> 2;             // kEP > 1: which share of the experts (columns) of the rows of quadrant q
         const int ep_tid = threadIdx.x - 128;
+        const CrossParts xp{xbuf_s + q * (kEP * 8 * 32), 2 + q, 32 * kEP};
         const uint32_t tempty_leader = (kCG == 2) ? ptx::mapa(tempty_bar, 0) : tempty_bar;
         int it = 0;
         int cur_layer = -1;
@@ -243,18 +249,18 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
             const int t = m0 + q * 32 + lane;
             if (p.do_gate && layer != cur_layer) {
                 // new layer: flush the histogram of the previous one, load this layer's select bias
-                asm volatile("bar.sync 1, 128;" ::: "memory");
+                asm volatile("bar.sync 1, %0;" ::"n"(kEpiThreads) : "memory");
                 if (cur_layer >= 0) {
                     int32_t* dst = p.A_step + (size_t)cur_layer * p.S * N;
-                    for (int i = ep_tid; i < p.S * N; i += 128) {
+                    for (int i = ep_tid; i < p.S * N; i += kEpiThreads) {
                         const int32_t c = hist[i];
                         if (c) atomicAdd(dst + i, c);
                     }
                 }
-                for (int i = ep_tid; i < p.S * N; i += 128) hist[i] = 0;
-                for (int i = ep_tid; i < N; i += 128) sb_s[i] = p.select_bias ? p.select_bias[(size_t)layer * N + i] : 0.0f;
+                for (int i = ep_tid; i < p.S * N; i += kEpiThreads) hist[i] = 0;
+                for (int i = ep_tid; i < N; i += kEpiThreads) sb_s[i] = p.select_bias ? p.select_bias[(size_t)layer * N + i] : 0.0f;
                 cur_layer = layer;
-                asm volatile("bar.sync 1, 128;" ::: "memory");
+                asm volatile("bar.sync 1, %0;" ::"n"(kEpiThreads) : "memory");
             }
             ptx::mbar_wait(tfull_bar + 8 * as, aphase);
             ptx::tc_fence_after();
@@ -262,6 +268,16 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
             const int s = find_source(off_s, p.S, min(t, p.T - 1));
             const float* bias = p.src_logit_bias ? p.src_logit_bias + ((size_t)layer * p.S + s) * N : nullptr;
             TmemRowSrc<N> src{taddr, bias};
+            if constexpr (kEP > 1) {
+                // counts only (the host picks kEP > 1 when neither logits nor ids / weights are asked for): this warp gates the
+                // experts [part * N / kEP, (part + 1) * N / kEP) of its quadrant's rows and meets the other parts in shared memory
+                constexpr int kPartCols = N / kEP;
+                TmemRowSrc<N> psrc{taddr + part * kPartCols, bias ? bias + part * kPartCols : nullptr};
+                int32_t ids[kTopK];
+                float w[kTopK];
+                const bool uni = p.hist_agg && __all_sync(0xffffffffu, s == __shfl_sync(0xffffffffu, s, 0));
+                gate_row<N, kSig, false, TmemRowSrc<N>, kEP, true>(p.gp, sb_s, psrc, t < p.T, hist + s * N, nullptr, 0, ids, w, part, uni, &xp);
+            } else {
             if (p.logits) {
                 constexpr int CH = TmemRowSrc<N>::CH;
                 float v[CH];
@@ -301,6 +317,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
                     gate_row<N, kSig, false>(p.gp, sb_s, src, valid, hist + s * N, nullptr, 0, ids, w, 0, uni);
                 }
             }
+            }
             // release this accumulator stage to the MMA issuer
             ptx::tc_fence_before();
             __syncwarp();
@@ -310,9 +327,9 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
             }
         }
         if (p.do_gate && cur_layer >= 0) {
-            asm volatile("bar.sync 1, 128;" ::: "memory");
+            asm volatile("bar.sync 1, %0;" ::"n"(kEpiThreads) : "memory");
             int32_t* dst = p.A_step + (size_t)cur_layer * p.S * N;
-            for (int i = ep_tid; i < p.S * N; i += 128) {
+            for (int i = ep_tid; i < p.S * N; i += kEpiThreads) {
                 const int32_t c = hist[i];
                 if (c) atomicAdd(dst + i, c);
             }

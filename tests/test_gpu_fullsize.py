@@ -54,6 +54,13 @@ def test_v3_full_size_bench_configuration():
     np.testing.assert_allclose(to_np(st.pressure_rel), d["pressure_rel"], rtol=1e-5)
     np.testing.assert_allclose(to_np(st.pressure_raw).sum(), A.sum(), rtol=1e-5)                     # loads sum to routed tokens
 
+    # ---- two epilogue warps per quadrant (GIMBAL_OPT_EPI_PARTS = 2, normally the small-batch kernel) over all 14,848 tiles
+    g.set_option(g.OPT_EPI_PARTS, 2)
+    st_p = g.StatsState(cfg, MODE_WINDOW, window_len=8)
+    g.route_stats(cfg, st_p, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off, workspace=ws)
+    g.set_option(g.OPT_EPI_PARTS, 0)
+    assert torch.equal(st_p.A_step, st.A_step)
+
     # ---- sampled layers: logits + ids written by a layer-sliced call must give the same counts; oracle on samples
     rng = np.random.default_rng(0)
     for l in sorted(rng.choice(r.L, 3, replace=False).tolist()):

@@ -473,6 +473,13 @@ def test_router_gemm_logits_and_full_path(name, cta_group):
     g.route_stats(cfg, st2, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off,
                   logits_mode=g.LOGITS_NONE, topk_ids=ids2, workspace=ws)
     assert torch.equal(ids2, ids) and torch.equal(st2.A_step, st.A_step)
+    # counts only, one and two epilogue warps per TMEM lane quadrant (GIMBAL_OPT_EPI_PARTS; two only exists for E >= 128)
+    for parts in (1, 2):
+        g.set_option(g.OPT_EPI_PARTS, parts)
+        st5 = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+        g.route_stats(cfg, st5, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off, workspace=ws)
+        assert torch.equal(st5.A_step, st.A_step), f"epilogue parts = {parts}"
+    g.set_option(g.OPT_EPI_PARTS, 0)
     # unfused two-kernel path (GEMM -> logits -> gating kernel): identical integers again
     g.set_option(g.OPT_FUSE_GATE, 0)
     st3 = g.StatsState(cfg, MODE_WINDOW, window_len=1)
@@ -1195,3 +1202,40 @@ def test_place_score_tma_kernel_matches_the_lane_load_kernel_and_the_oracle(P, L
     ref = oracle.objective_batch(to_np(cands)[pick], to_np(prev), to_np(A), to_np(B), to_np(D), None, 0.75, **_oracle_kw(cfg))
     _check_objective(to_np(outs[1]).astype(np.float64)[pick], ref)
     assert to_np(outs[1])[0, 3] == 0.0
+
+
+@pytest.mark.parametrize("name,hot", [("qwen3", (60, 71)), ("v3", (124, 136)), ("v3", (0, 256)), ("qwen3", (0, 128))])
+def test_router_epilogue_parts_meet_on_exact_ties(name, hot):
+    """Two epilogue warps per quadrant split a row's experts; ties with the k-th key that span both halves are resolved by the
+    total order (key desc, index asc) across the parts.  W rows of the `hot` experts are identical (the others zero), hidden is
+    positive: every token's logits tie exactly on the hot experts, and the k lowest hot indices straddle the part boundary
+    (E/2) -- or every expert ties.  Reference: the logits-out path (one thread per row), itself checked against the oracle."""
+    w = scaled(get_workload(name), L=2, T=700)
+    r = w.router
+    cfg = g.RouterCfg.from_workload(r)
+    gen_ = torch.Generator(device=DEV).manual_seed(5)
+    hidden = (torch.rand(r.L, w.T, r.H, device=DEV, generator=gen_) + 0.25).to(torch.bfloat16)
+    u = (torch.rand(r.H, device=DEV, generator=gen_) * 0.02 + 0.01).to(torch.bfloat16)
+    W = torch.zeros(r.L, r.E, r.H, dtype=torch.bfloat16, device=DEV)
+    W[:, hot[0]:hot[1]] = u
+    off = gen.src_offsets(w, 0, w.T, DEV)
+    ws = ws_tensor(g.route_stats_workspace_bytes(cfg, r.L, w.T))
+    st = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+    logits = torch.empty(r.L, w.T, r.E, device=DEV)
+    ids = torch.empty(r.L, w.T, r.k, dtype=torch.int32, device=DEV)
+    g.route_stats(cfg, st, T=w.T, hidden=hidden, w_router=W, src_offsets=off, logits_mode=g.LOGITS_OUT, logits=logits, topk_ids=ids, workspace=ws)
+    torch.cuda.synchronize()
+    offn = to_np(off)
+    for l in range(r.L):
+        gl = to_np(logits[l])
+        assert (gl[:, hot[0]:hot[1]] == gl[:, hot[0]:hot[0] + 1]).all()                 # exact ties on the hot experts
+        rid, _ = oracle.gate(gl, r, None, 1)
+        np.testing.assert_array_equal(to_np(ids[l]), rid)
+        np.testing.assert_array_equal(to_np(st.A_step[l]), oracle.counts(rid, offn, r.S, r.E))
+    if hot[1] - hot[0] < r.E and not r.n_groups > 1:
+        assert set(np.unique(to_np(ids)).tolist()) == set(range(hot[0], hot[0] + r.k))   # the k lowest hot indices, across E/2
+    for parts in (1, 2):
+        g.set_option(g.OPT_EPI_PARTS, parts)
+        st2 = g.StatsState(cfg, MODE_WINDOW, window_len=1)
+        g.route_stats(cfg, st2, T=w.T, hidden=hidden, w_router=W, src_offsets=off, workspace=ws)
+        assert torch.equal(st2.A_step, st.A_step), f"epilogue parts = {parts}"
