@@ -373,8 +373,13 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
     if (rc) return rc;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
 
-    // a3 accumulates into A_step: zero the slice of this call
-    CUDA_TRY(cudaMemsetAsync(st->A_step + (size_t)layer0 * cfg->S * cfg->E, 0, sizeof(int32_t) * (size_t)n_layers * cfg->S * cfg->E, stream));
+    // a3 accumulates into A_step with atomics: zero the slice of this call -- unless every layer is one tile with a CTA (pair)
+    // of its own (small-batch regime: T <= 256, n_layers <= pairs), where the fused router kernel stores a layer's counts
+    const int cg_pick = pick_cta_group(T);
+    const bool hist_stored = T > 0 && logits_mode != GIMBAL_LOGITS_IN && pick_fuse() && (size_t)cfg->S * cfg->E * 4 <= 64 * 1024 && T <= 128 * cg_pick &&
+                             n_layers <= device_info().sms / cg_pick;
+    if (!hist_stored)
+        CUDA_TRY(cudaMemsetAsync(st->A_step + (size_t)layer0 * cfg->S * cfg->E, 0, sizeof(int32_t) * (size_t)n_layers * cfg->S * cfg->E, stream));
     // stats_update_kernel's block counter starts at 0: the router kernel of this call clears it where there is one, else a memset
     const bool gemm_clears = layer0 == 0 && T > 0 && logits_mode != GIMBAL_LOGITS_IN;
     if (layer0 == 0 && !gemm_clears) CUDA_TRY(cudaMemsetAsync(ws.done, 0, sizeof(unsigned int), stream));
@@ -386,7 +391,8 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
         a.topk_ids = topk_ids; a.topk_w = topk_w; a.A_step = st->A_step; a.stream = stream;
         a.zero_word = gemm_clears ? ws.done : nullptr;
         if (map) { a.rep_off = map->rep_off; a.rep_slots = map->rep_slots; a.phys_ids = map->phys_ids; a.map_NS = map->NS; }
-        a.cta_group = pick_cta_group(T);
+        a.cta_group = cg_pick;
+        a.store_hist = hist_stored;
         a.hist_agg = g_opt[GIMBAL_OPT_HIST_AGG].load(std::memory_order_relaxed);
         {
             // epilogue parts: auto = 2 when no CTA (pair) gets more than two tiles, i.e. when the epilogue cannot hide behind the MMAs

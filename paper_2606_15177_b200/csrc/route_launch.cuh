@@ -32,6 +32,7 @@ int launch_gemm_t(const RouteArgs& a) {
     const int n_tiles = p.n_layers * p.m_tiles;
     int pairs = sms / kCG;
     if (pairs > n_tiles) pairs = n_tiles;
+    p.store_hist = a.store_hist && a.fuse_gate && p.m_tiles == 1 && n_tiles <= sms / kCG;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(pairs * kCG);
     cfg.blockDim = dim3(128 + 128 * kEP);

@@ -36,6 +36,8 @@ struct GemmParams {
     float* topk_w;
     int32_t* A_step;                // [L,S,E]
     unsigned int* zero_word;        // | nullptr: a workspace word this launch clears (stats_update_kernel's block counter)
+    int store_hist;                 // every layer of this call is ONE tile owned by one CTA (pair): the layer's counts are stored
+                                    // (the pair's two histograms are added through distributed shared memory), A_step needs no zeroing
     GateParams gp;
     ExpertMap map;
 };
@@ -326,7 +328,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
                 else ptx::mbar_arrive(tempty_bar + 8 * as);
             }
         }
-        if (p.do_gate && cur_layer >= 0) {
+        if (p.do_gate && cur_layer >= 0 && !p.store_hist) {
             asm volatile("bar.sync 1, %0;" ::"n"(kEpiThreads) : "memory");
             int32_t* dst = p.A_step + (size_t)cur_layer * p.S * N;
             for (int i = ep_tid; i < p.S * N; i += kEpiThreads) {
@@ -339,6 +341,27 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
     // ================= teardown =================
     ptx::tc_fence_before();
     if constexpr (kCG == 2) ptx::cluster_sync(); else __syncthreads();
+    if (p.do_gate && p.store_hist) {
+        // one tile per layer, one CTA (pair) per tile: the barrier above made both histograms of the pair complete and visible;
+        // the leader adds its peer's through distributed shared memory and STORES the layer's counts (zeros included)
+        if (warp >= 4 && leader) {
+            const int ep_tid = threadIdx.x - 128;
+            const int layer = p.layer0 + pair;                                   // tile == pair, m_tiles == 1
+            int32_t* dst = p.A_step + (size_t)layer * p.S * N;
+            const uint32_t peer = (kCG == 2) ? ptx::mapa(ptx::smem_u32(hist), 1) : 0u;
+            const int n4 = p.S * N / 4;                                          // N % 4 == 0, hist is 16-byte aligned
+#pragma unroll 4
+            for (int i = ep_tid; i < n4; i += kEpiThreads) {
+                int4 c = reinterpret_cast<const int4*>(hist)[i];
+                if constexpr (kCG == 2) {
+                    const uint4 o = ptx::ld_shared_cluster_v4(peer + 16u * (uint32_t)i);
+                    c.x += (int32_t)o.x; c.y += (int32_t)o.y; c.z += (int32_t)o.z; c.w += (int32_t)o.w;
+                }
+                reinterpret_cast<int4*>(dst)[i] = c;
+            }
+        }
+        if constexpr (kCG == 2) ptx::cluster_sync();                             // the peer's shared memory stays until it was read
+    }
     if (warp == 2) ptx::tmem_dealloc<kCG>(tmem_base, kTmemCols);
 }
 
