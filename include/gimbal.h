@@ -403,7 +403,10 @@ GIMBAL_API int gimbal_refine_placement(const gimbal_placement_cfg *cfg, int16_t 
  *   GIMBAL_OPT_EPI_PARTS         0 (default: auto), 1 or 2: epilogue warps per TMEM lane quadrant of the fused router kernel.
  *                                2 (E >= 128, counts only) splits a row's experts between two warps that meet in shared
  *                                memory; auto picks it when no CTA pair gets more than two tiles (small-batch regime, where
- *                                the epilogue is not hidden behind the MMAs)                                       */
+ *                                the epilogue is not hidden behind the MMAs)
+ *   GIMBAL_OPT_PDL               1 (default): stats_update_kernel, and the fused router kernel in the one-tile-per-layer regime,
+ *                                are launched with programmatic stream serialization (they wait for their predecessors
+ *                                themselves, so launch latency and prologues overlap); 0: plain stream order            */
 #define GIMBAL_OPT_CTA_GROUP 0
 #define GIMBAL_OPT_FUSE_GATE 1
 #define GIMBAL_OPT_SCORE_GENERIC 2
@@ -411,7 +414,8 @@ GIMBAL_API int gimbal_refine_placement(const gimbal_placement_cfg *cfg, int16_t 
 #define GIMBAL_OPT_HIST_AGG 4
 #define GIMBAL_OPT_SCORE_TMA 5
 #define GIMBAL_OPT_EPI_PARTS 6
-#define GIMBAL_OPT_COUNT_ 7
+#define GIMBAL_OPT_PDL 7
+#define GIMBAL_OPT_COUNT_ 8
 GIMBAL_API int gimbal_set_option(int option, int value);
 GIMBAL_API int gimbal_get_option(int option, int *value);
 

@@ -27,7 +27,7 @@ EXPORTED_SYMBOLS = [
 KERNEL_ROUTER, KERNEL_GATE, KERNEL_SCORE, KERNEL_MOVES, KERNEL_GREEDY, KERNEL_CHECK = 0, 1, 2, 3, 4, 5
 ENC_SLOT_TO_EXPERT_I16, ENC_EXPERT_TO_RANK_U8 = 0, 1
 PLACE_TRUSTED = 1
-OPT_CTA_GROUP, OPT_FUSE_GATE, OPT_SCORE_GENERIC, OPT_CHECK_SCORES_ALL, OPT_HIST_AGG, OPT_SCORE_TMA, OPT_EPI_PARTS = 0, 1, 2, 3, 4, 5, 6
+OPT_CTA_GROUP, OPT_FUSE_GATE, OPT_SCORE_GENERIC, OPT_CHECK_SCORES_ALL, OPT_HIST_AGG, OPT_SCORE_TMA, OPT_EPI_PARTS, OPT_PDL = 0, 1, 2, 3, 4, 5, 6, 7
 
 
 class GimbalError(RuntimeError):

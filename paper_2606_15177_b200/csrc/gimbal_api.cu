@@ -104,7 +104,7 @@ size_t route_ws_carve(const gimbal_router_cfg* c, void* ws, RouteWs* out) {
 }
 
 // process-wide switches set through gimbal_set_option (tests and A/B measurements); defaults = production
-std::atomic<int> g_opt[GIMBAL_OPT_COUNT_] = {{0}, {1}, {0}, {0}, {1}, {1}, {0}};
+std::atomic<int> g_opt[GIMBAL_OPT_COUNT_] = {{0}, {1}, {0}, {0}, {1}, {1}, {0}, {1}};
 
 int pick_cta_group(int T) {
     const int forced = g_opt[GIMBAL_OPT_CTA_GROUP].load(std::memory_order_relaxed);
@@ -393,6 +393,7 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
         if (map) { a.rep_off = map->rep_off; a.rep_slots = map->rep_slots; a.phys_ids = map->phys_ids; a.map_NS = map->NS; }
         a.cta_group = cg_pick;
         a.store_hist = hist_stored;
+        a.pdl = g_opt[GIMBAL_OPT_PDL].load(std::memory_order_relaxed);
         a.hist_agg = g_opt[GIMBAL_OPT_HIST_AGG].load(std::memory_order_relaxed);
         {
             // epilogue parts: auto = 2 when no CTA (pair) gets more than two tiles, i.e. when the epilogue cannot hide behind the MMAs
@@ -432,7 +433,13 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
         u.A_step = st->A_step; u.A_win = st->A_win; u.A_pub = st->A_pub; u.B_pub = st->B_pub; u.A_ema = st->A_ema; u.B = st->B;
         u.pressure_raw = st->pressure_raw; u.pressure_rel = st->pressure_rel; u.step_counter = st->step_counter; u.status = st->status;
         u.cur_placement = cur_placement; u.dp_of_rank = dp_of_rank; u.partial = ws.partial; u.done_counter = ws.done;
-        stats_update_kernel<<<cfg->L, kUpdateThreads, 0, stream>>>(u);
+        cudaLaunchConfig_t lc{};
+        lc.gridDim = dim3(cfg->L); lc.blockDim = dim3(kUpdateThreads); lc.dynamicSmemBytes = 0; lc.stream = stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        lc.attrs = at; lc.numAttrs = g_opt[GIMBAL_OPT_PDL].load(std::memory_order_relaxed) ? 1 : 0;
+        CUDA_TRY(cudaLaunchKernelEx(&lc, stats_update_kernel, u));
         LAUNCH_CHECK("stats_update_kernel");
     }
     return GIMBAL_OK;

@@ -38,10 +38,12 @@ int launch_gemm_t(const RouteArgs& a) {
     cfg.blockDim = dim3(128 + 128 * kEP);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = a.stream;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = kCG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr; cfg.numAttrs = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = (p.store_hist && a.pdl) ? 2 : 1;
     ktime_begin(GIMBAL_KERNEL_ROUTER, a.stream);
     CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, ta, tb, p));
     ktime_end(GIMBAL_KERNEL_ROUTER, a.stream);

@@ -153,7 +153,10 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
     const int n_tiles = p.n_layers * p.m_tiles;
     const int num_kb = (p.H + kBlockK - 1) / kBlockK;
 
-    if (blockIdx.x == 0 && threadIdx.x == 32 && p.zero_word) *p.zero_word = 0u;     // consumed by the next kernel of the stream
+    // Launched with programmatic stream serialization in the one-tile-per-layer regime (p.store_hist): everything up to the
+    // store of the counts may overlap the previous kernel of the stream (stats_update_kernel of the step before, which still
+    // reads A_step and its block counter); the next kernel may be scheduled right away (it waits for this grid itself).
+    if (p.store_hist) ptx::griddep_launch_dependents();
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tmap(&tmap_a);
         ptx::prefetch_tmap(&tmap_b);
@@ -341,7 +344,12 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
     // ================= teardown =================
     ptx::tc_fence_before();
     if constexpr (kCG == 2) ptx::cluster_sync(); else __syncthreads();
+    if (blockIdx.x == 0 && threadIdx.x == 32 && p.zero_word) {
+        ptx::griddep_wait();
+        *p.zero_word = 0u;                                                       // consumed by the next kernel of the stream
+    }
     if (p.do_gate && p.store_hist) {
+        if (warp >= 4 && leader) ptx::griddep_wait();                            // the previous step's stats_update_kernel is done with A_step
         // one tile per layer, one CTA (pair) per tile: the barrier above made both histograms of the pair complete and visible;
         // the leader adds its peer's through distributed shared memory and STORES the layer's counts (zeros included)
         if (warp >= 4 && leader) {

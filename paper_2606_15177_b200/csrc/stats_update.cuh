@@ -35,6 +35,10 @@ __global__ void __launch_bounds__(kUpdateThreads) stats_update_kernel(const Upda
     __shared__ bool last_s;
 
     const int l = blockIdx.x, e = threadIdx.x;
+    // programmatic dependent launch: this grid may have been scheduled while the router kernel still ran -- wait for it (and its
+    // memory) here; the next kernel of the stream may be scheduled from now on (it waits for this grid before it writes A_step)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     const int64_t step = *p.step_counter;
     const bool publish = p.mode == 0 && ((step + 1) % p.window_len) == 0;
     if (e == 0) bad_s = 0;
