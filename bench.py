@@ -57,7 +57,7 @@ def _profile_metrics(name: str) -> dict:
 
 
 K1_PROFILE = "r2_ncu_k1_router_gemm"       # V3 shape, `--layers 6`: counters are per launch of 6 layers x 65536 tokens
-K4_PROFILE = "r2_ncu_k4_place_score"       # V3 shape, P = 4096, 58 layers, GIMBAL_PLACE_TRUSTED (scoring only)
+K4_PROFILE = "r2_ncu_k4_place_score_tma"   # V3 shape, P = 4096, 58 layers, GIMBAL_PLACE_TRUSTED (scoring only): place_score_tma_kernel
 K4C_PROFILE = "r2_ncu_k4_place_score_checked"   # same, default call (validation fused in)
 
 
@@ -483,6 +483,8 @@ def run_ours(args, w):
         # step's default call: the same scoring with the exact validation fused in (a separate place_check_kernel on other shapes)
         place_score_kernel=dict(ms=t_ms, bound="hbm", achieved=cand_bytes / (t_ms * 1e-3) / 1e9, peak=peaks["hbm"], unit="GB/s",
                                 frac=cand_bytes / (t_ms * 1e-3) / 1e9 / peaks["hbm"], algorithmic_bytes="2*L*NS per candidate",
+                                kernel=("place_score_tma_kernel (candidate rows by TMA into per-warp rings)" if w.name == "v3" and g.get_option(g.OPT_SCORE_TMA)
+                                        else "place_score_kernel<.., kCheck = false>"),
                                 timed="outside the timed step: GIMBAL_PLACE_TRUSTED call after an L2 flush (clocks not held down by the router GEMM)",
                                 smem=smem_obj(K4_PROFILE, t_ms)),
         place_score_in_step=dict(ms=score_ms, bound="hbm", achieved=cand_bytes / (score_ms * 1e-3) / 1e9, peak=peaks["hbm"], unit="GB/s",
