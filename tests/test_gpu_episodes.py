@@ -128,6 +128,10 @@ def test_decode_episode_200_steps_from_one_cuda_graph():
     out = torch.zeros(w.P, 5, device=DEV); argmin = torch.zeros(1, dtype=torch.int32, device=DEV)
     snap_A = torch.zeros(r.L, r.S, r.E, device=DEV); snap_B = torch.zeros(r.L, r.E, device=DEV)
     st = g.StatsState(cfg, MODE_EMA, ema_decay=w.ema_decay)
+    # the bench's launch configuration of this regime: counts only (two epilogue warps per quadrant), counts stored through
+    # distributed shared memory, programmatic dependent launches captured into the graph -- stepped beside the logits-out state
+    st_b = g.StatsState(cfg, MODE_EMA, ema_decay=w.ema_decay)
+    ws_b = ws_tensor(g.route_stats_workspace_bytes(cfg, r.L, w.T))
     g.kernel_timing(False)
 
     def ten_steps(stream, rescore):
@@ -135,6 +139,8 @@ def test_decode_episode_200_steps_from_one_cuda_graph():
             g.route_stats(cfg, st, T=w.T, hidden=hidden[i], w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off,
                           logits_mode=g.LOGITS_OUT, logits=logits[i], cur_placement=place, dp_of_rank=dp, G=w.G,
                           slots_per_rank=w.slots_per_rank, workspace=ws, stream=stream)
+            g.route_stats(cfg, st_b, T=w.T, hidden=hidden[i], w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off,
+                          cur_placement=place, dp_of_rank=dp, G=w.G, slots_per_rank=w.slots_per_rank, workspace=ws_b, stream=stream)
         if rescore:
             g.eval_placements(pc, cands, st.A_ema, st.B, D, place, out, argmin=argmin, workspace=wsp, stream=stream)
             with torch.cuda.stream(stream):
@@ -149,7 +155,7 @@ def test_decode_episode_200_steps_from_one_cuda_graph():
         graphs[rescore] = torch.cuda.CUDAGraph()
         with torch.cuda.graph(graphs[rescore], stream=side):
             ten_steps(side, rescore)
-    for t in (st.A_ema, st.B, st.A_step, st.step_counter, st.status):
+    for t in (st.A_ema, st.B, st.A_step, st.step_counter, st.status, st_b.A_ema, st_b.B, st_b.A_step, st_b.step_counter, st_b.status):
         t.zero_()
     torch.cuda.synchronize()
     # per-step counts of the ring, once (the ring repeats every 10 steps)
@@ -169,6 +175,8 @@ def test_decode_episode_200_steps_from_one_cuda_graph():
             oracle.update_ema(A_ema, Cs[i], w.ema_decay)
         np.testing.assert_allclose(to_np(st.A_ema), A_ema, rtol=1e-5, atol=1e-30)
         assert int(st.step_counter.item()) == (rep + 1) * ring
+        assert torch.equal(st_b.A_ema, st.A_ema) and torch.equal(st_b.A_step, st.A_step) and torch.equal(st_b.B, st.B)
+        assert torch.equal(st_b.pressure_rel, st.pressure_rel) and int(st_b.step_counter.item()) == (rep + 1) * ring
         if rescore:
             rescored += 1
             np.testing.assert_allclose(to_np(snap_A), A_ema, rtol=1e-5, atol=1e-30)
