@@ -645,11 +645,16 @@ def run_episode(args, w):
     side.wait_stream(torch.cuda.current_stream())
     graph = torch.cuda.CUDAGraph()
     launches0 = g.launch_count()
+    # every input of the episode (the ring of hidden states, weights, biases, offsets) is resident before the first replay: the promise
+    # GIMBAL_OPT_PDL = 2 asks for, so a step's router kernel may overlap the previous step's update kernel (--opt PDL=1 / 0 for the A/B)
+    if not any(o.upper().startswith("PDL=") for o in (args.opt or [])):
+        g.set_option(g.OPT_PDL, 2)
     with torch.cuda.graph(graph, stream=side):
         for i in range(per):
             one(i, side)
         rescore(side)
     launches_per_graph = g.launch_count() - launches0
+    pdl_mode = g.get_option(g.OPT_PDL)
     for _ in range(max(args.warmup, 3)):
         graph.replay()
     torch.cuda.synchronize()
@@ -708,6 +713,9 @@ def run_episode(args, w):
                 config=dict(workload=f"decode episode: L={r.L} H={r.H} E={r.E} top-{r.k} S={r.S} T={w.T}/step x {K} consecutive steps, EMA "
                                      f"{w.ema_decay} every step; G={w.G}x{w.slots_per_rank} slots, P={w.P} candidates re-scored every {per} steps",
                             launch=f"one CUDA graph of {per} steps + 1 re-score ({launches_per_graph} kernels), replayed {K // per} times",
+                            pdl=("GIMBAL_OPT_PDL = %d: %s" % (pdl_mode, {0: "plain launches", 1: "programmatic launches, every kernel waits for its predecessor "
+                                 "before its first global access", 2: "programmatic launches; inputs are pre-staged, so a step's router kernel waits only before "
+                                 "it stores its counts and overlaps the previous step's update"}[pdl_mode])),
                             l2=f"ring of {ring} steps of hidden states ({hidden.numel() * 2 / 1e9:.1f} GB) + 213 MB of router weights cycle "
                                "through the 126 MB L2: every step's inputs come from HBM",
                             parallelism="single GPU"),

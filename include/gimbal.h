@@ -186,6 +186,14 @@ GIMBAL_API void gimbal_last_error(char *buf, size_t n);
  *                                      outputs only (both NULL: pressure is left untouched)
  *   G, slots_per_rank                  shape of cur_placement
  *   map           | NULL               expert mapping: phys_ids written next to the counts
+ * Stream order: the call behaves as if its kernels ran one after the other behind everything
+ * enqueued on `stream` before it.  Internally the update kernel (a4-a5) and, when every layer of
+ * the call is a single tile (T <= 256 and n_layers <= #SMs / 2), the router kernel are launched
+ * with programmatic stream serialization: they may be SCHEDULED while the previous kernel on the
+ * stream still runs and wait for it (griddepcontrol.wait) before their first global access.  In
+ * that regime A_step is stored by one CTA pair per layer instead of accumulated, so it is never
+ * zeroed first.  Capturable in a CUDA graph (programmatic edges).  See GIMBAL_OPT_PDL for the
+ * opt-in that lets the router kernel overlap the previous step's update, and for plain launches.
  * Errors: INVALID_ARG (NULL / shape / alignment), UNSUPPORTED (shape outside the compiled
  * range, no sm_100 device), WORKSPACE (workspace_bytes too small), CUDA.                  */
 GIMBAL_API size_t gimbal_route_stats_workspace_bytes(const gimbal_router_cfg *cfg, int n_layers, int T);
@@ -405,8 +413,13 @@ GIMBAL_API int gimbal_refine_placement(const gimbal_placement_cfg *cfg, int16_t 
  *                                memory; auto picks it when no CTA pair gets more than two tiles (small-batch regime, where
  *                                the epilogue is not hidden behind the MMAs)
  *   GIMBAL_OPT_PDL               1 (default): stats_update_kernel, and the fused router kernel in the one-tile-per-layer regime,
- *                                are launched with programmatic stream serialization (they wait for their predecessors
- *                                themselves, so launch latency and prologues overlap); 0: plain stream order            */
+ *                                are launched with programmatic stream serialization and wait for their predecessor themselves
+ *                                before their first global access (launch latency and prologues overlap; always safe);
+ *                                2: the caller PROMISES that the inputs of gimbal_route_stats (hidden, w_router, biases,
+ *                                src_offsets) were complete before the operation that precedes the call on the stream was
+ *                                enqueued -- e.g. steps replayed from pre-staged buffers -- and the router kernel then waits
+ *                                only before it stores its counts: it overlaps the previous step's update entirely;
+ *                                0: plain launches                                                                  */
 #define GIMBAL_OPT_CTA_GROUP 0
 #define GIMBAL_OPT_FUSE_GATE 1
 #define GIMBAL_OPT_SCORE_GENERIC 2

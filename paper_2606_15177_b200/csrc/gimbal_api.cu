@@ -304,9 +304,9 @@ int64_t gimbal_launch_count(void) { return gimbal::launches(); }
 
 int gimbal_set_option(int option, int value) {
     if (option < 0 || option >= GIMBAL_OPT_COUNT_) return fail(GIMBAL_ERR_INVALID_ARG, "option %d", option);
-    if ((option == GIMBAL_OPT_CTA_GROUP || option == GIMBAL_OPT_EPI_PARTS) && (value < 0 || value > 2))
-        return fail(GIMBAL_ERR_INVALID_ARG, "option %d takes 0 (auto), 1 or 2", option);
-    if (option != GIMBAL_OPT_CTA_GROUP && option != GIMBAL_OPT_EPI_PARTS && value != 0 && value != 1) return fail(GIMBAL_ERR_INVALID_ARG, "option %d takes 0 or 1", option);
+    const bool three = option == GIMBAL_OPT_CTA_GROUP || option == GIMBAL_OPT_EPI_PARTS || option == GIMBAL_OPT_PDL;
+    if (three && (value < 0 || value > 2)) return fail(GIMBAL_ERR_INVALID_ARG, "option %d takes 0, 1 or 2", option);
+    if (!three && value != 0 && value != 1) return fail(GIMBAL_ERR_INVALID_ARG, "option %d takes 0 or 1", option);
     g_opt[option].store(value, std::memory_order_relaxed);
     return GIMBAL_OK;
 }

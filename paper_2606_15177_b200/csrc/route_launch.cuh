@@ -43,7 +43,8 @@ int launch_gemm_t(const RouteArgs& a) {
     attr[0].val.clusterDim.x = kCG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[1].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr; cfg.numAttrs = (p.store_hist && a.pdl) ? 2 : 1;
+    p.pdl = p.store_hist ? a.pdl : 0;
+    cfg.attrs = attr; cfg.numAttrs = p.pdl ? 2 : 1;
     ktime_begin(GIMBAL_KERNEL_ROUTER, a.stream);
     CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, ta, tb, p));
     ktime_end(GIMBAL_KERNEL_ROUTER, a.stream);

@@ -36,6 +36,8 @@ struct GemmParams {
     float* topk_w;
     int32_t* A_step;                // [L,S,E]
     unsigned int* zero_word;        // | nullptr: a workspace word this launch clears (stats_update_kernel's block counter)
+    int pdl;                        // 0: plain launch; 1: programmatic launch, wait for the predecessor before the first global read;
+                                    // 2: (caller's promise that the inputs were ready earlier) wait only before the counts are stored
     int store_hist;                 // every layer of this call is ONE tile owned by one CTA (pair): the layer's counts are stored
                                     // (the pair's two histograms are added through distributed shared memory), A_step needs no zeroing
     GateParams gp;
@@ -153,10 +155,10 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
     const int n_tiles = p.n_layers * p.m_tiles;
     const int num_kb = (p.H + kBlockK - 1) / kBlockK;
 
-    // Launched with programmatic stream serialization in the one-tile-per-layer regime (p.store_hist): everything up to the
-    // store of the counts may overlap the previous kernel of the stream (stats_update_kernel of the step before, which still
+    // Launched with programmatic stream serialization in the one-tile-per-layer regime (p.pdl != 0).  pdl == 2: everything up to
+    // the store of the counts may overlap the previous kernel of the stream (stats_update_kernel of the step before, which still
     // reads A_step and its block counter); the next kernel may be scheduled right away (it waits for this grid itself).
-    if (p.store_hist) ptx::griddep_launch_dependents();
+    if (p.pdl == 2) ptx::griddep_launch_dependents();
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tmap(&tmap_a);
         ptx::prefetch_tmap(&tmap_b);
@@ -175,6 +177,11 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
     if (warp == 2) {
         ptx::tmem_alloc<kCG>(tmem_slot, kTmemCols);
         ptx::tmem_relinquish<kCG>();
+    }
+    if (p.pdl == 1) {
+        // barriers, TMEM and descriptors are set up: from here on global memory is read, so the predecessor must be complete
+        ptx::griddep_wait();
+        ptx::griddep_launch_dependents();
     }
     for (int i = threadIdx.x; i <= p.S; i += kThreads) off_s[i] = p.src_offsets[i];
     ptx::tc_fence_before();

@@ -132,6 +132,7 @@ def test_decode_episode_200_steps_from_one_cuda_graph():
     # distributed shared memory, programmatic dependent launches captured into the graph -- stepped beside the logits-out state
     st_b = g.StatsState(cfg, MODE_EMA, ema_decay=w.ema_decay)
     ws_b = ws_tensor(g.route_stats_workspace_bytes(cfg, r.L, w.T))
+    g.set_option(g.OPT_PDL, 2)          # every input below is staged before the first launch (the promise GIMBAL_OPT_PDL = 2 asks for)
     g.kernel_timing(False)
 
     def ten_steps(stream, rescore):

@@ -88,9 +88,9 @@ def test_options_are_validated_and_readable():
                 g.OPT_SCORE_TMA: 1, g.OPT_EPI_PARTS: 0, g.OPT_PDL: 1}
     for opt, val in defaults.items():
         assert g.get_option(opt) == val
-    for opt in (g.OPT_CTA_GROUP, g.OPT_EPI_PARTS):
+    for opt in (g.OPT_CTA_GROUP, g.OPT_EPI_PARTS, g.OPT_PDL):
         assert g.lib().gimbal_set_option(opt, 3) == -1 and g.lib().gimbal_set_option(opt, 2) == 0 and g.get_option(opt) == 2
-        g.set_option(opt, 0)
-    for opt in (g.OPT_SCORE_TMA, g.OPT_PDL, g.OPT_HIST_AGG):
+        g.set_option(opt, defaults[opt])
+    for opt in (g.OPT_SCORE_TMA, g.OPT_HIST_AGG):
         assert g.lib().gimbal_set_option(opt, 2) == -1 and g.get_option(opt) == 1
     assert g.lib().gimbal_set_option(99, 0) == -1
