@@ -94,7 +94,8 @@ typedef struct gimbal_router_cfg {
  *   pressure_raw [S] f32 out  MoE pressure of DP engine s: tokens processed by experts on its
  *                             EP ranks, sum_l sum_{g: dp_of_rank[g]=s} L[l,g]
  *   pressure_rel [S] f32 out  the same normalised to mean 1 (R14)
- *   step_counter [1] i64 inout  device-side step index; incremented by every call
+ *   step_counter [2] i64 inout  [0] device-side step index, incremented by every call that covers the last layer;
+ *                               [1] scratch of the library (a layer counter): zero it once with [0], it is 0 between calls
  *   status [1] i32 inout|NULL  bit 0 set on device-side data errors                        */
 typedef struct gimbal_stats_state {
     int32_t mode, window_len;
@@ -419,7 +420,10 @@ GIMBAL_API int gimbal_refine_placement(const gimbal_placement_cfg *cfg, int16_t 
  *                                src_offsets) were complete before the operation that precedes the call on the stream was
  *                                enqueued -- e.g. steps replayed from pre-staged buffers -- and the router kernel then waits
  *                                only before it stores its counts: it overlaps the previous step's update entirely;
- *                                0: plain launches                                                                  */
+ *                                0: plain launches
+ *   GIMBAL_OPT_FUSE_UPDATE       1 (default): a whole-step call (layer0 = 0, n_layers = L) in the one-tile-per-layer regime runs
+ *                                a4-a5 inside the router kernel (the CTA pair that stored a layer's counts updates that layer, the
+ *                                last pair finishes the step): one kernel per step; 0: separate stats_update_kernel          */
 #define GIMBAL_OPT_CTA_GROUP 0
 #define GIMBAL_OPT_FUSE_GATE 1
 #define GIMBAL_OPT_SCORE_GENERIC 2
@@ -428,7 +432,8 @@ GIMBAL_API int gimbal_refine_placement(const gimbal_placement_cfg *cfg, int16_t 
 #define GIMBAL_OPT_SCORE_TMA 5
 #define GIMBAL_OPT_EPI_PARTS 6
 #define GIMBAL_OPT_PDL 7
-#define GIMBAL_OPT_COUNT_ 8
+#define GIMBAL_OPT_FUSE_UPDATE 8
+#define GIMBAL_OPT_COUNT_ 9
 GIMBAL_API int gimbal_set_option(int option, int value);
 GIMBAL_API int gimbal_get_option(int option, int *value);
 

@@ -15,5 +15,5 @@ from .binding import (  # noqa: F401
     COUNTS_I32, COUNTS_F32, EXPORTED_SYMBOLS, kernel_timing, kernel_elapsed_ms, route_stats_result_bytes,
     KERNEL_ROUTER, KERNEL_GATE, KERNEL_SCORE, KERNEL_MOVES, KERNEL_GREEDY, KERNEL_CHECK, greedy_place, ExpertMap, select_engines,
     order_queues, refine_placement, HostCtx, eval_moves_host, set_option, get_option, ENC_SLOT_TO_EXPERT_I16,
-    ENC_EXPERT_TO_RANK_U8, PLACE_TRUSTED, OPT_CTA_GROUP, OPT_FUSE_GATE, OPT_SCORE_GENERIC, OPT_CHECK_SCORES_ALL, OPT_HIST_AGG, OPT_SCORE_TMA, OPT_EPI_PARTS, OPT_PDL,
+    ENC_EXPERT_TO_RANK_U8, PLACE_TRUSTED, OPT_CTA_GROUP, OPT_FUSE_GATE, OPT_SCORE_GENERIC, OPT_CHECK_SCORES_ALL, OPT_HIST_AGG, OPT_SCORE_TMA, OPT_EPI_PARTS, OPT_PDL, OPT_FUSE_UPDATE,
 )

@@ -27,7 +27,7 @@ EXPORTED_SYMBOLS = [
 KERNEL_ROUTER, KERNEL_GATE, KERNEL_SCORE, KERNEL_MOVES, KERNEL_GREEDY, KERNEL_CHECK = 0, 1, 2, 3, 4, 5
 ENC_SLOT_TO_EXPERT_I16, ENC_EXPERT_TO_RANK_U8 = 0, 1
 PLACE_TRUSTED = 1
-OPT_CTA_GROUP, OPT_FUSE_GATE, OPT_SCORE_GENERIC, OPT_CHECK_SCORES_ALL, OPT_HIST_AGG, OPT_SCORE_TMA, OPT_EPI_PARTS, OPT_PDL = 0, 1, 2, 3, 4, 5, 6, 7
+OPT_CTA_GROUP, OPT_FUSE_GATE, OPT_SCORE_GENERIC, OPT_CHECK_SCORES_ALL, OPT_HIST_AGG, OPT_SCORE_TMA, OPT_EPI_PARTS, OPT_PDL, OPT_FUSE_UPDATE = 0, 1, 2, 3, 4, 5, 6, 7, 8
 
 
 class GimbalError(RuntimeError):
@@ -191,7 +191,8 @@ class StatsState:
         self.B = torch.zeros(L, E, **(i32 if mode == MODE_WINDOW else f32))
         self.pressure_raw = torch.zeros(S, **f32)
         self.pressure_rel = torch.zeros(S, **f32)
-        self.step_counter = torch.zeros(1, dtype=torch.int64, device=device)
+        self._step_words = torch.zeros(2, dtype=torch.int64, device=device)     # [0] the step index, [1] the library's layer counter
+        self.step_counter = self._step_words[:1]
         self.status = torch.zeros(1, **i32)
 
     @property

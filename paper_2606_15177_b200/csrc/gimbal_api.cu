@@ -11,6 +11,7 @@
 #include <cstring>
 #include <new>
 
+#define GIMBAL_DEFINE_STATS_UPDATE_KERNEL
 #include "host_common.h"
 #include "greedy.cuh"
 #include "placement.cuh"
@@ -104,7 +105,7 @@ size_t route_ws_carve(const gimbal_router_cfg* c, void* ws, RouteWs* out) {
 }
 
 // process-wide switches set through gimbal_set_option (tests and A/B measurements); defaults = production
-std::atomic<int> g_opt[GIMBAL_OPT_COUNT_] = {{0}, {1}, {0}, {0}, {1}, {1}, {0}, {1}};
+std::atomic<int> g_opt[GIMBAL_OPT_COUNT_] = {{0}, {1}, {0}, {0}, {1}, {1}, {0}, {1}, {1}};
 
 int pick_cta_group(int T) {
     const int forced = g_opt[GIMBAL_OPT_CTA_GROUP].load(std::memory_order_relaxed);
@@ -380,9 +381,20 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
                              n_layers <= device_info().sms / cg_pick;
     if (!hist_stored)
         CUDA_TRY(cudaMemsetAsync(st->A_step + (size_t)layer0 * cfg->S * cfg->E, 0, sizeof(int32_t) * (size_t)n_layers * cfg->S * cfg->E, stream));
+    // whole-step call in that regime: the pair that stores a layer's counts also runs the layer's update (a4-a5) and the last pair
+    // finishes the step; its layer counter is the second word of state->step_counter (zero between calls), so nothing is zeroed
+    // and no stats_update_kernel is launched
+    const bool update_fused = hist_stored && layer0 == 0 && n_layers == cfg->L && g_opt[GIMBAL_OPT_FUSE_UPDATE].load(std::memory_order_relaxed);
+    UpdateParams u{};
+    u.L = cfg->L; u.S = cfg->S; u.E = cfg->E; u.G = G; u.sp = slots_per_rank;
+    u.mode = st->mode; u.window_len = st->window_len; u.ema_decay = st->ema_decay;
+    u.A_step = st->A_step; u.A_win = st->A_win; u.A_pub = st->A_pub; u.B_pub = st->B_pub; u.A_ema = st->A_ema; u.B = st->B;
+    u.pressure_raw = st->pressure_raw; u.pressure_rel = st->pressure_rel; u.step_counter = st->step_counter; u.status = st->status;
+    u.cur_placement = cur_placement; u.dp_of_rank = dp_of_rank; u.partial = ws.partial;
+    u.done_counter = update_fused ? reinterpret_cast<unsigned int*>(st->step_counter + 1) : ws.done;
     // stats_update_kernel's block counter starts at 0: the router kernel of this call clears it where there is one, else a memset
-    const bool gemm_clears = layer0 == 0 && T > 0 && logits_mode != GIMBAL_LOGITS_IN;
-    if (layer0 == 0 && !gemm_clears) CUDA_TRY(cudaMemsetAsync(ws.done, 0, sizeof(unsigned int), stream));
+    const bool gemm_clears = layer0 == 0 && T > 0 && logits_mode != GIMBAL_LOGITS_IN && !update_fused;
+    if (layer0 == 0 && !gemm_clears && !update_fused) CUDA_TRY(cudaMemsetAsync(ws.done, 0, sizeof(unsigned int), stream));
 
     if (T > 0) {
         RouteArgs a{};
@@ -390,6 +402,7 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
         a.select_bias = select_bias; a.src_logit_bias = src_logit_bias; a.src_offsets = src_offsets;
         a.topk_ids = topk_ids; a.topk_w = topk_w; a.A_step = st->A_step; a.stream = stream;
         a.zero_word = gemm_clears ? ws.done : nullptr;
+        a.upd = update_fused ? &u : nullptr;
         if (map) { a.rep_off = map->rep_off; a.rep_slots = map->rep_slots; a.phys_ids = map->phys_ids; a.map_NS = map->NS; }
         a.cta_group = cg_pick;
         a.store_hist = hist_stored;
@@ -426,13 +439,7 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
         }
     }
 
-    if (layer0 + n_layers == cfg->L) {
-        UpdateParams u{};
-        u.L = cfg->L; u.S = cfg->S; u.E = cfg->E; u.G = G; u.sp = slots_per_rank;
-        u.mode = st->mode; u.window_len = st->window_len; u.ema_decay = st->ema_decay;
-        u.A_step = st->A_step; u.A_win = st->A_win; u.A_pub = st->A_pub; u.B_pub = st->B_pub; u.A_ema = st->A_ema; u.B = st->B;
-        u.pressure_raw = st->pressure_raw; u.pressure_rel = st->pressure_rel; u.step_counter = st->step_counter; u.status = st->status;
-        u.cur_placement = cur_placement; u.dp_of_rank = dp_of_rank; u.partial = ws.partial; u.done_counter = ws.done;
+    if (layer0 + n_layers == cfg->L && !update_fused) {
         cudaLaunchConfig_t lc{};
         lc.gridDim = dim3(cfg->L); lc.blockDim = dim3(kUpdateThreads); lc.dynamicSmemBytes = 0; lc.stream = stream;
         cudaLaunchAttribute at[1];

@@ -7,6 +7,7 @@
 
 #include "../../include/gimbal.h"
 #include "gating.cuh"
+#include "stats_update.cuh"
 
 namespace gimbal {
 
@@ -57,6 +58,7 @@ struct RouteArgs {
     int fuse_gate;
     int cta_group;          // 1 or 2
     int hist_agg;           // epilogue counts by columns (GIMBAL_OPT_HIST_AGG)
+    const UpdateParams* upd; // | nullptr: the router kernel runs the window / EMA update of the layers it stores (whole-step call, one tile per layer)
     int pdl;                // programmatic dependent launch of the router kernel / stats_update_kernel (GIMBAL_OPT_PDL)
     int store_hist;         // the caller skipped the zeroing of A_step: every layer is one tile with its own CTA (pair)
     int epi_parts;          // 1 or 2 epilogue warps per TMEM lane quadrant (GIMBAL_OPT_EPI_PARTS; 2 only takes effect for E >= 128, counts only)

@@ -44,6 +44,8 @@ int launch_gemm_t(const RouteArgs& a) {
     attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[1].val.programmaticStreamSerializationAllowed = 1;
     p.pdl = p.store_hist ? a.pdl : 0;
+    p.fuse_update = p.store_hist && a.upd != nullptr;
+    if (p.fuse_update) p.upd = *a.upd;
     cfg.attrs = attr; cfg.numAttrs = p.pdl ? 2 : 1;
     ktime_begin(GIMBAL_KERNEL_ROUTER, a.stream);
     CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, ta, tb, p));

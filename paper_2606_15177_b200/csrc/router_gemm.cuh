@@ -15,6 +15,7 @@
 // the W tile, so W traffic out of L2 halves; the leader issues one M=256 MMA for both.
 #pragma once
 #include "gating.cuh"
+#include "stats_update.cuh"
 #include "ptx.cuh"
 
 namespace gimbal { constexpr size_t kGemmSmemLimit = 227 * 1024; }
@@ -38,6 +39,9 @@ struct GemmParams {
     unsigned int* zero_word;        // | nullptr: a workspace word this launch clears (stats_update_kernel's block counter)
     int pdl;                        // 0: plain launch; 1: programmatic launch, wait for the predecessor before the first global read;
                                     // 2: (caller's promise that the inputs were ready earlier) wait only before the counts are stored
+    int fuse_update;                // store_hist and the call covers all L layers: the pair that stored a layer's counts also runs its
+                                    // window / EMA update (`upd`), the last pair finishes the step -- no stats_update_kernel launch
+    UpdateParams upd;
     int store_hist;                 // every layer of this call is ONE tile owned by one CTA (pair): the layer's counts are stored
                                     // (the pair's two histograms are added through distributed shared memory), A_step needs no zeroing
     GateParams gp;
@@ -57,9 +61,13 @@ constexpr int kGemmMaxStages = 12;
 // bytes after the ring: [aux][select_bias N f32][src_offsets S+1 (padded)][hist S*N i32][selection list, when
 // ids / weights are written: kListWords x 128 epilogue threads]
 // ... [exchange buffers of the epilogue parts, ep > 1: 4 quadrants x [ep][8][32] words]
+// words of the histogram region: [S][N] counts, and at least the scratch of a fused layer update (UpdateScratch)
+__host__ __device__ constexpr size_t gemm_hist_words(int S, int N) {
+    return (size_t)S * N > (sizeof(UpdateScratch) + 3) / 4 ? (size_t)S * N : ((sizeof(UpdateScratch) + 3) / 4 + 3) / 4 * 4;
+}
 template <int N>
 constexpr size_t gemm_tail_bytes(int S, bool out, int ep = 1) {
-    return kGemmAuxBytes + sizeof(float) * N + sizeof(int32_t) * (size_t)((S + 1 + 3) & ~3) + sizeof(int32_t) * (size_t)S * N +
+    return kGemmAuxBytes + sizeof(float) * N + sizeof(int32_t) * (size_t)((S + 1 + 3) & ~3) + sizeof(int32_t) * gemm_hist_words(S, N) +
            (out ? sizeof(int32_t) * (size_t)kListWords * 128 : 0) + (ep > 1 ? sizeof(int32_t) * 4 * (size_t)ep * 8 * 32 : 0);
 }
 template <int N, int kCG>
@@ -143,7 +151,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
     float* sb_s = reinterpret_cast<float*>(base_ptr + kStages * kStageBytes + kGemmAuxBytes);
     int32_t* off_s = reinterpret_cast<int32_t*>(sb_s + N);
     int32_t* hist = off_s + ((p.S + 1 + 3) & ~3);
-    int32_t* list_s = hist + p.S * N;                    // [kListWords][128] (only when ids / weights are written)
+    int32_t* list_s = hist + gemm_hist_words(p.S, N);    // [kListWords][128] (only when ids / weights are written)
     int32_t* xbuf_s = list_s;                            // kEP > 1 (counts only, no list): [4 quadrants][kEP][8][32] exchange words
     constexpr int kThreads = 128 + 128 * kEP, kEpiThreads = 128 * kEP;
     static_assert(kEP == 1 || (N / 32) % kEP == 0, "epilogue parts split the 32-expert chunks of a row");
@@ -376,6 +384,14 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
             }
         }
         if constexpr (kCG == 2) ptx::cluster_sync();                             // the peer's shared memory stays until it was read
+        if (p.fuse_update && warp >= 4 && leader) {
+            // a4 + a5 of this layer right here: the counts just stored are complete; `hist` is free and serves as scratch
+            __threadfence();
+            asm volatile("bar.sync 1, %0;" ::"n"(kEpiThreads) : "memory");
+            UpdateScratch& sh = *reinterpret_cast<UpdateScratch*>(hist);
+            stats_update_layer(p.upd, p.layer0 + pair, (int)threadIdx.x - 128, kEpiThreads, sh,
+                               [] { asm volatile("bar.sync 1, %0;" ::"n"(kEpiThreads) : "memory"); });
+        }
     }
     if (warp == 2) ptx::tmem_dealloc<kCG>(tmem_base, kTmemCols);
 }

@@ -27,25 +27,28 @@ struct UpdateParams {
 
 constexpr int kUpdateThreads = 256;
 
-__global__ void __launch_bounds__(kUpdateThreads) stats_update_kernel(const UpdateParams p) {
-    __shared__ double b_s[256];          // live B of this layer (E <= 256)
-    __shared__ int r_s[256];             // replica count of each expert in cur_placement
-    __shared__ double lg_s[64];          // rank loads (G <= 64)
-    __shared__ int bad_s;
-    __shared__ bool last_s;
+// scratch of one layer's update: [E <= 256] live B, [E] replica counts, [G <= 64] rank loads, two flags
+struct UpdateScratch {
+    double b[256];
+    int r[256];
+    double lg[64];
+    int bad;
+    int last;
+};
 
-    const int l = blockIdx.x, e = threadIdx.x;
-    // programmatic dependent launch: this grid may have been scheduled while the router kernel still ran -- wait for it (and its
-    // memory) here; the next kernel of the stream may be scheduled from now on (it waits for this grid before it writes A_step)
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+// a4 + a5 of ONE layer by `nthr` threads (tid 0..nthr-1) that can synchronise through `sync()`; `done_counter` counts the layers
+// of the step: the caller that finishes the L-th layer reduces the pressure partials over layers in fixed order (deterministic),
+// advances the step counter and leaves the counter at 0.  Used by stats_update_kernel (one block per layer) and by the fused
+// router kernel in the one-tile-per-layer regime (the CTA pair that owns the layer's complete histogram).
+template <class Sync>
+__device__ __forceinline__ void stats_update_layer(const UpdateParams& p, int l, int tid, int nthr, UpdateScratch& sh, Sync sync) {
     const int64_t step = *p.step_counter;
     const bool publish = p.mode == 0 && ((step + 1) % p.window_len) == 0;
-    if (e == 0) bad_s = 0;
-    if (e < 256) r_s[e] = 0;
-    __syncthreads();
+    if (tid == 0) { sh.bad = 0; sh.last = 0; }
+    for (int e = tid; e < 256; e += nthr) sh.r[e] = 0;
+    sync();
 
-    if (e < p.E) {
+    for (int e = tid; e < p.E; e += nthr) {
         // sources are read eight at a time before anything is written back: the loads of a batch are in
         // flight together instead of one global round trip per source
         if (p.mode == 0) {
@@ -62,17 +65,17 @@ __global__ void __launch_bounds__(kUpdateThreads) stats_update_kernel(const Upda
                     if (s0 + j < p.S) {
                         const size_t i = ((size_t)l * p.S + s0 + j) * p.E + e;
                         const int64_t w = (int64_t)win[j] + stp[j];
-                        if (w > INT32_MAX) bad_s = 1;        // window sum must fit int32
+                        if (w > INT32_MAX) sh.bad = 1;       // window sum must fit int32
                         b += w;
                         if (publish) { p.A_pub[i] = (int32_t)w; p.A_win[i] = 0; }
                         else p.A_win[i] = (int32_t)w;
                     }
                 }
             }
-            if (b > INT32_MAX) bad_s = 1;
+            if (b > INT32_MAX) sh.bad = 1;
             reinterpret_cast<int32_t*>(p.B)[(size_t)l * p.E + e] = (int32_t)b;
             if (publish) p.B_pub[(size_t)l * p.E + e] = (int32_t)b;
-            b_s[e] = (double)b;
+            sh.b[e] = (double)b;
         } else {
             float b = 0.0f;
             for (int s0 = 0; s0 < p.S; s0 += 8) {
@@ -92,7 +95,7 @@ __global__ void __launch_bounds__(kUpdateThreads) stats_update_kernel(const Upda
                 }
             }
             reinterpret_cast<float*>(p.B)[(size_t)l * p.E + e] = b;
-            b_s[e] = (double)b;
+            sh.b[e] = (double)b;
         }
     }
 
@@ -100,54 +103,69 @@ __global__ void __launch_bounds__(kUpdateThreads) stats_update_kernel(const Upda
     if (want_pressure) {
         const int NS = p.G * p.sp;
         const int16_t* pl = p.cur_placement + (size_t)l * NS;
-        for (int j = e; j < NS; j += kUpdateThreads) {
+        for (int j = tid; j < NS; j += nthr) {
             const int x = pl[j];
-            if (x < 0 || x >= p.E) bad_s = 1; else atomicAdd(&r_s[x], 1);
+            if (x < 0 || x >= p.E) sh.bad = 1; else atomicAdd(&sh.r[x], 1);
         }
-        __syncthreads();
-        if (e < p.G) {
+        sync();
+        for (int g = tid; g < p.G; g += nthr) {
             double lg = 0.0;
             for (int j = 0; j < p.sp; ++j) {
-                const int x = pl[e * p.sp + j];
-                if (x >= 0 && x < p.E) lg += b_s[x] / (double)r_s[x];
+                const int x = pl[g * p.sp + j];
+                if (x >= 0 && x < p.E) lg += sh.b[x] / (double)sh.r[x];
             }
-            lg_s[e] = lg;
+            sh.lg[g] = lg;
         }
-        __syncthreads();
-        if (e < p.S) {
+        sync();
+        for (int s = tid; s < p.S; s += nthr) {
             double acc = 0.0;
             for (int g = 0; g < p.G; ++g)
-                if (p.dp_of_rank[g] == e) acc += lg_s[g];
-            p.partial[(size_t)l * p.S + e] = acc;
+                if (p.dp_of_rank[g] == s) acc += sh.lg[g];
+            p.partial[(size_t)l * p.S + s] = acc;
         }
     }
-    __syncthreads();
-    if (e == 0 && bad_s && p.status) atomicOr(p.status, 1);
+    sync();
+    if (tid == 0 && sh.bad && p.status) atomicOr(p.status, 1);
 
-    // last block: deterministic reduction over layers, then advance the step counter
+    // last layer of the step: deterministic reduction over layers, then advance the step counter
     __threadfence();
-    __syncthreads();
-    if (e == 0) last_s = (atomicAdd(p.done_counter, 1u) == (unsigned)p.L - 1u);
-    __syncthreads();
-    if (last_s) {
+    sync();
+    if (tid == 0) sh.last = (atomicAdd(p.done_counter, 1u) == (unsigned)p.L - 1u);
+    sync();
+    if (sh.last) {
         __threadfence();
-        if (want_pressure && e < p.S) {
-            double acc = 0.0;
-            for (int ll = 0; ll < p.L; ++ll) acc += __ldcg(p.partial + (size_t)ll * p.S + e);
-            lg_s[e] = acc;
+        if (want_pressure) {
+            for (int s = tid; s < p.S; s += nthr) {
+                double acc = 0.0;
+                for (int ll = 0; ll < p.L; ++ll) acc += __ldcg(p.partial + (size_t)ll * p.S + s);
+                sh.lg[s] = acc;
+            }
         }
-        __syncthreads();
-        if (want_pressure && e < p.S) {
-            double tot = 0.0;
-            for (int s = 0; s < p.S; ++s) tot += lg_s[s];
-            p.pressure_raw[e] = (float)lg_s[e];
-            p.pressure_rel[e] = tot > 0.0 ? (float)(lg_s[e] * p.S / tot) : 1.0f;
+        sync();
+        if (want_pressure) {
+            for (int s = tid; s < p.S; s += nthr) {
+                double tot = 0.0;
+                for (int q = 0; q < p.S; ++q) tot += sh.lg[q];
+                p.pressure_raw[s] = (float)sh.lg[s];
+                p.pressure_rel[s] = tot > 0.0 ? (float)(sh.lg[s] * p.S / tot) : 1.0f;
+            }
         }
-        if (e == 0) {
+        if (tid == 0) {
             *p.step_counter = step + 1;
             *p.done_counter = 0u;
         }
     }
 }
+
+#ifdef GIMBAL_DEFINE_STATS_UPDATE_KERNEL        // the kernel itself lives in one translation unit (gimbal_api.cu)
+__global__ void __launch_bounds__(kUpdateThreads) stats_update_kernel(const UpdateParams p) {
+    __shared__ UpdateScratch sh;
+    // programmatic dependent launch: this grid may have been scheduled while the router kernel still ran -- wait for it (and its
+    // memory) here; the next kernel of the stream may be scheduled from now on (it waits for this grid before it writes A_step)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    stats_update_layer(p, blockIdx.x, threadIdx.x, kUpdateThreads, sh, [] { __syncthreads(); });
+}
+#endif
 
 }  // namespace gimbal

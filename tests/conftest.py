@@ -34,7 +34,7 @@ def _default_library_options():
     try:
         import paper_2606_15177_b200 as g
         if os.path.exists(g.lib_path()):
-            for opt, val in ((g.OPT_CTA_GROUP, 0), (g.OPT_FUSE_GATE, 1), (g.OPT_SCORE_GENERIC, 0), (g.OPT_CHECK_SCORES_ALL, 0), (g.OPT_HIST_AGG, 1), (g.OPT_SCORE_TMA, 1), (g.OPT_EPI_PARTS, 0), (g.OPT_PDL, 1)):
+            for opt, val in ((g.OPT_CTA_GROUP, 0), (g.OPT_FUSE_GATE, 1), (g.OPT_SCORE_GENERIC, 0), (g.OPT_CHECK_SCORES_ALL, 0), (g.OPT_HIST_AGG, 1), (g.OPT_SCORE_TMA, 1), (g.OPT_EPI_PARTS, 0), (g.OPT_PDL, 1), (g.OPT_FUSE_UPDATE, 1)):
                 g.set_option(opt, val)
     except Exception:
         pass

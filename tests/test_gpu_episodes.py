@@ -188,3 +188,45 @@ def test_decode_episode_200_steps_from_one_cuda_graph():
     d = oracle.derived(A_ema, to_np(place), to_np(dp), w.G, w.slots_per_rank)
     np.testing.assert_allclose(to_np(st.B), d["B"], rtol=1e-5)
     np.testing.assert_allclose(to_np(st.pressure_rel), d["pressure_rel"], rtol=1e-5)
+
+
+@pytest.mark.parametrize("name,T,L,window_len", [("v3", 256, 3, 2), ("v3", 100, 2, 3), ("decode", 256, 4, 1), ("qwen3", 200, 3, 2),
+                                                   ("qwen3", 128, 2, 2), ("v2lite", 77, 3, 2)])
+def test_small_batch_regime_fused_update_matches_the_separate_kernels(name, T, L, window_len):
+    """One tile per layer (T <= 256, every layer with a CTA pair of its own): the router kernel stores the counts (no zeroing of
+    A_step) and, in a whole-step call, runs the window / EMA update of its layer in its tail (GIMBAL_OPT_FUSE_UPDATE).  Six steps
+    beside a state driven with the option off and programmatic launches off (memset-free store path + separate
+    stats_update_kernel) and a third one fed layer by layer (sliced calls: separate update kernel): every state array bit for bit,
+    incl. the publish / reset steps of the window mode; the counts against the oracle on the GPU's logits.  T <= 128 takes the
+    cta_group::1 kernel."""
+    w = scaled(get_workload(name), L=L, T=T)
+    r = w.router
+    cfg = g.RouterCfg.from_workload(r)
+    W = gen.w_router(w, DEV); sb = gen.select_bias(w, DEV); dp = gen.dp_of_rank(w, DEV)
+    place = gen.prev_placement(w, np.random.default_rng(5).integers(1, 1000, (r.L, r.E)), DEV)
+    ws = ws_tensor(g.route_stats_workspace_bytes(cfg, r.L, w.T))
+    states = [g.StatsState(cfg, w.mode, window_len=window_len, ema_decay=w.ema_decay) for _ in range(3)]
+    logits = torch.empty(r.L, w.T, r.E, device=DEV)
+    st_l = g.StatsState(cfg, w.mode, window_len=window_len, ema_decay=w.ema_decay)
+    for step in range(6):
+        hidden = gen.hidden_all(w, step, DEV); slb = gen.src_logit_bias(w, step, DEV); off = gen.src_offsets(w, step, w.T, DEV)
+        kw = dict(T=w.T, w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off, cur_placement=place, dp_of_rank=dp, G=w.G,
+                  slots_per_rank=w.slots_per_rank, workspace=ws)
+        g.set_option(g.OPT_FUSE_UPDATE, 1); g.set_option(g.OPT_PDL, 1)
+        g.route_stats(cfg, states[0], hidden=hidden, **kw)
+        g.route_stats(cfg, st_l, hidden=hidden, logits_mode=g.LOGITS_OUT, logits=logits, **kw)
+        g.set_option(g.OPT_FUSE_UPDATE, 0); g.set_option(g.OPT_PDL, 0)
+        g.route_stats(cfg, states[1], hidden=hidden, **kw)
+        g.set_option(g.OPT_FUSE_UPDATE, 1); g.set_option(g.OPT_PDL, 1)
+        for l in range(r.L):
+            g.route_stats(cfg, states[2], hidden=hidden[l:l + 1], layer0=l, n_layers=1, **kw)
+        torch.cuda.synchronize()
+        offn = to_np(off)
+        for l in range(r.L):
+            rid, _ = oracle.gate(to_np(logits[l]), r, None if sb is None else to_np(sb)[l], 1)
+            np.testing.assert_array_equal(to_np(states[0].A_step[l]), oracle.counts(rid, offn, r.S, r.E))
+        for other in states[1:] + [st_l]:
+            for f in ("A_step", "A_win", "A_pub", "B_pub", "A_ema", "B", "pressure_raw", "pressure_rel", "step_counter", "status"):
+                assert torch.equal(getattr(other, f), getattr(states[0], f)), (step, f)
+        assert int(states[0].step_counter.item()) == step + 1 and int(states[0].status.item()) == 0
+        assert int(states[0]._step_words[1].item()) == 0                      # the library's layer counter is 0 between calls

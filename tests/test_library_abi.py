@@ -85,12 +85,12 @@ def test_no_cpu_fallback_without_gpu():
 def test_options_are_validated_and_readable():
     """gimbal_set_option / gimbal_get_option: defaults, ranges (nothing reads the environment)."""
     defaults = {g.OPT_CTA_GROUP: 0, g.OPT_FUSE_GATE: 1, g.OPT_SCORE_GENERIC: 0, g.OPT_CHECK_SCORES_ALL: 0, g.OPT_HIST_AGG: 1,
-                g.OPT_SCORE_TMA: 1, g.OPT_EPI_PARTS: 0, g.OPT_PDL: 1}
+                g.OPT_SCORE_TMA: 1, g.OPT_EPI_PARTS: 0, g.OPT_PDL: 1, g.OPT_FUSE_UPDATE: 1}
     for opt, val in defaults.items():
         assert g.get_option(opt) == val
     for opt in (g.OPT_CTA_GROUP, g.OPT_EPI_PARTS, g.OPT_PDL):
         assert g.lib().gimbal_set_option(opt, 3) == -1 and g.lib().gimbal_set_option(opt, 2) == 0 and g.get_option(opt) == 2
         g.set_option(opt, defaults[opt])
-    for opt in (g.OPT_SCORE_TMA, g.OPT_HIST_AGG):
+    for opt in (g.OPT_SCORE_TMA, g.OPT_HIST_AGG, g.OPT_FUSE_UPDATE):
         assert g.lib().gimbal_set_option(opt, 2) == -1 and g.get_option(opt) == 1
     assert g.lib().gimbal_set_option(99, 0) == -1
