@@ -367,9 +367,11 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
         if (warp >= 4 && leader) ptx::griddep_wait();                            // the previous step's stats_update_kernel is done with A_step
         // one tile per layer, one CTA (pair) per tile: the barrier above made both histograms of the pair complete and visible;
         // the leader adds its peer's through distributed shared memory and STORES the layer's counts (zeros included)
+        int64_t step_now = 0;
         if (warp >= 4 && leader) {
             const int ep_tid = threadIdx.x - 128;
             const int layer = p.layer0 + pair;                                   // tile == pair, m_tiles == 1
+            if (p.fuse_update) step_now = *p.upd.step_counter;                   // (behind the wait above; its latency hides in the loop below)
             int32_t* dst = p.A_step + (size_t)layer * p.S * N;
             const uint32_t peer = (kCG == 2) ? ptx::mapa(ptx::smem_u32(hist), 1) : 0u;
             const int n4 = p.S * N / 4;                                          // N % 4 == 0, hist is 16-byte aligned
@@ -381,16 +383,18 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
                     c.x += (int32_t)o.x; c.y += (int32_t)o.y; c.z += (int32_t)o.z; c.w += (int32_t)o.w;
                 }
                 reinterpret_cast<int4*>(dst)[i] = c;
+                reinterpret_cast<int4*>(hist)[i] = c;                            // the layer's counts stay here for the update below
             }
         }
         if constexpr (kCG == 2) ptx::cluster_sync();                             // the peer's shared memory stays until it was read
         if (p.fuse_update && warp >= 4 && leader) {
-            // a4 + a5 of this layer right here: the counts just stored are complete; `hist` is free and serves as scratch
-            __threadfence();
+            // a4 + a5 of this layer right here, from the counts in `hist`; scratch = the (drained) operand ring
             asm volatile("bar.sync 1, %0;" ::"n"(kEpiThreads) : "memory");
-            UpdateScratch& sh = *reinterpret_cast<UpdateScratch*>(hist);
-            stats_update_layer(p.upd, p.layer0 + pair, (int)threadIdx.x - 128, kEpiThreads, sh,
-                               [] { asm volatile("bar.sync 1, %0;" ::"n"(kEpiThreads) : "memory"); });
+            UpdateScratch& sh = *reinterpret_cast<UpdateScratch*>(base_ptr);
+            const int32_t* hc = hist;
+            stats_update_layer(p.upd, p.layer0 + pair, (int)threadIdx.x - 128, kEpiThreads, sh, step_now,
+                               [] { asm volatile("bar.sync 1, %0;" ::"n"(kEpiThreads) : "memory"); },
+                               [hc](int s, int e) { return hc[s * N + e]; });
         }
     }
     if (warp == 2) ptx::tmem_dealloc<kCG>(tmem_base, kTmemCols);

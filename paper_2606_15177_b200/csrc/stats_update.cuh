@@ -27,41 +27,50 @@ struct UpdateParams {
 
 constexpr int kUpdateThreads = 256;
 
+constexpr int kUpdatePartStage = 2048;
+
 // scratch of one layer's update: [E <= 256] live B, [E] replica counts, [G <= 64] rank loads, two flags
 struct UpdateScratch {
     double b[256];
     int r[256];
     double lg[64];
+    int dp[64];
     int bad;
     int last;
+    double part[kUpdatePartStage];      // the [L][S] pressure partials, staged for the final reduction
 };
 
 // a4 + a5 of ONE layer by `nthr` threads (tid 0..nthr-1) that can synchronise through `sync()`; `done_counter` counts the layers
 // of the step: the caller that finishes the L-th layer reduces the pressure partials over layers in fixed order (deterministic),
 // advances the step counter and leaves the counter at 0.  Used by stats_update_kernel (one block per layer) and by the fused
 // router kernel in the one-tile-per-layer regime (the CTA pair that owns the layer's complete histogram).
-template <class Sync>
-__device__ __forceinline__ void stats_update_layer(const UpdateParams& p, int l, int tid, int nthr, UpdateScratch& sh, Sync sync) {
-    const int64_t step = *p.step_counter;
+// `step` = *p.step_counter read by the caller (as early as its ordering allows); `a_step(s, e)` = this layer's fresh counts (global
+// A_step for the kernel below, the router kernel's own shared-memory histogram in its tail).
+template <class Sync, class Counts>
+__device__ __forceinline__ void stats_update_layer(const UpdateParams& p, int l, int tid, int nthr, UpdateScratch& sh, int64_t step, Sync sync,
+                                                   Counts a_step) {
     const bool publish = p.mode == 0 && ((step + 1) % p.window_len) == 0;
     if (tid == 0) { sh.bad = 0; sh.last = 0; }
     for (int e = tid; e < 256; e += nthr) sh.r[e] = 0;
+    const bool want_pressure = p.cur_placement != nullptr && p.dp_of_rank != nullptr;
+    if (want_pressure)
+        for (int g = tid; g < p.G; g += nthr) sh.dp[g] = p.dp_of_rank[g];
     sync();
 
     for (int e = tid; e < p.E; e += nthr) {
-        // sources are read eight at a time before anything is written back: the loads of a batch are in
+        // sources are read sixteen at a time before anything is written back: the loads of a batch are in
         // flight together instead of one global round trip per source
         if (p.mode == 0) {
             int64_t b = 0;
-            for (int s0 = 0; s0 < p.S; s0 += 8) {
-                int32_t win[8], stp[8];
+            for (int s0 = 0; s0 < p.S; s0 += 16) {
+                int32_t win[16], stp[16];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const size_t i = ((size_t)l * p.S + min(s0 + j, p.S - 1)) * p.E + e;
-                    win[j] = p.A_win[i]; stp[j] = p.A_step[i];
+                for (int j = 0; j < 16; ++j) {
+                    const int sj = min(s0 + j, p.S - 1);
+                    win[j] = p.A_win[((size_t)l * p.S + sj) * p.E + e]; stp[j] = a_step(sj, e);
                 }
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
+                for (int j = 0; j < 16; ++j) {
                     if (s0 + j < p.S) {
                         const size_t i = ((size_t)l * p.S + s0 + j) * p.E + e;
                         const int64_t w = (int64_t)win[j] + stp[j];
@@ -78,15 +87,15 @@ __device__ __forceinline__ void stats_update_layer(const UpdateParams& p, int l,
             sh.b[e] = (double)b;
         } else {
             float b = 0.0f;
-            for (int s0 = 0; s0 < p.S; s0 += 8) {
-                float ema[8]; int32_t stp[8];
+            for (int s0 = 0; s0 < p.S; s0 += 16) {
+                float ema[16]; int32_t stp[16];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const size_t i = ((size_t)l * p.S + min(s0 + j, p.S - 1)) * p.E + e;
-                    ema[j] = p.A_ema[i]; stp[j] = p.A_step[i];
+                for (int j = 0; j < 16; ++j) {
+                    const int sj = min(s0 + j, p.S - 1);
+                    ema[j] = p.A_ema[((size_t)l * p.S + sj) * p.E + e]; stp[j] = a_step(sj, e);
                 }
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
+                for (int j = 0; j < 16; ++j) {
                     if (s0 + j < p.S) {
                         const float a = __fmaf_rn(p.ema_decay, ema[j], (float)stp[j]);
                         p.A_ema[((size_t)l * p.S + s0 + j) * p.E + e] = a;
@@ -99,7 +108,6 @@ __device__ __forceinline__ void stats_update_layer(const UpdateParams& p, int l,
         }
     }
 
-    const bool want_pressure = p.cur_placement != nullptr && p.dp_of_rank != nullptr;
     if (want_pressure) {
         const int NS = p.G * p.sp;
         const int16_t* pl = p.cur_placement + (size_t)l * NS;
@@ -120,7 +128,7 @@ __device__ __forceinline__ void stats_update_layer(const UpdateParams& p, int l,
         for (int s = tid; s < p.S; s += nthr) {
             double acc = 0.0;
             for (int g = 0; g < p.G; ++g)
-                if (p.dp_of_rank[g] == s) acc += sh.lg[g];
+                if (sh.dp[g] == s) acc += sh.lg[g];
             p.partial[(size_t)l * p.S + s] = acc;
         }
     }
@@ -135,9 +143,17 @@ __device__ __forceinline__ void stats_update_layer(const UpdateParams& p, int l,
     if (sh.last) {
         __threadfence();
         if (want_pressure) {
+            // every thread fetches its share of the [L][S] partials at once (one round trip instead of L dependent ones), then source
+            // s adds its column in layer order -- the same order, hence the same doubles, as a plain loop over the layers
+            const int n = p.L * p.S;
+            const bool staged = n <= kUpdatePartStage;
+            if (staged) {
+                for (int i = tid; i < n; i += nthr) sh.part[i] = __ldcg(p.partial + i);
+                sync();
+            }
             for (int s = tid; s < p.S; s += nthr) {
                 double acc = 0.0;
-                for (int ll = 0; ll < p.L; ++ll) acc += __ldcg(p.partial + (size_t)ll * p.S + s);
+                for (int ll = 0; ll < p.L; ++ll) acc += staged ? sh.part[ll * p.S + s] : __ldcg(p.partial + (size_t)ll * p.S + s);
                 sh.lg[s] = acc;
             }
         }
@@ -164,7 +180,11 @@ __global__ void __launch_bounds__(kUpdateThreads) stats_update_kernel(const Upda
     // memory) here; the next kernel of the stream may be scheduled from now on (it waits for this grid before it writes A_step)
     asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    stats_update_layer(p, blockIdx.x, threadIdx.x, kUpdateThreads, sh, [] { __syncthreads(); });
+    const int l = blockIdx.x;
+    const int32_t* a = p.A_step + (size_t)l * p.S * p.E;
+    const int E = p.E;
+    stats_update_layer(p, l, threadIdx.x, kUpdateThreads, sh, *p.step_counter, [] { __syncthreads(); },
+                       [a, E](int s, int e) { return a[(size_t)s * E + e]; });
 }
 #endif
 
