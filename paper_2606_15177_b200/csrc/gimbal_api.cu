@@ -733,7 +733,8 @@ int gimbal_eval_moves(const gimbal_placement_cfg* cfg, const int16_t* cur, const
         const int n_tasks = (int)(NS / 2);
         const size_t smem_all = move_all_smem_bytes((int)NS, cfg->G, M != nullptr);
         int per_sm = (int)((kSmemLimit - 1024) / (smem_all + 1024));
-        per_sm = per_sm > 4 ? 4 : (per_sm < 1 ? 1 : per_sm);
+        constexpr int kMaxResident = 2048 / kMoveAllThreads / 2;          // 64 registers per thread
+        per_sm = per_sm > kMaxResident ? kMaxResident : (per_sm < 1 ? 1 : per_sm);
         int bpl = per_sm * device_info().sms / cfg->L;
         const int max_bpl = (n_tasks + kMoveAllThreads / 32 - 1) / (kMoveAllThreads / 32);
         if (bpl > max_bpl) bpl = max_bpl;

@@ -1106,7 +1106,7 @@ __global__ void __launch_bounds__(256) move_delta_kernel(const MoveParams p) {
 //   dC_mig  = 2 M (n11 + n22 - n12 - n21), n = "x0 hosts the cell" (scalar M; with a table the four M's with those signs)
 //   dmaxload from the layer's three largest rank loads, in fp32 (compared relative to the largest load)
 // Same rank or same expert: zeros.  A second copy of an expert on a rank: NaN.  No data-dependent branch.
-constexpr int kMoveAllThreads = 256;
+constexpr int kMoveAllThreads = 512;
 
 __host__ __device__ inline size_t move_all_smem_bytes(int NS, int G, int has_M) {
     size_t b = sizeof(float) * (size_t)NS * (G + 1) * (has_M ? 2 : 1);   // Cs (+ Ms)
@@ -1163,7 +1163,7 @@ struct MoveAllParams {
 // depends on a (expert, rank, load, its table row) is warp-uniform, and the results of 32
 // consecutive b are contiguous in `delta`.
 template <bool kHasM>
-__global__ void __launch_bounds__(kMoveAllThreads, 4) move_all_kernel(const MoveAllParams p) {
+__global__ void __launch_bounds__(kMoveAllThreads, 2048 / kMoveAllThreads / 2) move_all_kernel(const MoveAllParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int NS = p.G * p.sp, PITCH = p.G + 1;
     const int l = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
