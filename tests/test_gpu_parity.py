@@ -1239,3 +1239,49 @@ def test_router_epilogue_parts_meet_on_exact_ties(name, hot):
         st2 = g.StatsState(cfg, MODE_WINDOW, window_len=1)
         g.route_stats(cfg, st2, T=w.T, hidden=hidden, w_router=W, src_offsets=off, workspace=ws)
         assert torch.equal(st2.A_step, st.A_step), f"epilogue parts = {parts}"
+
+
+def test_outputs_stay_inside_their_buffers():
+    """compute-sanitizer is closed on this pool, so the new store / copy paths are fenced by hand: every output and the workspace sit
+    inside larger buffers filled with a sentinel; after the calls the sentinels are intact and only the asked-for slices changed.
+    (1) the small-batch router path that STORES a layer's counts, called on a middle slice of the layers; (2) the TMA scoring
+    kernel with an odd P (its copies fetch a second candidate past the end) and a workspace of exactly the advertised size."""
+    # (1) layers 1..2 of 4, T = 200 (one tile per layer): A_step of layers 0 and 3 must keep the sentinel
+    w = scaled(get_workload("v3"), L=4, T=200)
+    r = w.router
+    cfg = g.RouterCfg.from_workload(r)
+    hidden = gen.hidden_all(w, 0, DEV); W = gen.w_router(w, DEV); slb = gen.src_logit_bias(w, 0, DEV); sb = gen.select_bias(w, DEV)
+    off = gen.src_offsets(w, 0, w.T, DEV)
+    st = g.StatsState(cfg, MODE_WINDOW, window_len=4)
+    st.A_step.fill_(-77)
+    need = g.route_stats_workspace_bytes(cfg, 2, w.T)
+    wsb = torch.full((need + 8192,), 0x5A, dtype=torch.uint8, device=DEV)
+    ws = wsb[4096:4096 + need]
+    g.route_stats(cfg, st, T=w.T, hidden=hidden[1:3], w_router=W, select_bias=sb, src_logit_bias=slb, src_offsets=off, layer0=1, n_layers=2,
+                  workspace=ws)
+    torch.cuda.synchronize()
+    A = to_np(st.A_step)
+    assert (A[0] == -77).all() and (A[3] == -77).all() and (A[1:3] >= 0).all()
+    assert A[1:3].sum() == 2 * w.T * r.k and int(st.step_counter.item()) == 0          # not the last slice: no update yet
+    assert bool((wsb[:4096] == 0x5A).all()) and bool((wsb[4096 + need:] == 0x5A).all())
+    # (2) TMA scoring kernel, P = 37 and 1001
+    for P in (37, 1001):
+        wp = scaled(get_workload("v3"), L=3, T=256, P=P)
+        rng = np.random.default_rng(P)
+        A_t = torch.from_numpy(rng.integers(0, 999, (3, r.S, r.E)).astype(np.int32)).to(DEV)
+        B_t = A_t.sum(1).to(torch.int32)
+        pc = g.PlacementCfg(L=3, E=r.E, G=wp.G, slots_per_rank=wp.slots_per_rank, S=r.S, flags=g.PLACE_TRUSTED)
+        D = gen.comm_cost_D(wp, "binary", DEV)
+        prev = gen.prev_placement(wp, to_np(B_t), DEV)
+        need = g.eval_placements_workspace_bytes(pc, P)
+        wsb = torch.full((need + 8192,), 0x5A, dtype=torch.uint8, device=DEV)
+        outb = torch.full((P + 64, 5), -5.0, device=DEV)
+        candb = torch.zeros(P + 8, 3, wp.NS, dtype=torch.int16, device=DEV)
+        candb[:P] = gen.candidates(wp, prev, P, DEV)
+        candb[P:] = 255                                                                  # rows past the end: valid ids, never scored
+        g.eval_placements(pc, candb[:P], A_t, B_t, D, prev, outb[32:32 + P], workspace=wsb[4096:4096 + need])
+        torch.cuda.synchronize()
+        assert bool((outb[:32] == -5.0).all()) and bool((outb[32 + P:] == -5.0).all()) and not bool(torch.isnan(outb[32:32 + P]).any())
+        assert bool((wsb[:4096] == 0x5A).all()) and bool((wsb[4096 + need:] == 0x5A).all())
+        ref = oracle.objective_batch(to_np(candb[:P])[:8], to_np(prev), to_np(A_t), to_np(B_t), to_np(D), None, 1.0, **_oracle_kw(pc))
+        _check_objective(to_np(outb[32:40]).astype(np.float64), ref)
