@@ -191,7 +191,7 @@ def test_decode_episode_200_steps_from_one_cuda_graph():
 
 
 @pytest.mark.parametrize("name,T,L,window_len", [("v3", 256, 3, 2), ("v3", 100, 2, 3), ("decode", 256, 4, 1), ("qwen3", 200, 3, 2),
-                                                   ("qwen3", 128, 2, 2), ("v2lite", 77, 3, 2)])
+                                                   ("qwen3", 128, 2, 2), ("v2lite", 77, 3, 2), ("tiny", 200, 1, 1), ("tiny", 64, 1, 2)])
 def test_small_batch_regime_fused_update_matches_the_separate_kernels(name, T, L, window_len):
     """One tile per layer (T <= 256, every layer with a CTA pair of its own): the router kernel stores the counts (no zeroing of
     A_step) and, in a whole-step call, runs the window / EMA update of its layer in its tail (GIMBAL_OPT_FUSE_UPDATE).  Six steps
