@@ -208,6 +208,53 @@ GIMBAL_API int gimbal_route_stats(const gimbal_router_cfg *cfg, int layer0, int 
                        gimbal_stats_state *state, const gimbal_expert_map *map /* | NULL */,
                        void *workspace, size_t workspace_bytes, gimbal_stream_t stream);
 
+/* ---------------------------------------------------------------------------------------
+ * gimbal_route_stats_static -- gimbal_route_stats for callers that have no device memory to give.
+ *
+ * Who needs it.  gimbal_route_stats wants a caller-owned workspace (the per-layer pressure partials and the
+ * layer counter of the a4-a5 update kernel).  A scheduler thread that lives inside a serving engine often
+ * cannot provide one: the engine has already handed all free HBM to its KV-cache pool, so a cudaMalloc made
+ * after start-up fails or steals from that pool; and a cudaMalloc / cudaFree issued from a side thread
+ * synchronises the whole device and stalls the decode loop it sits next to.  For those callers the scratch
+ * lives inside the library: a file-scope `static __device__` array of GIMBAL_STATIC_SCRATCH_BYTES (64 KiB)
+ * that every GPU on which the library's code is loaded keeps until the process exits.
+ *
+ * Arguments, outputs, stream order and errors are those of gimbal_route_stats, minus `workspace` /
+ * `workspace_bytes`; inputs, outputs and the state are still the caller's device memory.  Results are
+ * bit-identical to gimbal_route_stats on the same inputs (same kernels, same launch configuration).
+ *
+ * Limit.  The shape must satisfy gimbal_route_stats_workspace_bytes(cfg, ..) <= GIMBAL_STATIC_SCRATCH_BYTES,
+ * i.e. L * S <= 8128 (the DeepSeek-V3 shape has L * S = 928).  A larger shape is refused with
+ * GIMBAL_ERR_WORKSPACE and a message that states both sizes; nothing is launched.
+ *
+ * Set-up.  The first call on each device (the device current at the call) resolves the array's device
+ * address with cudaGetSymbolAddress -- the array's name in host code is only a handle, not something a
+ * kernel can dereference -- and remembers it for that device.  That first call may make the runtime load
+ * the library's device code, so make it once per device BEFORE any stream capture and before the part of
+ * the program that must not stall.  If the look-up fails the call returns GIMBAL_ERR_CUDA.
+ *
+ * No allocation.  Neither the set-up nor any later call uses cudaMalloc, cudaFree, a memory pool or any
+ * other allocating routine (host or device); with gimbal_kernel_timing switched on, the timing hooks'
+ * events exist already.
+ *
+ * Sharing.  There is ONE array per device, shared by every call, every stream and every host thread of
+ * the process, and it still holds whatever the previous call left there.  The entry point therefore
+ * zeroes the part it is about to use whenever the shape's scratch layout differs from that of the previous
+ * call on the device (the layer counter has to start at 0; the partials are always written before they
+ * are read).  Two calls whose kernels can overlap on the GPU -- different streams, or the same step issued
+ * from two threads -- race on the array and give wrong pressure values or a step that never completes its
+ * update: serialise them (one stream, or events), or give the concurrent caller its own workspace through
+ * gimbal_route_stats.                                                                              */
+#define GIMBAL_STATIC_SCRATCH_BYTES 65536
+GIMBAL_API int gimbal_route_stats_static(const gimbal_router_cfg *cfg, int layer0, int n_layers, int T,
+                              const void *hidden, const void *w_router,
+                              const float *select_bias, const float *src_logit_bias,
+                              const int32_t *src_offsets, int logits_mode, float *logits,
+                              int32_t *topk_ids, float *topk_w,
+                              const int16_t *cur_placement, const int32_t *dp_of_rank, int G, int slots_per_rank,
+                              gimbal_stats_state *state, const gimbal_expert_map *map /* | NULL */,
+                              gimbal_stream_t stream);
+
 /* Inverse of a slot -> expert placement [L,NS] for gimbal_expert_map: rep_off [L,E+1] and
  * rep_slots [L,NS] (device, caller-owned).  Ids out of range set bit 0 of `status`.         */
 GIMBAL_API int gimbal_build_expert_map(int L, int E, int G, int slots_per_rank, const int16_t *placement,

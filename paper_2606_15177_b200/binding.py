@@ -16,7 +16,7 @@ COUNTS_I32, COUNTS_F32 = 0, 1
 
 EXPORTED_SYMBOLS = [
     "gimbal_version", "gimbal_last_error", "gimbal_launch_count",
-    "gimbal_route_stats_workspace_bytes", "gimbal_route_stats", "gimbal_route_stats_result_bytes",
+    "gimbal_route_stats_workspace_bytes", "gimbal_route_stats", "gimbal_route_stats_static", "gimbal_route_stats_result_bytes",
     "gimbal_route_stats_host", "gimbal_host_ctx_create", "gimbal_host_ctx_destroy", "gimbal_eval_moves_host",
     "gimbal_set_option", "gimbal_get_option",
     "gimbal_eval_placements_workspace_bytes", "gimbal_eval_placements", "gimbal_eval_placements_host",
@@ -77,7 +77,7 @@ def lib():
         for n in ("gimbal_route_stats_workspace_bytes", "gimbal_route_stats_result_bytes",
                   "gimbal_eval_placements_workspace_bytes", "gimbal_eval_moves_workspace_bytes"):
             getattr(L, n).restype = C.c_size_t
-        for n in ("gimbal_route_stats", "gimbal_route_stats_host", "gimbal_eval_placements",
+        for n in ("gimbal_route_stats", "gimbal_route_stats_static", "gimbal_route_stats_host", "gimbal_eval_placements",
                   "gimbal_eval_placements_host", "gimbal_eval_moves", "gimbal_eval_moves_host", "gimbal_greedy_place",
                   "gimbal_build_expert_map", "gimbal_select_engines", "gimbal_order_queues", "gimbal_refine_placement",
                   "gimbal_host_ctx_create", "gimbal_host_ctx_destroy", "gimbal_set_option", "gimbal_get_option"):
@@ -231,6 +231,31 @@ def route_stats(cfg: RouterCfg, state: StatsState, *, T: int, hidden=None, w_rou
                                   C.c_size_t(0 if workspace is None else workspace.numel() * workspace.element_size()),
                                   _stream(stream))
     _check(rc, "gimbal_route_stats")
+
+
+STATIC_SCRATCH_BYTES = 65536
+
+
+def route_stats_static(cfg: RouterCfg, state: StatsState, *, T: int, hidden=None, w_router=None, select_bias=None,
+                       src_logit_bias=None, src_offsets=None, layer0: int = 0, n_layers: int | None = None,
+                       logits_mode: int = LOGITS_NONE, logits=None, topk_ids=None, topk_w=None, cur_placement=None,
+                       dp_of_rank=None, G: int = 0, slots_per_rank: int = 0, expert_map=None, phys_ids=None, stream=None):
+    """gimbal_route_stats_static: route_stats without a workspace argument, for a caller that cannot obtain device memory
+    (an engine that gave all of its HBM to the KV cache, a side thread that must not stall the device with cudaMalloc).
+    The update kernel's scratch is a 64 KiB array inside the library, one per GPU and shared by all calls: shapes with
+    L * S > 8128 are refused, calls that may overlap on the GPU must be serialised by the caller, and the first call on
+    a device (which looks the array up) belongs before any stream capture.  Same results as route_stats."""
+    n_layers = cfg.L - layer0 if n_layers is None else n_layers
+    c, s = cfg.c(), state.c()
+    m = None
+    if expert_map is not None:
+        m = _ExpertMap(expert_map.rep_off.data_ptr(), expert_map.rep_slots.data_ptr(), phys_ids.data_ptr(), expert_map.NS)
+    rc = lib().gimbal_route_stats_static(C.byref(c), C.c_int(layer0), C.c_int(n_layers), C.c_int(T), _ptr(hidden), _ptr(w_router),
+                                         _ptr(select_bias), _ptr(src_logit_bias), _ptr(src_offsets), C.c_int(logits_mode),
+                                         _ptr(logits), _ptr(topk_ids), _ptr(topk_w), _ptr(cur_placement), _ptr(dp_of_rank),
+                                         C.c_int(G), C.c_int(slots_per_rank), C.byref(s),
+                                         C.byref(m) if m is not None else C.c_void_p(None), _stream(stream))
+    _check(rc, "gimbal_route_stats_static")
 
 
 class ExpertMap:

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #define GIMBAL_DEFINE_STATS_UPDATE_KERNEL
@@ -450,6 +451,62 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
         LAUNCH_CHECK("stats_update_kernel");
     }
     return GIMBAL_OK;
+}
+
+// ---- gimbal_route_stats_static: the scratch of the a4-a5 update lives in the library ------------------
+// One array per device that has this module loaded, zero at load, kept until the process exits.  In HOST code the name below is
+// only the handle that cudaGetSymbolAddress understands; the pointer a kernel may use is what that call returns, per device.
+static __device__ __align__(256) unsigned char gimbal_static_scratch[GIMBAL_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+struct StaticScratchDev {
+    void* ptr = nullptr;     // device address of gimbal_static_scratch on this device (set-up done when non-null)
+    size_t layout = 0;       // bytes the previous call on this device carved (0: none yet)
+};
+std::mutex g_static_mu;
+StaticScratchDev g_static_dev[kStaticMaxDevices];
+}  // namespace
+
+int gimbal_route_stats_static(const gimbal_router_cfg* cfg, int layer0, int n_layers, int T, const void* hidden, const void* w_router,
+                              const float* select_bias, const float* src_logit_bias, const int32_t* src_offsets, int logits_mode,
+                              float* logits, int32_t* topk_ids, float* topk_w, const int16_t* cur_placement, const int32_t* dp_of_rank,
+                              int G, int slots_per_rank, gimbal_stats_state* st, const gimbal_expert_map* map, gimbal_stream_t stream_) {
+    int rc = validate_router_cfg(cfg);
+    if (rc) return rc;
+    const size_t need = route_ws_carve(cfg, nullptr, nullptr);
+    if (need > sizeof gimbal_static_scratch)
+        return fail(GIMBAL_ERR_WORKSPACE,
+                    "gimbal_route_stats_static: L=%d x S=%d needs %zu bytes of scratch, the built-in array holds %zu (L*S <= 8128); "
+                    "use gimbal_route_stats with a workspace of your own",
+                    cfg->L, cfg->S, need, sizeof gimbal_static_scratch);
+    rc = require_device();
+    if (rc) return rc;
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(GIMBAL_ERR_UNSUPPORTED, "gimbal_route_stats_static: device ordinal %d (max %d)", dev, kStaticMaxDevices - 1);
+    void* scratch = nullptr;
+    bool relayout = false;
+    {
+        std::lock_guard<std::mutex> lk(g_static_mu);
+        StaticScratchDev& d = g_static_dev[dev];
+        if (!d.ptr) {
+            // set-up, once per device, with that device current: ask the runtime where the array lives on it
+            void* p = nullptr;
+            const cudaError_t e = cudaGetSymbolAddress(&p, gimbal_static_scratch);
+            if (e != cudaSuccess || !p)
+                return fail(GIMBAL_ERR_CUDA, "cudaGetSymbolAddress(gimbal_static_scratch) on device %d: %s", dev, cudaGetErrorString(e));
+            d.ptr = p;
+        }
+        scratch = d.ptr;
+        relayout = d.layout != need;
+        d.layout = need;
+    }
+    // the array keeps the previous call's contents: under a new layout the layer counter may sit where partials were
+    if (relayout) CUDA_TRY(cudaMemsetAsync(scratch, 0, need, static_cast<cudaStream_t>(stream_)));
+    return gimbal_route_stats(cfg, layer0, n_layers, T, hidden, w_router, select_bias, src_logit_bias, src_offsets, logits_mode, logits,
+                              topk_ids, topk_w, cur_placement, dp_of_rank, G, slots_per_rank, st, map, scratch,
+                              sizeof gimbal_static_scratch, stream_);
 }
 
 struct gimbal_host_ctx {
