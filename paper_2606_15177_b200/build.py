@@ -24,6 +24,10 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
 
 
+# extra nvcc flags for A/B builds, e.g. GIMBAL_NVCC_EXTRA=-DGIMBAL_TMA_HANDOFF=1 (part of the staleness digest)
+NVCC_FLAGS += os.environ.get("GIMBAL_NVCC_EXTRA", "").split()
+
+
 def _nvcc() -> str:
     return os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 

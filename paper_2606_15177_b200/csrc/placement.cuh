@@ -173,7 +173,7 @@ struct ScoreParams {
     float4* partial;                    // [P,L] {sum_g d_g^2, comm, mig, maxL}; NaN in .x if invalid
     uint8_t* status;                    // [L,P] verdicts of the fused validation (kCheck): 0 same copies as x0, 1 invalid, 2 other replica counts
     int force_general;                  // tests: verdict 2 for every valid candidate
-    uint32_t zero;                      // 0, opaque to the compiler (place_score_tma_kernel's ordering dependency)
+    uint32_t zero;                      // 0 at run time, opaque to the compiler: place_score_tma_kernel's ordering dependency
 };
 
 constexpr int kScoreThreads = 512;
@@ -459,7 +459,8 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_kernel(const Sco
 constexpr int kTmaRowPitch = 640;                     // 4 pieces x 160 B
 constexpr int kTmaSlots = 2;                          // ring slots per warp, one pass (two rows) each
 inline size_t place_score_tma_smem_bytes() {
-    return (size_t)256 * 256 + (size_t)(kScoreThreads / 32) * kTmaSlots * kScoreU * kTmaRowPitch + (kScoreThreads / 32) * kTmaSlots * 8;
+    // table + per-warp ring + per-warp (full, empty) barrier of every slot
+    return (size_t)256 * 256 + (size_t)(kScoreThreads / 32) * kTmaSlots * kScoreU * kTmaRowPitch + (kScoreThreads / 32) * kTmaSlots * 16;
 }
 
 __device__ __forceinline__ uint32_t lds_u32_ordered(uint32_t addr) {      // ordered among the volatile asm statements (barrier wait before, refill after)
@@ -473,6 +474,12 @@ __device__ __forceinline__ float2 lds_f32x2(uint32_t addr) {               // a 
     return v;
 }
 
+// How a warp hands a ring slot it has read back to the copy engine (see the comment at the refill): 0 = the copy's coordinate
+// depends on every word the warp loaded (default, the only variant that is both correct and free), 1 = release / acquire on an
+// "empty" mbarrier, 2 = fence.proxy.async.  1 and 2 exist for the record in profiles/r3_k4_tma_handoff.md.
+#ifndef GIMBAL_TMA_HANDOFF
+#define GIMBAL_TMA_HANDOFF 0
+#endif
 __global__ void __launch_bounds__(kScoreThreads, 2) place_score_tma_kernel(const ScoreParams p, const __grid_constant__ CUtensorMap tm) {
     constexpr int SP = 9, G = 32, E = 256, NS = G * SP, NW = 5, kU = kScoreU, kWarps = kScoreThreads / 32;
     constexpr uint32_t kPassBytes = kU * kTmaRowPitch;
@@ -485,11 +492,14 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_tma_kernel(const
     const int c_first = p_begin + warp * kU;
     const uint32_t tab_a = __shfl_sync(0xffffffffu, ptx::smem_u32(smem_raw), 0);     // [E][32] float2
     const uint32_t ring_a = tab_a + (uint32_t)E * 256u + (uint32_t)warp * (kTmaSlots * kPassBytes);          // [slots][kU][640] of this warp
-    const uint32_t bar_a = tab_a + (uint32_t)E * 256u + (uint32_t)kWarps * (kTmaSlots * kPassBytes) + (uint32_t)warp * (kTmaSlots * 8);
+    // this warp's barriers: "full" of slot s at bar_a + 8 s (the copy's bytes have landed); the "empty" barriers behind them are
+    // only used by the GIMBAL_TMA_HANDOFF == 1 build
+    const uint32_t bar_a = tab_a + (uint32_t)E * 256u + (uint32_t)kWarps * (kTmaSlots * kPassBytes) + (uint32_t)warp * (kTmaSlots * 16);
+    constexpr uint32_t kEmptyOff = kTmaSlots * 8;
     const uint64_t pol = ptx::policy_evict_first();
     if (ptx::elect_one()) {
 #pragma unroll
-        for (int s = 0; s < kTmaSlots; ++s) ptx::mbar_init(bar_a + 8 * s, 1);
+        for (int s = 0; s < kTmaSlots; ++s) { ptx::mbar_init(bar_a + 8 * s, 1); ptx::mbar_init(bar_a + kEmptyOff + 8 * s, 1); }
         ptx::fence_barrier_init();
         ptx::fence_proxy_async();
         // the first rows are on their way while the table is staged
@@ -535,25 +545,49 @@ __global__ void __launch_bounds__(kScoreThreads, 2) place_score_tma_kernel(const
     uint32_t kept[2 * kU];
     uint32_t it = 0;
     auto pass = [&](int c0, int q) {
-        const uint32_t slot = it & (kTmaSlots - 1);
+        const uint32_t slot = it & (kTmaSlots - 1), phase = (it / kTmaSlots) & 1u;
         const uint32_t bar = bar_a + 8 * slot, rows = ring_a + slot * kPassBytes;
-        ptx::mbar_wait(bar, (it / kTmaSlots) & 1u);
+        ptx::mbar_wait(bar, phase);
         ++it;
         uint32_t w[kU][NW];
 #pragma unroll
         for (int u = 0; u < kU; ++u)
 #pragma unroll
             for (int j = 0; j < NW; ++j) w[u][j] = lds_u32_ordered(rows + u * kTmaRowPitch + 4 * j + lane_off);
-        // refill the slot with the pass after next: the copy (async proxy) overwrites what the loads above read, and ptxas is free to
-        // issue it while they are still queued -- at kernel start, when all warps fire at once, a queued load has been seen to lose
-        // that race.  So the copy's candidate coordinate carries a true dependency on the words of every lane: an OR-reduction over
-        // the warp of (first | last word of both rows) & p.zero, which the host sets to 0 and the compiler cannot fold.
+        // refill the slot with the pass after next.  The copy (async proxy) overwrites what the loads above read, and it must not
+        // start before every lane's loads have RETURNED: at kernel start, when all warps of an SM fire at once behind the table's
+        // stores, queued loads lose that race.  Measured on the bench grid (4096 candidates x 58 layers, 300 launches,
+        // profiles/r3_k4_tma_handoff.md): the textbook hand-off -- arrive on an "empty" mbarrier after the loads, wait on it, then
+        // expect_tx + copy -- still returned wrong rows in 14 launches (the barrier unit is not ordered behind the warp's queued
+        // shared-memory loads, and nothing waits for their scoreboard); fence.proxy.async before the copy was correct but 2 us
+        // slower.  What holds by construction, at no cost: the copy's candidate coordinate carries a true dependency on ALL ten
+        // words of every lane (warp OR-reduction, AND-ed with a kernel argument that is 0 at run time and that the compiler
+        // cannot fold), so UTMALDG cannot issue before the last load has delivered its register.
         if (c0 + kTmaSlots * kPassStride < p_end) {
-            const uint32_t dep = __reduce_or_sync(0xffffffffu, (w[0][0] | w[0][NW - 1] | w[kU - 1][0] | w[kU - 1][NW - 1]) & p.zero);
+#if GIMBAL_TMA_HANDOFF == 0
+            uint32_t acc = 0u;
+#pragma unroll
+            for (int u = 0; u < kU; ++u)
+#pragma unroll
+                for (int j = 0; j < NW; ++j) acc |= w[u][j];
+            const uint32_t dep = __reduce_or_sync(0xffffffffu, acc & p.zero);
             if (ptx::elect_one()) {
                 ptx::mbar_arrive_expect_tx(bar, kPassBytes);
                 ptx::tma_load_4d(rows, &tm, bar, 0, 0, l, c0 + kTmaSlots * kPassStride + (int)dep, pol);
             }
+#else
+            __syncwarp();
+            if (ptx::elect_one()) {
+#if GIMBAL_TMA_HANDOFF == 1
+                ptx::mbar_arrive(bar + kEmptyOff);          // the slot's k-th refill completes phase k: same parity as the full barrier
+                ptx::mbar_wait(bar + kEmptyOff, phase);
+#else
+                ptx::fence_proxy_async();
+#endif
+                ptx::mbar_arrive_expect_tx(bar, kPassBytes);
+                ptx::tma_load_4d(rows, &tm, bar, 0, 0, l, c0 + kTmaSlots * kPassStride, pol);
+            }
+#endif
         }
 #pragma unroll
         for (int u = 0; u < kU; ++u) {

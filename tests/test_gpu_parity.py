@@ -1168,13 +1168,14 @@ def test_eval_placements_and_moves_on_other_shapes(L, E, G, sp, S, table_M, coun
         assert int(best[l].item()) == l * per + int(np.nanargmin(to_np(delta)[l * per:(l + 1) * per, 0]))
 
 
-@pytest.mark.parametrize("P,L", [(1, 2), (2, 3), (31, 2), (33, 1), (97, 4), (1000, 5), (2051, 58)])
+@pytest.mark.parametrize("P,L", [(1, 2), (2, 3), (31, 2), (33, 1), (97, 4), (1000, 5), (2051, 58), (4096, 58)])
 def test_place_score_tma_kernel_matches_the_lane_load_kernel_and_the_oracle(P, L):
     """The 9 x 32 x 256 shape, scalar M, GIMBAL_PLACE_TRUSTED: rows delivered by TMA (place_score_tma_kernel, the default) against
     the per-lane-load kernel (GIMBAL_OPT_SCORE_TMA = 0) bit for bit -- odd and ragged P (a copy's second candidate past the end,
     chunks that are not a multiple of a warp pass), one block per layer up to the bench grid -- and against the oracle on a
     sample.  Repeated right after a large memset so that every warp's first passes really wait on their barriers; the ring's
-    write-after-read ordering (K4) once failed exactly there."""
+    write-after-read ordering (K4) once failed exactly there -- the last case is the bench's own grid
+    (P = 4096 candidates x 58 layers, 290 blocks), launched fifty times."""
     w = scaled(get_workload("v3"), L=L, T=256, P=P)
     r = w.router
     rng = np.random.default_rng(11 + P)
@@ -1189,7 +1190,7 @@ def test_place_score_tma_kernel_matches_the_lane_load_kernel_and_the_oracle(P, L
     outs = {}
     for tma in (0, 1):
         g.set_option(g.OPT_SCORE_TMA, tma)
-        for rep in range(1 if tma == 0 else 12):
+        for rep in range(1 if tma == 0 else (50 if P == 4096 else 12)):
             out = torch.full((P, 5), -3.0, device=DEV)
             flush.zero_()
             g.eval_placements(cfg, cands, A, B, D, prev, out, M_scalar=0.75, workspace=ws)
