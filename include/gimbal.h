@@ -38,6 +38,16 @@ extern "C" {
 #define GIMBAL_API
 #endif
 
+/* Version of this interface = the value gimbal_version() returns.  It changes whenever a struct layout, a buffer size or
+ * an argument list of this header changes, so that a caller compiled against another header is refused instead of
+ * reading or writing past its buffers:
+ *   100  round 1
+ *   300  gimbal_stats_state: step_counter is i64[2] (was [1]) and `reserved` became `abi_version`; gimbal_placement_cfg
+ *        gained `encoding` and `flags`; gimbal_route_stats_host gained the leading `ctx`; gimbal_route_stats_static added.
+ * Every gimbal_stats_state must carry abi_version = GIMBAL_ABI_VERSION (GIMBAL_ERR_INVALID_ARG otherwise, nothing is
+ * launched); a caller can also compare gimbal_version() with the GIMBAL_ABI_VERSION it was compiled with at load time.   */
+#define GIMBAL_ABI_VERSION 300
+
 #define GIMBAL_OK 0
 #define GIMBAL_ERR_INVALID_ARG (-1)
 #define GIMBAL_ERR_UNSUPPORTED (-2)
@@ -100,7 +110,7 @@ typedef struct gimbal_router_cfg {
 typedef struct gimbal_stats_state {
     int32_t mode, window_len;
     float ema_decay;
-    int32_t reserved;
+    int32_t abi_version;   /* = GIMBAL_ABI_VERSION: the header this state was laid out by (step_counter [2]) */
     int32_t *A_step;
     int32_t *A_win;
     int32_t *A_pub;
@@ -128,7 +138,9 @@ typedef struct gimbal_stats_state {
  *             e.g. the output of gimbal_refine_placement or a rebalancer's own proposals); the
  *             validation pass is skipped.  A candidate that breaks the promise gets finite but
  *             meaningless numbers -- never a fault (ids are masked to the tables).
- * Supported: E <= 256 and even, G a power of two <= 64, slots_per_rank <= 16, S <= 64.       */
+ * Supported: E <= 256 and even, G a power of two <= 64, slots_per_rank <= 16, G*slots_per_rank even, S <= 64.  An `encoding` other than the two
+ * below or a bit of `flags` the library does not know is GIMBAL_ERR_INVALID_ARG (it is what a struct laid out by an older
+ * header would carry there).                                                                 */
 #define GIMBAL_ENC_SLOT_TO_EXPERT_I16 0
 #define GIMBAL_ENC_EXPERT_TO_RANK_U8 1
 #define GIMBAL_PLACE_TRUSTED 1
@@ -159,7 +171,7 @@ typedef struct gimbal_expert_map {
     int32_t NS;
 } gimbal_expert_map;
 
-/* Library / device probe.  gimbal_version() never touches CUDA. */
+/* Library / device probe.  gimbal_version() returns the library's GIMBAL_ABI_VERSION and never touches CUDA. */
 GIMBAL_API int gimbal_version(void);
 /* Writes the last CUDA / validation error string (NUL-terminated, truncated to n). */
 GIMBAL_API void gimbal_last_error(char *buf, size_t n);

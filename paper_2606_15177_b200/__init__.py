@@ -9,7 +9,7 @@ when no sm_100 device is present.
 """
 from .binding import (  # noqa: F401
     GimbalError, RouterCfg, PlacementCfg, StatsState, lib, lib_path, last_error, launch_count,
-    route_stats, route_stats_static, STATIC_SCRATCH_BYTES, route_stats_host, eval_placements, eval_placements_host, eval_moves,
+    route_stats, route_stats_static, STATIC_SCRATCH_BYTES, ABI_VERSION, route_stats_host, eval_placements, eval_placements_host, eval_moves,
     route_stats_workspace_bytes, eval_placements_workspace_bytes, eval_moves_workspace_bytes,
     LOGITS_NONE, LOGITS_OUT, LOGITS_IN, MODE_WINDOW, MODE_EMA, SCORE_SOFTMAX, SCORE_SIGMOID,
     COUNTS_I32, COUNTS_F32, EXPORTED_SYMBOLS, kernel_timing, kernel_elapsed_ms, route_stats_result_bytes,

@@ -9,6 +9,7 @@ import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
+ABI_VERSION = 300          # GIMBAL_ABI_VERSION of the include/gimbal.h this binding was written against
 LOGITS_NONE, LOGITS_OUT, LOGITS_IN = 0, 1, 2
 MODE_WINDOW, MODE_EMA = 0, 1
 SCORE_SOFTMAX, SCORE_SIGMOID = 0, 1
@@ -40,7 +41,7 @@ class _RouterCfg(C.Structure):
 
 
 class _StatsState(C.Structure):
-    _fields_ = [("mode", C.c_int32), ("window_len", C.c_int32), ("ema_decay", C.c_float), ("reserved", C.c_int32),
+    _fields_ = [("mode", C.c_int32), ("window_len", C.c_int32), ("ema_decay", C.c_float), ("abi_version", C.c_int32),
                 ("A_step", C.c_void_p), ("A_win", C.c_void_p), ("A_pub", C.c_void_p), ("B_pub", C.c_void_p),
                 ("A_ema", C.c_void_p), ("B", C.c_void_p), ("pressure_raw", C.c_void_p), ("pressure_rel", C.c_void_p),
                 ("step_counter", C.c_void_p), ("status", C.c_void_p)]
@@ -73,6 +74,8 @@ def lib():
                               "(there is no CPU fallback)")
         L = C.CDLL(path)
         L.gimbal_version.restype = C.c_int
+        if L.gimbal_version() != ABI_VERSION:
+            raise GimbalError(f"{path} has interface version {L.gimbal_version()}, this binding expects {ABI_VERSION}: rebuild it")
         L.gimbal_launch_count.restype = C.c_int64
         for n in ("gimbal_route_stats_workspace_bytes", "gimbal_route_stats_result_bytes",
                   "gimbal_eval_placements_workspace_bytes", "gimbal_eval_moves_workspace_bytes"):
@@ -200,7 +203,7 @@ class StatsState:
         return self.A_win if self.mode == MODE_WINDOW else self.A_ema
 
     def c(self):
-        return _StatsState(self.mode, self.window_len, self.ema_decay, 0, self.A_step.data_ptr(), self.A_win.data_ptr(),
+        return _StatsState(self.mode, self.window_len, self.ema_decay, ABI_VERSION, self.A_step.data_ptr(), self.A_win.data_ptr(),
                            self.A_pub.data_ptr(), self.B_pub.data_ptr(), self.A_ema.data_ptr(), self.B.data_ptr(),
                            self.pressure_raw.data_ptr(), self.pressure_rel.data_ptr(), self.step_counter.data_ptr(),
                            self.status.data_ptr())

@@ -127,6 +127,10 @@ static int validate_place_cfg(const gimbal_placement_cfg* c) {
     if ((long)c->G * c->slots_per_rank < c->E) return fail(GIMBAL_ERR_INVALID_ARG, "G*slots_per_rank < E");
     if (c->counts_dtype != GIMBAL_COUNTS_I32 && c->counts_dtype != GIMBAL_COUNTS_F32) return fail(GIMBAL_ERR_INVALID_ARG, "counts_dtype=%d", c->counts_dtype);
     if (c->E % 2 != 0) return fail(GIMBAL_ERR_UNSUPPORTED, "E must be even");
+    // candidate / placement rows [NS] int16 are read as 32-bit words: an odd row length would misalign every other row
+    if (((long)c->G * c->slots_per_rank) % 2 != 0) return fail(GIMBAL_ERR_UNSUPPORTED, "G*slots_per_rank=%ld must be even", (long)c->G * c->slots_per_rank);
+    if (c->encoding != GIMBAL_ENC_SLOT_TO_EXPERT_I16 && c->encoding != GIMBAL_ENC_EXPERT_TO_RANK_U8) return fail(GIMBAL_ERR_INVALID_ARG, "encoding=%d", c->encoding);
+    if (c->flags & ~GIMBAL_PLACE_TRUSTED) return fail(GIMBAL_ERR_INVALID_ARG, "flags=0x%x has bits this library does not know", c->flags);
     return GIMBAL_OK;
 }
 
@@ -295,7 +299,7 @@ __global__ void __launch_bounds__(256) expert_map_kernel(int E, int NS, const in
 
 extern "C" {
 
-int gimbal_version(void) { return 100; }
+int gimbal_version(void) { return GIMBAL_ABI_VERSION; }
 
 void gimbal_last_error(char* buf, size_t n) {
     if (!buf || n == 0) return;
@@ -346,7 +350,12 @@ int gimbal_route_stats(const gimbal_router_cfg* cfg, int layer0, int n_layers, i
     if (layer0 < 0 || n_layers < 1 || layer0 + n_layers > cfg->L) return fail(GIMBAL_ERR_INVALID_ARG, "layer range [%d,%d) outside [0,%d)", layer0, layer0 + n_layers, cfg->L);
     if (T < 0) return fail(GIMBAL_ERR_INVALID_ARG, "T=%d", T);
     if (!src_offsets) return fail(GIMBAL_ERR_INVALID_ARG, "src_offsets is NULL");
-    if (!st || !st->A_step || !st->step_counter || !st->B) return fail(GIMBAL_ERR_INVALID_ARG, "state / A_step / B / step_counter is NULL");
+    if (!st) return fail(GIMBAL_ERR_INVALID_ARG, "state is NULL");
+    // a state laid out by another header (round 1: step_counter [1], this field `reserved` = 0) would be written out of bounds
+    if (st->abi_version != GIMBAL_ABI_VERSION)
+        return fail(GIMBAL_ERR_INVALID_ARG, "state->abi_version=%d, this library is %d: rebuild against include/gimbal.h (step_counter is i64[2])",
+                    st->abi_version, GIMBAL_ABI_VERSION);
+    if (!st->A_step || !st->step_counter || !st->B) return fail(GIMBAL_ERR_INVALID_ARG, "state: A_step / B / step_counter is NULL");
     if (st->mode == GIMBAL_MODE_WINDOW) {
         if (!st->A_win || !st->A_pub || !st->B_pub || st->window_len < 1) return fail(GIMBAL_ERR_INVALID_ARG, "WINDOW mode needs A_win, A_pub, B_pub, window_len >= 1");
     } else if (st->mode == GIMBAL_MODE_EMA) {
@@ -516,19 +525,35 @@ struct gimbal_host_ctx {
     cudaEvent_t ev_copied[kHostCtxSlots], ev_done[kHostCtxSlots];
 };
 
+// destroys whatever a (possibly half-built) context holds; handles that were never created are null
+static void host_ctx_release(gimbal_host_ctx* c) {
+    for (int i = 0; i < kHostCtxSlots; ++i) {
+        if (c->ev_copied[i]) cudaEventDestroy(c->ev_copied[i]);
+        if (c->ev_done[i]) cudaEventDestroy(c->ev_done[i]);
+    }
+    if (c->ev_start) cudaEventDestroy(c->ev_start);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    delete c;
+}
+
 int gimbal_host_ctx_create(gimbal_host_ctx** out) {
     if (!out) return fail(GIMBAL_ERR_INVALID_ARG, "ctx out pointer is NULL");
     *out = nullptr;
     int rc = require_device();
     if (rc) return rc;
-    gimbal_host_ctx* c = new (std::nothrow) gimbal_host_ctx();
+    gimbal_host_ctx* c = new (std::nothrow) gimbal_host_ctx();     // value-initialised: every handle starts null
     if (!c) return fail(GIMBAL_ERR_CUDA, "out of host memory");
-    CUDA_TRY(cudaGetDevice(&c->device));
-    CUDA_TRY(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
-    CUDA_TRY(cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));
-    for (int i = 0; i < kHostCtxSlots; ++i) {
-        CUDA_TRY(cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming));
-        CUDA_TRY(cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming));
+    // a failure half-way must not leak the stream and the events made so far
+    cudaError_t e = cudaGetDevice(&c->device);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming);
+    for (int i = 0; i < kHostCtxSlots && e == cudaSuccess; ++i) {
+        e = cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming);
+    }
+    if (e != cudaSuccess) {
+        host_ctx_release(c);
+        return fail(GIMBAL_ERR_CUDA, "gimbal_host_ctx_create: %s", cudaGetErrorString(e));
     }
     *out = c;
     return GIMBAL_OK;
@@ -537,10 +562,7 @@ int gimbal_host_ctx_create(gimbal_host_ctx** out) {
 int gimbal_host_ctx_destroy(gimbal_host_ctx* c) {
     if (!c) return GIMBAL_OK;
     cudaStreamSynchronize(c->copy_stream);
-    for (int i = 0; i < kHostCtxSlots; ++i) { cudaEventDestroy(c->ev_copied[i]); cudaEventDestroy(c->ev_done[i]); }
-    cudaEventDestroy(c->ev_start);
-    cudaStreamDestroy(c->copy_stream);
-    delete c;
+    host_ctx_release(c);
     return GIMBAL_OK;
 }
 

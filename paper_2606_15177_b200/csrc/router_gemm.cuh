@@ -61,10 +61,9 @@ constexpr int kGemmMaxStages = 12;
 // bytes after the ring: [aux][select_bias N f32][src_offsets S+1 (padded)][hist S*N i32][selection list, when
 // ids / weights are written: kListWords x 128 epilogue threads]
 // ... [exchange buffers of the epilogue parts, ep > 1: 4 quadrants x [ep][8][32] words]
-// words of the histogram region: [S][N] counts, and at least the scratch of a fused layer update (UpdateScratch)
-__host__ __device__ constexpr size_t gemm_hist_words(int S, int N) {
-    return (size_t)S * N > (sizeof(UpdateScratch) + 3) / 4 ? (size_t)S * N : ((sizeof(UpdateScratch) + 3) / 4 + 3) / 4 * 4;
-}
+// words of the histogram region: [S][N] counts (a multiple of 16 words).  The scratch of a fused layer update (UpdateScratch)
+// does not live here: it reuses the drained operand ring, which holds at least two stages
+__host__ __device__ constexpr size_t gemm_hist_words(int S, int N) { return (size_t)S * N; }
 template <int N>
 constexpr size_t gemm_tail_bytes(int S, bool out, int ep = 1) {
     return kGemmAuxBytes + sizeof(float) * N + sizeof(int32_t) * (size_t)((S + 1 + 3) & ~3) + sizeof(int32_t) * gemm_hist_words(S, N) +
@@ -390,6 +389,7 @@ router_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_cons
         if (p.fuse_update && warp >= 4 && leader) {
             // a4 + a5 of this layer right here, from the counts in `hist`; scratch = the (drained) operand ring
             asm volatile("bar.sync 1, %0;" ::"n"(kEpiThreads) : "memory");
+            static_assert(2 * gemm_stage_bytes<N, kCG>() >= (int)sizeof(UpdateScratch), "the scratch of the fused update must fit two ring stages");
             UpdateScratch& sh = *reinterpret_cast<UpdateScratch*>(base_ptr);
             const int32_t* hc = hist;
             stats_update_layer(p.upd, p.layer0 + pair, (int)threadIdx.x - 128, kEpiThreads, sh, step_now,

@@ -21,7 +21,7 @@ def _declared_symbols():
 def test_build_is_current_and_loads():
     from paper_2606_15177_b200 import build
     build.build()
-    assert g.lib().gimbal_version() >= 100
+    assert g.lib().gimbal_version() == g.ABI_VERSION == 300
 
 
 def test_every_declared_symbol_is_exported():
@@ -66,6 +66,11 @@ def test_host_side_validation():
     rc = g.lib().gimbal_eval_placements(C.byref(pc), 1, None, None, None, None, None, C.c_float(1.0), None, None, None, None,
                                         C.c_size_t(0), None)
     assert rc == -2 and "power of two" in g.last_error()
+    # one rank with an odd number of slots: rows of odd length would be read through misaligned 32-bit words
+    pc = g.PlacementCfg(L=2, E=2, G=1, slots_per_rank=3, S=2).c()
+    rc = g.lib().gimbal_eval_placements(C.byref(pc), 1, None, None, None, None, None, C.c_float(1.0), None, None, None, None,
+                                        C.c_size_t(0), None)
+    assert rc == -2 and "must be even" in g.last_error()
     assert g.eval_placements_workspace_bytes(g.PlacementCfg(L=58, E=256, G=32, slots_per_rank=9, S=16), 4096) > 58 * 256 * 32 * 8
 
 
@@ -76,7 +81,7 @@ def test_no_cpu_fallback_without_gpu():
     st = g.binding._StatsState()
     one = C.c_void_p(16)          # fake non-NULL, 16-byte aligned "device" pointers: never dereferenced on the host
     st.A_step = st.A_win = st.A_pub = st.B_pub = st.B = st.step_counter = 16
-    st.mode, st.window_len = 0, 1
+    st.mode, st.window_len, st.abi_version = 0, 1, g.ABI_VERSION
     rc = g.lib().gimbal_route_stats(C.byref(c), 0, 1, 16, one, one, None, None, one, 0, None, None, None, None, None, 0, 0,
                                     C.byref(st), None, one, C.c_size_t(1 << 20), None)
     assert rc == -2 and "CUDA" in g.last_error()
@@ -94,3 +99,28 @@ def test_options_are_validated_and_readable():
     for opt in (g.OPT_SCORE_TMA, g.OPT_HIST_AGG, g.OPT_FUSE_UPDATE):
         assert g.lib().gimbal_set_option(opt, 2) == -1 and g.get_option(opt) == 1
     assert g.lib().gimbal_set_option(99, 0) == -1
+
+
+def test_structs_laid_out_by_another_header_are_refused():
+    """A caller compiled against the round-1 header passes a state whose step_counter is i64[1] and whose `reserved` word is 0,
+    and a placement cfg that ends before `encoding` / `flags` (whatever follows it in memory is read there): both are refused on
+    the host, before anything is launched, instead of being written or read out of bounds."""
+    cfg = g.RouterCfg(L=1, H=256, E=16, k=2, S=2)
+    c = cfg.c()
+    st = g.binding._StatsState()
+    one = C.c_void_p(16)
+    st.A_step = st.A_win = st.A_pub = st.B_pub = st.B = st.step_counter = 16
+    st.mode, st.window_len = 0, 1                                   # abi_version left at 0, as `reserved` was
+    rc = g.lib().gimbal_route_stats(C.byref(c), 0, 1, 16, one, one, None, None, one, 0, None, None, None, None, None, 0, 0,
+                                    C.byref(st), None, one, C.c_size_t(1 << 20), None)
+    assert rc == -1 and "abi_version=0" in g.last_error() and "300" in g.last_error()
+    rc = g.lib().gimbal_route_stats_static(C.byref(c), 0, 1, 16, one, one, None, None, one, 0, None, None, None, None, None, 0, 0,
+                                           C.byref(st), None, None)
+    assert rc in (-1, -2)                                          # -2 on a CPU box (the device probe comes first on this entry point)
+    for enc, flags, what in ((2, 0, "encoding=2"), (0, 6, "flags=0x6"), (-1, 0, "encoding=-1")):
+        pc = g.PlacementCfg(L=1, E=16, G=4, slots_per_rank=4, S=2, encoding=enc, flags=flags).c()
+        rc = g.lib().gimbal_eval_placements(C.byref(pc), 1, None, None, None, None, None, C.c_float(1.0), None, None, None, None,
+                                            C.c_size_t(0), None)
+        assert rc == -1 and what in g.last_error()
+        assert g.lib().gimbal_eval_moves(C.byref(pc), None, None, C.c_int64(0), None, None, None, None, None, C.c_float(1.0), None, None,
+                                         None, C.c_size_t(0), None) == -1
