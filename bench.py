@@ -79,6 +79,18 @@ class ClockSampler:
 
     def __init__(self, gpu_index: int):
         self.gpu, self.proc, self.path = gpu_index, None, f"/tmp/gimbal_clocks_{os.getpid()}.csv"
+        self.nvml, self.e0_mj, self.t0 = None, None, None
+
+    def _energy_mj(self):
+        """NVML's total-energy counter of the board (mJ since the driver loaded) | None"""
+        try:
+            if self.nvml is None:
+                import pynvml
+                pynvml.nvmlInit()
+                self.nvml = (pynvml, pynvml.nvmlDeviceGetHandleByIndex(self.gpu))
+            return int(self.nvml[0].nvmlDeviceGetTotalEnergyConsumption(self.nvml[1]))
+        except Exception:
+            return None
 
     def start(self):
         try:
@@ -86,6 +98,7 @@ class ClockSampler:
                                           "-i", str(self.gpu)], stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
+            self.e0_mj, self.t0 = self._energy_mj(), time.perf_counter()
             return
         # nvidia-smi needs a moment to attach: the timed region starts once the first sample is on disk
         t0 = time.perf_counter()
@@ -96,9 +109,17 @@ class ClockSampler:
             except OSError:
                 pass
             time.sleep(0.01)
+        self.e0_mj, self.t0 = self._energy_mj(), time.perf_counter()
 
     def stop(self):
+        """call right after the synchronize that ends the timed region"""
+        e1, t1 = self._energy_mj(), time.perf_counter()
         out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[])
+        if self.e0_mj is not None and e1 is not None:
+            out.update(energy_j=(e1 - self.e0_mj) / 1e3, energy_window_ms=(t1 - self.t0) * 1e3,
+                       avg_power_w=((e1 - self.e0_mj) / 1e3 / (t1 - self.t0) if t1 > self.t0 else None),
+                       energy_note="nvmlDeviceGetTotalEnergyConsumption read right before the first and right after the last timed step "
+                                   "(host wall window, includes the L2 flushes between steps)")
         if self.proc is None:
             return out
         self.proc.terminate()
@@ -292,6 +313,57 @@ def _config(w, args):
                         + ("written" if getattr(args, "with_ids", False) else "not written"))
 
 
+def _best_ms(fn, reps=5):
+    """device time of one call of `fn` between two CUDA events on the current stream, best of `reps`"""
+    best = None
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); fn(); e1.record()
+        torch.cuda.synchronize()
+        t = e0.elapsed_time(e1)
+        best = t if best is None else min(best, t)
+    return best
+
+
+def aux_rates(g, w, pc, cur, prev, A, B, D, ws_p, dev):
+    """Throughput of the entry points outside the timed step (parity is in tests/): whole calls between
+    CUDA events, warm, best of five.  Synthetic instances: uniform traces / request lengths / arrival times."""
+    r = w.router
+    gen_ = torch.Generator(device=dev); gen_.manual_seed(5)
+    out = {}
+    nb, N, R = 8192, 16, 64                                               # Algorithm 1: nb scheduler instances x R requests over N engines
+    trace = torch.rand(nb, N, 4, generator=gen_, device=dev)
+    trace[..., 1:3] *= 4000.0
+    trace[..., 3] += 0.5
+    req = torch.rand(nb, R, generator=gen_, device=dev) * 2000.0 + 16.0
+    comp = torch.zeros(nb, N, dtype=torch.float64, device=dev); rr = torch.zeros(nb, dtype=torch.int32, device=dev)
+    eng = torch.empty(nb, R, dtype=torch.int32, device=dev)
+    t = _best_ms(lambda: g.select_engines(trace, req, comp, rr, eng, lambda_kv=2000.0, lambda_moe=500.0, close_frac=0.05))
+    out["select_engines"] = dict(ms=t, instances=nb, engines=N, requests_per_instance=R, instances_per_s=nb / (t * 1e-3),
+                                 decisions_per_s=nb * R / (t * 1e-3))
+    nq, Q = 4096, 1024                                                    # Algorithm 2: nq waiting queues of up to Q requests
+    arrival = torch.rand(nq, Q, generator=gen_, device=dev) * 10.0
+    prefill = torch.randint(1, 8192, (nq, Q), generator=gen_, device=dev, dtype=torch.int32)
+    qlen = torch.randint(Q // 2, Q + 1, (nq,), generator=gen_, device=dev, dtype=torch.int32)
+    order = torch.empty(nq, Q, dtype=torch.int32, device=dev)
+    t = _best_ms(lambda: g.order_queues(arrival, prefill, qlen, 10.0, order))
+    out["order_queues"] = dict(ms=t, queues=nq, max_len=Q, queues_per_s=nq / (t * 1e-3), requests_per_s=float(qlen.sum().item()) / (t * 1e-3))
+    n_moves = r.L * w.NS * (w.NS - 1) // 2                               # swap search: rounds of "best exchange per layer"
+    delta = torch.empty(n_moves, 5, device=dev); best = torch.empty(r.L, dtype=torch.int32, device=dev)
+    iters = 4
+    work = cur.clone()
+
+    def refine():
+        work.copy_(cur)
+        g.refine_placement(pc, work, prev, A, B, D, delta, best, iters=iters, workspace=ws_p)
+    t = _best_ms(refine)
+    out["refine_placement"] = dict(ms=t, iters=iters, layers=r.L, rounds_per_s=iters / (t * 1e-3), moves_scored_per_s=iters * n_moves / (t * 1e-3))
+    t = _best_ms(lambda: g.ExpertMap(r.L, r.E, w.G, w.slots_per_rank, cur))
+    out["build_expert_map"] = dict(ms=t, layers=r.L, layers_per_s=r.L / (t * 1e-3), note="includes the two torch.empty of the binding's ExpertMap")
+    out["note"] = "outside the timed step; whole entry-point calls (all their kernels) between CUDA events, warm, best of 5"
+    return out
+
+
 def _check_ms(g):
     """device time of the last place_check_kernel; 0 where the validation is fused into place_score_kernel (the five config shapes)"""
     try:
@@ -386,6 +458,23 @@ def run_ours(args, w):
         flush.zero_()
         g.eval_moves(pc, cur, prev, A_live, B_live, D, delta, best_per_layer=best, workspace=ws_p)
         moves_alone_ms.append(g.kernel_elapsed_ms(g.KERNEL_MOVES))
+    # a7 on an EXPLICIT list (the heuristic's own use: the feasible ranks of one expert are a list of moves):
+    # move_delta_kernel, one thread per move with global gathers; 12 B read + 20 B written per move
+    n_list = 1 << 22
+    gl = torch.Generator(device=dev); gl.manual_seed(77)
+    ma = torch.randint(0, w.NS, (n_list,), generator=gl, device=dev, dtype=torch.int32)
+    mb = torch.randint(0, w.NS - 1, (n_list,), generator=gl, device=dev, dtype=torch.int32)
+    mb = mb + (mb >= ma).to(torch.int32)
+    move_list = torch.stack([torch.randint(0, r.L, (n_list,), generator=gl, device=dev, dtype=torch.int32), torch.minimum(ma, mb),
+                             torch.maximum(ma, mb)], dim=1).contiguous()
+    delta_list = torch.empty(n_list, 5, device=dev)
+    moves_list_ms = []
+    for _ in range(4):
+        flush.zero_()
+        g.eval_moves(pc, cur, prev, A_live, B_live, D, delta_list, moves=move_list, workspace=ws_p)
+        moves_list_ms.append(g.kernel_elapsed_ms(g.KERNEL_MOVES))
+    del delta_list, move_list, ma, mb
+    aux = aux_rates(g, w, pc, cur, prev, A_live, B_live, D, ws_p, dev) if rank == 0 else None
     # K2 (not part of the timed step): the standalone gating + histogram kernel on given logits (LOGITS_IN), the
     # kernel whose roofline is plain HBM: 4*E bytes read per token-layer.  Logits of `nl` layers (> L2) are
     # written once by the fused kernel's LOGITS_OUT mode, then re-read from HBM.
@@ -510,7 +599,15 @@ def run_ours(args, w):
                                timed="inside the timed step, at the clocks the power-capped router GEMM leaves behind",
                                alone=dict(ms=min(moves_alone_ms[1:]), achieved=20.0 * n_moves / (min(moves_alone_ms[1:]) * 1e-3) / 1e9, unit="GB/s",
                                           frac=20.0 * n_moves / (min(moves_alone_ms[1:]) * 1e-3) / 1e9 / peaks["hbm"],
-                                          timed="outside the timed step, after an L2 flush (as place_score_kernel)")))
+                                          timed="outside the timed step, after an L2 flush (as place_score_kernel)"),
+                               kernel="move_all_kernel (the implicit whole neighbourhood)"),
+        move_list_kernel=dict(ms=min(moves_list_ms[1:]), moves=n_list, moves_per_s=n_list / (min(moves_list_ms[1:]) * 1e-3), bound="hbm",
+                              achieved=32.0 * n_list / (min(moves_list_ms[1:]) * 1e-3) / 1e9, peak=peaks["hbm"], unit="GB/s",
+                              frac=32.0 * n_list / (min(moves_list_ms[1:]) * 1e-3) / 1e9 / peaks["hbm"],
+                              algorithmic_bytes="12 B read + 20 B written per move (explicit list)",
+                              kernel="move_delta_kernel: one thread per listed move, tables gathered from global memory / L2",
+                              timed="outside the timed step, after an L2 flush; uniformly random (layer, slot a < slot b) moves"),
+        aux_rates=aux)
 
     # ---- e2e: the same step through the *_host entry points ------------------------------------------
     e2e = None
@@ -540,10 +637,50 @@ def run_ours(args, w):
         line = dict(metric=METRIC, value=value, unit="routed tokens/s", n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
                     ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16",
                     data="synthetic", config=_config(w, args), clocks=clocks, e2e=e2e, gpu_launches=int(launches),
-                    roofline=roofline, cpu_baseline=cpu, topk_flip_rate=flips, token_layers_per_s=value * r.L, **extra)
-        print(json.dumps(line))
+                    roofline=roofline, cpu_baseline=cpu, topk_flip_rate=flips, token_layers_per_s=value * r.L,
+                    energy_j_per_step=(clocks["energy_j"] / args.steps if clocks.get("energy_j") is not None else None), **extra)
     if dist:
         td.destroy_process_group()
+    return line if rank == 0 else None
+
+
+# routed tokens/s of the whole stats step at the HBM peak, fully fused, before launch overhead
+FUSED_BOUND_TOKENS_PER_S = dict(v2lite=61e6, qwen3=33e6, v3=7.8e6, decode=3.9e6)
+
+
+def collect_configs(args):
+    """The other four BASELINE.json configs (one step each, timed as the headline is) and the decode episode, each in a process of
+    its own (`bench.py --workload X`, no CPU baseline, no host leg) so that every config starts from an empty GPU; the line of each
+    run is cut down to the figures DESIGN.md section 8 quotes.  A failed run is reported as such, never replaced."""
+    # step counts: a timed window of >= 0.3 s each, so that the 20 ms clock sampler sees it more than ten times
+    runs = [("tiny", ["--workload", "tiny", "--steps", "2000"]), ("v2lite", ["--workload", "v2lite", "--steps", "800"]),
+            ("qwen3", ["--workload", "qwen3", "--steps", "300"]), ("decode", ["--workload", "decode", "--steps", "500"]),
+            ("decode_episode", ["--workload", "decode", "--episode"])]
+    keep = ("value", "unit", "ms_per_step", "steps", "gpu_launches", "clocks", "energy_j_per_step", "placements_per_s", "placements_per_s_trusted",
+            "moves_per_s", "pdl2_ab", "bound_tokens_per_s")
+    out = {}
+    for name, extra in runs:
+        cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--no-configs", "--no-cpu-baseline", "--no-e2e", "--warmup", str(max(args.warmup, 3))] + extra
+        try:
+            r = subprocess.run(cmd, capture_output=True, text=True, timeout=900)
+            d = json.loads(r.stdout.strip().splitlines()[-1])
+        except Exception as ex:  # report, never fake
+            out[name] = dict(error=f"{type(ex).__name__}: {str(ex)[:200]}", command=" ".join(cmd[1:]))
+            continue
+        c = {k: d[k] for k in keep if k in d}
+        c["workload"] = d["config"]["workload"]
+        c["command"] = "python bench.py " + " ".join(cmd[2:])
+        rf = d.get("roofline") or {}
+        c["router_kernel"] = {k: rf[k] for k in ("kernel", "ms", "bound", "achieved", "peak", "unit", "frac", "share_of_step", "hbm") if k in rf}
+        for k in ("gate_hist_kernel", "place_score_kernel", "place_score_in_step", "place_check_kernel", "move_delta_kernel", "move_list_kernel"):
+            if k in d:
+                c[k] = {f: d[k][f] for f in ("ms", "achieved", "unit", "frac", "kernel") if f in d[k]}
+        bound = FUSED_BOUND_TOKENS_PER_S.get(name.split("_")[0])
+        if bound and "bound_tokens_per_s" not in c:
+            c["fused_bound_tokens_per_s"] = bound
+            c["frac_of_fused_bound"] = d["value"] / bound
+        out[name] = c
+    return out
 
 
 def run_e2e(g, w, cfg, pc, st, hidden, off, cands, W, sb, slb, cur, dp, D, prev, delta, ws_r, ws_p, args, dev):
@@ -653,39 +790,58 @@ def run_episode(args, w):
     torch.cuda.synchronize()
     side = torch.cuda.Stream()
     side.wait_stream(torch.cuda.current_stream())
-    graph = torch.cuda.CUDAGraph()
-    launches0 = g.launch_count()
-    # every input of the episode (the ring of hidden states, weights, biases, offsets) is resident before the first replay: the promise
-    # GIMBAL_OPT_PDL = 2 asks for, so a step's router kernel may overlap the previous step's update kernel (--opt PDL=1 / 0 for the A/B)
-    if not any(o.upper().startswith("PDL=") for o in (args.opt or [])):
-        g.set_option(g.OPT_PDL, 2)
-    with torch.cuda.graph(graph, stream=side):
+
+    def timed_replays(body, n_replays, with_clocks):
+        """capture `body` on the side stream, warm up, time n_replays replays with CUDA events -> (ms, clocks, kernels per graph)"""
+        graph = torch.cuda.CUDAGraph()
+        l0 = g.launch_count()
+        with torch.cuda.graph(graph, stream=side):
+            body(side)
+        per_graph = g.launch_count() - l0
+        for _ in range(max(args.warmup, 3)):
+            graph.replay()
+        torch.cuda.synchronize()
+        sampler = ClockSampler(0) if with_clocks else None
+        if sampler:
+            sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n_replays):
+            graph.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1), (sampler.stop() if sampler else None), per_graph
+
+    def episode_body(stream):
         for i in range(per):
-            one(i, side)
-        rescore(side)
-    launches_per_graph = g.launch_count() - launches0
+            one(i, stream)
+        rescore(stream)
+
+    # The episode's value is taken with the library's default launch mode (GIMBAL_OPT_PDL = 1: every kernel waits for its
+    # predecessor before its first global access), which is what a serving loop whose hidden states come from the kernel just
+    # before can rely on; `--opt PDL=x` overrides it.  PDL = 2 needs the caller's promise that the inputs were staged earlier --
+    # true of this bench (ring of pre-staged hidden states), not of serving -- and is reported beside it as a labelled A/B.
     pdl_mode = g.get_option(g.OPT_PDL)
-    for _ in range(max(args.warmup, 3)):
-        graph.replay()
-    torch.cuda.synchronize()
-    sampler = ClockSampler(0)
-    sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(K // per):
-        graph.replay()
-    e1.record()
-    torch.cuda.synchronize()
-    clocks = sampler.stop()
-    ms = e0.elapsed_time(e1)
+    ms, clocks, launches_per_graph = timed_replays(episode_body, K // per, True)
     ms_per_step = ms / K
     value = w.T * K / (ms * 1e-3)
+    # the re-score's share, measured the same way: a graph that holds only the re-score, replayed as often
+    rescore_graph_ms = timed_replays(rescore, K // per, False)[0] / (K // per)
+    ab = None
+    if pdl_mode != 2:
+        g.set_option(g.OPT_PDL, 2)
+        ms2, clocks2, _ = timed_replays(episode_body, K // per, True)
+        g.set_option(g.OPT_PDL, pdl_mode)
+        ab = dict(option="GIMBAL_OPT_PDL = 2", ms_per_step=ms2 / K, value=w.T * K / (ms2 * 1e-3), unit="routed tokens/s", clocks=clocks2,
+                  note="A/B, not the headline: programmatic launches under the caller's promise that hidden / w_router / biases / src_offsets "
+                       "were complete before the previous call was enqueued (true here: steps replay pre-staged buffers), so a step's router "
+                       "kernel waits only before it stores its counts and overlaps the previous step's update")
     k1_eager_ms = statistics.median(k1[2:])
     step_bytes = 2.0 * r.L * (w.T * r.H + r.E * r.H)            # hidden + W_router of every layer, each read once per step
     # Inside the graph the router kernel is the step (the update runs in its tail, GIMBAL_OPT_FUSE_UPDATE) and consecutive launches
     # overlap under programmatic dependent launch, so a launch has no duration of its own: the kernel's average duration over the
-    # timed region is the region's time per launch, less the re-score's share (event-bracketed around its kernels above).
-    rescore_share_ms = (statistics.median(ksc) + statistics.median(kck)) / per
+    # timed region is the region's time per launch, less the re-score's share (a graph holding only the re-score, replayed and timed the same way).
+    rescore_share_ms = rescore_graph_ms / per
     k1_ms = max(ms_per_step - rescore_share_ms, 1e-6)
     roofline = dict(bound="hbm", achieved=step_bytes / (k1_ms * 1e-3) / 1e9, peak=peaks["hbm"], unit="GB/s",
                     frac=step_bytes / (k1_ms * 1e-3) / 1e9 / peaks["hbm"], traffic=None,
@@ -693,7 +849,7 @@ def run_episode(args, w):
                     ms_eager_event_bracketed=k1_eager_ms,
                     algorithmic_bytes=step_bytes, share_of_step=k1_ms / ms_per_step,
                     note="decode regime: one tile per CTA pair, the GEMM is bound by streaming hidden and W_router once; ms = time of the timed "
-                         "region per launch less the re-score's share (launches overlap inside the graph); ms_eager_event_bracketed = one eager "
+                         "region per launch less the re-score's share (a re-score-only graph replayed the same way); ms_eager_event_bracketed = one eager "
                          "launch between two events (no overlap, update included)")
     bound_lo, bound_hi = 3.6e6, 3.9e6                           # unfused / fused traffic at HBM peak, before launch overhead
     cand_bytes = 2.0 * r.L * w.NS * w.P
@@ -744,7 +900,8 @@ def run_episode(args, w):
                 roofline=roofline, cpu_baseline=None,
                 bound_tokens_per_s=dict(lo=bound_lo, hi=bound_hi, frac_of_lo=value / bound_lo,
                                         note="SURVEY.md section 8d: 3.6 M (unfused) - 3.9 M (fused) tokens/s at HBM peak, before launch overhead"),
-                rescore=dict(score_ms=statistics.median(ksc), check_ms=statistics.median(kck),
+                energy_j_per_step=(clocks["energy_j"] / K if clocks.get("energy_j") is not None else None), pdl2_ab=ab,
+                rescore=dict(score_ms=statistics.median(ksc), check_ms=statistics.median(kck), graph_ms=rescore_graph_ms,
                              place_score_frac_hbm=cand_bytes / (statistics.median(ksc) * 1e-3) / 1e9 / peaks["hbm"],
                              amortised_ms_per_step=(statistics.median(ksc) + statistics.median(kck)) / per))
     print(json.dumps(line))
@@ -761,6 +918,8 @@ def main():
     ap.add_argument("--ring", type=int, default=32, help="--episode: step buffers of hidden states that the steps cycle through")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    ap.add_argument("--no-configs", action="store_true", help="default run only: skip the `configs` object (the other four configs and the "
+                                                                "decode episode, each timed in a process of its own)")
     ap.add_argument("--with-ids", action="store_true", help="also write top-k ids and weights (a2 outputs) inside the timed step")
     ap.add_argument("--layers", type=int, default=0, help="profiling only: run the first N MoE layers (named in config.workload)")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
@@ -784,7 +943,14 @@ def main():
             raise SystemExit("--episode is defined for the decode workload (BASELINE.json config 5)")
         run_episode(args, w)
     else:
-        run_ours(args, w)
+        line = run_ours(args, w)
+        if line is not None:
+            # the default invocation (what the driver records) also carries the other configs
+            if (args.workload == "v3" and not args.no_configs and args.layers == 0 and not args.opt and
+                    int(os.environ.get("WORLD_SIZE", "1")) == 1):
+                torch.cuda.empty_cache()
+                line["configs"] = collect_configs(args)
+            print(json.dumps(line))
 
 
 if __name__ == "__main__":
