@@ -57,8 +57,8 @@ def _profile_metrics(name: str) -> dict:
 
 
 K1_PROFILE = "r2_ncu_k1_router_gemm"       # V3 shape, `--layers 6`: counters are per launch of 6 layers x 65536 tokens
-K4_PROFILE = "r2_ncu_k4_place_score_tma"   # V3 shape, P = 4096, 58 layers, GIMBAL_PLACE_TRUSTED (scoring only): place_score_tma_kernel
-K4C_PROFILE = "r2_ncu_k4_place_score_checked"   # same, default call (validation fused in)
+K4_PROFILE = "r3_ncu_k4_place_score_tma"   # V3 shape, P = 4096, 58 layers, GIMBAL_PLACE_TRUSTED (scoring only): place_score_tma_kernel
+K4C_PROFILE = "r3_ncu_k4_place_score_checked"   # same, default call (validation fused in)
 
 
 def _peaks():
@@ -475,6 +475,53 @@ def run_ours(args, w):
         moves_list_ms.append(g.kernel_elapsed_ms(g.KERNEL_MOVES))
     del delta_list, move_list, ma, mb
     aux = aux_rates(g, w, pc, cur, prev, A_live, B_live, D, ws_p, dev) if rank == 0 else None
+    # EXPERT_TO_RANK_U8 (half the candidate bytes; defined without replicas only) against the default
+    # slot -> expert int16 encoding: the same candidates, the same validated call, the scoring kernel of each timed alone
+    e2r = None
+    if w.NS == r.E and r.E % 4 == 0 and rank == 0:
+        ranks = (torch.arange(w.NS, device=dev) // w.slots_per_rank).to(torch.uint8).expand(w.P, r.L, w.NS)
+        cands_u8 = torch.empty(w.P, r.L, r.E, dtype=torch.uint8, device=dev).scatter_(2, cands.long(), ranks).contiguous()
+        pc_u8 = g.PlacementCfg(**{**pc.__dict__, "encoding": g.ENC_EXPERT_TO_RANK_U8})
+        out_u8 = torch.empty(w.P, 5, device=dev)
+        t_u8, t_i16 = [], []
+        for _ in range(4):
+            flush.zero_()
+            g.eval_placements(pc_u8, cands_u8, A_live, B_live, D, prev, out_u8, workspace=ws_p)
+            t_u8.append(g.kernel_elapsed_ms(g.KERNEL_SCORE))
+            flush.zero_()
+            g.eval_placements(pc, cands, A_live, B_live, D, prev, out, workspace=ws_p)
+            t_i16.append(g.kernel_elapsed_ms(g.KERNEL_SCORE) + _check_ms(g))
+        torch.cuda.synchronize()
+        e2r = dict(expert_to_rank_u8_ms=min(t_u8[1:]), slot_to_expert_i16_ms=min(t_i16[1:]), ratio=min(t_u8[1:]) / min(t_i16[1:]),
+                   same_objective=bool(torch.allclose(out_u8, out, rtol=1e-5, atol=0.0, equal_nan=True)),
+                   candidate_bytes=dict(u8=int(cands_u8.numel()), i16=int(cands.numel() * 2)),
+                   note="validated default call on the same candidates in both encodings, scoring (+ validation) kernels timed alone after an L2 flush")
+        del cands_u8, out_u8
+    # Counting fused into the router kernel's epilogue against the two-kernel path (GEMM writes logits, the gating kernel reads them
+    # and counts): the build's analogue of the paper's Fig. 13 "count fusion" experiment
+    fusion = None
+    if rank == 0:
+        lg_all = None
+        try:
+            lg_all = torch.empty(r.L, w.T, r.E, device=dev)
+        except torch.cuda.OutOfMemoryError:
+            pass
+        if lg_all is not None:
+            def stats_only(fused):
+                g.set_option(g.OPT_FUSE_GATE, 1 if fused else 0)
+                try:
+                    return _best_ms(lambda: g.route_stats(cfg, st, T=w.T, hidden=hidden, w_router=W, select_bias=sb, src_logit_bias=slb,
+                                                          src_offsets=off, logits_mode=g.LOGITS_NONE if fused else g.LOGITS_OUT,
+                                                          logits=None if fused else lg_all, cur_placement=cur, dp_of_rank=dp, G=w.G,
+                                                          slots_per_rank=w.slots_per_rank, workspace=ws_r), reps=3)
+                finally:
+                    g.set_option(g.OPT_FUSE_GATE, 1)
+            t_f, t_u = stats_only(True), stats_only(False)
+            fusion = dict(fused_ms=t_f, two_kernels_ms=t_u, ratio=t_u / t_f,
+                          note="gimbal_route_stats alone (a1-a5), whole call between CUDA events, best of 3: counting and gating in the GEMM "
+                               "epilogue (logits never leave the chip) vs GEMM -> fp32 logits in HBM -> gating + counting kernel "
+                               "(GIMBAL_OPT_FUSE_GATE = 0); PAPER.md:360-368 is the paper's own count-fusion experiment")
+            del lg_all
     # K2 (not part of the timed step): the standalone gating + histogram kernel on given logits (LOGITS_IN), the
     # kernel whose roofline is plain HBM: 4*E bytes read per token-layer.  Logits of `nl` layers (> L2) are
     # written once by the fused kernel's LOGITS_OUT mode, then re-read from HBM.
@@ -607,7 +654,7 @@ def run_ours(args, w):
                               algorithmic_bytes="12 B read + 20 B written per move (explicit list)",
                               kernel="move_delta_kernel: one thread per listed move, tables gathered from global memory / L2",
                               timed="outside the timed step, after an L2 flush; uniformly random (layer, slot a < slot b) moves"),
-        aux_rates=aux)
+        aux_rates=aux, e2r_encoding=e2r, count_fusion=fusion)
 
     # ---- e2e: the same step through the *_host entry points ------------------------------------------
     e2e = None
@@ -675,6 +722,9 @@ def collect_configs(args):
         for k in ("gate_hist_kernel", "place_score_kernel", "place_score_in_step", "place_check_kernel", "move_delta_kernel", "move_list_kernel"):
             if k in d:
                 c[k] = {f: d[k][f] for f in ("ms", "achieved", "unit", "frac", "kernel") if f in d[k]}
+        for k in ("e2r_encoding", "count_fusion"):
+            if d.get(k):
+                c[k] = {f: v for f, v in d[k].items() if f != "note"}
         bound = FUSED_BOUND_TOKENS_PER_S.get(name.split("_")[0])
         if bound and "bound_tokens_per_s" not in c:
             c["fused_bound_tokens_per_s"] = bound

@@ -51,27 +51,32 @@ void copy_last_error(char* buf, size_t n) {
     snprintf(buf, n, "%s", g_err);
 }
 
+// One record per device ordinal, filled on the first call made with that device current: a process that drives several
+// GPUs gets each one's SM count (grid sizes follow it), not the count of whichever device came first.
 const DeviceInfo& device_info() {
-    static DeviceInfo info = [] {
+    constexpr int kMaxDevices = 64;
+    static DeviceInfo info[kMaxDevices];
+    static std::atomic<int> state[kMaxDevices];          // 0 = not probed, 2 = ready
+    static std::mutex mu;
+    static DeviceInfo none = [] { DeviceInfo d; snprintf(d.why, sizeof d.why, "no CUDA device"); return d; }();
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) {
+        cudaGetLastError();
+        return none;
+    }
+    if (state[dev].load(std::memory_order_acquire) == 2) return info[dev];
+    std::lock_guard<std::mutex> lk(mu);
+    if (state[dev].load(std::memory_order_relaxed) != 2) {
         DeviceInfo d;
-        int n = 0;
-        if (cudaGetDeviceCount(&n) != cudaSuccess || n == 0) {
-            snprintf(d.why, sizeof d.why, "no CUDA device");
-            cudaGetLastError();
-            return d;
-        }
-        int dev = 0, major = 0;
-        cudaGetDevice(&dev);
+        int major = 0;
         cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
         cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev);
-        if (major != 10) {
-            snprintf(d.why, sizeof d.why, "device compute capability %d.x, need 10.x (sm_100a)", major);
-            return d;
-        }
-        d.ok = true;
-        return d;
-    }();
-    return info;
+        if (major != 10) snprintf(d.why, sizeof d.why, "device %d: compute capability %d.x, need 10.x (sm_100a)", dev, major);
+        else d.ok = true;
+        info[dev] = d;
+        state[dev].store(2, std::memory_order_release);
+    }
+    return info[dev];
 }
 
 int require_device() {
